@@ -1,0 +1,203 @@
+/*
+ * spmv_b200.h -- C ABI of the B200-native autotuned fp64 CSR SpMV library.
+ *
+ *      y = alpha * A * x + beta * y        A: CSR, fp64 values, int32 indices
+ *
+ * The operation and its boundary are those of BASELINE.json:north_star (a)
+ * ("spmv_create / spmv_tune / spmv_apply / spmv_destroy, with arguments following
+ * the paper's problem statement of matrix, vectors and scalars"); the paper states
+ * the problem only as "sparse kernels vs cuSPARSE and CUSP" (sec. 3)
+ * and the method as annotate -> generate variants -> run -> compare outputs with
+ * the reference -> keep the fastest (sec. 2).
+ * fixes the conventions below.
+ *
+ * General rules
+ *   - C linkage, no exceptions or aborts cross this boundary; every call returns a
+ *     spmv_status_t (except the string/getter helpers).
+ *   - "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers.
+ *   - `stream` arguments are a cudaStream_t passed as void* (NULL = legacy default
+ *     stream).  spmv_apply / spmv_apply_batch are asynchronous and never
+ *     synchronise; spmv_create, spmv_tune, spmv_select synchronise the stream they
+ *     use.
+ *   - The handle BORROWS d_row_ptr / d_col_idx / d_val: the caller keeps them alive
+ *     and unmodified until spmv_destroy.  Converted formats and workspaces are OWNED
+ *     by the handle (allocated through the spmv_allocator_t callbacks, or
+ *     cudaMalloc/cudaFree when none is given).  x and y are caller-owned and must
+ *     not alias each other or the matrix.
+ *   - Limits: rows, cols, nnz <= 2^31-1 (int32 indices, BASELINE.json:configs[0]);
+ *     rows == 0 and nnz == 0 are valid.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point
+ *     returns SPMV_ERR_CUDA.
+ */
+#ifndef SPMV_B200_H
+#define SPMV_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define SPMV_API __attribute__((visibility("default")))
+#else
+#define SPMV_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spmv_handle_s* spmv_handle_t;
+
+typedef enum {
+  SPMV_OK = 0,
+  SPMV_ERR_INVALID_ARG = 1,     /* NULL pointer, negative size, unknown descriptor   */
+  SPMV_ERR_INVALID_MATRIX = 2,  /* row_ptr not monotone / wrong ends, col out of range */
+  SPMV_ERR_UNSUPPORTED = 3,     /* size over the int32 limits, variant not eligible  */
+  SPMV_ERR_ALLOC = 4,
+  SPMV_ERR_CUDA = 5,            /* text via spmv_last_error()                        */
+  SPMV_ERR_VERIFY_FAILED = 6,   /* no candidate matched the reference result          */
+  SPMV_ERR_INTERNAL = 7
+} spmv_status_t;
+
+/* Optional device allocator (e.g. the torch caching allocator). */
+typedef struct {
+  void* (*alloc)(size_t bytes, void* stream, void* ctx);
+  void (*free)(void* ptr, void* ctx);
+  void* ctx;
+} spmv_allocator_t;
+
+/* Matrix statistics, structure signature and the selected variant. */
+typedef struct {
+  int64_t rows, cols, nnz;
+  int32_t min_row_len, max_row_len;
+  double mean_row_len, var_row_len;
+  int64_t len_hist[32];     /* [0]: empty rows; [b>=1]: rows with 2^(b-1) <= len < 2^b */
+  int64_t bandwidth;        /* max |col - row| over stored entries                    */
+  int32_t cols_sorted;      /* 1: every row strictly ascending (sorted, no duplicates) */
+  int32_t block3_full;      /* 1: matrix is a union of dense, aligned 3x3 blocks       */
+  int64_t n_blocks3;        /* number of 3x3 blocks touched (valid if cols_sorted)     */
+  uint64_t sig_row_ptr;     /* order-independent 64-bit hashes of the structure        */
+  uint64_t sig_col_idx;
+  int32_t tuned;            /* 1 after a successful spmv_tune / cache hit              */
+  int32_t sm_count;
+  int64_t l2_bytes;
+  int64_t format_bytes;     /* matrix bytes streamed per apply by the selected variant */
+  int64_t owned_bytes;      /* device bytes currently owned by the handle              */
+  char variant[128];        /* descriptor of the selected variant                      */
+  char device_name[64];
+} spmv_info_t;
+
+/* Tuning options; zero-initialise for defaults. */
+typedef struct {
+  int32_t has_scalars;        /* 0: tune for alpha=1, beta=0; 1: use alpha/beta below */
+  double alpha, beta;
+  const double* d_x_probe;    /* cols  entries, device; NULL: tuner draws U[-1,1) from seed */
+  const double* d_y0_probe;   /* rows  entries, device; NULL: idem                      */
+  const double* d_y_ref;      /* optional externally computed reference result (device) */
+  const double* d_scale;      /*   and its per-row tolerance denominators; both or none.
+                                   When NULL the reference is the library's own unfused,
+                                   stored-order, one-thread-per-row device kernel -- the
+                                   "un-annotated program" of PAPER.md:19.                */
+  double tolerance;           /* 0 -> 1e-12 (north_star)                                */
+  int32_t warmup;             /* 0 -> 2 untimed launches per candidate                  */
+  int32_t reps;               /* 0 -> 5 timed batches per candidate (median)            */
+  double min_batch_ms;        /* 0 -> 0.5 ms per batch                                  */
+  double time_budget_s;       /* 0 -> unlimited                                         */
+  const char* variant_filter; /* comma-separated family prefixes, e.g. "csr_vector,sell"; NULL = all */
+  int32_t n_carveouts;        /* 0 -> {-1 (driver default)}                             */
+  int32_t carveouts[8];       /* shared-memory carve-out percentages, -1 = default      */
+  int32_t use_cache;          /* 0 -> use the in-process cache; 2 -> bypass it           */
+  const char* cache_path;     /* optional file persisted across processes               */
+  const char* fault_inject;   /* TEST ONLY: descriptor prefix of candidates whose output
+                                 is perturbed before verification                       */
+  uint64_t seed;
+  int32_t flush_l2;           /* 1: overwrite a > L2-sized buffer before each timed launch */
+  void* stream;
+} spmv_tune_opts_t;
+
+typedef struct {
+  char winner[128];
+  double winner_us;            /* median time per apply of the winner                  */
+  double default_us;           /* same protocol, the fixed default variant             */
+  int32_t n_enumerated, n_pruned_structural, n_pruned_slow, n_rejected, n_timed;
+  double tune_seconds;
+  int32_t cache_hit;
+  char runner_up[128];
+  double runner_up_us;
+  /* optional per-candidate log: "descriptor status time_us max_err_over_scale\n" */
+  char* log_buf;
+  size_t log_cap;
+  size_t log_len;
+} spmv_tune_report_t;
+
+/* Build a handle: validates the CSR arrays on the device and gathers statistics.
+ * Errors: INVALID_ARG (NULL out / negative size / NULL array with nnz > 0),
+ * UNSUPPORTED (over int32 limits), INVALID_MATRIX, CUDA, ALLOC.  *out untouched on
+ * failure. */
+SPMV_API spmv_status_t spmv_create(spmv_handle_t* out, int64_t rows, int64_t cols, int64_t nnz,
+                          const int32_t* d_row_ptr, const int32_t* d_col_idx,
+                          const double* d_val, const spmv_allocator_t* alloc, void* stream);
+
+/* The paper's loop: enumerate candidates (variant x launch config x
+ * carve-out), run each on the actual matrix, compare its output with the reference
+ * result, time the ones that match, keep the fastest, cache it per matrix signature. */
+SPMV_API spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts, spmv_tune_report_t* report);
+
+/* y = alpha*A*x + beta*y with the selected variant (the fixed default variant until
+ * spmv_tune / spmv_select).  beta == 0: y is write-only (never read).  alpha == 0:
+ * y = beta*y, A and x are not referenced.  Asynchronous on `stream`. */
+SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta,
+                         double* d_y, void* stream);
+
+/* Same operation with HOST vectors: copies x (and y when beta != 0) to the device,
+ * applies, copies y back; synchronises `stream` before returning. */
+SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
+                              double* h_y, void* stream);
+
+/* n independent applies, handle i on streams[i % nstreams] ("number of
+ * asynchronous streams").  No synchronisation. */
+SPMV_API spmv_status_t spmv_apply_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,
+                               const double* const* d_xs, const double* betas,
+                               double* const* d_ys, void* const* streams, int32_t nstreams);
+
+/* Times spmv_apply_batch over 1, 2, 4, ... <= max_streams of the caller's streams and
+ * returns the fastest count; us_per_count[i] (may be NULL) receives the batch time for
+ * the i-th count tried. */
+SPMV_API spmv_status_t spmv_tune_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,
+                              const double* const* d_xs, const double* betas,
+                              double* const* d_ys, void* const* streams, int32_t max_streams,
+                              int32_t* best_nstreams, double* us_per_count);
+
+/* Force a variant by descriptor ("default" = the fixed default).  Builds the format it
+ * needs.  Errors: INVALID_ARG (unparsable), UNSUPPORTED (not eligible for this matrix). */
+SPMV_API spmv_status_t spmv_select(spmv_handle_t h, const char* variant_descriptor, void* stream);
+
+/* Writes the newline-separated descriptors of every candidate the tuner would
+ * enumerate for this matrix (after structural pruning) into buf; *len = bytes needed. */
+SPMV_API spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap, size_t* len);
+
+SPMV_API spmv_status_t spmv_get_info(spmv_handle_t h, spmv_info_t* out);
+
+/* Inspection (tests): copy an owned array of the selected variant's format to the host.
+ * name in {"slice_ptr","sval","scol","perm","brow_ptr","bcol","bval","tile_row"};
+ * *bytes receives the array size; copies min(cap, size) bytes when h_buf != NULL. */
+SPMV_API spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_buf,
+                                   size_t cap, size_t* bytes, void* stream);
+
+/* Errors: INVALID_ARG on NULL or on a handle that was already destroyed. */
+SPMV_API spmv_status_t spmv_destroy(spmv_handle_t h);
+
+/* Measured ceilings with the library's own kernels, for the bench report:
+ * kind 0: device copy GB/s (read+write bytes), 1: read-only streaming sum GB/s,
+ * 2: empty-kernel launch latency in microseconds. */
+SPMV_API spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_t reps, void* stream,
+                                   double* result);
+
+SPMV_API const char* spmv_status_string(spmv_status_t s);
+SPMV_API const char* spmv_last_error(void);   /* thread-local text of the last CUDA/internal error */
+SPMV_API const char* spmv_version(void);
+SPMV_API void spmv_clear_cache(void);          /* drops the in-process tuning cache */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPMV_B200_H */

@@ -1,0 +1,311 @@
+"""Thin ctypes binding over libspmv_b200.so (include/spmv_b200.h): argument marshalling
+only -- every step of the path runs in the library's CUDA kernels.  PyTorch is used for
+device memory and streams, nothing else.  There is no fallback: if the shared library is
+missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libspmv_b200.so")
+_lib = None
+
+SPMV_OK = 0
+STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "SPMV_ERR_UNSUPPORTED",
+                "SPMV_ERR_ALLOC", "SPMV_ERR_CUDA", "SPMV_ERR_VERIFY_FAILED", "SPMV_ERR_INTERNAL"]
+
+EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
+           "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
+           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_status_string",
+           "spmv_last_error", "spmv_version", "spmv_clear_cache"]
+
+
+class SpmvError(RuntimeError):
+    def __init__(self, status: int, where: str, text: str = ""):
+        self.status = status
+        name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        super().__init__(f"{where}: {name}" + (f" ({text})" if text else ""))
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class Allocator(C.Structure):
+    _fields_ = [("alloc", ALLOC_FN), ("free", FREE_FN), ("ctx", C.c_void_p)]
+
+
+class Info(C.Structure):
+    _fields_ = [("rows", C.c_int64), ("cols", C.c_int64), ("nnz", C.c_int64),
+                ("min_row_len", C.c_int32), ("max_row_len", C.c_int32),
+                ("mean_row_len", C.c_double), ("var_row_len", C.c_double),
+                ("len_hist", C.c_int64 * 32), ("bandwidth", C.c_int64),
+                ("cols_sorted", C.c_int32), ("block3_full", C.c_int32), ("n_blocks3", C.c_int64),
+                ("sig_row_ptr", C.c_uint64), ("sig_col_idx", C.c_uint64),
+                ("tuned", C.c_int32), ("sm_count", C.c_int32), ("l2_bytes", C.c_int64),
+                ("format_bytes", C.c_int64), ("owned_bytes", C.c_int64),
+                ("variant", C.c_char * 128), ("device_name", C.c_char * 64)]
+
+
+class TuneOpts(C.Structure):
+    _fields_ = [("has_scalars", C.c_int32), ("alpha", C.c_double), ("beta", C.c_double),
+                ("d_x_probe", C.c_void_p), ("d_y0_probe", C.c_void_p),
+                ("d_y_ref", C.c_void_p), ("d_scale", C.c_void_p),
+                ("tolerance", C.c_double), ("warmup", C.c_int32), ("reps", C.c_int32),
+                ("min_batch_ms", C.c_double), ("time_budget_s", C.c_double),
+                ("variant_filter", C.c_char_p), ("n_carveouts", C.c_int32), ("carveouts", C.c_int32 * 8),
+                ("use_cache", C.c_int32), ("cache_path", C.c_char_p), ("fault_inject", C.c_char_p),
+                ("seed", C.c_uint64), ("flush_l2", C.c_int32), ("stream", C.c_void_p)]
+
+
+class TuneReport(C.Structure):
+    _fields_ = [("winner", C.c_char * 128), ("winner_us", C.c_double), ("default_us", C.c_double),
+                ("n_enumerated", C.c_int32), ("n_pruned_structural", C.c_int32),
+                ("n_pruned_slow", C.c_int32), ("n_rejected", C.c_int32), ("n_timed", C.c_int32),
+                ("tune_seconds", C.c_double), ("cache_hit", C.c_int32),
+                ("runner_up", C.c_char * 128), ("runner_up_us", C.c_double),
+                ("log_buf", C.c_void_p), ("log_cap", C.c_size_t), ("log_len", C.c_size_t)]
+
+
+def lib():
+    """Loads libspmv_b200.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1309_1894_b200.build` "
+                           "(there is no CPU or PyTorch fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+    L.spmv_create.argtypes = [C.POINTER(vp), i64, i64, i64, vp, vp, vp, C.POINTER(Allocator), vp]
+    L.spmv_tune.argtypes = [vp, C.POINTER(TuneOpts), C.POINTER(TuneReport)]
+    L.spmv_apply.argtypes = [vp, dbl, vp, dbl, vp, vp]
+    L.spmv_apply_host.argtypes = [vp, dbl, vp, dbl, vp, vp]
+    L.spmv_apply_batch.argtypes = [i32, C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), C.POINTER(dbl),
+                                   C.POINTER(vp), C.POINTER(vp), i32]
+    L.spmv_tune_batch.argtypes = [i32, C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), C.POINTER(dbl),
+                                  C.POINTER(vp), C.POINTER(vp), i32, C.POINTER(i32), C.POINTER(dbl)]
+    L.spmv_select.argtypes = [vp, C.c_char_p, vp]
+    L.spmv_list_variants.argtypes = [vp, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
+    L.spmv_get_info.argtypes = [vp, C.POINTER(Info)]
+    L.spmv_format_download.argtypes = [vp, C.c_char_p, vp, C.c_size_t, C.POINTER(C.c_size_t), vp]
+    L.spmv_destroy.argtypes = [vp]
+    L.spmv_measure_ceiling.argtypes = [i32, C.c_size_t, i32, vp, C.POINTER(dbl)]
+    for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
+              "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
+              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling"):
+        getattr(L, n).restype = C.c_int
+    L.spmv_status_string.argtypes = [C.c_int]
+    L.spmv_status_string.restype = C.c_char_p
+    L.spmv_last_error.restype = C.c_char_p
+    L.spmv_version.restype = C.c_char_p
+    L.spmv_clear_cache.restype = None
+    _lib = L
+    return L
+
+
+def _check(st: int, where: str):
+    if st != SPMV_OK:
+        raise SpmvError(st, where, lib().spmv_last_error().decode(errors="replace"))
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+# torch caching allocator behind the spmv_allocator_t callbacks (device memory plumbing only)
+def _torch_allocator():
+    import torch
+
+    def _alloc(nbytes, stream, ctx):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+        except Exception:
+            return 0
+
+    def _free(ptr, ctx):
+        torch.cuda.caching_allocator_delete(int(ptr))
+
+    a = Allocator(ALLOC_FN(_alloc), FREE_FN(_free), None)
+    return a
+
+
+class SpMV:
+    """Handle wrapper.  row_ptr/col_idx (int32) and val (float64) are CUDA torch tensors that
+    this object keeps alive (the C handle borrows them)."""
+
+    def __init__(self, rows, cols, row_ptr, col_idx, val, *, use_torch_allocator=True, stream=None):
+        import torch
+        assert row_ptr.is_cuda and row_ptr.dtype == torch.int32 and row_ptr.is_contiguous()
+        assert col_idx.dtype == torch.int32 and val.dtype == torch.float64
+        assert col_idx.is_contiguous() and val.is_contiguous()
+        self._keep = (row_ptr, col_idx, val)
+        self._alloc = _torch_allocator() if use_torch_allocator else None
+        self.rows, self.cols, self.nnz = int(rows), int(cols), int(val.numel())
+        h = C.c_void_p(0)
+        st = lib().spmv_create(C.byref(h), self.rows, self.cols, self.nnz, _dptr(row_ptr),
+                               _dptr(col_idx) if self.nnz else C.c_void_p(col_idx.data_ptr() or 0),
+                               _dptr(val) if self.nnz else C.c_void_p(val.data_ptr() or 0),
+                               C.byref(self._alloc) if self._alloc is not None else None, _stream_ptr(stream))
+        _check(st, "spmv_create")
+        self.h = h
+
+    @classmethod
+    def from_csr(cls, A, device="cuda:0", **kw):
+        """A: workloads.CSR (numpy).  Copies the arrays to the device."""
+        import torch
+        rp = torch.from_numpy(np.ascontiguousarray(A.row_ptr, dtype=np.int32)).to(device)
+        ci = torch.from_numpy(np.ascontiguousarray(A.col_idx, dtype=np.int32)).to(device)
+        va = torch.from_numpy(np.ascontiguousarray(A.val, dtype=np.float64)).to(device)
+        return cls(A.rows, A.cols, rp, ci, va, **kw)
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            _check(lib().spmv_destroy(self.h), "spmv_destroy")
+            self.h = C.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> Info:
+        out = Info()
+        _check(lib().spmv_get_info(self.h, C.byref(out)), "spmv_get_info")
+        return out
+
+    @property
+    def variant(self) -> str:
+        return self.info().variant.decode()
+
+    def select(self, desc: str, stream=None):
+        _check(lib().spmv_select(self.h, desc.encode(), _stream_ptr(stream)), f"spmv_select({desc})")
+
+    def variants(self) -> list[str]:
+        n = C.c_size_t(0)
+        _check(lib().spmv_list_variants(self.h, None, 0, C.byref(n)), "spmv_list_variants")
+        buf = C.create_string_buffer(n.value + 1)
+        _check(lib().spmv_list_variants(self.h, buf, n.value + 1, C.byref(n)), "spmv_list_variants")
+        return [l for l in buf.value.decode().split("\n") if l]
+
+    def apply(self, alpha, x, beta, y, stream=None):
+        """y = alpha*A*x + beta*y on the device, asynchronous on the (current) stream."""
+        assert x.is_cuda and y.is_cuda and x.numel() == self.cols and y.numel() == self.rows
+        _check(lib().spmv_apply(self.h, float(alpha), _dptr(x), float(beta), _dptr(y), _stream_ptr(stream)),
+               "spmv_apply")
+        return y
+
+    def apply_host(self, alpha, x_host, beta, y_host, stream=None):
+        """Host-buffer form: x_host/y_host are CPU tensors or numpy arrays (pinned is faster)."""
+        xp = x_host.data_ptr() if hasattr(x_host, "data_ptr") else x_host.ctypes.data
+        yp = y_host.data_ptr() if hasattr(y_host, "data_ptr") else y_host.ctypes.data
+        _check(lib().spmv_apply_host(self.h, float(alpha), C.c_void_p(xp), float(beta), C.c_void_p(yp),
+                                     _stream_ptr(stream)), "spmv_apply_host")
+        return y_host
+
+    def tune(self, *, alpha=1.0, beta=0.0, x=None, y0=None, y_ref=None, scale=None, tolerance=0.0,
+             warmup=0, reps=0, min_batch_ms=0.0, time_budget_s=0.0, variant_filter=None,
+             carveouts=None, use_cache=0, cache_path=None, fault_inject=None, seed=0, flush_l2=False,
+             stream=None, log_bytes=1 << 20) -> dict:
+        o = TuneOpts()
+        o.has_scalars, o.alpha, o.beta = 1, float(alpha), float(beta)
+        o.d_x_probe, o.d_y0_probe = _dptr(x), _dptr(y0)
+        o.d_y_ref, o.d_scale = _dptr(y_ref), _dptr(scale)
+        o.tolerance, o.warmup, o.reps = float(tolerance), int(warmup), int(reps)
+        o.min_batch_ms, o.time_budget_s = float(min_batch_ms), float(time_budget_s)
+        o.variant_filter = variant_filter.encode() if variant_filter else None
+        if carveouts:
+            o.n_carveouts = len(carveouts)
+            for i, c in enumerate(carveouts[:8]):
+                o.carveouts[i] = int(c)
+        o.use_cache = int(use_cache)
+        o.cache_path = cache_path.encode() if cache_path else None
+        o.fault_inject = fault_inject.encode() if fault_inject else None
+        o.seed, o.flush_l2, o.stream = int(seed), int(bool(flush_l2)), _stream_ptr(stream)
+        rep = TuneReport()
+        logbuf = C.create_string_buffer(log_bytes) if log_bytes else None
+        if logbuf is not None:
+            rep.log_buf, rep.log_cap = C.cast(logbuf, C.c_void_p), log_bytes
+        st = lib().spmv_tune(self.h, C.byref(o), C.byref(rep))
+        log = logbuf.value.decode() if logbuf is not None else ""
+        out = {"status": st, "winner": rep.winner.decode(), "winner_us": rep.winner_us,
+               "default_us": rep.default_us, "n_enumerated": rep.n_enumerated,
+               "n_pruned_structural": rep.n_pruned_structural, "n_pruned_slow": rep.n_pruned_slow,
+               "n_rejected": rep.n_rejected, "n_timed": rep.n_timed, "tune_seconds": rep.tune_seconds,
+               "cache_hit": bool(rep.cache_hit), "runner_up": rep.runner_up.decode(),
+               "runner_up_us": rep.runner_up_us,
+               "log": [l.split() for l in log.split("\n") if l]}
+        if st != SPMV_OK:
+            err = SpmvError(st, "spmv_tune", lib().spmv_last_error().decode(errors="replace"))
+            err.report = out
+            raise err
+        return out
+
+    def download(self, name: str, dtype) -> np.ndarray:
+        n = C.c_size_t(0)
+        _check(lib().spmv_format_download(self.h, name.encode(), None, 0, C.byref(n), _stream_ptr()),
+               f"spmv_format_download({name})")
+        out = np.empty(n.value // np.dtype(dtype).itemsize, dtype=dtype)
+        if n.value:
+            _check(lib().spmv_format_download(self.h, name.encode(), C.c_void_p(out.ctypes.data), n.value,
+                                              C.byref(n), _stream_ptr()), f"spmv_format_download({name})")
+        return out
+
+
+def apply_batch(handles, alphas, xs, betas, ys, streams):
+    """spmv_apply_batch: handle i on streams[i % len(streams)]; no synchronisation."""
+    n = len(handles)
+    vp, dbl = C.c_void_p, C.c_double
+    hs = (vp * n)(*[h.h for h in handles])
+    al = (dbl * n)(*[float(a) for a in alphas])
+    be = (dbl * n)(*[float(b) for b in betas])
+    dx = (vp * n)(*[x.data_ptr() for x in xs])
+    dy = (vp * n)(*[y.data_ptr() for y in ys])
+    ss = (vp * len(streams))(*[s.cuda_stream for s in streams])
+    _check(lib().spmv_apply_batch(n, hs, al, dx, be, dy, ss, len(streams)), "spmv_apply_batch")
+
+
+def tune_batch(handles, alphas, xs, betas, ys, streams):
+    """spmv_tune_batch: returns (best stream count, {count: microseconds per batch})."""
+    n = len(handles)
+    vp, dbl = C.c_void_p, C.c_double
+    hs = (vp * n)(*[h.h for h in handles])
+    al = (dbl * n)(*[float(a) for a in alphas])
+    be = (dbl * n)(*[float(b) for b in betas])
+    dx = (vp * n)(*[x.data_ptr() for x in xs])
+    dy = (vp * n)(*[y.data_ptr() for y in ys])
+    ss = (vp * len(streams))(*[s.cuda_stream for s in streams])
+    best = C.c_int32(0)
+    us = (dbl * 8)()
+    _check(lib().spmv_tune_batch(n, hs, al, dx, be, dy, ss, len(streams), C.byref(best), us), "spmv_tune_batch")
+    counts, c, i = {}, 1, 0
+    while c <= len(streams):
+        counts[c] = us[i]
+        c *= 2
+        i += 1
+    return best.value, counts
+
+
+def measure_ceiling(kind: int, nbytes: int = 1 << 30, reps: int = 10) -> float:
+    out = C.c_double(0.0)
+    _check(lib().spmv_measure_ceiling(kind, nbytes, reps, _stream_ptr(), C.byref(out)), "spmv_measure_ceiling")
+    return out.value
+
+
+def clear_cache():
+    lib().spmv_clear_cache()
+
+
+def version() -> str:
+    return lib().spmv_version().decode()

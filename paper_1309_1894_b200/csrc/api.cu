@@ -1,0 +1,248 @@
+// C ABI entry points (include/spmv_b200.h) except spmv_tune / spmv_tune_batch (tuner.cu)
+// and spmv_measure_ceiling (verify.cu).
+#include <math.h>
+#include <string.h>
+
+#include <mutex>
+#include <set>
+
+#include "handle.h"
+
+namespace spmv {
+const char* last_error_text();
+
+static std::mutex g_live_mu;
+static std::set<void*> g_live;
+
+bool handle_alive(spmv_handle_t h) {
+  if (!h) return false;
+  std::lock_guard<std::mutex> lk(g_live_mu);
+  return g_live.count((void*)h) && h->magic == kHandleMagic;
+}
+
+static void refresh_info(spmv_handle_s* h) {
+  h->info.tuned = h->tuned ? 1 : 0;
+  h->info.format_bytes = variant_format_bytes(h, h->sel);
+  h->info.owned_bytes = h->al.owned;
+  std::string d = variant_to_string(h->sel);
+  strncpy(h->info.variant, d.c_str(), sizeof(h->info.variant) - 1);
+}
+void handle_refresh_info(spmv_handle_s* h) { refresh_info(h); }
+
+}  // namespace spmv
+
+using namespace spmv;
+
+extern "C" {
+
+const char* spmv_status_string(spmv_status_t s) {
+  switch (s) {
+    case SPMV_OK: return "SPMV_OK";
+    case SPMV_ERR_INVALID_ARG: return "SPMV_ERR_INVALID_ARG";
+    case SPMV_ERR_INVALID_MATRIX: return "SPMV_ERR_INVALID_MATRIX";
+    case SPMV_ERR_UNSUPPORTED: return "SPMV_ERR_UNSUPPORTED";
+    case SPMV_ERR_ALLOC: return "SPMV_ERR_ALLOC";
+    case SPMV_ERR_CUDA: return "SPMV_ERR_CUDA";
+    case SPMV_ERR_VERIFY_FAILED: return "SPMV_ERR_VERIFY_FAILED";
+    case SPMV_ERR_INTERNAL: return "SPMV_ERR_INTERNAL";
+  }
+  return "SPMV_ERR_UNKNOWN";
+}
+const char* spmv_last_error(void) { return last_error_text(); }
+const char* spmv_version(void) { return kVersion; }
+
+spmv_status_t spmv_create(spmv_handle_t* out, int64_t rows, int64_t cols, int64_t nnz, const int32_t* d_row_ptr,
+                          const int32_t* d_col_idx, const double* d_val, const spmv_allocator_t* alloc,
+                          void* stream) {
+  if (!out || rows < 0 || cols < 0 || nnz < 0 || !d_row_ptr) return SPMV_ERR_INVALID_ARG;
+  if (nnz > 0 && (!d_col_idx || !d_val)) return SPMV_ERR_INVALID_ARG;
+  if (alloc && (!alloc->alloc || !alloc->free)) return SPMV_ERR_INVALID_ARG;
+  if (rows > 0x7fffffffll || cols > 0x7fffffffll || nnz > 0x7fffffffll) return SPMV_ERR_UNSUPPORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  int dev = 0;
+  SPMV_CUDA_TRY(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  SPMV_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+
+  spmv_handle_s* h = new (std::nothrow) spmv_handle_s();
+  if (!h) return SPMV_ERR_ALLOC;
+  h->magic = kHandleMagic;
+  h->device = dev;
+  h->A.rows = rows; h->A.cols = cols; h->A.nnz = nnz;
+  h->A.row_ptr = d_row_ptr; h->A.col_idx = d_col_idx; h->A.val = d_val;
+  if (alloc) { h->al.cb = *alloc; h->al.has_cb = true; }
+  h->dev.sm_count = prop.multiProcessorCount;
+  h->dev.l2_bytes = prop.l2CacheSize;
+  strncpy(h->dev.name, prop.name, sizeof(h->dev.name) - 1);
+
+  RawStats rs;
+  cudaError_t e = compute_stats(h->A, &rs, s);
+  if (e != cudaSuccess) {
+    set_last_error("spmv_create: statistics pass failed: %s", cudaGetErrorString(e));
+    delete h;
+    return SPMV_ERR_CUDA;
+  }
+  if (rs.bad_row_ptr || rs.bad_col) {
+    set_last_error("spmv_create: invalid CSR (%llu bad row_ptr entries, %llu columns out of range)",
+                   rs.bad_row_ptr, rs.bad_col);
+    delete h;
+    return SPMV_ERR_INVALID_MATRIX;
+  }
+  spmv_info_t& in = h->info;
+  in.rows = rows; in.cols = cols; in.nnz = nnz;
+  in.min_row_len = rows ? rs.min_len : 0;
+  in.max_row_len = rs.max_len;
+  in.mean_row_len = rows ? (double)rs.sum_len / (double)rows : 0.0;
+  in.var_row_len = rows ? (double)rs.sum_len_sq / (double)rows - in.mean_row_len * in.mean_row_len : 0.0;
+  if (in.var_row_len < 0) in.var_row_len = 0;
+  for (int b = 0; b < 32; ++b) in.len_hist[b] = (int64_t)rs.hist[b];
+  in.bandwidth = rs.bandwidth;
+  in.cols_sorted = rs.unsorted_rows == 0;
+  in.block3_full = (rs.block3_bad == 0 && rows > 0 && rows % 3 == 0 && cols % 3 == 0) ? 1 : 0;
+  in.n_blocks3 = in.block3_full ? (int64_t)rs.n_blocks3 : 0;
+  in.sig_row_ptr = rs.sig_row_ptr;
+  in.sig_col_idx = rs.sig_col_idx;
+  in.sm_count = h->dev.sm_count;
+  in.l2_bytes = h->dev.l2_bytes;
+  strncpy(in.device_name, h->dev.name, sizeof(in.device_name) - 1);
+  h->sel = default_variant();
+  refresh_info(h);
+  {
+    std::lock_guard<std::mutex> lk(g_live_mu);
+    g_live.insert((void*)h);
+  }
+  *out = h;
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_destroy(spmv_handle_t h) {
+  if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
+  {
+    std::lock_guard<std::mutex> lk(g_live_mu);
+    g_live.erase((void*)h);
+  }
+  release_all_formats(h);
+  if (h->d_x_stage) h->al.free(h->d_x_stage, sizeof(double) * h->A.cols);
+  if (h->d_y_stage) h->al.free(h->d_y_stage, sizeof(double) * h->A.rows);
+  h->magic = 0;
+  delete h;
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_get_info(spmv_handle_t h, spmv_info_t* out) {
+  if (!handle_alive(h) || !out) return SPMV_ERR_INVALID_ARG;
+  refresh_info(h);
+  *out = h->info;
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_select(spmv_handle_t h, const char* desc, void* stream) {
+  if (!handle_alive(h) || !desc) return SPMV_ERR_INVALID_ARG;
+  Variant v;
+  if (!variant_from_string(desc, &v)) { set_last_error("cannot parse variant '%s'", desc); return SPMV_ERR_INVALID_ARG; }
+  std::string why;
+  if (!variant_eligible(h, v, &why)) { set_last_error("variant %s not eligible: %s", desc, why.c_str()); return SPMV_ERR_UNSUPPORTED; }
+  spmv_status_t st = ensure_format(h, v, (cudaStream_t)stream);
+  if (st != SPMV_OK) return st;
+  h->sel = v;
+  release_formats_except(h, v);
+  refresh_info(h);
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y, void* stream) {
+  if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
+  if (h->A.rows > 0 && !d_y) return SPMV_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (alpha == 0.0 || h->A.rows == 0) {           // reading A2: A and x are not referenced
+    cudaError_t e = scale_y_launch(h->A.rows, beta, d_y, s);
+    if (e != cudaSuccess) { set_last_error("scale kernel: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+    return SPMV_OK;
+  }
+  if (h->A.cols > 0 && !d_x) return SPMV_ERR_INVALID_ARG;
+  ApplyArgs a{alpha, beta, d_x, d_y, s};
+  return launch_variant(h, h->sel, a);
+}
+
+spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
+                              void* stream) {
+  if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
+  if ((h->A.rows > 0 && !h_y) || (h->A.cols > 0 && !h_x)) return SPMV_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (!h->d_x_stage) h->d_x_stage = (double*)h->al.alloc(sizeof(double) * h->A.cols, s);
+  if (!h->d_y_stage) h->d_y_stage = (double*)h->al.alloc(sizeof(double) * h->A.rows, s);
+  if (!h->d_x_stage || !h->d_y_stage) return SPMV_ERR_ALLOC;
+  if (h->A.cols) SPMV_CUDA_TRY(cudaMemcpyAsync(h->d_x_stage, h_x, sizeof(double) * h->A.cols, cudaMemcpyHostToDevice, s));
+  if (beta != 0.0 && h->A.rows)
+    SPMV_CUDA_TRY(cudaMemcpyAsync(h->d_y_stage, h_y, sizeof(double) * h->A.rows, cudaMemcpyHostToDevice, s));
+  spmv_status_t st = spmv_apply(h, alpha, h->d_x_stage, beta, h->d_y_stage, stream);
+  if (st != SPMV_OK) return st;
+  if (h->A.rows) SPMV_CUDA_TRY(cudaMemcpyAsync(h_y, h->d_y_stage, sizeof(double) * h->A.rows, cudaMemcpyDeviceToHost, s));
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_apply_batch(int32_t n, const spmv_handle_t* hs, const double* alphas, const double* const* d_xs,
+                               const double* betas, double* const* d_ys, void* const* streams, int32_t nstreams) {
+  if (n < 0 || (n > 0 && (!hs || !alphas || !d_xs || !betas || !d_ys))) return SPMV_ERR_INVALID_ARG;
+  if (nstreams < 0 || (nstreams > 0 && !streams)) return SPMV_ERR_INVALID_ARG;
+  for (int i = 0; i < n; ++i) {
+    void* s = nstreams > 0 ? streams[i % nstreams] : nullptr;
+    spmv_status_t st = spmv_apply(hs[i], alphas[i], d_xs[i], betas[i], d_ys[i], s);
+    if (st != SPMV_OK) return st;
+  }
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap, size_t* len) {
+  if (!handle_alive(h) || !len) return SPMV_ERR_INVALID_ARG;
+  int pruned = 0;
+  std::vector<Variant> c = enumerate_candidates(h, nullptr, &pruned);
+  std::string all;
+  for (const auto& v : c) { all += variant_to_string(v); all += '\n'; }
+  *len = all.size() + 1;
+  if (buf && cap > 0) {
+    size_t n = all.size() < cap - 1 ? all.size() : cap - 1;
+    memcpy(buf, all.data(), n);
+    buf[n] = 0;
+  }
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_buf, size_t cap, size_t* bytes,
+                                   void* stream) {
+  if (!handle_alive(h) || !name || !bytes) return SPMV_ERR_INVALID_ARG;
+  const Variant& v = h->sel;
+  const void* src = nullptr;
+  size_t n = 0;
+  const SellFormat* sf = nullptr;
+  if (v.fam == FAM_SELL) {
+    auto it = h->sells.find(std::make_pair(v.C, v.S));
+    if (it != h->sells.end()) sf = &it->second;
+  } else if (v.fam == FAM_ELL && h->has_ell) {
+    sf = &h->ell;
+  }
+  if (sf) {
+    if (!strcmp(name, "slice_ptr")) { src = sf->slice_ptr; n = sizeof(int64_t) * (sf->nslices + 1); }
+    else if (!strcmp(name, "sval")) { src = sf->val; n = sizeof(double) * sf->padded; }
+    else if (!strcmp(name, "scol")) { src = sf->col; n = sizeof(int32_t) * sf->padded; }
+    else if (!strcmp(name, "perm") && sf->perm) { src = sf->perm; n = sizeof(int32_t) * sf->nslices * sf->C; }
+  } else if (v.fam == FAM_BCSR3 && h->has_bcsr) {
+    if (!strcmp(name, "brow_ptr")) { src = h->bcsr.brow_ptr; n = sizeof(int32_t) * (h->bcsr.brows + 1); }
+    else if (!strcmp(name, "bcol")) { src = h->bcsr.bcol; n = sizeof(int32_t) * h->bcsr.nblocks; }
+    else if (!strcmp(name, "bval")) { src = h->bcsr.bval; n = sizeof(double) * 9 * h->bcsr.nblocks; }
+  } else if (v.fam == FAM_MERGE) {
+    auto it = h->plans.find(v.block * v.I);
+    if (it != h->plans.end() && !strcmp(name, "tile_row")) { src = it->second.tile_row; n = sizeof(int32_t) * (it->second.ntiles + 1); }
+  }
+  if (!src) { set_last_error("no array '%s' in the selected format", name); return SPMV_ERR_INVALID_ARG; }
+  *bytes = n;
+  if (h_buf && cap > 0) {
+    cudaStream_t s = (cudaStream_t)stream;
+    SPMV_CUDA_TRY(cudaMemcpyAsync(h_buf, src, n < cap ? n : cap, cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  }
+  return SPMV_OK;
+}
+
+}  // extern "C"

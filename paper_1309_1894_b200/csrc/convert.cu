@@ -1,0 +1,271 @@
+// On-device format converters (north_star (b)):
+// CSR -> SELL-C-sigma, CSR -> ELL (one-slice SELL), CSR -> 3x3 BCSR.
+// Integer work and copies only; hand-written sort (bitonic per sigma-window) and scan.
+#include <algorithm>
+
+#include "spmv_internal.h"
+
+namespace spmv {
+
+// ------------------------------------------------------------------ single-block inclusive scan
+// In place over a[1..n]; a[0] must already hold 0.  Off the apply path.
+template <typename T>
+__global__ void scan_inclusive_kernel(T* __restrict__ a, int64_t n) {
+  __shared__ T s_w[32];
+  __shared__ T s_carry;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  for (int64_t base = 1; base <= n; base += blockDim.x) {
+    const int64_t i = base + tid;
+    T v = i <= n ? a[i] : 0;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      T u = __shfl_up_sync(0xffffffffu, v, d);
+      if (lane >= d) v += u;
+    }
+    if (lane == 31) s_w[w] = v;
+    __syncthreads();
+    if (w == 0) {
+      T x = lane < (blockDim.x >> 5) ? s_w[lane] : 0;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        T u = __shfl_up_sync(0xffffffffu, x, d);
+        if (lane >= d) x += u;
+      }
+      s_w[lane] = x;
+    }
+    __syncthreads();
+    const T carry = s_carry;
+    v += carry + (w > 0 ? s_w[w - 1] : 0);
+    if (i <= n) a[i] = v;
+    __syncthreads();
+    if (tid == blockDim.x - 1) s_carry = v;
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------ SELL-C-sigma
+// perm[p] = original row stored at SELL position p (or -1).  Within each window of sigma
+// positions, rows are ordered by descending length, ties by ascending row (stable).
+__global__ void sell_sort_kernel(int64_t rows, int64_t rows_padded, int sigma, const int* __restrict__ rp,
+                                 int* __restrict__ perm) {
+  extern __shared__ unsigned long long s_key[];
+  const int64_t w0 = (int64_t)blockIdx.x * sigma;
+  for (int j = threadIdx.x; j < sigma; j += blockDim.x) {
+    const int64_t r = w0 + j;
+    unsigned long long key = ~0ull;
+    if (r < rows) {
+      const unsigned len = (unsigned)(rp[r + 1] - rp[r]);
+      key = ((unsigned long long)(0x7fffffffu - len) << 32) | (unsigned)j;
+    }
+    s_key[j] = key;
+  }
+  __syncthreads();
+  for (int k = 2; k <= sigma; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = threadIdx.x; i < sigma; i += blockDim.x) {
+        const int p = i ^ j;
+        if (p > i) {
+          const unsigned long long a = s_key[i], b = s_key[p];
+          const bool up = (i & k) == 0;
+          if ((a > b) == up) { s_key[i] = b; s_key[p] = a; }
+        }
+      }
+      __syncthreads();
+    }
+  }
+  for (int j = threadIdx.x; j < sigma; j += blockDim.x) {
+    const int64_t p = w0 + j;
+    if (p < rows_padded) {
+      const unsigned long long key = s_key[j];
+      perm[p] = key == ~0ull ? -1 : (int)(w0 + (key & 0xffffffffu));
+    }
+  }
+}
+
+// slice_ptr[s+1] = C * max row length in slice s (scanned afterwards)
+__global__ void sell_width_kernel(int64_t rows, int64_t nslices, int C, const int* __restrict__ rp,
+                                  const int* __restrict__ perm, int64_t* __restrict__ slice_ptr) {
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (warp >= nslices) return;
+  int mx = 0;
+  for (int j = lane; j < C; j += 32) {
+    const int64_t p = warp * C + j;
+    const int64_t r = perm ? perm[p] : (p < rows ? p : -1);
+    if (r >= 0) mx = max(mx, rp[r + 1] - rp[r]);
+  }
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+  if (lane == 0) {
+    slice_ptr[warp + 1] = (int64_t)mx * C;
+    if (warp == 0) slice_ptr[0] = 0;
+  }
+}
+
+__global__ void sell_fill_kernel(int64_t rows, int64_t rows_padded, int C, int logC, const int* __restrict__ rp,
+                                 const int* __restrict__ ci, const double* __restrict__ va,
+                                 const int* __restrict__ perm, const int64_t* __restrict__ slice_ptr,
+                                 double* __restrict__ sval, int* __restrict__ scol) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= rows_padded) return;
+  const int64_t s = logC >= 0 ? (p >> logC) : 0;
+  const int off = (int)(p - s * C);
+  const int64_t base = slice_ptr[s];
+  const int w = (int)((slice_ptr[s + 1] - base) / C);
+  const int64_t r = perm ? perm[p] : (p < rows ? p : -1);
+  const int a = r >= 0 ? rp[r] : 0;
+  const int len = r >= 0 ? rp[r + 1] - a : 0;
+  for (int j = 0; j < w; ++j) {
+    const int64_t q = base + (int64_t)j * C + off;
+    if (j < len) {
+      sval[q] = va[a + j];
+      scol[q] = ci[a + j];
+    } else {
+      sval[q] = 0.0;
+      scol[q] = -1;       // padding marker: skipped by the kernel, never multiplied (A7)
+    }
+  }
+}
+
+void free_sell(SellFormat& f, Allocator& al) {
+  if (f.slice_ptr) al.free(f.slice_ptr, sizeof(int64_t) * (f.nslices + 1));
+  if (f.val) al.free(f.val, sizeof(double) * f.padded);
+  if (f.col) al.free(f.col, sizeof(int32_t) * f.padded);
+  if (f.perm) al.free(f.perm, sizeof(int32_t) * f.nslices * f.C);
+  f = SellFormat();
+}
+
+spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, Allocator& al, cudaStream_t s,
+                         SellFormat* out) {
+  SellFormat f;
+  f.is_ell = ell;
+  if (ell) {
+    int64_t padded_rows = ((A.rows + 127) / 128) * 128;
+    if (padded_rows == 0) padded_rows = 128;
+    if (padded_rows > 0x7fffff80) return SPMV_ERR_UNSUPPORTED;
+    f.C = (int)padded_rows;
+    f.logC = -1;
+    f.sigma = 1;
+    f.nslices = 1;
+  } else {
+    f.C = C;
+    f.logC = 0;
+    while ((1 << f.logC) < C) ++f.logC;
+    f.sigma = sigma;
+    f.nslices = (A.rows + C - 1) / C;
+    if (f.nslices == 0) f.nslices = 1;
+  }
+  const int64_t rows_padded = f.nslices * f.C;
+  f.slice_ptr = (int64_t*)al.alloc(sizeof(int64_t) * (f.nslices + 1), s);
+  if (!f.slice_ptr) return SPMV_ERR_ALLOC;
+  if (f.sigma > 1) {
+    f.perm = (int32_t*)al.alloc(sizeof(int32_t) * rows_padded, s);
+    if (!f.perm) { free_sell(f, al); return SPMV_ERR_ALLOC; }
+    const int64_t nwin = (rows_padded + f.sigma - 1) / f.sigma;
+    const size_t smem = sizeof(unsigned long long) * f.sigma;
+    if (smem > 48 * 1024)
+      SPMV_CUDA_TRY(cudaFuncSetAttribute((const void*)sell_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sell_sort_kernel<<<(unsigned)nwin, std::min(1024, std::max(32, f.sigma / 2)), smem, s>>>(A.rows, rows_padded, f.sigma,
+                                                                                          A.row_ptr, f.perm);
+    SPMV_CUDA_TRY(cudaGetLastError());
+  }
+  sell_width_kernel<<<(unsigned)((f.nslices * 32 + 255) / 256), 256, 0, s>>>(A.rows, f.nslices, f.C, A.row_ptr, f.perm,
+                                                                         f.slice_ptr);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  scan_inclusive_kernel<int64_t><<<1, 1024, 0, s>>>(f.slice_ptr, f.nslices);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  int64_t total = 0;
+  SPMV_CUDA_TRY(cudaMemcpyAsync(&total, f.slice_ptr + f.nslices, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  f.padded = total;
+  const int64_t n_alloc = total > 0 ? total : 2;
+  f.val = (double*)al.alloc(sizeof(double) * n_alloc, s);
+  f.col = (int32_t*)al.alloc(sizeof(int32_t) * n_alloc, s);
+  if (!f.val || !f.col) { f.padded = n_alloc; free_sell(f, al); return SPMV_ERR_ALLOC; }
+  f.padded = n_alloc;
+  if (total > 0) {
+    sell_fill_kernel<<<(unsigned)((rows_padded + 127) / 128), 128, 0, s>>>(A.rows, rows_padded, f.C, f.logC, A.row_ptr,
+                                                                        A.col_idx, A.val, f.perm, f.slice_ptr, f.val,
+                                                                        f.col);
+    SPMV_CUDA_TRY(cudaGetLastError());
+  }
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  *out = f;
+  return SPMV_OK;
+}
+
+// ------------------------------------------------------------------ 3x3 BCSR
+// Three-way merge over the block columns (col/3) of the three rows of a block row.
+// FILL = false: count unique block columns; FILL = true: write bcol and scatter values.
+template <bool FILL>
+__global__ void bcsr3_merge_kernel(int64_t brows, const int* __restrict__ rp, const int* __restrict__ ci,
+                                   const double* __restrict__ va, int* __restrict__ brow_ptr,
+                                   int* __restrict__ bcol, double* __restrict__ bval) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= brows) return;
+  int p[3], e[3];
+#pragma unroll
+  for (int r = 0; r < 3; ++r) { p[r] = rp[3 * b + r]; e[r] = rp[3 * b + r + 1]; }
+  const int start = FILL ? brow_ptr[b] : 0;
+  const int nb = FILL ? brow_ptr[b + 1] - start : 0;
+  int count = 0;
+  while (true) {
+    int bc = 0x7fffffff;
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+      if (p[r] < e[r]) bc = min(bc, ci[p[r]] / 3);
+    if (bc == 0x7fffffff) break;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+      while (p[r] < e[r] && ci[p[r]] / 3 == bc) {
+        if (FILL) bval[9 * (int64_t)start + (int64_t)(3 * r + ci[p[r]] % 3) * nb + count] = va[p[r]];
+        ++p[r];
+      }
+    }
+    if (FILL) bcol[start + count] = bc;
+    ++count;
+  }
+  if (!FILL) {
+    brow_ptr[b + 1] = count;
+    if (b == 0) brow_ptr[0] = 0;
+  }
+}
+
+void free_bcsr3(BcsrFormat& f, Allocator& al) {
+  if (f.brow_ptr) al.free(f.brow_ptr, sizeof(int32_t) * (f.brows + 1));
+  if (f.bcol) al.free(f.bcol, sizeof(int32_t) * std::max<int64_t>(f.nblocks, 1));
+  if (f.bval) al.free(f.bval, sizeof(double) * 9 * std::max<int64_t>(f.nblocks, 1));
+  f = BcsrFormat();
+}
+
+spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out) {
+  if (A.rows % 3 || A.cols % 3 || A.rows == 0) return SPMV_ERR_UNSUPPORTED;
+  BcsrFormat f;
+  f.brows = A.rows / 3;
+  f.brow_ptr = (int32_t*)al.alloc(sizeof(int32_t) * (f.brows + 1), s);
+  if (!f.brow_ptr) return SPMV_ERR_ALLOC;
+  const unsigned grid = (unsigned)((f.brows + 127) / 128);
+  bcsr3_merge_kernel<false><<<grid, 128, 0, s>>>(f.brows, A.row_ptr, A.col_idx, A.val, f.brow_ptr, nullptr, nullptr);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(f.brow_ptr, f.brows);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  int total = 0;
+  SPMV_CUDA_TRY(cudaMemcpyAsync(&total, f.brow_ptr + f.brows, sizeof(int), cudaMemcpyDeviceToHost, s));
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  f.nblocks = total;
+  const int64_t n_alloc = std::max<int64_t>(f.nblocks, 1);
+  f.bcol = (int32_t*)al.alloc(sizeof(int32_t) * n_alloc, s);
+  f.bval = (double*)al.alloc(sizeof(double) * 9 * n_alloc, s);
+  if (!f.bcol || !f.bval) { free_bcsr3(f, al); return SPMV_ERR_ALLOC; }
+  SPMV_CUDA_TRY(cudaMemsetAsync(f.bval, 0, sizeof(double) * 9 * n_alloc, s));
+  bcsr3_merge_kernel<true><<<grid, 128, 0, s>>>(f.brows, A.row_ptr, A.col_idx, A.val, f.brow_ptr, f.bcol, f.bval);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  f.fill = f.nblocks ? (double)A.nnz / (9.0 * (double)f.nblocks) : 1.0;
+  *out = f;
+  return SPMV_OK;
+}
+
+}  // namespace spmv

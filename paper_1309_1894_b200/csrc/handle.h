@@ -1,0 +1,55 @@
+// The handle behind spmv_handle_t and the helpers api.cu / tuner.cu share.
+#pragma once
+#include <map>
+#include <string>
+#include <utility>
+
+#include "spmv_internal.h"
+
+struct spmv_handle_s {
+  uint64_t magic = 0;
+  spmv::CsrView A;
+  spmv::Allocator al;
+  spmv::DeviceProps dev;
+  int device = 0;
+  spmv_info_t info{};
+  spmv::Variant sel;
+  bool tuned = false;
+
+  // owned formats, built on demand
+  std::map<std::pair<int, int>, spmv::SellFormat> sells;   // key (C, sigma)
+  spmv::SellFormat ell;
+  bool has_ell = false;
+  spmv::BcsrFormat bcsr;
+  bool has_bcsr = false;
+  std::map<int, spmv::MergePlan> plans;                    // key tile_items
+
+  // staging for spmv_apply_host
+  double* d_x_stage = nullptr;
+  double* d_y_stage = nullptr;
+};
+
+namespace spmv {
+
+constexpr uint64_t kHandleMagic = 0x53504D5642323030ull;   // "SPMVB200"
+constexpr const char* kVersion = "0.1.0";
+
+bool handle_alive(spmv_handle_t h);
+
+// Structural eligibility of a variant for this matrix (SURVEY.md sec. 8(d) "pruning").
+bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why);
+// Builds (or finds) the format the variant needs.  UNSUPPORTED if the built format turns
+// out too padded to be worth keeping.
+spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s);
+// Launches the variant (format must exist).  Resolves grid size and carve-out.
+spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs& a);
+// Bytes of matrix data the variant streams per apply (format-actual, not algorithmic).
+int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v);
+// Frees every owned format the given variant does not need.
+void release_formats_except(spmv_handle_s* h, const Variant& keep);
+void release_all_formats(spmv_handle_s* h);
+// Candidate list of the tuner's first phase for this matrix.
+std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* filter, int* n_pruned_structural);
+std::string signature_key(const spmv_handle_s* h, bool beta_nonzero);
+
+}  // namespace spmv

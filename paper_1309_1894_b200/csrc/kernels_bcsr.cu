@@ -1,0 +1,94 @@
+// 3x3 BCSR kernel (north_star (c) "3x3 BCSR").
+//
+// T lanes share a block row; lane l takes blocks l, l+T, ...  The values of a block row
+// are stored TRANSPOSED inside the block row (element k of block j at 9*start + k*nb + j),
+// a library-owned layout, so that each of the 9 value loads is contiguous across lanes
+// instead of striding by 72 bytes.  One int32 block column per 9 values: 8.44 B/nnz
+// instead of CSR's 12.  x is read as the 3-vector x[3*bc .. 3*bc+2].
+#include "device_utils.cuh"
+#include "spmv_internal.h"
+
+namespace spmv {
+
+template <int T, int U, int X>
+__global__ void __launch_bounds__(1024)
+bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol,
+             const double* __restrict__ bval, double alpha, const double* __restrict__ x,
+             double beta, double* __restrict__ y) {
+  const int lane = threadIdx.x & (T - 1);
+  const int sub_in_warp = (threadIdx.x & 31) / T;
+  const int64_t nsub = ((int64_t)gridDim.x * blockDim.x) / T;
+  const int64_t warp_first = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / T - sub_in_warp;
+  for (int64_t base = warp_first; base < brows; base += nsub) {
+    const int64_t br = base + sub_in_warp;
+    const bool ok = br < brows;
+    const int start = ok ? __ldg(bp + br) : 0;
+    const int nb = ok ? __ldg(bp + br + 1) - start : 0;
+    const double* pv = bval + 9 * (int64_t)start;
+    const int* pc = bcol + start;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int j = lane; j < nb; j += T * U) {
+      double v[U][9];
+      int c[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int jj = j + u * T;
+        const bool in = jj < nb;
+        c[u] = in ? ld_stream(pc + jj) : -1;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) v[u][k] = in ? ld_stream(pv + (int64_t)k * nb + jj) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        if (c[u] >= 0) {
+          const double* px = x + 3 * (int64_t)c[u];
+          const double x0 = ldx<X>(px, 0), x1 = ldx<X>(px, 1), x2 = ldx<X>(px, 2);
+          s0 = fma(v[u][0], x0, fma(v[u][1], x1, fma(v[u][2], x2, s0)));
+          s1 = fma(v[u][3], x0, fma(v[u][4], x1, fma(v[u][5], x2, s1)));
+          s2 = fma(v[u][6], x0, fma(v[u][7], x1, fma(v[u][8], x2, s2)));
+        }
+      }
+    }
+    s0 = butterfly_sum<T>(s0);
+    s1 = butterfly_sum<T>(s1);
+    s2 = butterfly_sum<T>(s2);
+    if (ok && lane == 0) {
+      store_y(y, 3 * br + 0, alpha, s0, beta);
+      store_y(y, 3 * br + 1, alpha, s1, beta);
+      store_y(y, 3 * br + 2, alpha, s2, beta);
+    }
+  }
+}
+
+typedef void (*bcsr_kernel_t)(int, const int*, const int*, const double*, double, const double*, double,
+                              double*);
+
+template <int X>
+static bcsr_kernel_t pick_tu(int T, int U) {
+#define P(t, u) if (T == t && U == u) return bcsr3_kernel<t, u, X>;
+  P(4, 1) P(4, 2) P(8, 1) P(8, 2) P(16, 1) P(16, 2) P(32, 1) P(32, 2)
+#undef P
+  return nullptr;
+}
+static bcsr_kernel_t pick(const Variant& v) {
+  return v.X == 0 ? pick_tu<0>(v.W, v.U) : v.X == 1 ? pick_tu<1>(v.W, v.U) : nullptr;
+}
+
+bool bcsr_supported(const Variant& v) {
+  return v.block >= 32 && v.block <= 1024 && v.block % 32 == 0 && pick(v) != nullptr;
+}
+const void* bcsr_func(const Variant& v) { return (const void*)pick(v); }
+
+cudaError_t bcsr_launch(const Variant& v, const BcsrFormat& f, const ApplyArgs& a, int grid_blocks) {
+  bcsr_kernel_t k = pick(v);
+  if (!k) return cudaErrorInvalidValue;
+  if (f.brows == 0) return cudaSuccess;
+  int64_t per_block = v.block / v.W;
+  int64_t exact = (f.brows + per_block - 1) / per_block;
+  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>((int)f.brows, f.brow_ptr, f.bcol, f.bval, a.alpha, a.x, a.beta,
+                                              a.y);
+  return cudaGetLastError();
+}
+
+}  // namespace spmv

@@ -1,0 +1,242 @@
+// Merge-path CSR kernel (north_star (c): "merge-path CSR for
+// skewed row lengths").  Restates the published merge-path decomposition: the list of row
+// ends (row_ptr[1..rows]) is merged with the list of non-zero indices 0..nnz-1; the merged
+// path of rows+nnz items is cut into equal tiles (one per thread block, precomputed once per
+// matrix in MergePlan::tile_row) and, inside a tile, into equal per-thread pieces.
+//
+// Determinism (reading A20): no floating-point atomics.  Partial sums that cross thread
+// boundaries are combined by a fixed-shape segmented scan; partial sums that cross tile
+// boundaries go to (carry_row, carry_val) and are added in tile order by merge_fixup_kernel.
+#include <limits.h>
+
+#include "device_utils.cuh"
+#include "spmv_internal.h"
+
+namespace spmv {
+
+template <int B, int I>
+struct MergeSmem {
+  static constexpr int TI = B * I;
+  static constexpr size_t bytes = sizeof(double) * TI * 2 + sizeof(int) * (TI + 2) +
+                                  sizeof(int) * B + sizeof(double) * B + 32 * (sizeof(int) + sizeof(double)) + 16;
+};
+
+template <int B, int I, int X>
+__global__ void __launch_bounds__(B)
+merge_kernel(int rows, int nnz, const int* __restrict__ rp, const int* __restrict__ ci,
+             const double* __restrict__ va, const int* __restrict__ tile_row,
+             int* __restrict__ carry_row, double* __restrict__ carry_val, double alpha,
+             const double* __restrict__ x, double beta, double* __restrict__ y) {
+  constexpr int TI = B * I;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* s_prod = reinterpret_cast<double*>(smem_raw);
+  double* s_rowsum = s_prod + TI;
+  double* s_cval = s_rowsum + TI;
+  double* s_wval = s_cval + B;
+  int* s_rowend = reinterpret_cast<int*>(s_wval + 32);
+  int* s_ckey = s_rowend + TI + 2;
+  int* s_wkey = s_ckey + B;
+
+  const int t = blockIdx.x;
+  const int tid = threadIdx.x;
+  const int64_t P = (int64_t)rows + nnz;
+  const int64_t d0 = (int64_t)t * TI;
+  const int64_t d1 = (d0 + TI < P) ? d0 + TI : P;
+  const int i0 = __ldg(tile_row + t), i1 = __ldg(tile_row + t + 1);
+  const int k0 = (int)(d0 - i0), k1 = (int)(d1 - i1);
+  const int nrows_t = i1 - i0;       // rows finished inside this tile
+  const int nk = k1 - k0;            // non-zeros consumed inside this tile
+  const int tile_len = (int)(d1 - d0);
+
+  // stage row ends (one extra: the row the tile ends inside) and the products
+  for (int j = tid; j <= nrows_t; j += B) {
+    int r = i0 + j;
+    s_rowend[j] = (r < rows) ? __ldg(rp + r + 1) : INT_MAX;
+  }
+  {
+    double v[I];
+    int c[I];
+#pragma unroll
+    for (int u = 0; u < I; ++u) {
+      int k = tid + u * B;
+      bool in = k < nk;
+      v[u] = in ? ld_stream(va + k0 + k) : 0.0;
+      c[u] = in ? ld_stream(ci + k0 + k) : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < I; ++u) {
+      int k = tid + u * B;
+      if (c[u] >= 0) s_prod[k] = v[u] * ldx<X>(x, c[u]);
+    }
+  }
+  __syncthreads();
+
+  // per-thread start on the tile-local merge path
+  int ld = tid * I;
+  if (ld > tile_len) ld = tile_len;
+  int lo = ld - nk > 0 ? ld - nk : 0;
+  int hi = ld < nrows_t ? ld : nrows_t;
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    if (s_rowend[mid] - k0 <= ld - mid - 1) lo = mid + 1; else hi = mid;
+  }
+  int i = lo, k = ld - lo;
+  double s = 0.0;
+  int end = ld + I < tile_len ? ld + I : tile_len;
+  for (int it = ld; it < end; ++it) {
+    if (k < nk && k + k0 < s_rowend[i]) {
+      s += s_prod[k];
+      ++k;
+    } else {
+      s_rowsum[i] = s;      // row i0+i ends here; carry-ins are added below
+      s = 0.0;
+      ++i;
+    }
+  }
+
+  // segmented inclusive scan of (key = local row the thread ended in, val = open partial sum)
+  const int lane = tid & 31, w = tid >> 5;
+  int key = i;
+  double val = s;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    int kk = __shfl_up_sync(0xffffffffu, key, d);
+    double vv = __shfl_up_sync(0xffffffffu, val, d);
+    if (lane >= d && kk == key) val += vv;
+  }
+  if (lane == 31) { s_wkey[w] = key; s_wval[w] = val; }
+  __syncthreads();
+  if (w == 0) {
+    constexpr int NW = B / 32;
+    int wk = lane < NW ? s_wkey[lane] : INT_MAX;
+    double wv = lane < NW ? s_wval[lane] : 0.0;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      int kk = __shfl_up_sync(0xffffffffu, wk, d);
+      double vv = __shfl_up_sync(0xffffffffu, wv, d);
+      if (lane >= d && kk == wk) wv += vv;
+    }
+    if (lane < NW) s_wval[lane] = wv;
+  }
+  __syncthreads();
+  if (w > 0 && s_wkey[w - 1] == key) val += s_wval[w - 1];
+  s_ckey[tid] = key;
+  s_cval[tid] = val;
+  __syncthreads();
+  const bool seg_last = (tid == B - 1) || (s_ckey[tid + 1] != key);
+  if (seg_last) {
+    if (key < nrows_t) {
+      s_rowsum[key] += val;              // finished by the next thread of this tile
+    } else if (tid == B - 1) {           // the row the tile ends inside
+      int row_start = (i1 < rows) ? __ldg(rp + i1) : nnz;
+      int from = row_start > k0 ? row_start : k0;
+      bool open = (i1 < rows) && (k1 > from);
+      carry_row[t] = open ? i1 : -1;
+      carry_val[t] = open ? val : 0.0;
+    }
+  }
+  __syncthreads();
+  for (int j = tid; j < nrows_t; j += B) store_y(y, i0 + j, alpha, s_rowsum[j], beta);
+}
+
+// Adds the tile carry-outs in tile order: one thread per run of equal carry_row.
+__global__ void merge_fixup_kernel(int64_t ntiles, const int* __restrict__ carry_row,
+                                   const double* __restrict__ carry_val, double alpha,
+                                   double* __restrict__ y) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntiles) return;
+  int r = carry_row[t];
+  if (r < 0) return;
+  if (t > 0 && carry_row[t - 1] == r) return;    // not a run head
+  double s = carry_val[t];
+  for (int64_t u = t + 1; u < ntiles && carry_row[u] == r; ++u) s += carry_val[u];
+  y[r] = fma(alpha, s, y[r]);
+}
+
+// One thread per tile boundary: diagonal search on the global row_ptr (done once per matrix).
+__global__ void merge_partition_kernel(int rows, int nnz, const int* __restrict__ rp, int tile_items,
+                                       int64_t ntiles, int* __restrict__ tile_row) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t > ntiles) return;
+  int64_t P = (int64_t)rows + nnz;
+  int64_t d = t * tile_items;
+  if (d > P) d = P;
+  int64_t lo = d - nnz > 0 ? d - nnz : 0;
+  int64_t hi = d < rows ? d : rows;
+  while (lo < hi) {
+    int64_t mid = (lo + hi) >> 1;
+    if ((int64_t)__ldg(rp + mid + 1) <= d - mid - 1) lo = mid + 1; else hi = mid;
+  }
+  tile_row[t] = (int)lo;
+}
+
+typedef void (*merge_kernel_t)(int, int, const int*, const int*, const double*, const int*, int*, double*,
+                               double, const double*, double, double*);
+
+struct MergeEntry { int B, I, X; merge_kernel_t k; size_t smem; };
+#define ME(b, i) {b, i, 0, merge_kernel<b, i, 0>, MergeSmem<b, i>::bytes}, {b, i, 1, merge_kernel<b, i, 1>, MergeSmem<b, i>::bytes}
+static const MergeEntry g_merge[] = {ME(128, 5), ME(128, 7), ME(128, 11), ME(256, 5), ME(256, 7), ME(256, 11),
+                                     ME(512, 5), ME(512, 7)};
+#undef ME
+
+static const MergeEntry* merge_pick(const Variant& v) {
+  for (const auto& e : g_merge)
+    if (e.B == v.block && e.I == v.I && e.X == v.X) return &e;
+  return nullptr;
+}
+
+bool merge_supported(const Variant& v) { return merge_pick(v) != nullptr; }
+const void* merge_func(const Variant& v) {
+  const MergeEntry* e = merge_pick(v);
+  return e ? (const void*)e->k : nullptr;
+}
+
+cudaError_t merge_launch(const Variant& v, const CsrView& A, const MergePlan& p, const ApplyArgs& a) {
+  const MergeEntry* e = merge_pick(v);
+  if (!e || p.tile_items != v.block * v.I) return cudaErrorInvalidValue;
+  if (A.rows == 0) return cudaSuccess;
+  static thread_local const void* last_attr = nullptr;
+  if (e->smem > 48 * 1024 && last_attr != (const void*)e->k) {
+    cudaError_t err = cudaFuncSetAttribute((const void*)e->k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem);
+    if (err != cudaSuccess) return err;
+    last_attr = (const void*)e->k;
+  }
+  e->k<<<(unsigned)p.ntiles, e->B, e->smem, a.stream>>>((int)A.rows, (int)A.nnz, A.row_ptr, A.col_idx, A.val,
+                                                       p.tile_row, p.carry_row, p.carry_val, a.alpha, a.x,
+                                                       a.beta, a.y);
+  cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  merge_fixup_kernel<<<(unsigned)((p.ntiles + 255) / 256), 256, 0, a.stream>>>(p.ntiles, p.carry_row,
+                                                                            p.carry_val, a.alpha, a.y);
+  return cudaGetLastError();
+}
+
+spmv_status_t build_merge_plan(const CsrView& A, int tile_items, Allocator& al, cudaStream_t s,
+                               MergePlan* out) {
+  MergePlan p;
+  p.tile_items = tile_items;
+  int64_t P = A.rows + A.nnz;
+  p.ntiles = (P + tile_items - 1) / tile_items;
+  if (p.ntiles == 0) p.ntiles = 1;
+  p.tile_row = (int32_t*)al.alloc(sizeof(int32_t) * (p.ntiles + 1), s);
+  p.carry_row = (int32_t*)al.alloc(sizeof(int32_t) * p.ntiles, s);
+  p.carry_val = (double*)al.alloc(sizeof(double) * p.ntiles, s);
+  if (!p.tile_row || !p.carry_row || !p.carry_val) {
+    free_merge_plan(p, al);
+    return SPMV_ERR_ALLOC;
+  }
+  merge_partition_kernel<<<(unsigned)((p.ntiles + 1 + 255) / 256), 256, 0, s>>>((int)A.rows, (int)A.nnz, A.row_ptr,
+                                                                           tile_items, p.ntiles, p.tile_row);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  *out = p;
+  return SPMV_OK;
+}
+
+void free_merge_plan(MergePlan& p, Allocator& al) {
+  if (p.tile_row) al.free(p.tile_row, sizeof(int32_t) * (p.ntiles + 1));
+  if (p.carry_row) al.free(p.carry_row, sizeof(int32_t) * p.ntiles);
+  if (p.carry_val) al.free(p.carry_val, sizeof(double) * p.ntiles);
+  p = MergePlan();
+}
+
+}  // namespace spmv

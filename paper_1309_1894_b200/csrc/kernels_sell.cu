@@ -1,0 +1,143 @@
+// SELL-C-sigma / ELL kernel (north_star (c): "SELL-C-sigma
+// with coalesced 128-bit vectorised loads of values and column indices").
+//
+// Row-vectorised layout (SURVEY "SELL layout" option 1): entry (slice s, position j, row r)
+// lives at slice_ptr[s] + j*C + r; a thread owns R ADJACENT rows, so one step is one
+// R*8-byte load of values and one R*4-byte load of column indices (R=2: double2 + int2,
+// R=4: 2 x double2 + int4), fully coalesced across the warp, with no width padding.
+// Padding entries have col = -1 and are skipped, never multiplied (reading A7), so a
+// NaN/Inf in x cannot leak into a row that CSR would leave clean.
+#include "device_utils.cuh"
+#include "spmv_internal.h"
+
+namespace spmv {
+
+template <int R>
+struct VecLoad;
+template <>
+struct VecLoad<1> {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+    v[0] = ld_stream(pv);
+    c[0] = ld_stream(pc);
+  }
+};
+template <>
+struct VecLoad<2> {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+    double2 a = ld_stream2(pv);
+    int2 b = ld_stream2(pc);
+    v[0] = a.x; v[1] = a.y; c[0] = b.x; c[1] = b.y;
+  }
+};
+template <>
+struct VecLoad<4> {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+    double2 a0 = ld_stream2(pv);
+    double2 a1 = ld_stream2(pv + 2);
+    int4 b = ld_stream4(pc);
+    v[0] = a0.x; v[1] = a0.y; v[2] = a1.x; v[3] = a1.y;
+    c[0] = b.x; c[1] = b.y; c[2] = b.z; c[3] = b.w;
+  }
+};
+
+template <int R, int U, int PERM, int X>
+__global__ void __launch_bounds__(1024)
+sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
+            const int64_t* __restrict__ slice_ptr, const double* __restrict__ sval,
+            const int* __restrict__ scol, const int* __restrict__ perm, double alpha,
+            const double* __restrict__ x, double beta, double* __restrict__ y) {
+  const int64_t G = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows_padded; g += G) {
+    const int64_t r0 = g * R;
+    const int64_t s = logC >= 0 ? (r0 >> logC) : 0;
+    const int off = (int)(r0 - s * C);
+    const int64_t base = __ldg(slice_ptr + s);
+    const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
+    const double* pv = sval + base + off;
+    const int* pc = scol + base + off;
+    double acc[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = 0.0;
+    int j = 0;
+    for (; j + U <= w; j += U) {
+      double v[U][R];
+      int c[U][R];
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        VecLoad<R>::load(pv + (int64_t)(j + u) * C, pc + (int64_t)(j + u) * C, v[u], c[u]);
+      double xv[U][R];
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int r = 0; r < R; ++r) xv[u][r] = c[u][r] >= 0 ? ldx<X>(x, c[u][r]) : 0.0;
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          if (c[u][r] >= 0) acc[r] = fma(v[u][r], xv[u][r], acc[r]);
+    }
+    for (; j < w; ++j) {
+      double v[R];
+      int c[R];
+      VecLoad<R>::load(pv + (int64_t)j * C, pc + (int64_t)j * C, v, c);
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        if (c[r] >= 0) acc[r] = fma(v[r], ldx<X>(x, c[r]), acc[r]);
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      int64_t row = r0 + r;
+      if (PERM) {
+        int o = __ldg(perm + row);
+        if (o >= 0) store_y(y, o, alpha, acc[r], beta);
+      } else if (row < rows) {
+        store_y(y, row, alpha, acc[r], beta);
+      }
+    }
+  }
+}
+
+typedef void (*sell_kernel_t)(int64_t, int64_t, int, int, const int64_t*, const double*, const int*,
+                              const int*, double, const double*, double, double*);
+
+template <int PERM, int X>
+static sell_kernel_t pick_ru(int R, int U) {
+#define P(r, u) if (R == r && U == u) return sell_kernel<r, u, PERM, X>;
+  P(1, 1) P(1, 2) P(1, 4) P(1, 8) P(2, 1) P(2, 2) P(2, 4) P(2, 8) P(4, 1) P(4, 2) P(4, 4)
+#undef P
+  return nullptr;
+}
+static sell_kernel_t pick(const Variant& v, bool perm) {
+  if (v.X == 0) return perm ? pick_ru<1, 0>(v.R, v.U) : pick_ru<0, 0>(v.R, v.U);
+  if (v.X == 1) return perm ? pick_ru<1, 1>(v.R, v.U) : pick_ru<0, 1>(v.R, v.U);
+  return nullptr;
+}
+
+bool sell_supported(const Variant& v) {
+  if (v.block < 32 || v.block > 1024 || v.block % 32) return false;
+  if (pick(v, false) == nullptr) return false;
+  if (v.fam == FAM_SELL) {
+    if (v.C < 128 || v.C > 4096 || (v.C & (v.C - 1))) return false;   // power of two, multiple of 32*Rmax
+    if (v.S < 1) return false;
+    if (v.S > 1 && (v.S % v.C != 0 || v.S > 8192 || (v.S & (v.S - 1)))) return false;
+  }
+  return true;
+}
+const void* sell_func(const Variant& v, bool perm) { return (const void*)pick(v, perm); }
+
+cudaError_t sell_launch(const Variant& v, int64_t rows, const SellFormat& f, const ApplyArgs& a,
+                        int grid_blocks) {
+  const bool perm = f.perm != nullptr;
+  sell_kernel_t k = pick(v, perm);
+  if (!k) return cudaErrorInvalidValue;
+  if (rows == 0) return cudaSuccess;
+  const int64_t rows_padded = f.nslices * (int64_t)f.C;
+  const int64_t threads = (rows_padded + v.R - 1) / v.R;
+  int64_t exact = (threads + v.block - 1) / v.block;
+  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, rows_padded, f.C, f.logC, f.slice_ptr, f.val, f.col,
+                                              f.perm, a.alpha, a.x, a.beta, a.y);
+  return cudaGetLastError();
+}
+
+}  // namespace spmv

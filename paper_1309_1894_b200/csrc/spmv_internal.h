@@ -1,0 +1,176 @@
+// Internal declarations shared by the translation units of libspmv_b200.so.
+// Nothing here is shared with oracle/ (independent paths).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/spmv_b200.h"
+
+namespace spmv {
+
+// ---------------------------------------------------------------- formats
+struct CsrView {
+  int64_t rows = 0, cols = 0, nnz = 0;
+  const int32_t* row_ptr = nullptr;
+  const int32_t* col_idx = nullptr;
+  const double* val = nullptr;
+};
+
+// SELL-C-sigma (ELL is the one-slice case).  Storage is slice-column-major:
+//   entry (row r of slice s, position j) at  slice_ptr[s] + j*C + r.
+// Padding carries col = -1 and is never multiplied (reading A7).
+struct SellFormat {
+  int C = 0;                 // rows per slice (multiple of 128; ELL: padded row count)
+  int logC = -1;             // log2(C), or -1 when there is a single slice (ELL)
+  int sigma = 1;             // sorting window (1: no permutation)
+  int64_t nslices = 0;
+  int64_t padded = 0;        // stored entries including padding
+  int64_t* slice_ptr = nullptr;   // [nslices+1]
+  double* val = nullptr;          // [padded]
+  int32_t* col = nullptr;         // [padded]
+  int32_t* perm = nullptr;        // [nslices*C] sell row -> original row (or -1); null if sigma==1
+  bool is_ell = false;
+};
+
+// 3x3 BCSR, values transposed per block row:
+//   element k (= 3*r + c) of block j of block row b at  9*brow_ptr[b] + k*nb_b + j.
+struct BcsrFormat {
+  int64_t brows = 0, nblocks = 0;
+  int32_t* brow_ptr = nullptr;   // [brows+1]
+  int32_t* bcol = nullptr;       // [nblocks] block column
+  double* bval = nullptr;        // [9*nblocks]
+  double fill = 0.0;             // nnz / (9*nblocks)
+};
+
+// Merge-path plan: tile t covers merge-path diagonals [t*tile_items, (t+1)*tile_items);
+// tile_row[t] = number of row-end items consumed before that diagonal.
+struct MergePlan {
+  int tile_items = 0;
+  int64_t ntiles = 0;
+  int32_t* tile_row = nullptr;   // [ntiles+1]
+  int32_t* carry_row = nullptr;  // [ntiles]
+  double* carry_val = nullptr;   // [ntiles]
+};
+
+// ---------------------------------------------------------------- variants
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_COUNT };
+
+struct Variant {
+  int fam = FAM_CSR_SCALAR;
+  int block = 256;   // b: threads per block                       (PAPER.md:23 knob 1)
+  int grid = 0;      // g: 0 exact cover, k>0: k * SMs * resident blocks, grid-stride (knob 2)
+  int carve = -1;    // co: shared-memory carve-out percent, -1 default         (knob 4)
+  int U = 1;         // u: unroll factor                                         (knob 5)
+  int R = 1;         // r: rows per thread (csr_scalar, sell)
+  int W = 1;         // w: lanes per row (csr_vector), lanes per block row (bcsr3)
+  int X = 0;         // x: 0 read-only path (ld.global.nc), 1 plain ld.global
+  int C = 0;         // c: SELL slice height
+  int S = 1;         // s: SELL sorting window sigma
+  int I = 0;         // i: merge-path items per thread
+};
+
+std::string variant_to_string(const Variant& v);
+bool variant_from_string(const char* s, Variant* out);
+Variant default_variant();
+
+struct ApplyArgs {
+  double alpha, beta;
+  const double* x;
+  double* y;
+  cudaStream_t stream;
+};
+
+struct DeviceProps {
+  int sm_count = 0;
+  int64_t l2_bytes = 0;
+  char name[64] = {0};
+};
+
+// Per-family entry points (kernels_*.cu).  `supported` checks template-parameter
+// availability only; structural eligibility is decided by the tuner / select.
+bool csr_scalar_supported(const Variant&);
+const void* csr_scalar_func(const Variant&);
+cudaError_t csr_scalar_launch(const Variant&, const CsrView&, const ApplyArgs&, int grid_blocks);
+
+bool csr_vector_supported(const Variant&);
+const void* csr_vector_func(const Variant&);
+cudaError_t csr_vector_launch(const Variant&, const CsrView&, const ApplyArgs&, int grid_blocks);
+
+bool sell_supported(const Variant&);
+const void* sell_func(const Variant&, bool perm);
+cudaError_t sell_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int grid_blocks);
+
+bool merge_supported(const Variant&);
+const void* merge_func(const Variant&);
+cudaError_t merge_launch(const Variant&, const CsrView&, const MergePlan&, const ApplyArgs&);
+
+bool bcsr_supported(const Variant&);
+const void* bcsr_func(const Variant&);
+cudaError_t bcsr_launch(const Variant&, const BcsrFormat&, const ApplyArgs&, int grid_blocks);
+
+// y = beta*y (or 0): the alpha == 0 path (reading A2)
+cudaError_t scale_y_launch(int64_t rows, double beta, double* y, cudaStream_t s);
+
+// ---------------------------------------------------------------- allocator
+struct Allocator {
+  spmv_allocator_t cb{};
+  bool has_cb = false;
+  int64_t owned = 0;
+  void* alloc(size_t bytes, cudaStream_t s);
+  void free(void* p, size_t bytes);
+};
+
+// ---------------------------------------------------------------- converters / stats (convert.cu)
+struct RawStats {   // filled on the device, copied back once
+  unsigned long long bad_row_ptr, bad_col;
+  unsigned long long sum_len, sum_len_sq;
+  unsigned long long hist[32];
+  unsigned long long sig_row_ptr, sig_col_idx;
+  unsigned long long unsorted_rows;     // rows whose columns are not strictly ascending
+  unsigned long long block3_bad;        // block rows violating the dense aligned 3x3 pattern
+  unsigned long long n_blocks3;
+  long long bandwidth;
+  int min_len, max_len;
+};
+cudaError_t compute_stats(const CsrView& A, RawStats* h_out, cudaStream_t s);
+
+spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, Allocator& al,
+                         cudaStream_t s, SellFormat* out);
+void free_sell(SellFormat& f, Allocator& al);
+spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out);
+void free_bcsr3(BcsrFormat& f, Allocator& al);
+spmv_status_t build_merge_plan(const CsrView& A, int tile_items, Allocator& al, cudaStream_t s,
+                               MergePlan* out);
+void free_merge_plan(MergePlan& p, Allocator& al);
+
+// ---------------------------------------------------------------- verification kernels (verify.cu)
+struct VerifyResult {
+  unsigned long long n_fail;
+  long long first_fail;
+  double max_ratio;
+};
+// reference: unfused, stored-order, one thread per row; also emits scale
+cudaError_t reference_launch(const CsrView& A, double alpha, const double* x, double beta,
+                             double* y, double* scale, cudaStream_t s);
+cudaError_t compare_launch(int64_t rows, const double* y_test, const double* y_ref,
+                           const double* scale, double tol, VerifyResult* d_result, cudaStream_t s);
+cudaError_t fill_uniform_launch(double* p, int64_t n, uint64_t seed, cudaStream_t s);
+cudaError_t perturb_launch(double* y, int64_t rows, cudaStream_t s);
+cudaError_t flush_l2_launch(double* buf, int64_t n, cudaStream_t s);
+
+// error text
+void set_last_error(const char* fmt, ...);
+const char* last_error_text();
+#define SPMV_CUDA_TRY(expr)                                                        \
+  do {                                                                             \
+    cudaError_t _e = (expr);                                                       \
+    if (_e != cudaSuccess) {                                                       \
+      spmv::set_last_error("%s:%d %s -> %s", __FILE__, __LINE__, #expr, cudaGetErrorString(_e)); \
+      return SPMV_ERR_CUDA;                                                        \
+    }                                                                              \
+  } while (0)
+
+}  // namespace spmv

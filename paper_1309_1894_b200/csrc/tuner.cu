@@ -1,0 +1,474 @@
+// The autotuner (sec. 2): enumerate variants, run each on
+// the actual matrix, compare its output with the reference result, time the ones that match,
+// keep the fastest, cache the winner per matrix signature.  Knobs follow PAPER.md:23: threads per
+// block, blocks per grid, L1/shared carve-out, unroll (stream count: spmv_tune_batch).
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <chrono>
+#include <map>
+#include <mutex>
+
+#include "handle.h"
+
+namespace spmv {
+void handle_refresh_info(spmv_handle_s* h);
+
+struct CacheEntry { std::string variant; double us; };
+static std::mutex g_cache_mu;
+static std::map<std::string, CacheEntry> g_cache;
+
+std::string signature_key(const spmv_handle_s* h, bool beta_nonzero) {
+  char buf[320];
+  const spmv_info_t& in = h->info;
+  snprintf(buf, sizeof(buf), "%lld:%lld:%lld:%016llx:%016llx:%s:%d:%s:b%d", (long long)in.rows, (long long)in.cols,
+           (long long)in.nnz, (unsigned long long)in.sig_row_ptr, (unsigned long long)in.sig_col_idx, in.device_name,
+           in.sm_count, kVersion, beta_nonzero ? 1 : 0);
+  for (char* p = buf; *p; ++p) if (*p == ' ' || *p == '\t') *p = '_';
+  return std::string(buf);
+}
+
+static bool filter_match(const char* filter, const std::string& desc) {
+  if (!filter || !*filter) return true;
+  std::string f(filter);
+  size_t pos = 0;
+  while (pos <= f.size()) {
+    size_t c = f.find(',', pos);
+    if (c == std::string::npos) c = f.size();
+    std::string tok = f.substr(pos, c - pos);
+    if (!tok.empty() && desc.compare(0, tok.size(), tok) == 0) return true;
+    pos = c + 1;
+  }
+  return false;
+}
+
+// First-phase candidates: family x template parameters x threads per block, exact grid, default
+// carve-out.  The second phase (spmv_tune) sweeps grid multipliers and carve-outs on the leaders.
+std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* filter, int* n_pruned) {
+  std::vector<Variant> all, out;
+  const spmv_info_t& in = h->info;
+  const int blocks[3] = {128, 256, 512};
+  for (int b : blocks) {
+    for (int R : {1, 2, 4}) for (int U : {1, 2, 4}) {
+      Variant v; v.fam = FAM_CSR_SCALAR; v.block = b; v.R = R; v.U = U; all.push_back(v);
+    }
+    for (int W : {2, 4, 8, 16, 32}) for (int U : {1, 2, 4}) {
+      Variant v; v.fam = FAM_CSR_VECTOR; v.block = b; v.W = W; v.U = U;
+      // lanes far wider than the rows are long (or far narrower) cannot win
+      if (W > 2 && (double)W > 8.0 * std::max(1.0, in.mean_row_len)) { ++*n_pruned; continue; }
+      if ((double)W * 64.0 < in.mean_row_len) { ++*n_pruned; continue; }
+      all.push_back(v);
+    }
+    for (int C : {128, 512}) for (int S : {1, 8192}) for (int R : {1, 2, 4}) for (int U : {1, 2, 4, 8}) {
+      Variant v; v.fam = FAM_SELL; v.block = b; v.C = C; v.S = S; v.R = R; v.U = U;
+      if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }       // sorting equal rows is a no-op
+      if (S == 1 && in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0) { ++*n_pruned; continue; }
+      if ((double)in.max_row_len > 64.0 * in.mean_row_len + 64.0 && S < 8192) { ++*n_pruned; continue; }
+      all.push_back(v);
+    }
+    for (int R : {1, 2, 4}) for (int U : {1, 2, 4, 8}) {
+      Variant v; v.fam = FAM_ELL; v.block = b; v.R = R; v.U = U; all.push_back(v);
+    }
+    for (int I : {5, 7, 11}) {
+      Variant v; v.fam = FAM_MERGE; v.block = b; v.I = I; all.push_back(v);
+    }
+    for (int W : {4, 8, 16, 32}) for (int U : {1, 2}) {
+      Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; all.push_back(v);
+    }
+  }
+  // family, then format key, outermost: formats are then built once per key
+  std::stable_sort(all.begin(), all.end(), [](const Variant& a, const Variant& b) {
+    if (a.fam != b.fam) return a.fam < b.fam;
+    if (a.C != b.C) return a.C < b.C;
+    return a.S < b.S;
+  });
+  for (const Variant& v : all) {
+    std::string why;
+    if (!variant_eligible(h, v, &why)) { ++*n_pruned; continue; }
+    if (!filter_match(filter, variant_to_string(v))) continue;
+    out.push_back(v);
+  }
+  return out;
+}
+
+namespace {
+
+struct Tuner {
+  spmv_handle_s* h;
+  cudaStream_t s;
+  double alpha, beta, tol;
+  int warmup, reps;
+  double min_batch_ms;
+  bool flush;
+  const char* fault;
+  double *x = nullptr, *y0 = nullptr, *y = nullptr, *yref = nullptr, *scale = nullptr, *flushbuf = nullptr;
+  bool own_x = false, own_y0 = false, own_ref = false;
+  int64_t flush_n = 0;
+  VerifyResult* d_res = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  spmv_tune_report_t* rep;
+
+  void log(const std::string& desc, const char* status, double us, double err) {
+    if (!rep || !rep->log_buf || rep->log_cap == 0) return;
+    char line[256];
+    int n = snprintf(line, sizeof(line), "%s %s %.3f %.3e\n", desc.c_str(), status, us, err);
+    if (rep->log_len + n + 1 <= rep->log_cap) {
+      memcpy(rep->log_buf + rep->log_len, line, n);
+      rep->log_len += n;
+      rep->log_buf[rep->log_len] = 0;
+    }
+  }
+
+  spmv_status_t reset_y() {
+    if (h->A.rows == 0) return SPMV_OK;
+    if (beta != 0.0) SPMV_CUDA_TRY(cudaMemcpyAsync(y, y0, sizeof(double) * h->A.rows, cudaMemcpyDeviceToDevice, s));
+    else SPMV_CUDA_TRY(cudaMemsetAsync(y, 0xff, sizeof(double) * h->A.rows, s));   // NaN: must be overwritten
+    return SPMV_OK;
+  }
+
+  // one launch from y0, compared with the reference; returns pass/fail and the launch time
+  spmv_status_t verify(const Variant& v, bool* pass, double* err, double* us) {
+    spmv_status_t st = reset_y();
+    if (st != SPMV_OK) return st;
+    ApplyArgs a{alpha, beta, x, y, s};
+    SPMV_CUDA_TRY(cudaEventRecord(e0, s));
+    st = launch_variant(h, v, a);
+    if (st != SPMV_OK) return st;
+    SPMV_CUDA_TRY(cudaEventRecord(e1, s));
+    if (fault && *fault && variant_to_string(v).compare(0, strlen(fault), fault) == 0) {
+      cudaError_t e = perturb_launch(y, h->A.rows, s);
+      if (e != cudaSuccess) return SPMV_ERR_CUDA;
+    }
+    cudaError_t e = compare_launch(h->A.rows, y, yref, scale, tol, d_res, s);
+    if (e != cudaSuccess) { set_last_error("compare: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+    VerifyResult r;
+    SPMV_CUDA_TRY(cudaMemcpyAsync(&r, d_res, sizeof(r), cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+    float ms = 0.f;
+    SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    *pass = r.n_fail == 0;
+    *err = r.max_ratio;
+    *us = (double)ms * 1e3;
+    return SPMV_OK;
+  }
+
+  // median time per apply over `reps` batches (warm) or `reps*4` flushed single launches (cold)
+  spmv_status_t time(const Variant& v, double est_us, double* us) {
+    ApplyArgs a{alpha, beta, x, y, s};
+    for (int i = 0; i < warmup; ++i) {
+      spmv_status_t st = launch_variant(h, v, a);
+      if (st != SPMV_OK) return st;
+    }
+    std::vector<double> t;
+    if (flush) {
+      for (int i = 0; i < reps * 4; ++i) {
+        cudaError_t e = flush_l2_launch(flushbuf, flush_n, s);
+        if (e != cudaSuccess) return SPMV_ERR_CUDA;
+        SPMV_CUDA_TRY(cudaEventRecord(e0, s));
+        spmv_status_t st = launch_variant(h, v, a);
+        if (st != SPMV_OK) return st;
+        SPMV_CUDA_TRY(cudaEventRecord(e1, s));
+        SPMV_CUDA_TRY(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        t.push_back((double)ms * 1e3);
+      }
+    } else {
+      int K = (int)(min_batch_ms * 1e3 / std::max(est_us, 1.0)) + 1;
+      K = std::min(K, 2000);
+      for (int i = 0; i < reps; ++i) {
+        SPMV_CUDA_TRY(cudaEventRecord(e0, s));
+        for (int k = 0; k < K; ++k) {
+          spmv_status_t st = launch_variant(h, v, a);
+          if (st != SPMV_OK) return st;
+        }
+        SPMV_CUDA_TRY(cudaEventRecord(e1, s));
+        SPMV_CUDA_TRY(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        t.push_back((double)ms * 1e3 / K);
+      }
+    }
+    std::sort(t.begin(), t.end());
+    *us = t[t.size() / 2];
+    return SPMV_OK;
+  }
+
+  void cleanup() {
+    Allocator& al = h->al;
+    const int64_t r = h->A.rows, c = h->A.cols;
+    if (own_x && x) al.free(x, sizeof(double) * c);
+    if (own_y0 && y0) al.free(y0, sizeof(double) * r);
+    if (y) al.free(y, sizeof(double) * r);
+    if (own_ref && yref) al.free(yref, sizeof(double) * r);
+    if (own_ref && scale) al.free(scale, sizeof(double) * r);
+    if (flushbuf) al.free(flushbuf, sizeof(double) * flush_n);
+    if (d_res) al.free(d_res, sizeof(VerifyResult));
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+  }
+};
+
+struct Scored { Variant v; double us; };
+
+}  // namespace
+}  // namespace spmv
+
+using namespace spmv;
+
+extern "C" void spmv_clear_cache(void) {
+  std::lock_guard<std::mutex> lk(g_cache_mu);
+  g_cache.clear();
+}
+
+static void cache_file_load(const char* path) {
+  FILE* f = fopen(path, "r");
+  if (!f) return;
+  char key[400], var[160];
+  double us;
+  while (fscanf(f, "%399s %159s %lf", key, var, &us) == 3) {
+    Variant v;
+    if (variant_from_string(var, &v)) g_cache[key] = CacheEntry{var, us};   // malformed lines are skipped
+  }
+  fclose(f);
+}
+
+extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts, spmv_tune_report_t* report) {
+  if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
+  spmv_tune_opts_t o{};
+  if (opts) o = *opts;
+  if ((o.d_y_ref == nullptr) != (o.d_scale == nullptr)) return SPMV_ERR_INVALID_ARG;
+  if (o.d_y_ref && !o.d_x_probe) return SPMV_ERR_INVALID_ARG;   // an external reference needs its x
+  const auto t_start = std::chrono::steady_clock::now();
+  char* log_buf = report ? report->log_buf : nullptr;
+  size_t log_cap = report ? report->log_cap : 0;
+  if (report) { memset(report, 0, sizeof(*report)); report->log_buf = log_buf; report->log_cap = log_cap; if (log_buf && log_cap) log_buf[0] = 0; }
+
+  Tuner T{};
+  T.h = h;
+  T.s = (cudaStream_t)o.stream;
+  T.alpha = o.has_scalars ? o.alpha : 1.0;
+  T.beta = o.has_scalars ? o.beta : 0.0;
+  if (T.alpha == 0.0) return SPMV_ERR_INVALID_ARG;
+  T.tol = o.tolerance > 0 ? o.tolerance : 1e-12;
+  T.warmup = o.warmup > 0 ? o.warmup : 2;
+  T.reps = o.reps > 0 ? o.reps : 5;
+  T.min_batch_ms = o.min_batch_ms > 0 ? o.min_batch_ms : 0.5;
+  T.flush = o.flush_l2 != 0;
+  T.fault = o.fault_inject;
+  T.rep = report;
+  const int64_t rows = h->A.rows, cols = h->A.cols;
+
+  const std::string key = signature_key(h, T.beta != 0.0);
+  if (o.use_cache != 2 && !(o.fault_inject && *o.fault_inject)) {
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    if (o.cache_path && *o.cache_path) cache_file_load(o.cache_path);
+    auto it = g_cache.find(key);
+    if (it != g_cache.end()) {
+      Variant v;
+      std::string why;
+      if (variant_from_string(it->second.variant.c_str(), &v) && variant_eligible(h, v, &why) &&
+          ensure_format(h, v, T.s) == SPMV_OK) {
+        h->sel = v;
+        h->tuned = true;
+        release_formats_except(h, v);
+        handle_refresh_info(h);
+        if (report) {
+          strncpy(report->winner, it->second.variant.c_str(), sizeof(report->winner) - 1);
+          report->winner_us = it->second.us;
+          report->cache_hit = 1;
+          report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+        }
+        return SPMV_OK;
+      }
+    }
+  }
+
+  // ---- probes, reference result, scratch
+  Allocator& al = h->al;
+  spmv_status_t st = SPMV_OK;
+  auto fail = [&](spmv_status_t code) { T.cleanup(); return code; };
+  if (cudaEventCreate(&T.e0) != cudaSuccess || cudaEventCreate(&T.e1) != cudaSuccess) return fail(SPMV_ERR_CUDA);
+  T.x = (double*)o.d_x_probe;
+  if (!T.x) { T.x = (double*)al.alloc(sizeof(double) * cols, T.s); T.own_x = true; if (!T.x) return fail(SPMV_ERR_ALLOC);
+              if (fill_uniform_launch(T.x, cols, o.seed * 2 + 1, T.s) != cudaSuccess) return fail(SPMV_ERR_CUDA); }
+  T.y0 = (double*)o.d_y0_probe;
+  if (!T.y0 && T.beta != 0.0) { T.y0 = (double*)al.alloc(sizeof(double) * rows, T.s); T.own_y0 = true; if (!T.y0) return fail(SPMV_ERR_ALLOC);
+              if (fill_uniform_launch(T.y0, rows, o.seed * 2 + 2, T.s) != cudaSuccess) return fail(SPMV_ERR_CUDA); }
+  T.y = (double*)al.alloc(sizeof(double) * rows, T.s);
+  T.d_res = (VerifyResult*)al.alloc(sizeof(VerifyResult), T.s);
+  if (!T.y || !T.d_res) return fail(SPMV_ERR_ALLOC);
+  if (o.d_y_ref) { T.yref = (double*)o.d_y_ref; T.scale = (double*)o.d_scale; }
+  else {
+    T.own_ref = true;
+    T.yref = (double*)al.alloc(sizeof(double) * rows, T.s);
+    T.scale = (double*)al.alloc(sizeof(double) * rows, T.s);
+    if (!T.yref || !T.scale) return fail(SPMV_ERR_ALLOC);
+    if (T.beta != 0.0 && rows) { if (cudaMemcpyAsync(T.yref, T.y0, sizeof(double) * rows, cudaMemcpyDeviceToDevice, T.s) != cudaSuccess) return fail(SPMV_ERR_CUDA); }
+    if (reference_launch(h->A, T.alpha, T.x, T.beta, T.yref, T.scale, T.s) != cudaSuccess) return fail(SPMV_ERR_CUDA);
+  }
+  if (T.flush) {
+    T.flush_n = (int64_t)(2 * h->dev.l2_bytes / sizeof(double));
+    T.flushbuf = (double*)al.alloc(sizeof(double) * T.flush_n, T.s);
+    if (!T.flushbuf) return fail(SPMV_ERR_ALLOC);
+  }
+
+  // ---- phase 1: every candidate, verify then time
+  int n_pruned = 0;
+  std::vector<Variant> cand = enumerate_candidates(h, o.variant_filter, &n_pruned);
+  const Variant dflt = default_variant();
+  std::vector<Scored> ok;
+  double best_us = 1e300, default_us = 0.0;
+  int n_rej = 0, n_slow = 0, n_timed = 0, n_enum = (int)cand.size();
+  auto budget_left = [&]() {
+    if (o.time_budget_s <= 0) return true;
+    return std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count() < o.time_budget_s;
+  };
+  auto try_candidate = [&](const Variant& v, bool force_time) -> spmv_status_t {
+    const std::string d = variant_to_string(v);
+    spmv_status_t s1 = ensure_format(h, v, T.s);
+    if (s1 == SPMV_ERR_UNSUPPORTED) { ++n_pruned; T.log(d, "pruned_format", 0, 0); return SPMV_OK; }
+    if (s1 != SPMV_OK) return s1;
+    bool pass = false; double err = 0, vus = 0;
+    s1 = T.verify(v, &pass, &err, &vus);
+    if (s1 != SPMV_OK) return s1;
+    if (!pass) { ++n_rej; T.log(d, "rejected", vus, err); return SPMV_OK; }   // can never win
+    if (!force_time && vus > 4.0 * best_us + 20.0) { ++n_slow; T.log(d, "pruned_slow", vus, err); return SPMV_OK; }
+    double us = 0;
+    s1 = T.time(v, vus, &us);
+    if (s1 != SPMV_OK) return s1;
+    ++n_timed;
+    T.log(d, "timed", us, err);
+    ok.push_back(Scored{v, us});
+    if (us < best_us) best_us = us;
+    return SPMV_OK;
+  };
+  // the fixed default first: it is the denominator of the reported speedup
+  {
+    size_t before = ok.size();
+    st = try_candidate(dflt, true);
+    if (st != SPMV_OK) return fail(st);
+    if (ok.size() > before) default_us = ok.back().us;
+  }
+  Variant last_fmt = dflt;
+  for (const Variant& v : cand) {
+    if (!budget_left()) break;
+    if (variant_to_string(v) == variant_to_string(dflt)) continue;
+    // keep device memory bounded: drop formats when the family / format key changes
+    if (v.fam != last_fmt.fam || v.C != last_fmt.C || v.S != last_fmt.S) {
+      Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
+      release_formats_except(h, keep);
+      last_fmt = v;
+    }
+    st = try_candidate(v, false);
+    if (st != SPMV_OK) return fail(st);
+  }
+  // ---- phase 2: grid multipliers and carve-outs on the three leaders
+  std::sort(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; });
+  std::vector<Variant> leaders;
+  for (size_t i = 0; i < ok.size() && i < 3; ++i) leaders.push_back(ok[i].v);
+  std::vector<int> carves;
+  for (int i = 0; i < o.n_carveouts && i < 8; ++i) carves.push_back(o.carveouts[i]);
+  if (carves.empty()) carves = {-1, 0, 100};
+  for (const Variant& L : leaders) {
+    for (int g : {0, 1, 2, 4, 8}) for (int co : carves) {
+      if (g == 0 && co == -1) continue;
+      if (L.fam == FAM_MERGE && g != 0) continue;
+      if (!budget_left()) break;
+      Variant v = L; v.grid = g; v.carve = co;
+      if (!filter_match(o.variant_filter, variant_to_string(v))) continue;
+      ++n_enum;
+      st = try_candidate(v, false);
+      if (st != SPMV_OK) return fail(st);
+    }
+  }
+  std::sort(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; });
+
+  if (report) {
+    report->n_enumerated = n_enum + 1;
+    report->n_pruned_structural = n_pruned;
+    report->n_pruned_slow = n_slow;
+    report->n_rejected = n_rej;
+    report->n_timed = n_timed;
+    report->default_us = default_us;
+  }
+  if (ok.empty()) {
+    T.cleanup();
+    release_all_formats(h);
+    h->sel = dflt;
+    h->tuned = false;
+    handle_refresh_info(h);
+    if (report) report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+    set_last_error("spmv_tune: no candidate matched the reference result");
+    return SPMV_ERR_VERIFY_FAILED;
+  }
+  const Scored& win = ok[0];
+  st = ensure_format(h, win.v, T.s);
+  if (st != SPMV_OK) return fail(st);
+  h->sel = win.v;
+  h->tuned = true;
+  release_formats_except(h, win.v);
+  T.cleanup();
+  handle_refresh_info(h);
+  const std::string wd = variant_to_string(win.v);
+  if (!(o.fault_inject && *o.fault_inject)) {
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    g_cache[key] = CacheEntry{wd, win.us};
+    if (o.cache_path && *o.cache_path) {
+      FILE* f = fopen(o.cache_path, "a");
+      if (f) { fprintf(f, "%s %s %.6f\n", key.c_str(), wd.c_str(), win.us); fclose(f); }
+    }
+  }
+  if (report) {
+    strncpy(report->winner, wd.c_str(), sizeof(report->winner) - 1);
+    report->winner_us = win.us;
+    if (ok.size() > 1) {
+      strncpy(report->runner_up, variant_to_string(ok[1].v).c_str(), sizeof(report->runner_up) - 1);
+      report->runner_up_us = ok[1].us;
+    }
+    report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+  }
+  return SPMV_OK;
+}
+
+extern "C" spmv_status_t spmv_tune_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,
+                                         const double* const* d_xs, const double* betas, double* const* d_ys,
+                                         void* const* streams, int32_t max_streams, int32_t* best_nstreams,
+                                         double* us_per_count) {
+  if (n <= 0 || !hs || !alphas || !d_xs || !betas || !d_ys || !streams || max_streams <= 0 || !best_nstreams)
+    return SPMV_ERR_INVALID_ARG;
+  cudaEvent_t e0, e1, join[64];
+  if (max_streams > 64) max_streams = 64;
+  SPMV_CUDA_TRY(cudaEventCreate(&e0));
+  SPMV_CUDA_TRY(cudaEventCreate(&e1));
+  for (int i = 0; i < max_streams; ++i) SPMV_CUDA_TRY(cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming));
+  cudaStream_t s0 = (cudaStream_t)streams[0];
+  double best = 1e300;
+  int best_c = 1, idx = 0;
+  spmv_status_t st = SPMV_OK;
+  for (int c = 1; c <= max_streams && st == SPMV_OK; c *= 2, ++idx) {
+    std::vector<double> t;
+    for (int rep = 0; rep < 7 && st == SPMV_OK; ++rep) {
+      cudaEventRecord(e0, s0);
+      for (int i = 1; i < c; ++i) cudaStreamWaitEvent((cudaStream_t)streams[i], e0, 0);
+      st = spmv_apply_batch(n, hs, alphas, d_xs, betas, d_ys, streams, c);
+      for (int i = 1; i < c; ++i) { cudaEventRecord(join[i], (cudaStream_t)streams[i]); cudaStreamWaitEvent(s0, join[i], 0); }
+      cudaEventRecord(e1, s0);
+      cudaEventSynchronize(e1);
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep >= 2) t.push_back((double)ms * 1e3);
+    }
+    if (st != SPMV_OK) break;
+    std::sort(t.begin(), t.end());
+    const double med = t[t.size() / 2];
+    if (us_per_count) us_per_count[idx] = med;
+    if (med < best) { best = med; best_c = c; }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  for (int i = 0; i < max_streams; ++i) cudaEventDestroy(join[i]);
+  if (st == SPMV_OK) *best_nstreams = best_c;
+  return st;
+}

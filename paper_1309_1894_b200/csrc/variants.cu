@@ -1,0 +1,303 @@
+// Variant descriptors, eligibility, format management and launch dispatch.
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <mutex>
+
+#include "handle.h"
+
+namespace spmv {
+
+// ------------------------------------------------------------------ error text
+static thread_local char g_err[512] = "";
+void set_last_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+const char* last_error_text() { return g_err; }
+
+// ------------------------------------------------------------------ allocator
+void* Allocator::alloc(size_t bytes, cudaStream_t s) {
+  if (bytes == 0) bytes = 8;
+  void* p = nullptr;
+  if (has_cb) {
+    p = cb.alloc(bytes, (void*)s, cb.ctx);
+  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    p = nullptr;
+  }
+  if (p) owned += (int64_t)bytes;
+  else set_last_error("device allocation of %zu bytes failed", bytes);
+  return p;
+}
+void Allocator::free(void* p, size_t bytes) {
+  if (!p) return;
+  if (bytes == 0) bytes = 8;
+  if (has_cb) cb.free(p, cb.ctx);
+  else cudaFree(p);
+  owned -= (int64_t)bytes;
+}
+
+// ------------------------------------------------------------------ descriptors
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3"};
+
+Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
+
+std::string variant_to_string(const Variant& v) {
+  char buf[160];
+  int n = snprintf(buf, sizeof(buf), "%s:b%d", kFamName[v.fam], v.block);
+  auto add = [&](const char* k, int val) { n += snprintf(buf + n, sizeof(buf) - n, ":%s%d", k, val); };
+  switch (v.fam) {
+    case FAM_CSR_SCALAR: add("r", v.R); add("u", v.U); break;
+    case FAM_CSR_VECTOR: add("w", v.W); add("u", v.U); break;
+    case FAM_SELL: add("c", v.C); add("s", v.S); add("r", v.R); add("u", v.U); break;
+    case FAM_ELL: add("r", v.R); add("u", v.U); break;
+    case FAM_MERGE: add("i", v.I); break;
+    case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
+  }
+  add("x", v.X);
+  if (v.grid > 0) add("g", v.grid);
+  if (v.carve >= 0) add("co", v.carve);
+  return std::string(buf);
+}
+
+bool variant_from_string(const char* s, Variant* out) {
+  if (!s) return false;
+  Variant v;
+  if (!strcmp(s, "default")) { *out = v; return true; }
+  char tmp[160];
+  strncpy(tmp, s, sizeof(tmp) - 1);
+  tmp[sizeof(tmp) - 1] = 0;
+  char* save = nullptr;
+  char* tok = strtok_r(tmp, ":", &save);
+  if (!tok) return false;
+  int fam = -1;
+  for (int f = 0; f < FAM_COUNT; ++f)
+    if (!strcmp(tok, kFamName[f])) fam = f;
+  if (fam < 0) return false;
+  v.fam = fam;
+  if (fam == FAM_MERGE) v.I = 7;
+  if (fam == FAM_SELL) { v.C = 128; v.S = 1; }
+  if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
+  while ((tok = strtok_r(nullptr, ":", &save))) {
+    char* end = nullptr;
+    if (!strncmp(tok, "co", 2)) { v.carve = (int)strtol(tok + 2, &end, 10); }
+    else {
+      const int val = (int)strtol(tok + 1, &end, 10);
+      switch (tok[0]) {
+        case 'b': v.block = val; break;
+        case 'g': v.grid = val; break;
+        case 'u': v.U = val; break;
+        case 'r': v.R = val; break;
+        case 'w': v.W = val; break;
+        case 'x': v.X = val; break;
+        case 'c': v.C = val; break;
+        case 's': v.S = val; break;
+        case 'i': v.I = val; break;
+        default: return false;
+      }
+    }
+    if (!end || *end != 0) return false;
+  }
+  *out = v;
+  return true;
+}
+
+static bool template_supported(const Variant& v) {
+  switch (v.fam) {
+    case FAM_CSR_SCALAR: return csr_scalar_supported(v);
+    case FAM_CSR_VECTOR: return csr_vector_supported(v);
+    case FAM_SELL:
+    case FAM_ELL: return sell_supported(v);
+    case FAM_MERGE: return merge_supported(v);
+    case FAM_BCSR3: return bcsr_supported(v);
+  }
+  return false;
+}
+
+bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why) {
+  auto no = [&](const char* m) { if (why) *why = m; return false; };
+  if (v.grid < 0 || v.grid > 64 || v.carve < -1 || v.carve > 100) return no("bad grid/carve-out");
+  if (!template_supported(v)) return no("no such template instantiation");
+  const spmv_info_t& in = h->info;
+  if (v.fam == FAM_ELL) {
+    // eligibility rule of SURVEY 8(a) a3: width*rows <= 1.5*nnz
+    if ((double)in.max_row_len * (double)in.rows > 1.5 * (double)in.nnz + 1024.0) return no("ELL padding > 1.5x");
+  }
+  if (v.fam == FAM_BCSR3) {
+    if (in.rows % 3 || in.cols % 3 || in.rows == 0) return no("rows/cols not multiples of 3");
+    if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
+    if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
+  }
+  if (v.fam == FAM_SELL || v.fam == FAM_ELL || v.fam == FAM_MERGE) {
+    if (in.rows + in.nnz > 0x7ffffff0ll) return no("rows+nnz over int32");
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------ formats
+spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) {
+  switch (v.fam) {
+    case FAM_SELL: {
+      auto key = std::make_pair(v.C, v.S);
+      if (h->sells.count(key)) return SPMV_OK;
+      SellFormat f;
+      spmv_status_t st = build_sell(h->A, v.C, v.S, false, h->al, s, &f);
+      if (st != SPMV_OK) return st;
+      if ((double)f.padded > 2.0 * (double)h->A.nnz + 65536.0) {   // too padded to be a candidate
+        free_sell(f, h->al);
+        set_last_error("SELL c%d s%d: padding over 2x nnz", v.C, v.S);
+        return SPMV_ERR_UNSUPPORTED;
+      }
+      h->sells[key] = f;
+      return SPMV_OK;
+    }
+    case FAM_ELL: {
+      if (h->has_ell) return SPMV_OK;
+      spmv_status_t st = build_sell(h->A, 0, 1, true, h->al, s, &h->ell);
+      if (st == SPMV_OK) h->has_ell = true;
+      return st;
+    }
+    case FAM_BCSR3: {
+      if (h->has_bcsr) return SPMV_OK;
+      spmv_status_t st = build_bcsr3(h->A, h->al, s, &h->bcsr);
+      if (st == SPMV_OK) h->has_bcsr = true;
+      return st;
+    }
+    case FAM_MERGE: {
+      const int ti = v.block * v.I;
+      if (h->plans.count(ti)) return SPMV_OK;
+      MergePlan p;
+      spmv_status_t st = build_merge_plan(h->A, ti, h->al, s, &p);
+      if (st != SPMV_OK) return st;
+      SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+      h->plans[ti] = p;
+      return SPMV_OK;
+    }
+    default: return SPMV_OK;
+  }
+}
+
+void release_formats_except(spmv_handle_s* h, const Variant& keep) {
+  for (auto it = h->sells.begin(); it != h->sells.end();) {
+    if (keep.fam == FAM_SELL && it->first == std::make_pair(keep.C, keep.S)) { ++it; continue; }
+    free_sell(it->second, h->al);
+    it = h->sells.erase(it);
+  }
+  if (h->has_ell && keep.fam != FAM_ELL) { free_sell(h->ell, h->al); h->has_ell = false; }
+  if (h->has_bcsr && keep.fam != FAM_BCSR3) { free_bcsr3(h->bcsr, h->al); h->has_bcsr = false; }
+  for (auto it = h->plans.begin(); it != h->plans.end();) {
+    if (keep.fam == FAM_MERGE && it->first == keep.block * keep.I) { ++it; continue; }
+    free_merge_plan(it->second, h->al);
+    it = h->plans.erase(it);
+  }
+}
+
+void release_all_formats(spmv_handle_s* h) {
+  Variant none;   // csr_scalar keeps nothing
+  release_formats_except(h, none);
+}
+
+int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
+  const CsrView& A = h->A;
+  const int64_t csr = A.nnz * 12 + (A.rows + 1) * 4;
+  switch (v.fam) {
+    case FAM_SELL: {
+      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      if (it == h->sells.end()) return 0;
+      const SellFormat& f = it->second;
+      return f.padded * 12 + (f.nslices + 1) * 8 + (f.perm ? f.nslices * (int64_t)f.C * 4 : 0);
+    }
+    case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
+    case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
+    case FAM_MERGE: {
+      auto it = h->plans.find(v.block * v.I);
+      return csr + (it == h->plans.end() ? 0 : it->second.ntiles * 16 + 4);
+    }
+    default: return csr;
+  }
+}
+
+// ------------------------------------------------------------------ launch
+static std::mutex g_attr_mu;
+static std::map<const void*, int> g_carve;                          // current carve-out per kernel
+static std::map<std::pair<const void*, int>, int> g_occ;            // resident blocks per SM
+
+static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
+  switch (v.fam) {
+    case FAM_CSR_SCALAR: return csr_scalar_func(v);
+    case FAM_CSR_VECTOR: return csr_vector_func(v);
+    case FAM_SELL: {
+      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      return sell_func(v, it != h->sells.end() && it->second.perm != nullptr);
+    }
+    case FAM_ELL: return sell_func(v, false);
+    case FAM_MERGE: return merge_func(v);
+    case FAM_BCSR3: return bcsr_func(v);
+  }
+  return nullptr;
+}
+
+spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs& a) {
+  const void* fn = variant_func(h, v);
+  if (!fn) { set_last_error("variant %s has no kernel", variant_to_string(v).c_str()); return SPMV_ERR_INTERNAL; }
+  int grid_blocks = 0;
+  {
+    std::lock_guard<std::mutex> lk(g_attr_mu);
+    auto ci = g_carve.find(fn);
+    const int cur = ci == g_carve.end() ? -1 : ci->second;
+    if (cur != v.carve) {   // PAPER.md:23 "size of L1 cache" -> shared-memory carve-out hint
+      SPMV_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve));
+      g_carve[fn] = v.carve;
+    }
+    if (v.grid > 0 && v.fam != FAM_MERGE) {
+      auto key = std::make_pair(fn, v.block);
+      auto oi = g_occ.find(key);
+      int occ = 0;
+      if (oi == g_occ.end()) {
+        SPMV_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, v.block, 0));
+        if (occ < 1) occ = 1;
+        g_occ[key] = occ;
+      } else {
+        occ = oi->second;
+      }
+      grid_blocks = v.grid * h->dev.sm_count * occ;
+    }
+  }
+  cudaError_t e = cudaSuccess;
+  switch (v.fam) {
+    case FAM_CSR_SCALAR: e = csr_scalar_launch(v, h->A, a, grid_blocks); break;
+    case FAM_CSR_VECTOR: e = csr_vector_launch(v, h->A, a, grid_blocks); break;
+    case FAM_SELL: {
+      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
+      e = sell_launch(v, h->A.rows, it->second, a, grid_blocks);
+      break;
+    }
+    case FAM_ELL:
+      if (!h->has_ell) return SPMV_ERR_INTERNAL;
+      e = sell_launch(v, h->A.rows, h->ell, a, grid_blocks);
+      break;
+    case FAM_MERGE: {
+      auto it = h->plans.find(v.block * v.I);
+      if (it == h->plans.end()) return SPMV_ERR_INTERNAL;
+      e = merge_launch(v, h->A, it->second, a);
+      break;
+    }
+    case FAM_BCSR3:
+      if (!h->has_bcsr) return SPMV_ERR_INTERNAL;
+      e = bcsr_launch(v, h->bcsr, a, grid_blocks);
+      break;
+  }
+  if (e != cudaSuccess) {
+    set_last_error("launch of %s failed: %s", variant_to_string(v).c_str(), cudaGetErrorString(e));
+    return SPMV_ERR_CUDA;
+  }
+  return SPMV_OK;
+}
+
+}  // namespace spmv

@@ -1,0 +1,64 @@
+"""CPU-side checks of the boundary: the shared library builds, loads and exports every symbol
+include/spmv_b200.h declares; error paths that need no GPU return codes, never abort."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_1309_1894_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    build.build()
+    return binding.lib()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "spmv_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(spmv_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    names = _declared_symbols()
+    assert len(names) >= 16
+    for n in names:
+        assert hasattr(L, n), n
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_status_strings_and_version(L):
+    assert L.spmv_status_string(0) == b"SPMV_OK"
+    assert L.spmv_status_string(6) == b"SPMV_ERR_VERIFY_FAILED"
+    assert L.spmv_status_string(99) == b"SPMV_ERR_UNKNOWN"
+    assert binding.version() == "0.1.0"
+
+
+def test_null_and_bad_arguments_return_codes(L):
+    h = ctypes.c_void_p(0)
+    # NULL out pointer / negative sizes / NULL row_ptr
+    assert L.spmv_create(None, 1, 1, 0, ctypes.c_void_p(8), None, None, None, None) == 1
+    assert L.spmv_create(ctypes.byref(h), -1, 1, 0, ctypes.c_void_p(8), None, None, None, None) == 1
+    assert L.spmv_create(ctypes.byref(h), 1, 1, 0, None, None, None, None, None) == 1
+    assert L.spmv_create(ctypes.byref(h), 1, 1, 5, ctypes.c_void_p(8), None, None, None, None) == 1
+    # over the int32 limits
+    assert L.spmv_create(ctypes.byref(h), 1 << 31, 1, 0, ctypes.c_void_p(8), None, None, None, None) == 3
+    assert h.value is None
+    # NULL / never-created handles
+    assert L.spmv_destroy(None) == 1
+    assert L.spmv_destroy(ctypes.c_void_p(0x1234)) == 1
+    assert L.spmv_apply(None, 1.0, None, 0.0, None, None) == 1
+    assert L.spmv_tune(None, None, None) == 1
+    assert L.spmv_select(None, b"default", None) == 1
+    assert L.spmv_get_info(None, None) == 1
+    L.spmv_clear_cache()
+
+
+def test_struct_sizes_match_header():
+    # guards the ctypes mirrors against drift from include/spmv_b200.h (x86-64 layout)
+    assert ctypes.sizeof(binding.Info) == 3 * 8 + 2 * 4 + 2 * 8 + 32 * 8 + 8 + 2 * 4 + 8 + 2 * 8 + 2 * 4 + 3 * 8 + 128 + 64
+    assert ctypes.sizeof(binding.Allocator) == 24

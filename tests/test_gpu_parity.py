@@ -1,0 +1,142 @@
+"""GPU parity: every kernel family / template axis against the oracle, element by element,
+through the C ABI.  Floating point: |y - y_ref| <= 1e-12 * scale
+(north_star); exactness cases (x = e_j, small integers, val = x = 1) bitwise."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1309_1894_b200 import binding
+from paper_1309_1894_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+ZOO = H.zoo()
+
+
+def _select_or_skip(S, desc):
+    try:
+        S.select(desc)
+        return True
+    except binding.SpmvError as e:
+        assert e.status == 3, e          # only SPMV_ERR_UNSUPPORTED may refuse a parsable variant
+        return False
+
+
+@pytest.mark.parametrize("name,A", ZOO, ids=[z[0] for z in ZOO])
+def test_zoo_all_representative_variants(cuda, name, A):
+    S = binding.SpMV.from_csr(A)
+    x = W.uniform(70, A.cols)
+    y0 = W.uniform(71, A.rows)
+    ran = 0
+    for desc in H.REPRESENTATIVE_VARIANTS:
+        if not _select_or_skip(S, desc):
+            continue
+        ran += 1
+        for alpha, beta in ((1.0, 0.0), (1.0, 0.5), (-2.5, 1.0)):
+            H.check_against_oracle(S, A, alpha, x, beta, None if beta == 0.0 else y0, what=name)
+    assert ran >= 10          # CSR and merge families are always eligible
+    S.close()
+
+
+@pytest.mark.parametrize("name,A", [z for z in ZOO if z[0] in ("lap3d_11", "fem_5", "powerlaw_3k", "lengths_ladder")],
+                         ids=["lap3d_11", "fem_5", "powerlaw_3k", "lengths_ladder"])
+def test_every_enumerated_candidate(cuda, name, A):
+    """Everything the tuner would enumerate for this matrix passes parity."""
+    S = binding.SpMV.from_csr(A)
+    x = W.uniform(72, A.cols)
+    y0 = W.uniform(73, A.rows)
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x, 0.5, y0)
+    cands = S.variants()
+    assert len(cands) > 50
+    fams = {c.split(":")[0] for c in cands}
+    assert {"csr_scalar", "csr_vector", "merge"} <= fams
+    for desc in cands:
+        if not _select_or_skip(S, desc):
+            continue
+        y = H.gpu_apply(S, 1.0, x, 0.5, y0)
+        ok, mr, ff, nf = oracle.accept(y, y_ref, scale, H.TOL)
+        assert ok, (desc, nf, ff, mr)
+    S.close()
+
+
+def test_exactness_cases_bitwise(cuda):
+    """P5/P6/P7 for every family: x = e_j, small integers, val = x = 1 are exact in any order."""
+    lengths = np.random.default_rng(3).integers(0, 90, 1200)
+    lengths[5] = 3000
+    A = W.csr_from_lengths(lengths, 6000, 31, values="smallint")
+    xi = np.round(W.uniform(32, A.cols) * 8)
+    yi = np.round(W.uniform(33, A.rows) * 8)
+    B = W.fem_block27(4)
+    B.val[:] = np.round(B.val * 2)
+    xb = np.round(W.uniform(34, B.cols) * 8)
+    for M, x, y0 in ((A, xi, yi), (B, xb, np.round(W.uniform(35, B.rows) * 8))):
+        S = binding.SpMV.from_csr(M)
+        y_ref, _ = oracle.spmv(M.row_ptr, M.col_idx, M.val, 3.0, x, -2.0, y0)
+        e = np.zeros(M.cols); e[M.cols // 3] = 1.0
+        ye_ref, _ = oracle.spmv(M.row_ptr, M.col_idx, M.val, 2.0, e, 0.0)
+        ones_ref = M.row_lengths().astype(np.float64)
+        Mones = W.CSR(M.rows, M.cols, M.row_ptr, M.col_idx, np.ones(M.nnz))
+        S1 = binding.SpMV.from_csr(Mones)
+        for desc in H.REPRESENTATIVE_VARIANTS:
+            if not _select_or_skip(S, desc):
+                continue
+            assert np.array_equal(H.gpu_apply(S, 3.0, x, -2.0, y0), y_ref), desc
+            assert np.array_equal(H.gpu_apply(S, 2.0, e, 0.0, None), ye_ref), desc
+            S1.select(desc)
+            assert np.array_equal(H.gpu_apply(S1, 1.0, np.ones(M.cols), 0.0, None), ones_ref), desc
+        S.close(); S1.close()
+
+
+def test_nonfinite_x_touches_only_real_entries(cuda):
+    """A7: padding (SELL/ELL) is never multiplied, so NaN/Inf in x reaches exactly the rows
+    CSR semantics say; beta = 0 ignores NaN in incoming y (A1); alpha = 0 ignores A and x (A2)."""
+    A = W.csr_from_lengths(np.random.default_rng(4).integers(1, 12, 2000), 2000, 41)
+    x = W.uniform(42, A.cols)
+    x[17] = np.nan
+    x[900] = np.inf
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x, 0.0)
+    assert np.isfinite(y_ref).sum() > 1000 and (~np.isfinite(y_ref)).sum() > 0
+    S = binding.SpMV.from_csr(A)
+    for desc in H.REPRESENTATIVE_VARIANTS:
+        if not _select_or_skip(S, desc):
+            continue
+        y = H.gpu_apply(S, 1.0, x, 0.0, None)          # incoming y is NaN-filled
+        assert oracle.accept(y, y_ref, scale, H.TOL)[0], desc
+        y0 = W.uniform(43, A.rows)
+        y = H.gpu_apply(S, 0.0, x, 1.0, y0)
+        assert np.array_equal(y, y0), desc
+        y = H.gpu_apply(S, 0.0, x, 0.0, None)
+        assert np.array_equal(y, np.zeros(A.rows)), desc
+    S.close()
+
+
+def test_bit_identical_across_repeated_runs(cuda):
+    """north_star: 'the selected variant must give bit-identical results across repeated runs'."""
+    A = W.powerlaw(20000, lmax=5000)
+    x = W.uniform(44, A.cols)
+    y0 = W.uniform(45, A.rows)
+    S = binding.SpMV.from_csr(A)
+    for desc in H.REPRESENTATIVE_VARIANTS:
+        if not _select_or_skip(S, desc):
+            continue
+        first = H.gpu_apply(S, 1.5, x, 0.5, y0)
+        for _ in range(9):
+            assert np.array_equal(H.gpu_apply(S, 1.5, x, 0.5, y0), first), desc
+    S.close()
+
+
+def test_apply_host_matches_device_apply(cuda):
+    import torch
+    prob = W.config(2, 0.25)
+    A = prob.A
+    S = binding.SpMV.from_csr(A)
+    S.select("sell:b256:c128:s1:r2:u4:x0")
+    y_dev = H.gpu_apply(S, prob.alpha, prob.x, prob.beta, prob.y0)
+    xh = torch.from_numpy(prob.x).pin_memory()
+    yh = torch.from_numpy(prob.y0.copy()).pin_memory()
+    S.apply_host(prob.alpha, xh, prob.beta, yh)
+    assert np.array_equal(yh.numpy(), y_dev)
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, prob.alpha, prob.x, prob.beta, prob.y0)
+    assert oracle.accept(yh.numpy(), y_ref, scale, H.TOL)[0]
+    S.close()
