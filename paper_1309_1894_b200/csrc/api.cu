@@ -216,7 +216,7 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
   const void* src = nullptr;
   size_t n = 0;
   const SellFormat* sf = nullptr;
-  if (v.fam == FAM_SELL) {
+  if (v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) {
     auto it = h->sells.find(std::make_pair(v.C, v.S));
     if (it != h->sells.end()) sf = &it->second;
   } else if (v.fam == FAM_ELL && h->has_ell) {

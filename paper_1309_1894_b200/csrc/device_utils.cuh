@@ -42,6 +42,11 @@ __device__ __forceinline__ int4 ld_stream4(const int* p) {         // 16-byte al
   return v;
 }
 
+// Compiler-level fence: keeps the phases of an unrolled trip (all matrix loads | all x
+// gathers | all FMAs) in that order in the generated code.  Warps issue in order, so a
+// dependent use placed between two loads would delay every load behind it.
+__device__ __forceinline__ void phase_fence() { asm volatile("" ::: "memory"); }
+
 // BLAS-style epilogue (reading A1): y is not read when beta == 0.
 __device__ __forceinline__ void store_y(double* __restrict__ y, int64_t i, double alpha, double s, double beta) {
   y[i] = (beta == 0.0) ? alpha * s : fma(alpha, s, beta * y[i]);

@@ -40,8 +40,11 @@ struct VecLoad<4> {
   }
 };
 
+// heavier instantiations trade occupancy for registers (loads in flight per thread)
+constexpr int sell_max_block(int R, int U) { return R * U >= 16 ? 256 : 512; }
+
 template <int R, int U, int PERM, int X>
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(sell_max_block(R, U))
 sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
             const int64_t* __restrict__ slice_ptr, const double* __restrict__ sval,
             const int* __restrict__ scol, const int* __restrict__ perm, double alpha,
@@ -58,42 +61,53 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
     double acc[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0;
-    int j = 0;
-    for (; j + U <= w; j += U) {
+    // destination rows and (beta != 0) the old y values are fetched up front so that their
+    // latency overlaps the matrix stream instead of trailing it
+    int64_t orow[R];
+    double yold[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int64_t row = r0 + r;
+      if (PERM) orow[r] = __ldg(perm + row);
+      else orow[r] = row < rows ? row : -1;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && orow[r] >= 0) ? y[orow[r]] : 0.0;
+    // U steps per trip, every load of the trip issued before the first use; steps beyond
+    // the slice width are predicated off (warp-uniform), so U >= w streams a short row in
+    // one batch
+    for (int j = 0; j < w; j += U) {
       double v[U][R];
       int c[U][R];
 #pragma unroll
+      for (int u = 0; u < U; ++u) {
+        // steps past the slice width re-read the last valid step (in bounds, L2-resident) and
+        // are masked afterwards: unconditional loads let the compiler batch all U of them
+        const int jj = min(j + u, w - 1);
+        VecLoad<R>::load(pv + (int64_t)jj * C, pc + (int64_t)jj * C, v[u], c[u]);
+      }
+#pragma unroll
       for (int u = 0; u < U; ++u)
-        VecLoad<R>::load(pv + (int64_t)(j + u) * C, pc + (int64_t)(j + u) * C, v[u], c[u]);
+        if (j + u >= w) {
+#pragma unroll
+          for (int r = 0; r < R; ++r) c[u][r] = -1;
+        }
+      phase_fence();
       double xv[U][R];
 #pragma unroll
       for (int u = 0; u < U; ++u)
 #pragma unroll
-        for (int r = 0; r < R; ++r) xv[u][r] = c[u][r] >= 0 ? ldx<X>(x, c[u][r]) : 0.0;
+        for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, max(c[u][r], 0));   // padding reads x[0], masked below
+      phase_fence();
 #pragma unroll
       for (int u = 0; u < U; ++u)
 #pragma unroll
         for (int r = 0; r < R; ++r)
-          if (c[u][r] >= 0) acc[r] = fma(v[u][r], xv[u][r], acc[r]);
-    }
-    for (; j < w; ++j) {
-      double v[R];
-      int c[R];
-      VecLoad<R>::load(pv + (int64_t)j * C, pc + (int64_t)j * C, v, c);
-#pragma unroll
-      for (int r = 0; r < R; ++r)
-        if (c[r] >= 0) acc[r] = fma(v[r], ldx<X>(x, c[r]), acc[r]);
+          acc[r] = c[u][r] >= 0 ? fma(v[u][r], xv[u][r], acc[r]) : acc[r];
     }
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      int64_t row = r0 + r;
-      if (PERM) {
-        int o = __ldg(perm + row);
-        if (o >= 0) store_y(y, o, alpha, acc[r], beta);
-      } else if (row < rows) {
-        store_y(y, row, alpha, acc[r], beta);
-      }
-    }
+    for (int r = 0; r < R; ++r)
+      if (orow[r] >= 0) y[orow[r]] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
   }
 }
 
@@ -103,7 +117,7 @@ typedef void (*sell_kernel_t)(int64_t, int64_t, int, int, const int64_t*, const 
 template <int PERM, int X>
 static sell_kernel_t pick_ru(int R, int U) {
 #define P(r, u) if (R == r && U == u) return sell_kernel<r, u, PERM, X>;
-  P(1, 1) P(1, 2) P(1, 4) P(1, 8) P(2, 1) P(2, 2) P(2, 4) P(2, 8) P(4, 1) P(4, 2) P(4, 4)
+  P(1, 1) P(1, 2) P(1, 4) P(1, 8) P(2, 1) P(2, 2) P(2, 4) P(2, 8) P(4, 1) P(4, 2) P(4, 4) P(4, 8)
 #undef P
   return nullptr;
 }
@@ -114,8 +128,8 @@ static sell_kernel_t pick(const Variant& v, bool perm) {
 }
 
 bool sell_supported(const Variant& v) {
-  if (v.block < 32 || v.block > 1024 || v.block % 32) return false;
   if (pick(v, false) == nullptr) return false;
+  if (v.block < 32 || v.block > sell_max_block(v.R, v.U) || v.block % 32) return false;
   if (v.fam == FAM_SELL) {
     if (v.C < 128 || v.C > 4096 || (v.C & (v.C - 1))) return false;   // power of two, multiple of 32*Rmax
     if (v.S < 1) return false;

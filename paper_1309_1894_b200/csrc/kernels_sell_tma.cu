@@ -1,0 +1,225 @@
+// SELL-C-sigma with the matrix stream moved by the TMA engine (sm_100a):
+// cp.async.bulk (1-D bulk copy, SASS UBLKCP) + mbarrier producer/consumer ring.
+//
+// Why: SpMV on short rows is latency-bound when the bytes in flight depend on how many
+// loads each warp has issued (warps issue in order and ptxas sinks loads next to their
+// uses).  A slice of the SELL format is one contiguous run of values and one of column
+// indices, so ONE elected producer thread can keep STAGES x (J*C*12) bytes per CTA in
+// flight with two bulk copies per stage, independent of what the consumer warps do.
+// Consumers read values/indices from shared memory (conflict-free: consecutive threads,
+// consecutive addresses), gather x through L1 and accumulate in registers.
+//
+// Layout and padding semantics are those of kernels_sell.cu (same SellFormat).
+// Work split: CTA b owns slices b, b+gridDim, ...; a slice wider than J steps is streamed
+// as ceil(w/J) stages.  Deterministic: each row is summed by one thread in stored order.
+#include "device_utils.cuh"
+#include "spmv_internal.h"
+
+namespace spmv {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+template <int R>
+struct SmemVec;
+template <>
+struct SmemVec<1> {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) { v[0] = *pv; c[0] = *pc; }
+};
+template <>
+struct SmemVec<2> {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+    double2 a = *reinterpret_cast<const double2*>(pv);
+    int2 b = *reinterpret_cast<const int2*>(pc);
+    v[0] = a.x; v[1] = a.y; c[0] = b.x; c[1] = b.y;
+  }
+};
+
+// blockDim.x = C/R consumer threads + 32 (warp C/R/32 is the producer warp)
+template <int R, int STAGES, int J, int PERM, int X>
+__global__ void __launch_bounds__(512 + 32)
+sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict__ slice_ptr,
+                const double* __restrict__ sval, const int* __restrict__ scol, const int* __restrict__ perm,
+                double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int nconsumers = C / R;
+  const size_t val_bytes = (size_t)J * C * sizeof(double);
+  const size_t col_bytes = (size_t)J * C * sizeof(int);
+  double* s_val = reinterpret_cast<double*>(smem_raw);                       // [STAGES][J*C]
+  int* s_col = reinterpret_cast<int*>(smem_raw + STAGES * val_bytes);        // [STAGES][J*C]
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * (val_bytes + col_bytes));
+  uint64_t* empty = full + STAGES;
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], nconsumers / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (tid >= nconsumers) {
+    // ---------------- producer warp: one elected lane streams the slices
+    if (tid == nconsumers) {
+      uint32_t stage = 0, phase = 0;
+      for (int64_t s = blockIdx.x; s < nslices; s += gridDim.x) {
+        const int64_t base = __ldg(slice_ptr + s);
+        const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
+        for (int j0 = 0; j0 < w; j0 += J) {
+          const int nj = min(J, w - j0);
+          mbar_wait(&empty[stage], phase ^ 1);
+          const uint32_t vb = (uint32_t)nj * C * sizeof(double), cb = (uint32_t)nj * C * sizeof(int);
+          mbar_expect_tx(&full[stage], vb + cb);
+          bulk_g2s(s_val + (size_t)stage * J * C, sval + base + (int64_t)j0 * C, vb, &full[stage]);
+          bulk_g2s(s_col + (size_t)stage * J * C, scol + base + (int64_t)j0 * C, cb, &full[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+    return;
+  }
+
+  // ---------------- consumers: thread t owns rows [t*R, t*R+R) of the current slice
+  uint32_t stage = 0, phase = 0;
+  const int lane = tid & 31;
+  for (int64_t s = blockIdx.x; s < nslices; s += gridDim.x) {
+    const int64_t base = __ldg(slice_ptr + s);
+    const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
+    const int64_t r0 = s * C + (int64_t)tid * R;
+    int64_t orow[R];
+    double yold[R], acc[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int64_t row = r0 + r;
+      if (PERM) orow[r] = __ldg(perm + row);
+      else orow[r] = row < rows ? row : -1;
+      acc[r] = 0.0;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && orow[r] >= 0) ? y[orow[r]] : 0.0;
+    for (int j0 = 0; j0 < w; j0 += J) {
+      const int nj = min(J, w - j0);
+      mbar_wait(&full[stage], phase);
+      const double* pv = s_val + (size_t)stage * J * C + tid * R;
+      const int* pc = s_col + (size_t)stage * J * C + tid * R;
+      {
+        double v[J][R];
+        int c[J][R];
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          SmemVec<R>::load(pv + j * C, pc + j * C, v[j], c[j]);
+          if (j >= nj) {          // beyond this stage's steps: stale shared memory, masked off
+#pragma unroll
+            for (int r = 0; r < R; ++r) c[j][r] = -1;
+          }
+        }
+        double xv[J][R];
+#pragma unroll
+        for (int j = 0; j < J; ++j)
+#pragma unroll
+          for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, max(c[j][r], 0));
+#pragma unroll
+        for (int j = 0; j < J; ++j)
+#pragma unroll
+          for (int r = 0; r < R; ++r) acc[r] = c[j][r] >= 0 ? fma(v[j][r], xv[j][r], acc[r]) : acc[r];
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[stage]);     // this warp is done with the stage
+      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if (orow[r] >= 0) y[orow[r]] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  }
+}
+
+typedef void (*sell_tma_kernel_t)(int64_t, int64_t, int, const int64_t*, const double*, const int*, const int*,
+                                  double, const double*, double, double*);
+
+struct TmaEntry { int R, STAGES, J, X; sell_tma_kernel_t k[2]; };
+#define TE(r, st, j) {r, st, j, 0, {sell_tma_kernel<r, st, j, 0, 0>, sell_tma_kernel<r, st, j, 1, 0>}}
+static const TmaEntry g_tma[] = {TE(1, 2, 8), TE(1, 3, 8), TE(1, 4, 8), TE(1, 3, 4), TE(1, 4, 4), TE(1, 6, 4),
+                                 TE(2, 2, 8), TE(2, 3, 8), TE(2, 4, 8), TE(2, 3, 4), TE(2, 4, 4), TE(2, 6, 4),
+                                 TE(1, 3, 16), TE(2, 3, 16), TE(1, 2, 16), TE(2, 2, 16)};
+#undef TE
+
+static const TmaEntry* tma_pick(const Variant& v) {
+  for (const auto& e : g_tma)
+    if (e.R == v.R && e.STAGES == v.I && e.J == v.U && e.X == v.X) return &e;
+  return nullptr;
+}
+static size_t tma_smem(const Variant& v) { return (size_t)v.I * v.U * v.C * 12 + 2 * v.I * 8 + 128; }
+
+bool sell_tma_supported(const Variant& v) {
+  if (!tma_pick(v)) return false;
+  if (v.C < 128 || v.C > 1024 || (v.C & (v.C - 1))) return false;
+  if (v.S < 1 || (v.S > 1 && (v.S % v.C != 0 || v.S > 8192 || (v.S & (v.S - 1))))) return false;
+  const int consumers = v.C / v.R;
+  if (consumers < 32 || consumers > 512 || v.block != consumers + 32) return false;
+  return tma_smem(v) <= 200 * 1024;
+}
+const void* sell_tma_func(const Variant& v, bool perm) {
+  const TmaEntry* e = tma_pick(v);
+  return e ? (const void*)e->k[perm ? 1 : 0] : nullptr;
+}
+
+cudaError_t sell_tma_launch(const Variant& v, int64_t rows, const SellFormat& f, const ApplyArgs& a, int sm_count) {
+  const TmaEntry* e = tma_pick(v);
+  if (!e || f.C != v.C) return cudaErrorInvalidValue;
+  if (rows == 0) return cudaSuccess;
+  sell_tma_kernel_t k = e->k[f.perm ? 1 : 0];
+  const size_t smem = tma_smem(v);
+  static thread_local const void* last_attr = nullptr;
+  static thread_local size_t last_smem = 0;
+  if (last_attr != (const void*)k || last_smem != smem) {
+    cudaError_t err = cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    last_attr = (const void*)k;
+    last_smem = smem;
+  }
+  static thread_local int occ = 1;
+  static thread_local const void* occ_k = nullptr;
+  static thread_local size_t occ_smem = 0;
+  if (occ_k != (const void*)k || occ_smem != smem) {
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)k, v.block, smem);
+    if (err != cudaSuccess) return err;
+    if (occ < 1) occ = 1;
+    occ_k = (const void*)k;
+    occ_smem = smem;
+  }
+  // persistent: g (default 1) waves of resident CTAs, never more CTAs than slices
+  int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;
+  if (grid > f.nslices) grid = f.nslices;
+  k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, f.nslices, f.C, f.slice_ptr, f.val, f.col, f.perm, a.alpha,
+                                                 a.x, a.beta, a.y);
+  return cudaGetLastError();
+}
+
+}  // namespace spmv

@@ -56,20 +56,20 @@ struct MergePlan {
 };
 
 // ---------------------------------------------------------------- variants
-enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_COUNT };
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_COUNT };
 
 struct Variant {
   int fam = FAM_CSR_SCALAR;
   int block = 256;   // b: threads per block                       (PAPER.md:23 knob 1)
   int grid = 0;      // g: 0 exact cover, k>0: k * SMs * resident blocks, grid-stride (knob 2)
   int carve = -1;    // co: shared-memory carve-out percent, -1 default         (knob 4)
-  int U = 1;         // u: unroll factor                                         (knob 5)
+  int U = 1;         // u: unroll factor (sell_tma: steps per stage)             (knob 5)
   int R = 1;         // r: rows per thread (csr_scalar, sell)
   int W = 1;         // w: lanes per row (csr_vector), lanes per block row (bcsr3)
   int X = 0;         // x: 0 read-only path (ld.global.nc), 1 plain ld.global
   int C = 0;         // c: SELL slice height
   int S = 1;         // s: SELL sorting window sigma
-  int I = 0;         // i: merge-path items per thread
+  int I = 0;         // i: merge-path items per thread (sell_tma: pipeline stages)
 };
 
 std::string variant_to_string(const Variant& v);
@@ -102,6 +102,10 @@ cudaError_t csr_vector_launch(const Variant&, const CsrView&, const ApplyArgs&, 
 bool sell_supported(const Variant&);
 const void* sell_func(const Variant&, bool perm);
 cudaError_t sell_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int grid_blocks);
+
+bool sell_tma_supported(const Variant&);
+const void* sell_tma_func(const Variant&, bool perm);
+cudaError_t sell_tma_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int sm_count);
 
 bool merge_supported(const Variant&);
 const void* merge_func(const Variant&);

@@ -77,9 +77,16 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
       Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; all.push_back(v);
     }
   }
+  for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
+    Variant v; v.fam = FAM_SELL_TMA; v.C = C; v.S = S; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;
+    if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
+    if (S == 1 && in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0) { ++*n_pruned; continue; }
+    all.push_back(v);
+  }
   // family, then format key, outermost: formats are then built once per key
   std::stable_sort(all.begin(), all.end(), [](const Variant& a, const Variant& b) {
-    if (a.fam != b.fam) return a.fam < b.fam;
+    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : v.fam; };
+    if (grp(a) != grp(b)) return grp(a) < grp(b);
     if (a.C != b.C) return a.C < b.C;
     return a.S < b.S;
   });
@@ -356,7 +363,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!budget_left()) break;
     if (variant_to_string(v) == variant_to_string(dflt)) continue;
     // keep device memory bounded: drop formats when the family / format key changes
-    if (v.fam != last_fmt.fam || v.C != last_fmt.C || v.S != last_fmt.S) {
+    if ((v.fam != last_fmt.fam && !(v.C == last_fmt.C && v.C > 0)) || v.C != last_fmt.C || v.S != last_fmt.S) {
       Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
       release_formats_except(h, keep);
       last_fmt = v;
@@ -375,6 +382,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     for (int g : {0, 1, 2, 4, 8}) for (int co : carves) {
       if (g == 0 && co == -1) continue;
       if (L.fam == FAM_MERGE && g != 0) continue;
+      if (L.fam == FAM_SELL_TMA && (g == 0 || g == 8)) continue;   // persistent: g = waves of resident CTAs
       if (!budget_left()) break;
       Variant v = L; v.grid = g; v.carve = co;
       if (!filter_match(o.variant_filter, variant_to_string(v))) continue;

@@ -43,7 +43,7 @@ void Allocator::free(void* p, size_t bytes) {
 }
 
 // ------------------------------------------------------------------ descriptors
-static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3"};
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma"};
 
 Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
 
@@ -58,6 +58,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_ELL: add("r", v.R); add("u", v.U); break;
     case FAM_MERGE: add("i", v.I); break;
     case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
+    case FAM_SELL_TMA: add("c", v.C); add("s", v.S); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
   if (v.grid > 0) add("g", v.grid);
@@ -82,6 +83,7 @@ bool variant_from_string(const char* s, Variant* out) {
   v.fam = fam;
   if (fam == FAM_MERGE) v.I = 7;
   if (fam == FAM_SELL) { v.C = 128; v.S = 1; }
+  if (fam == FAM_SELL_TMA) { v.C = 256; v.S = 1; v.U = 8; v.I = 3; v.block = 288; }
   if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
   while ((tok = strtok_r(nullptr, ":", &save))) {
     char* end = nullptr;
@@ -115,6 +117,7 @@ static bool template_supported(const Variant& v) {
     case FAM_ELL: return sell_supported(v);
     case FAM_MERGE: return merge_supported(v);
     case FAM_BCSR3: return bcsr_supported(v);
+    case FAM_SELL_TMA: return sell_tma_supported(v);
   }
   return false;
 }
@@ -133,7 +136,7 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
   }
-  if (v.fam == FAM_SELL || v.fam == FAM_ELL || v.fam == FAM_MERGE) {
+  if (v.fam == FAM_SELL || v.fam == FAM_ELL || v.fam == FAM_MERGE || v.fam == FAM_SELL_TMA) {
     if (in.rows + in.nnz > 0x7ffffff0ll) return no("rows+nnz over int32");
   }
   return true;
@@ -142,6 +145,7 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
 // ------------------------------------------------------------------ formats
 spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) {
   switch (v.fam) {
+    case FAM_SELL_TMA:
     case FAM_SELL: {
       auto key = std::make_pair(v.C, v.S);
       if (h->sells.count(key)) return SPMV_OK;
@@ -184,7 +188,7 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
 
 void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   for (auto it = h->sells.begin(); it != h->sells.end();) {
-    if (keep.fam == FAM_SELL && it->first == std::make_pair(keep.C, keep.S)) { ++it; continue; }
+    if ((keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA) && it->first == std::make_pair(keep.C, keep.S)) { ++it; continue; }
     free_sell(it->second, h->al);
     it = h->sells.erase(it);
   }
@@ -206,6 +210,7 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
   const CsrView& A = h->A;
   const int64_t csr = A.nnz * 12 + (A.rows + 1) * 4;
   switch (v.fam) {
+    case FAM_SELL_TMA:
     case FAM_SELL: {
       auto it = h->sells.find(std::make_pair(v.C, v.S));
       if (it == h->sells.end()) return 0;
@@ -236,6 +241,10 @@ static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
       return sell_func(v, it != h->sells.end() && it->second.perm != nullptr);
     }
     case FAM_ELL: return sell_func(v, false);
+    case FAM_SELL_TMA: {
+      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      return sell_tma_func(v, it != h->sells.end() && it->second.perm != nullptr);
+    }
     case FAM_MERGE: return merge_func(v);
     case FAM_BCSR3: return bcsr_func(v);
   }
@@ -254,7 +263,7 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       SPMV_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve));
       g_carve[fn] = v.carve;
     }
-    if (v.grid > 0 && v.fam != FAM_MERGE) {
+    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA) {
       auto key = std::make_pair(fn, v.block);
       auto oi = g_occ.find(key);
       int occ = 0;
@@ -276,6 +285,12 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       auto it = h->sells.find(std::make_pair(v.C, v.S));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
       e = sell_launch(v, h->A.rows, it->second, a, grid_blocks);
+      break;
+    }
+    case FAM_SELL_TMA: {
+      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
+      e = sell_tma_launch(v, h->A.rows, it->second, a, h->dev.sm_count);
       break;
     }
     case FAM_ELL:
