@@ -95,6 +95,10 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
         for (int j0 = 0; j0 < w; j0 += J) {
           const int nj = min(J, w - j0);
           mbar_wait(&empty[stage], phase ^ 1);
+          // The consumers read this stage through the generic proxy; the refill is an async-proxy
+          // write.  Without this cross-proxy fence the refill was observed (B200, full-size
+          // cfg5, sorted slices) to land under reads that had been ordered before the arrive.
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           const uint32_t vb = (uint32_t)nj * C * sizeof(double), cb = (uint32_t)nj * C * sizeof(int);
           mbar_expect_tx(&full[stage], vb + cb);
           bulk_g2s(s_val + (size_t)stage * J * C, sval + base + (int64_t)j0 * C, vb, &full[stage]);
@@ -129,29 +133,30 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
       mbar_wait(&full[stage], phase);
       const double* pv = s_val + (size_t)stage * J * C + tid * R;
       const int* pc = s_col + (size_t)stage * J * C + tid * R;
-      {
-        double v[J][R];
-        int c[J][R];
+      double v[J][R];
+      int c[J][R];
 #pragma unroll
-        for (int j = 0; j < J; ++j) {
-          SmemVec<R>::load(pv + j * C, pc + j * C, v[j], c[j]);
-          if (j >= nj) {          // beyond this stage's steps: stale shared memory, masked off
+      for (int j = 0; j < J; ++j) {
+        SmemVec<R>::load(pv + j * C, pc + j * C, v[j], c[j]);
+        if (j >= nj) {          // beyond this stage's steps: stale shared memory, masked off
 #pragma unroll
-            for (int r = 0; r < R; ++r) c[j][r] = -1;
-          }
+          for (int r = 0; r < R; ++r) c[j][r] = -1;
         }
-        double xv[J][R];
-#pragma unroll
-        for (int j = 0; j < J; ++j)
-#pragma unroll
-          for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, max(c[j][r], 0));
-#pragma unroll
-        for (int j = 0; j < J; ++j)
-#pragma unroll
-          for (int r = 0; r < R; ++r) acc[r] = c[j][r] >= 0 ? fma(v[j][r], xv[j][r], acc[r]) : acc[r];
       }
+      // The stage is now in registers: hand it back to the producer before the x gathers.
+      // The fence orders every lane's shared-memory reads before the arrive.
+      asm volatile("fence.acq_rel.cta;" ::: "memory");
       __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[stage]);     // this warp is done with the stage
+      if (lane == 0) mbar_arrive(&empty[stage]);
+      double xv[J][R];
+#pragma unroll
+      for (int j = 0; j < J; ++j)
+#pragma unroll
+        for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, max(c[j][r], 0));
+#pragma unroll
+      for (int j = 0; j < J; ++j)
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = c[j][r] >= 0 ? fma(v[j][r], xv[j][r], acc[r]) : acc[r];
       if (++stage == STAGES) { stage = 0; phase ^= 1; }
     }
 #pragma unroll

@@ -112,6 +112,7 @@ struct Tuner {
   double *x = nullptr, *y0 = nullptr, *y = nullptr, *yref = nullptr, *scale = nullptr, *flushbuf = nullptr;
   bool own_x = false, own_y0 = false, own_ref = false;
   int64_t flush_n = 0;
+  double flush_us = 0.0;
   VerifyResult* d_res = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   spmv_tune_report_t* rep;
@@ -160,7 +161,7 @@ struct Tuner {
     return SPMV_OK;
   }
 
-  // median time per apply over `reps` batches (warm) or `reps*4` flushed single launches (cold)
+  // median time per apply over `reps` batches (warm: K applies; cold: K x (flush, apply) - K flushes)
   spmv_status_t time(const Variant& v, double est_us, double* us) {
     ApplyArgs a{alpha, beta, x, y, s};
     for (int i = 0; i < warmup; ++i) {
@@ -169,17 +170,42 @@ struct Tuner {
     }
     std::vector<double> t;
     if (flush) {
-      for (int i = 0; i < reps * 4; ++i) {
-        cudaError_t e = flush_l2_launch(flushbuf, flush_n, s);
-        if (e != cudaSuccess) return SPMV_ERR_CUDA;
+      // Cold protocol: K x (overwrite a 2xL2 buffer, apply) back to back inside one event pair,
+      // minus K flushes timed the same way (once per tune).  Per-launch event pairs would add the
+      // ~3-5 us launch gap to every candidate and quantise at the event resolution.
+      const int K = 8;
+      auto batch = [&](bool with_apply, double* out_us) -> spmv_status_t {
         SPMV_CUDA_TRY(cudaEventRecord(e0, s));
-        spmv_status_t st = launch_variant(h, v, a);
-        if (st != SPMV_OK) return st;
+        for (int k = 0; k < K; ++k) {
+          if (flush_l2_launch(flushbuf, flush_n, s) != cudaSuccess) return SPMV_ERR_CUDA;
+          if (with_apply) {
+            spmv_status_t st = launch_variant(h, v, a);
+            if (st != SPMV_OK) return st;
+          }
+        }
         SPMV_CUDA_TRY(cudaEventRecord(e1, s));
         SPMV_CUDA_TRY(cudaEventSynchronize(e1));
         float ms = 0.f;
         SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
-        t.push_back((double)ms * 1e3);
+        *out_us = (double)ms * 1e3 / K;
+        return SPMV_OK;
+      };
+      if (flush_us <= 0.0) {
+        std::vector<double> f;
+        for (int i = 0; i < 7; ++i) {
+          double u = 0;
+          spmv_status_t st = batch(false, &u);
+          if (st != SPMV_OK) return st;
+          if (i >= 2) f.push_back(u);
+        }
+        std::sort(f.begin(), f.end());
+        flush_us = f[f.size() / 2];
+      }
+      for (int i = 0; i < reps; ++i) {
+        double u = 0;
+        spmv_status_t st = batch(true, &u);
+        if (st != SPMV_OK) return st;
+        t.push_back(std::max(u - flush_us, 0.01));
       }
     } else {
       int K = (int)(min_batch_ms * 1e3 / std::max(est_us, 1.0)) + 1;

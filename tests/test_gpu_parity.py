@@ -140,3 +140,26 @@ def test_apply_host_matches_device_apply(cuda):
     y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, prob.alpha, prob.x, prob.beta, prob.y0)
     assert oracle.accept(yh.numpy(), y_ref, scale, H.TOL)[0]
     S.close()
+
+
+@pytest.mark.slow
+def test_tma_pipeline_race_regression_full_size(cuda):
+    """Regression: on full-size cfg5 with sorted slices the TMA refill (async proxy) used to land
+    under shared-memory reads of the previous occupant unless the producer issues
+    fence.proxy.async -- whole half-warps of rows were off by ~1e-3, in ~1 of 3 launches."""
+    import torch
+    prob = W.config(5)
+    A = prob.A
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, prob.x, 0.0)
+    S = binding.SpMV.from_csr(A)
+    x = torch.from_numpy(prob.x).cuda()
+    for desc in ("sell_tma:b96:c128:s8192:r2:u4:i3:x0", "sell_tma:b160:c128:s8192:r1:u8:i2:x0",
+                 "sell_tma:b288:c256:s1:r1:u8:i2:x0"):
+        S.select(desc)
+        for _ in range(12):
+            y = torch.full((A.rows,), float("nan"), dtype=torch.float64, device="cuda")
+            S.apply(1.0, x, 0.0, y)
+            torch.cuda.synchronize()
+            ok, mr, ff, nf = oracle.accept(y.cpu().numpy(), y_ref, scale, H.TOL)
+            assert ok, (desc, nf, ff, mr)
+    S.close()
