@@ -236,7 +236,8 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     streams, nstreams = [torch.cuda.current_stream()], 1
     tsum_d, tmed_d, _ = timed(max(10, args.steps // 10), 3)
     t0 = time.perf_counter()
-    reports = [h.tune(alpha=alpha, beta=beta, use_cache=(0 if i else 2), flush_l2=(mode != "warm"), seed=cfg)
+    reports = [h.tune(alpha=alpha, beta=beta, use_cache=(0 if (i or args.tune_cache) else 2),
+                      cache_path=args.tune_cache, flush_l2=(mode != "warm"), seed=cfg)
                for i, h in enumerate(handles)]
     stream_times = {}
     if members > 1:
@@ -323,6 +324,8 @@ def main():
     ap.add_argument("--configs", default="2", help="comma list; the first is the headline (default cfg2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune-cache", default=None,
+                    help="file persisting tuning winners (spmv_tune cache_path); a second run then skips the search")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
 
