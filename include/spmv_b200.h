@@ -188,7 +188,9 @@ SPMV_API spmv_status_t spmv_destroy(spmv_handle_t h);
 
 /* Measured ceilings with the library's own kernels, for the bench report:
  * kind 0: device copy GB/s (read+write bytes), 1: read-only streaming sum GB/s,
- * 2: empty-kernel launch latency in microseconds. */
+ * 2: empty-kernel launch latency in microseconds, 3: random 8-byte gathers out of a vector of
+ * `bytes` bytes, in giga-gathers per second (the ceiling of the x path when columns are
+ * unstructured). */
 SPMV_API spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_t reps, void* stream,
                                    double* result);
 

@@ -138,6 +138,23 @@ __global__ void ceiling_read_kernel(const double2* __restrict__ src, int64_t n, 
   if (s == 1.2345e300) out[0] = s;   // keeps the loads alive without a write stream
 }
 __global__ void ceiling_empty_kernel() {}
+// Random 8-byte gathers out of an L2-resident vector: the ceiling of the x path for matrices
+// with unstructured columns (cfg3).  idx[i] is a counter hash, so the index stream is free.
+__global__ void ceiling_gather_kernel(const double* __restrict__ x, int64_t nx, int64_t n, double* __restrict__ out) {
+  const int64_t G = (int64_t)gridDim.x * blockDim.x;
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += 4 * G) {
+    double v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      unsigned long long z = (unsigned long long)(i + u * G) * 0x9E3779B97F4A7C15ull;
+      z ^= z >> 29; z *= 0xBF58476D1CE4E5B9ull; z ^= z >> 32;
+      v[u] = (i + u * G < n) ? __ldg(x + (int64_t)__umul64hi(z, (unsigned long long)nx)) : 0.0;
+    }
+    s += (v[0] + v[1]) + (v[2] + v[3]);
+  }
+  if (s == 1.2345e300) out[0] = s;
+}
 
 }  // namespace spmv
 
@@ -181,6 +198,27 @@ extern "C" spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_
     *result = best;
     cudaFree(a);
     if (b) cudaFree(b);
+    cudaFree(o);
+  } else if (kind == 3) {
+    // bytes = size of the gathered vector; reps * 16M gathers per timed launch
+    const int64_t nx = (int64_t)(bytes / 8), n = (int64_t)1 << 26;
+    if (nx <= 0) return SPMV_ERR_INVALID_ARG;
+    double *xv = nullptr, *o = nullptr;
+    SPMV_CUDA_TRY(cudaMalloc(&xv, nx * 8));
+    SPMV_CUDA_TRY(cudaMalloc(&o, 8));
+    SPMV_CUDA_TRY(cudaMemsetAsync(xv, 0, nx * 8, s));
+    double best = 0.0;
+    for (int i = 0; i < reps + 2; ++i) {
+      SPMV_CUDA_TRY(cudaEventRecord(e0, s));
+      ceiling_gather_kernel<<<148 * 8, 512, 0, s>>>(xv, nx, n, o);
+      SPMV_CUDA_TRY(cudaEventRecord(e1, s));
+      SPMV_CUDA_TRY(cudaEventSynchronize(e1));
+      SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+      const double gps = (double)n / ((double)ms * 1e6);     // giga-gathers per second
+      if (i >= 2 && gps > best) best = gps;
+    }
+    *result = best;
+    cudaFree(xv);
     cudaFree(o);
   } else {
     return SPMV_ERR_INVALID_ARG;
