@@ -217,7 +217,7 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
   size_t n = 0;
   const SellFormat* sf = nullptr;
   if (v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) {
-    auto it = h->sells.find(std::make_pair(v.C, v.S));
+    auto it = h->sells.find(sell_key(v));
     if (it != h->sells.end()) sf = &it->second;
   } else if (v.fam == FAM_ELL && h->has_ell) {
     sf = &h->ell;

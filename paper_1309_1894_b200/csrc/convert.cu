@@ -129,18 +129,114 @@ __global__ void sell_fill_kernel(int64_t rows, int64_t rows_padded, int C, int l
   }
 }
 
+// ---- row splitting (SellFormat::split): virtual rows
+// pass 1: per row, number of virtual rows / partial-sum slots / split flag (scanned afterwards)
+__global__ void split_count_kernel(int64_t rows, int L, const int* __restrict__ rp, int* __restrict__ vstart,
+                                   int* __restrict__ pstart, int* __restrict__ sidx) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r == 0) { vstart[0] = 0; pstart[0] = 0; sidx[0] = 0; }
+  if (r >= rows) return;
+  const int len = rp[r + 1] - rp[r];
+  const bool split = len > L;
+  const int nseg = split ? (len + L - 1) / L : 1;
+  vstart[r + 1] = nseg;
+  pstart[r + 1] = split ? nseg : 0;
+  sidx[r + 1] = split ? 1 : 0;
+}
+// pass 2: virtual row pointers and targets (original row, or -(2+slot) for a segment)
+__global__ void split_fill_kernel(int64_t rows, int64_t vrows, int nnz, int L, const int* __restrict__ rp,
+                                  const int* __restrict__ vstart, const int* __restrict__ pstart,
+                                  const int* __restrict__ sidx, int* __restrict__ vrp, int* __restrict__ vtarget,
+                                  int* __restrict__ srow, int* __restrict__ sptr) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r == 0) { vrp[vrows] = nnz; sptr[sidx[rows]] = pstart[rows]; }
+  if (r >= rows) return;
+  const int a = rp[r], len = rp[r + 1] - a, v0 = vstart[r];
+  if (len <= L) {
+    vrp[v0] = a;
+    vtarget[v0] = (int)r;
+    return;
+  }
+  const int nseg = vstart[r + 1] - v0, p0 = pstart[r];
+  for (int sgm = 0; sgm < nseg; ++sgm) {
+    vrp[v0 + sgm] = a + sgm * L;
+    vtarget[v0 + sgm] = -(2 + p0 + sgm);
+  }
+  srow[sidx[r]] = (int)r;
+  sptr[sidx[r]] = p0;
+}
+__global__ void split_compose_kernel(int64_t rows_padded, const int* __restrict__ vtarget, int* __restrict__ perm) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= rows_padded) return;
+  const int v = perm[p];
+  perm[p] = v >= 0 ? vtarget[v] : -1;
+}
+
 void free_sell(SellFormat& f, Allocator& al) {
   if (f.slice_ptr) al.free(f.slice_ptr, sizeof(int64_t) * (f.nslices + 1));
   if (f.val) al.free(f.val, sizeof(double) * f.padded);
   if (f.col) al.free(f.col, sizeof(int32_t) * f.padded);
   if (f.perm) al.free(f.perm, sizeof(int32_t) * f.nslices * f.C);
+  if (f.part) al.free(f.part, sizeof(double) * std::max<int64_t>(f.nparts, 1));
+  if (f.srow) al.free(f.srow, sizeof(int32_t) * std::max<int64_t>(f.nsplit, 1));
+  if (f.sptr) al.free(f.sptr, sizeof(int32_t) * (f.nsplit + 1));
   f = SellFormat();
 }
 
-spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, Allocator& al, cudaStream_t s,
+spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int split, Allocator& al, cudaStream_t s,
                          SellFormat* out) {
   SellFormat f;
   f.is_ell = ell;
+  CsrView A = A0;
+  f.vrows = A0.rows;
+  // temporaries of the split pre-pass, released on every exit path
+  int *vstart = nullptr, *pstart = nullptr, *sidx = nullptr, *vrp = nullptr, *vtarget = nullptr;
+  const int64_t rows0 = A0.rows;
+  int64_t vrows_alloc = 0;
+  struct Tmp {
+    Allocator& al; int*& a; int*& b; int*& c; int*& d; int*& e; const int64_t& n; int64_t& v;
+    ~Tmp() {
+      if (a) al.free(a, sizeof(int) * (n + 1));
+      if (b) al.free(b, sizeof(int) * (n + 1));
+      if (c) al.free(c, sizeof(int) * (n + 1));
+      if (d) al.free(d, sizeof(int) * (v + 1));
+      if (e) al.free(e, sizeof(int) * std::max<int64_t>(v, 1));
+    }
+  } tmp{al, vstart, pstart, sidx, vrp, vtarget, rows0, vrows_alloc};
+  if (split > 0 && !ell && sigma > 1 && rows0 > 0) {
+    f.split = split;
+    vstart = (int*)al.alloc(sizeof(int) * (rows0 + 1), s);
+    pstart = (int*)al.alloc(sizeof(int) * (rows0 + 1), s);
+    sidx = (int*)al.alloc(sizeof(int) * (rows0 + 1), s);
+    if (!vstart || !pstart || !sidx) return SPMV_ERR_ALLOC;
+    const unsigned g = (unsigned)((rows0 + 255) / 256);
+    split_count_kernel<<<g, 256, 0, s>>>(rows0, split, A0.row_ptr, vstart, pstart, sidx);
+    SPMV_CUDA_TRY(cudaGetLastError());
+    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(vstart, rows0);
+    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(pstart, rows0);
+    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(sidx, rows0);
+    SPMV_CUDA_TRY(cudaGetLastError());
+    int tot[3] = {0, 0, 0};
+    SPMV_CUDA_TRY(cudaMemcpyAsync(&tot[0], vstart + rows0, sizeof(int), cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaMemcpyAsync(&tot[1], pstart + rows0, sizeof(int), cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaMemcpyAsync(&tot[2], sidx + rows0, sizeof(int), cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+    f.vrows = tot[0];
+    f.nparts = tot[1];
+    f.nsplit = tot[2];
+    vrows_alloc = f.vrows;
+    vrp = (int*)al.alloc(sizeof(int) * (f.vrows + 1), s);
+    vtarget = (int*)al.alloc(sizeof(int) * std::max<int64_t>(f.vrows, 1), s);
+    f.part = (double*)al.alloc(sizeof(double) * std::max<int64_t>(f.nparts, 1), s);
+    f.srow = (int32_t*)al.alloc(sizeof(int32_t) * std::max<int64_t>(f.nsplit, 1), s);
+    f.sptr = (int32_t*)al.alloc(sizeof(int32_t) * (f.nsplit + 1), s);
+    if (!vrp || !vtarget || !f.part || !f.srow || !f.sptr) { free_sell(f, al); return SPMV_ERR_ALLOC; }
+    split_fill_kernel<<<g, 256, 0, s>>>(rows0, f.vrows, (int)A0.nnz, split, A0.row_ptr, vstart, pstart, sidx, vrp,
+                                        vtarget, f.srow, f.sptr);
+    SPMV_CUDA_TRY(cudaGetLastError());
+    A.rows = f.vrows;
+    A.row_ptr = vrp;
+  }
   if (ell) {
     int64_t padded_rows = ((A.rows + 127) / 128) * 128;
     if (padded_rows == 0) padded_rows = 128;
@@ -189,6 +285,10 @@ spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, Allocator
     sell_fill_kernel<<<(unsigned)((rows_padded + 127) / 128), 128, 0, s>>>(A.rows, rows_padded, f.C, f.logC, A.row_ptr,
                                                                         A.col_idx, A.val, f.perm, f.slice_ptr, f.val,
                                                                         f.col);
+    SPMV_CUDA_TRY(cudaGetLastError());
+  }
+  if (f.split) {
+    split_compose_kernel<<<(unsigned)((rows_padded + 255) / 256), 256, 0, s>>>(rows_padded, vtarget, f.perm);
     SPMV_CUDA_TRY(cudaGetLastError());
   }
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));

@@ -2,6 +2,7 @@
 #pragma once
 #include <map>
 #include <string>
+#include <tuple>
 #include <utility>
 
 #include "spmv_internal.h"
@@ -17,7 +18,7 @@ struct spmv_handle_s {
   bool tuned = false;
 
   // owned formats, built on demand
-  std::map<std::pair<int, int>, spmv::SellFormat> sells;   // key (C, sigma)
+  std::map<std::tuple<int, int, int>, spmv::SellFormat> sells;   // key (C, sigma, split)
   spmv::SellFormat ell;
   bool has_ell = false;
   spmv::BcsrFormat bcsr;
@@ -30,6 +31,8 @@ struct spmv_handle_s {
 };
 
 namespace spmv {
+
+inline std::tuple<int, int, int> sell_key(const Variant& v) { return std::make_tuple(v.C, v.S, v.L); }
 
 constexpr uint64_t kHandleMagic = 0x53504D5642323030ull;   // "SPMVB200"
 constexpr const char* kVersion = "0.1.0";

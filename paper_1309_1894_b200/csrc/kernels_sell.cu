@@ -47,7 +47,7 @@ template <int R, int U, int PERM, int X>
 __global__ void __launch_bounds__(sell_max_block(R, U))
 sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
             const int64_t* __restrict__ slice_ptr, const double* __restrict__ sval,
-            const int* __restrict__ scol, const int* __restrict__ perm, double alpha,
+            const int* __restrict__ scol, const int* __restrict__ perm, double* __restrict__ part, double alpha,
             const double* __restrict__ x, double beta, double* __restrict__ y) {
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows_padded; g += G) {
@@ -106,13 +106,37 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
           acc[r] = c[u][r] >= 0 ? fma(v[u][r], xv[u][r], acc[r]) : acc[r];
     }
 #pragma unroll
-    for (int r = 0; r < R; ++r)
+    for (int r = 0; r < R; ++r) {
       if (orow[r] >= 0) y[orow[r]] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+      else if (PERM && orow[r] < -1) part[-(orow[r] + 2)] = acc[r];   // segment of a split row
+    }
   }
 }
 
+// One warp per split row: lane-strided sums over its segments, then the fixed butterfly -- the
+// order depends only on the format, so results are bit-identical across runs (reading A20).
+__global__ void sell_split_fixup_kernel(int64_t nsplit, const int* __restrict__ srow, const int* __restrict__ sptr,
+                                        const double* __restrict__ part, double alpha, double beta,
+                                        double* __restrict__ y) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (w >= nsplit) return;
+  const int a = __ldg(sptr + w), b = __ldg(sptr + w + 1);
+  double s = 0.0;
+  for (int k = a + lane; k < b; k += 32) s += part[k];
+  s = butterfly_sum<32>(s);
+  if (lane == 0) store_y(y, __ldg(srow + w), alpha, s, beta);
+}
+
+cudaError_t sell_split_fixup_launch(const SellFormat& f, const ApplyArgs& a) {
+  if (!f.split || f.nsplit == 0) return cudaSuccess;
+  sell_split_fixup_kernel<<<(unsigned)((f.nsplit * 32 + 255) / 256), 256, 0, a.stream>>>(f.nsplit, f.srow, f.sptr, f.part,
+                                                                                      a.alpha, a.beta, a.y);
+  return cudaGetLastError();
+}
+
 typedef void (*sell_kernel_t)(int64_t, int64_t, int, int, const int64_t*, const double*, const int*,
-                              const int*, double, const double*, double, double*);
+                              const int*, double*, double, const double*, double, double*);
 
 template <int PERM, int X>
 static sell_kernel_t pick_ru(int R, int U) {
@@ -150,7 +174,7 @@ cudaError_t sell_launch(const Variant& v, int64_t rows, const SellFormat& f, con
   int64_t exact = (threads + v.block - 1) / v.block;
   int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
   k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, rows_padded, f.C, f.logC, f.slice_ptr, f.val, f.col,
-                                              f.perm, a.alpha, a.x, a.beta, a.y);
+                                              f.perm, f.part, a.alpha, a.x, a.beta, a.y);
   return cudaGetLastError();
 }
 

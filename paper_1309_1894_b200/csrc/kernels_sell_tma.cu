@@ -65,7 +65,8 @@ template <int R, int STAGES, int J, int PERM, int X>
 __global__ void __launch_bounds__(512 + 32)
 sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict__ slice_ptr,
                 const double* __restrict__ sval, const int* __restrict__ scol, const int* __restrict__ perm,
-                double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+                double* __restrict__ part, double alpha, const double* __restrict__ x, double beta,
+                double* __restrict__ y) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nconsumers = C / R;
   const size_t val_bytes = (size_t)J * C * sizeof(double);
@@ -160,13 +161,15 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
       if (++stage == STAGES) { stage = 0; phase ^= 1; }
     }
 #pragma unroll
-    for (int r = 0; r < R; ++r)
+    for (int r = 0; r < R; ++r) {
       if (orow[r] >= 0) y[orow[r]] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+      else if (PERM && orow[r] < -1) part[-(orow[r] + 2)] = acc[r];   // segment of a split row
+    }
   }
 }
 
 typedef void (*sell_tma_kernel_t)(int64_t, int64_t, int, const int64_t*, const double*, const int*, const int*,
-                                  double, const double*, double, double*);
+                                  double*, double, const double*, double, double*);
 
 struct TmaEntry { int R, STAGES, J, X; sell_tma_kernel_t k[2]; };
 #define TE(r, st, j) {r, st, j, 0, {sell_tma_kernel<r, st, j, 0, 0>, sell_tma_kernel<r, st, j, 1, 0>}}
@@ -222,8 +225,8 @@ cudaError_t sell_tma_launch(const Variant& v, int64_t rows, const SellFormat& f,
   // persistent: g (default 1) waves of resident CTAs, never more CTAs than slices
   int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;
   if (grid > f.nslices) grid = f.nslices;
-  k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, f.nslices, f.C, f.slice_ptr, f.val, f.col, f.perm, a.alpha,
-                                                 a.x, a.beta, a.y);
+  k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, f.nslices, f.C, f.slice_ptr, f.val, f.col, f.perm, f.part,
+                                                 a.alpha, a.x, a.beta, a.y);
   return cudaGetLastError();
 }
 

@@ -33,6 +33,18 @@ struct SellFormat {
   int32_t* col = nullptr;         // [padded]
   int32_t* perm = nullptr;        // [nslices*C] sell row -> original row (or -1); null if sigma==1
   bool is_ell = false;
+  // Row splitting (split = L > 0): a row longer than L is cut into ceil(len/L) segments of at most L
+  // entries; every segment is a "virtual row" of the SELL structure, so one heavy row can no longer
+  // stretch a slice.  perm[p] >= 0: original row (written with the epilogue); -1: padding row;
+  // <= -2: the virtual row is a segment, its plain sum goes to part[-(perm[p]+2)] and
+  // sell_split_fixup adds the segments of each split row in a fixed order.
+  int split = 0;
+  int64_t vrows = 0;              // virtual rows (== rows when split == 0)
+  int64_t nparts = 0;             // segments of split rows
+  int64_t nsplit = 0;             // rows that were split
+  double* part = nullptr;         // [nparts] workspace, rewritten by every apply
+  int32_t* srow = nullptr;        // [nsplit] original row of split row i
+  int32_t* sptr = nullptr;        // [nsplit+1] its segments are part[sptr[i] .. sptr[i+1])
 };
 
 // 3x3 BCSR, values transposed per block row:
@@ -70,6 +82,7 @@ struct Variant {
   int C = 0;         // c: SELL slice height
   int S = 1;         // s: SELL sorting window sigma
   int I = 0;         // i: merge-path items per thread (sell_tma: pipeline stages)
+  int L = 0;         // l: SELL row-split length (0: rows are not split)
 };
 
 std::string variant_to_string(const Variant& v);
@@ -106,6 +119,8 @@ cudaError_t sell_launch(const Variant&, int64_t rows, const SellFormat&, const A
 bool sell_tma_supported(const Variant&);
 const void* sell_tma_func(const Variant&, bool perm);
 cudaError_t sell_tma_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int sm_count);
+// adds the segment sums of split rows in a fixed order (after a SELL kernel ran on a split format)
+cudaError_t sell_split_fixup_launch(const SellFormat&, const ApplyArgs&);
 
 bool merge_supported(const Variant&);
 const void* merge_func(const Variant&);
@@ -141,7 +156,7 @@ struct RawStats {   // filled on the device, copied back once
 };
 cudaError_t compute_stats(const CsrView& A, RawStats* h_out, cudaStream_t s);
 
-spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, Allocator& al,
+spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, int split, Allocator& al,
                          cudaStream_t s, SellFormat* out);
 void free_sell(SellFormat& f, Allocator& al);
 spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out);

@@ -49,6 +49,7 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
   std::vector<Variant> all, out;
   const spmv_info_t& in = h->info;
   const int blocks[3] = {128, 256, 512};
+  const bool skewed = in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0;
   for (int b : blocks) {
     for (int R : {1, 2, 4}) for (int U : {1, 2, 4}) {
       Variant v; v.fam = FAM_CSR_SCALAR; v.block = b; v.R = R; v.U = U; all.push_back(v);
@@ -65,6 +66,13 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
       if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }       // sorting equal rows is a no-op
       if (S == 1 && in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0) { ++*n_pruned; continue; }
       if ((double)in.max_row_len > 64.0 * in.mean_row_len + 64.0 && S < 8192) { ++*n_pruned; continue; }
+      if (skewed && S > 1) {
+        // heavy rows: cut them into segments of L entries (virtual rows) so that no slice is stretched
+        for (int L : {16, 32, 64, 128}) {
+          if (in.max_row_len <= L || R == 4 || U == 1) continue;
+          Variant w = v; w.L = L; all.push_back(w);
+        }
+      }
       all.push_back(v);
     }
     for (int R : {1, 2, 4}) for (int U : {1, 2, 4, 8}) {
@@ -81,6 +89,12 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     Variant v; v.fam = FAM_SELL_TMA; v.C = C; v.S = S; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;
     if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
     if (S == 1 && in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0) { ++*n_pruned; continue; }
+    if (skewed && S > 1) {
+      for (int L : {16, 32, 64, 128}) {
+        if (in.max_row_len <= L) continue;
+        Variant w = v; w.L = L; all.push_back(w);
+      }
+    }
     all.push_back(v);
   }
   // family, then format key, outermost: formats are then built once per key
@@ -88,7 +102,8 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : v.fam; };
     if (grp(a) != grp(b)) return grp(a) < grp(b);
     if (a.C != b.C) return a.C < b.C;
-    return a.S < b.S;
+    if (a.S != b.S) return a.S < b.S;
+    return a.L < b.L;
   });
   for (const Variant& v : all) {
     std::string why;
@@ -389,7 +404,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!budget_left()) break;
     if (variant_to_string(v) == variant_to_string(dflt)) continue;
     // keep device memory bounded: drop formats when the family / format key changes
-    if ((v.fam != last_fmt.fam && !(v.C == last_fmt.C && v.C > 0)) || v.C != last_fmt.C || v.S != last_fmt.S) {
+    if ((v.fam != last_fmt.fam && !(v.C == last_fmt.C && v.C > 0)) || v.C != last_fmt.C || v.S != last_fmt.S || v.L != last_fmt.L) {
       Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
       release_formats_except(h, keep);
       last_fmt = v;

@@ -54,11 +54,11 @@ std::string variant_to_string(const Variant& v) {
   switch (v.fam) {
     case FAM_CSR_SCALAR: add("r", v.R); add("u", v.U); break;
     case FAM_CSR_VECTOR: add("w", v.W); add("u", v.U); break;
-    case FAM_SELL: add("c", v.C); add("s", v.S); add("r", v.R); add("u", v.U); break;
+    case FAM_SELL: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); break;
     case FAM_ELL: add("r", v.R); add("u", v.U); break;
     case FAM_MERGE: add("i", v.I); break;
     case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
-    case FAM_SELL_TMA: add("c", v.C); add("s", v.S); add("r", v.R); add("u", v.U); add("i", v.I); break;
+    case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
   if (v.grid > 0) add("g", v.grid);
@@ -100,6 +100,7 @@ bool variant_from_string(const char* s, Variant* out) {
         case 'c': v.C = val; break;
         case 's': v.S = val; break;
         case 'i': v.I = val; break;
+        case 'l': v.L = val; break;
         default: return false;
       }
     }
@@ -136,6 +137,11 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
   }
+  if (v.L != 0) {
+    if (v.fam != FAM_SELL && v.fam != FAM_SELL_TMA) return no("row splitting is a SELL option");
+    if (v.L < 4 || v.L > 65536) return no("split length out of range");
+    if (v.S <= 1) return no("row splitting needs a sorting window (s > 1)");
+  }
   if (v.fam == FAM_SELL || v.fam == FAM_ELL || v.fam == FAM_MERGE || v.fam == FAM_SELL_TMA) {
     if (in.rows + in.nnz > 0x7ffffff0ll) return no("rows+nnz over int32");
   }
@@ -147,10 +153,10 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
   switch (v.fam) {
     case FAM_SELL_TMA:
     case FAM_SELL: {
-      auto key = std::make_pair(v.C, v.S);
+      auto key = sell_key(v);
       if (h->sells.count(key)) return SPMV_OK;
       SellFormat f;
-      spmv_status_t st = build_sell(h->A, v.C, v.S, false, h->al, s, &f);
+      spmv_status_t st = build_sell(h->A, v.C, v.S, false, v.L, h->al, s, &f);
       if (st != SPMV_OK) return st;
       if ((double)f.padded > 2.0 * (double)h->A.nnz + 65536.0) {   // too padded to be a candidate
         free_sell(f, h->al);
@@ -162,7 +168,7 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
     }
     case FAM_ELL: {
       if (h->has_ell) return SPMV_OK;
-      spmv_status_t st = build_sell(h->A, 0, 1, true, h->al, s, &h->ell);
+      spmv_status_t st = build_sell(h->A, 0, 1, true, 0, h->al, s, &h->ell);
       if (st == SPMV_OK) h->has_ell = true;
       return st;
     }
@@ -188,7 +194,7 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
 
 void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   for (auto it = h->sells.begin(); it != h->sells.end();) {
-    if ((keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA) && it->first == std::make_pair(keep.C, keep.S)) { ++it; continue; }
+    if ((keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA) && it->first == sell_key(keep)) { ++it; continue; }
     free_sell(it->second, h->al);
     it = h->sells.erase(it);
   }
@@ -212,10 +218,11 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
   switch (v.fam) {
     case FAM_SELL_TMA:
     case FAM_SELL: {
-      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return 0;
       const SellFormat& f = it->second;
-      return f.padded * 12 + (f.nslices + 1) * 8 + (f.perm ? f.nslices * (int64_t)f.C * 4 : 0);
+      return f.padded * 12 + (f.nslices + 1) * 8 + (f.perm ? f.nslices * (int64_t)f.C * 4 : 0) +
+             f.nparts * 16 + f.nsplit * 8;
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
     case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
@@ -237,12 +244,12 @@ static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
     case FAM_CSR_SCALAR: return csr_scalar_func(v);
     case FAM_CSR_VECTOR: return csr_vector_func(v);
     case FAM_SELL: {
-      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      auto it = h->sells.find(sell_key(v));
       return sell_func(v, it != h->sells.end() && it->second.perm != nullptr);
     }
     case FAM_ELL: return sell_func(v, false);
     case FAM_SELL_TMA: {
-      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      auto it = h->sells.find(sell_key(v));
       return sell_tma_func(v, it != h->sells.end() && it->second.perm != nullptr);
     }
     case FAM_MERGE: return merge_func(v);
@@ -282,15 +289,17 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
     case FAM_CSR_SCALAR: e = csr_scalar_launch(v, h->A, a, grid_blocks); break;
     case FAM_CSR_VECTOR: e = csr_vector_launch(v, h->A, a, grid_blocks); break;
     case FAM_SELL: {
-      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
       e = sell_launch(v, h->A.rows, it->second, a, grid_blocks);
+      if (e == cudaSuccess && it->second.split) e = sell_split_fixup_launch(it->second, a);
       break;
     }
     case FAM_SELL_TMA: {
-      auto it = h->sells.find(std::make_pair(v.C, v.S));
+      auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
       e = sell_tma_launch(v, h->A.rows, it->second, a, h->dev.sm_count);
+      if (e == cudaSuccess && it->second.split) e = sell_split_fixup_launch(it->second, a);
       break;
     }
     case FAM_ELL:
