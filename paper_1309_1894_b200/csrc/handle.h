@@ -24,6 +24,8 @@ struct spmv_handle_s {
   spmv::BcsrFormat bcsr;
   bool has_bcsr = false;
   std::map<int, spmv::MergePlan> plans;                    // key tile_items
+  std::map<int, spmv::DiaFormat> dias;                     // key C
+  int dia_state = 0;                                       // 0 not tried, 1 built once, -1 pattern is not diagonal
 
   // staging for spmv_apply_host
   double* d_x_stage = nullptr;

@@ -1,0 +1,434 @@
+// Stencil-aware DIA format: converter and kernel (the paper's own GPU
+// work is "stencil-aware" / "stencil-based", PAPER.md:33 ref [1], PAPER.md:39 ref [2]).
+//
+// A matrix whose stored entries lie on nd <= 32 diagonals (col - row in a small set) is stored
+// WITHOUT column indices, slice-major (slices of C rows, C in {128, 256, 512}):
+//     dval[((row / C) * nd + d) * C + row % C] = value of entry (row, row + off[d])
+//     mask[row] bit d                          = 1 iff that entry is stored in the CSR matrix
+// so the values of consecutive diagonals of one slice are one contiguous run (one bulk copy).
+// 8 bytes per non-zero instead of CSR's 12 (plus 4 bytes per row for the mask).  Entries that are
+// absent from the CSR matrix (Dirichlet-truncated neighbours) are never multiplied (reading A7): the
+// mask bit predicates both the x load and the FMA, so NaN/Inf in x reaches exactly the rows CSR
+// semantics say.  x[row + off] is a shifted contiguous stream: coalesced, no gather.
+// Deterministic: one thread sums a row over the diagonals in ascending-offset order.
+#include <algorithm>
+
+#include "device_utils.cuh"
+#include "spmv_internal.h"
+
+namespace spmv {
+
+struct DiaOffsets { int off[32]; };
+
+template <int R>
+struct DiaVec;
+template <>
+struct DiaVec<1> {
+  static __device__ __forceinline__ void load(const double* p, double* v) { v[0] = ld_stream(p); }
+};
+template <>
+struct DiaVec<2> {
+  static __device__ __forceinline__ void load(const double* p, double* v) {
+    double2 a = ld_stream2(p);
+    v[0] = a.x; v[1] = a.y;
+  }
+};
+template <>
+struct DiaVec<4> {
+  static __device__ __forceinline__ void load(const double* p, double* v) {
+    double2 a = ld_stream2(p), b = ld_stream2(p + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  }
+};
+
+// thread owns R adjacent rows of one slice; U diagonals per trip, all loads of a trip issued before the FMAs
+template <int R, int U, int X>
+__global__ void __launch_bounds__(512)
+dia_kernel(int64_t rows, int64_t ld, int C, int logC, int nd, DiaOffsets offs, const double* __restrict__ dval,
+           const unsigned* __restrict__ mask, double alpha, const double* __restrict__ x, double beta,
+           double* __restrict__ y) {
+  const int64_t G = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < ld; g += G) {
+    const int64_t r0 = g * R;
+    const int64_t sl = r0 >> logC;
+    const double* pv = dval + sl * nd * C + (r0 - (sl << logC));      // diagonal d of this slice at pv + d*C
+    unsigned m[R];
+    double acc[R], yold[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
+      acc[r] = 0.0;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
+    for (int d0 = 0; d0 < nd; d0 += U) {
+      double v[U][R], xv[U][R];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int d = min(d0 + u, nd - 1);          // past-the-end trips re-read the last diagonal, masked below
+        DiaVec<R>::load(pv + (int64_t)d * C, v[u]);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int d = d0 + u;
+        const int o = offs.off[min(d, nd - 1)];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const bool on = d < nd && ((m[r] >> d) & 1u);
+          xv[u][r] = on ? ldx<X>(x, (int)(r0 + r) + o) : 0.0;   // absent entries are never loaded (A7)
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int d = d0 + u;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const bool on = d < nd && ((m[r] >> d) & 1u);
+          acc[r] = on ? fma(v[u][r], xv[u][r], acc[r]) : acc[r];
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  }
+}
+
+typedef void (*dia_kernel_t)(int64_t, int64_t, int, int, int, DiaOffsets, const double*, const unsigned*, double,
+                             const double*, double, double*);
+
+template <int X>
+static dia_kernel_t dia_pick_ru(int R, int U) {
+#define P(r, u) if (R == r && U == u) return dia_kernel<r, u, X>;
+  P(1, 1) P(1, 2) P(1, 4) P(1, 8) P(2, 1) P(2, 2) P(2, 4) P(2, 8) P(4, 2) P(4, 4)
+#undef P
+  return nullptr;
+}
+static dia_kernel_t dia_pick(const Variant& v) {
+  return v.X == 0 ? dia_pick_ru<0>(v.R, v.U) : v.X == 1 ? dia_pick_ru<1>(v.R, v.U) : nullptr;
+}
+static bool dia_c_ok(int C) { return C == 128 || C == 256 || C == 512; }
+
+bool dia_supported(const Variant& v) {
+  return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && dia_c_ok(v.C) && dia_pick(v) != nullptr;
+}
+const void* dia_func(const Variant& v) { return (const void*)dia_pick(v); }
+
+static DiaOffsets dia_offsets(const DiaFormat& f) {
+  DiaOffsets o;
+  for (int i = 0; i < 32; ++i) o.off[i] = f.off[i];
+  return o;
+}
+
+cudaError_t dia_launch(const Variant& v, int64_t rows, const DiaFormat& f, const ApplyArgs& a, int grid_blocks) {
+  dia_kernel_t k = dia_pick(v);
+  if (!k || f.C != v.C) return cudaErrorInvalidValue;
+  if (rows == 0) return cudaSuccess;
+  const int64_t threads = (f.ld + v.R - 1) / v.R;
+  const int64_t exact = (threads + v.block - 1) / v.block;
+  const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, f.ld, f.C, f.logC, f.nd, dia_offsets(f), f.val, f.mask, a.alpha, a.x,
+                                              a.beta, a.y);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ DIA with the value stream on the TMA engine
+// Same producer/consumer ring as kernels_sell_tma.cu: the values of J diagonals of one slice are ONE
+// contiguous run (slice-major layout), so a stage is a single cp.async.bulk.  The x addresses do not
+// depend on loaded data (row + offset), so the consumers issue their x loads BEFORE waiting for the stage.
+__device__ __forceinline__ uint32_t dsmem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void dbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(dsmem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void dbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(dsmem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void dbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(dsmem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void dbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "DWAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DWAIT_DONE;\n"
+      "bra DWAIT_LOOP;\n"
+      "DWAIT_DONE:\n"
+      "}\n" ::"r"(dsmem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void dbulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   dsmem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(dsmem_u32(bar))
+               : "memory");
+}
+
+// blockDim.x = C/R consumer threads + 32 (the last warp is the producer warp).
+// With the first stage of a slice the producer also brings the slice's mask words and (beta != 0, Y_BULK)
+// its old y values, so a consumer never waits on a dependent global load: the x loads are issued
+// unpredicated (index clamped into [0, cols), never multiplied when the mask bit is off -- reading A7)
+// before the stage wait, everything else arrives through the ring.
+template <int R, int STAGES, int J, int X>
+__global__ void __launch_bounds__(512 + 32)
+dia_tma_kernel(int64_t rows, int64_t cols, int64_t nslices, int C, int nd, DiaOffsets offs,
+               const double* __restrict__ dval, const unsigned* __restrict__ mask, double alpha,
+               const double* __restrict__ x, double beta, double* __restrict__ y, int y_bulk) {
+  extern __shared__ __align__(128) unsigned char dia_smem[];
+  const int nconsumers = C / R;
+  double* s_val = reinterpret_cast<double*>(dia_smem);                                  // [STAGES][J*C]
+  double* s_y = s_val + (size_t)STAGES * J * C;                                         // [STAGES][C]
+  unsigned* s_mask = reinterpret_cast<unsigned*>(s_y + (size_t)STAGES * C);             // [STAGES][C]
+  uint64_t* full = reinterpret_cast<uint64_t*>(s_mask + (size_t)STAGES * C);
+  uint64_t* empty = full + STAGES;
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) {
+      dbar_init(&full[s], 1);
+      dbar_init(&empty[s], nconsumers / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const bool want_y = beta != 0.0 && y_bulk;
+
+  if (tid >= nconsumers) {
+    if (tid == nconsumers) {      // one elected lane streams the slices
+      uint32_t stage = 0, phase = 0;
+      for (int64_t s = blockIdx.x; s < nslices; s += gridDim.x) {
+        const double* src = dval + s * nd * C;
+        const bool ybulk = want_y && (s + 1) * C <= rows;
+        for (int d0 = 0; d0 < nd; d0 += J) {
+          const int nj = min(J, nd - d0);
+          dbar_wait(&empty[stage], phase ^ 1);
+          // generic-proxy reads of the previous occupant are ordered before this async-proxy refill
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          const uint32_t vb = (uint32_t)nj * C * sizeof(double);
+          const uint32_t mb = d0 == 0 ? (uint32_t)C * sizeof(unsigned) : 0u;
+          const uint32_t yb = (d0 == 0 && ybulk) ? (uint32_t)C * sizeof(double) : 0u;
+          dbar_expect_tx(&full[stage], vb + mb + yb);
+          dbulk_g2s(s_val + (size_t)stage * J * C, src + (int64_t)d0 * C, vb, &full[stage]);
+          if (mb) dbulk_g2s(s_mask + (size_t)stage * C, mask + s * C, mb, &full[stage]);
+          if (yb) dbulk_g2s(s_y + (size_t)stage * C, y + s * C, yb, &full[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+    return;
+  }
+
+  uint32_t stage = 0, phase = 0;
+  const int lane = tid & 31;
+  const int xmax = (int)cols - 1;
+  for (int64_t s = blockIdx.x; s < nslices; s += gridDim.x) {
+    const int64_t r0 = s * C + (int64_t)tid * R;
+    const bool ybulk = want_y && (s + 1) * C <= rows;
+    unsigned m[R];
+    double acc[R], yold[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { acc[r] = 0.0; yold[r] = 0.0; m[r] = 0u; }
+    if (beta != 0.0 && !ybulk) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) yold[r] = r0 + r < rows ? y[r0 + r] : 0.0;
+    }
+    for (int d0 = 0; d0 < nd; d0 += J) {
+      double xv[J][R];
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        const int o = offs.off[min(d0 + j, nd - 1)];
+#pragma unroll
+        for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
+      }
+      dbar_wait(&full[stage], phase);
+      if (d0 == 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          m[r] = s_mask[(size_t)stage * C + tid * R + r];
+          if (ybulk) yold[r] = s_y[(size_t)stage * C + tid * R + r];
+        }
+      }
+      const double* pv = s_val + (size_t)stage * J * C + tid * R;
+      double v[J][R];
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        if (R == 2) {
+          const double2 a = *reinterpret_cast<const double2*>(pv + j * C);
+          v[j][0] = a.x; v[j][R - 1] = a.y;
+        } else {
+          v[j][0] = pv[j * C];
+        }
+      }
+      // the stage is in registers: hand it back before the FMAs
+      asm volatile("fence.acq_rel.cta;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) dbar_arrive(&empty[stage]);
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        const int d = d0 + j;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const bool on = d < nd && ((m[r] >> d) & 1u);     // absent entries / stale shared memory: never multiplied
+          acc[r] = on ? fma(v[j][r], xv[j][r], acc[r]) : acc[r];
+        }
+      }
+      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  }
+}
+
+typedef void (*dia_tma_kernel_t)(int64_t, int64_t, int64_t, int, int, DiaOffsets, const double*, const unsigned*, double,
+                                 const double*, double, double*, int);
+struct DiaTmaEntry { int R, STAGES, J; dia_tma_kernel_t k; };
+#define DE(r, st, j) {r, st, j, dia_tma_kernel<r, st, j, 0>}
+#define DE_J(j) DE(1, 2, j), DE(1, 3, j), DE(1, 4, j), DE(2, 2, j), DE(2, 3, j), DE(2, 4, j)
+static const DiaTmaEntry g_dia_tma[] = {DE_J(4), DE_J(7), DE_J(8), DE_J(9), DE_J(14)};
+#undef DE_J
+#undef DE
+
+static const DiaTmaEntry* dia_tma_pick(const Variant& v) {
+  if (v.X != 0) return nullptr;
+  for (const auto& e : g_dia_tma)
+    if (e.R == v.R && e.STAGES == v.I && e.J == v.U) return &e;
+  return nullptr;
+}
+static size_t dia_tma_smem(const Variant& v) { return (size_t)v.I * (v.U + 1) * v.C * 8 + (size_t)v.I * v.C * 4 + 2 * v.I * 8 + 128; }
+
+bool dia_tma_supported(const Variant& v) {
+  if (!dia_tma_pick(v) || !dia_c_ok(v.C)) return false;
+  const int consumers = v.C / v.R;
+  if (consumers < 32 || consumers > 512 || v.block != consumers + 32) return false;
+  return dia_tma_smem(v) <= 200 * 1024;
+}
+const void* dia_tma_func(const Variant& v) {
+  const DiaTmaEntry* e = dia_tma_pick(v);
+  return e ? (const void*)e->k : nullptr;
+}
+
+cudaError_t dia_tma_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
+                           int sm_count) {
+  const DiaTmaEntry* e = dia_tma_pick(v);
+  if (!e || f.C != v.C) return cudaErrorInvalidValue;
+  if (rows == 0) return cudaSuccess;
+  const size_t smem = dia_tma_smem(v);
+  static thread_local const void* attr_k = nullptr;
+  static thread_local size_t attr_smem = 0;
+  static thread_local int occ = 1;
+  if (attr_k != (const void*)e->k || attr_smem != smem) {
+    cudaError_t err = cudaFuncSetAttribute((const void*)e->k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)e->k, v.block, smem);
+    if (err != cudaSuccess) return err;
+    if (occ < 1) occ = 1;
+    attr_k = (const void*)e->k;
+    attr_smem = smem;
+  }
+  const int64_t nslices = f.ld / f.C;
+  int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;   // persistent: g waves of resident CTAs
+  if (grid > nslices) grid = nslices;
+  const int y_bulk = ((uintptr_t)a.y & 15) == 0;     // cp.async.bulk needs 16-byte aligned global addresses
+  e->k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, cols, nslices, f.C, f.nd, dia_offsets(f), f.val, f.mask, a.alpha,
+                                                   a.x, a.beta, a.y, y_bulk);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ converter
+// pass 1: flag every occupied diagonal (benign write race: all writers store 1)
+__global__ void dia_flag_kernel(int64_t rows, const int* __restrict__ rp, const int* __restrict__ ci,
+                                unsigned char* __restrict__ flags) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= rows) return;
+  for (int k = rp[r]; k < rp[r + 1]; ++k) flags[(int64_t)ci[k] - r + rows] = 1;
+}
+// pass 2: collect up to 64 flagged diagonals (unordered; sorted on the host)
+__global__ void dia_collect_kernel(int64_t n, int64_t rows, const unsigned char* __restrict__ flags,
+                                   int* __restrict__ count, int* __restrict__ list) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || !flags[i]) return;
+  const int pos = atomicAdd(count, 1);
+  if (pos < 64) list[pos] = (int)(i - rows);
+}
+// pass 3: scatter values diagonal-major and build the masks
+__global__ void dia_fill_kernel(int64_t rows, int64_t ld, int C, int nd, DiaOffsets offs, const int* __restrict__ rp,
+                                const int* __restrict__ ci, const double* __restrict__ va,
+                                double* __restrict__ dval, unsigned* __restrict__ mask) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= ld) return;
+  unsigned m = 0;
+  if (r < rows) {
+    for (int k = rp[r]; k < rp[r + 1]; ++k) {
+      const int o = (int)((int64_t)ci[k] - r);
+      int lo = 0, hi = nd - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (offs.off[mid] < o) lo = mid + 1; else hi = mid;
+      }
+      dval[((r / C) * nd + lo) * C + r % C] = va[k];     // slice-major: (slice, diagonal, row in slice)
+      m |= 1u << lo;
+    }
+  }
+  mask[r] = m;
+}
+
+void free_dia(DiaFormat& f, Allocator& al) {
+  if (f.val) al.free(f.val, sizeof(double) * std::max<int64_t>((int64_t)f.nd * f.ld, 1));
+  if (f.mask) al.free(f.mask, sizeof(unsigned) * std::max<int64_t>(f.ld, 1));
+  f = DiaFormat();
+}
+
+// UNSUPPORTED when the pattern has more than 32 diagonals or is less than half full.
+spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, DiaFormat* out) {
+  if (!dia_c_ok(C)) return SPMV_ERR_UNSUPPORTED;
+  if (A.rows == 0 || A.nnz == 0 || A.rows + A.cols > 0x7ffffff0ll) return SPMV_ERR_UNSUPPORTED;
+  DiaFormat f;
+  const int64_t nflag = A.rows + A.cols + 1;
+  unsigned char* flags = (unsigned char*)al.alloc(nflag, s);
+  int* d_cnt = (int*)al.alloc(sizeof(int) * 65, s);
+  if (!flags || !d_cnt) {
+    if (flags) al.free(flags, nflag);
+    if (d_cnt) al.free(d_cnt, sizeof(int) * 65);
+    return SPMV_ERR_ALLOC;
+  }
+  auto drop_tmp = [&]() { al.free(flags, nflag); al.free(d_cnt, sizeof(int) * 65); };
+  int h_cnt[65];
+  cudaError_t e = cudaMemsetAsync(flags, 0, nflag, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_cnt, 0, sizeof(int) * 65, s);
+  if (e == cudaSuccess) {
+    dia_flag_kernel<<<(unsigned)((A.rows + 255) / 256), 256, 0, s>>>(A.rows, A.row_ptr, A.col_idx, flags);
+    dia_collect_kernel<<<(unsigned)((nflag + 255) / 256), 256, 0, s>>>(nflag, A.rows, flags, d_cnt, d_cnt + 1);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h_cnt, d_cnt, sizeof(int) * 65, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  drop_tmp();
+  if (e != cudaSuccess) { set_last_error("build_dia: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+  const int nd = h_cnt[0];
+  if (nd < 1 || nd > 32) { set_last_error("DIA: %d diagonals (limit 32)", nd); return SPMV_ERR_UNSUPPORTED; }
+  if ((double)A.nnz < 0.5 * (double)nd * (double)A.rows) {
+    set_last_error("DIA: fill %.3f below 0.5", (double)A.nnz / ((double)nd * (double)A.rows));
+    return SPMV_ERR_UNSUPPORTED;
+  }
+  std::sort(h_cnt + 1, h_cnt + 1 + nd);
+  f.nd = nd;
+  for (int i = 0; i < 32; ++i) f.off[i] = h_cnt[1 + std::min(i, nd - 1)];
+  f.C = C;
+  f.logC = C == 128 ? 7 : C == 256 ? 8 : 9;
+  f.ld = ((A.rows + C - 1) / C) * C;
+  f.val = (double*)al.alloc(sizeof(double) * nd * f.ld, s);
+  f.mask = (unsigned*)al.alloc(sizeof(unsigned) * f.ld, s);
+  if (!f.val || !f.mask) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+  SPMV_CUDA_TRY(cudaMemsetAsync(f.val, 0, sizeof(double) * nd * f.ld, s));
+  DiaOffsets o;
+  for (int i = 0; i < 32; ++i) o.off[i] = f.off[i];
+  dia_fill_kernel<<<(unsigned)((f.ld + 255) / 256), 256, 0, s>>>(A.rows, f.ld, C, nd, o, A.row_ptr, A.col_idx, A.val,
+                                                             f.val, f.mask);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  *out = f;
+  return SPMV_OK;
+}
+
+}  // namespace spmv

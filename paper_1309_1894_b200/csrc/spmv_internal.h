@@ -57,6 +57,17 @@ struct BcsrFormat {
   double fill = 0.0;             // nnz / (9*nblocks)
 };
 
+// DIA (stencil-aware): nd <= 32 diagonals, diagonal-major values, no column
+// indices; mask[row] bit d says whether entry (row, row + off[d]) is stored.
+struct DiaFormat {
+  int nd = 0;
+  int off[32] = {0};             // ascending; entries past nd repeat the last one
+  int C = 0, logC = 0;           // slice height (128, 256 or 512)
+  int64_t ld = 0;                // rows rounded up to a multiple of C
+  double* val = nullptr;         // [nd * ld], slice-major: ((row / C) * nd + d) * C + row % C
+  unsigned* mask = nullptr;      // [ld]
+};
+
 // Merge-path plan: tile t covers merge-path diagonals [t*tile_items, (t+1)*tile_items);
 // tile_row[t] = number of row-end items consumed before that diagonal.
 struct MergePlan {
@@ -68,7 +79,7 @@ struct MergePlan {
 };
 
 // ---------------------------------------------------------------- variants
-enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_COUNT };
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_COUNT };
 
 struct Variant {
   int fam = FAM_CSR_SCALAR;
@@ -130,6 +141,13 @@ bool bcsr_supported(const Variant&);
 const void* bcsr_func(const Variant&);
 cudaError_t bcsr_launch(const Variant&, const BcsrFormat&, const ApplyArgs&, int grid_blocks);
 
+bool dia_supported(const Variant&);
+const void* dia_func(const Variant&);
+cudaError_t dia_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+bool dia_tma_supported(const Variant&);
+const void* dia_tma_func(const Variant&);
+cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);
+
 // y = beta*y (or 0): the alpha == 0 path (reading A2)
 cudaError_t scale_y_launch(int64_t rows, double beta, double* y, cudaStream_t s);
 
@@ -161,6 +179,8 @@ spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, int split
 void free_sell(SellFormat& f, Allocator& al);
 spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out);
 void free_bcsr3(BcsrFormat& f, Allocator& al);
+spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, DiaFormat* out);
+void free_dia(DiaFormat& f, Allocator& al);
 spmv_status_t build_merge_plan(const CsrView& A, int tile_items, Allocator& al, cudaStream_t s,
                                MergePlan* out);
 void free_merge_plan(MergePlan& p, Allocator& al);

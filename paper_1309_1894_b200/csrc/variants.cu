@@ -43,7 +43,7 @@ void Allocator::free(void* p, size_t bytes) {
 }
 
 // ------------------------------------------------------------------ descriptors
-static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma"};
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma"};
 
 Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
 
@@ -58,6 +58,8 @@ std::string variant_to_string(const Variant& v) {
     case FAM_ELL: add("r", v.R); add("u", v.U); break;
     case FAM_MERGE: add("i", v.I); break;
     case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
+    case FAM_DIA: add("c", v.C); add("r", v.R); add("u", v.U); break;
+    case FAM_DIA_TMA: add("c", v.C); add("r", v.R); add("u", v.U); add("i", v.I); break;
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
@@ -85,6 +87,8 @@ bool variant_from_string(const char* s, Variant* out) {
   if (fam == FAM_SELL) { v.C = 128; v.S = 1; }
   if (fam == FAM_SELL_TMA) { v.C = 256; v.S = 1; v.U = 8; v.I = 3; v.block = 288; }
   if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
+  if (fam == FAM_DIA) v.C = 128;
+  if (fam == FAM_DIA_TMA) { v.C = 256; v.U = 8; v.I = 3; v.block = 288; }
   while ((tok = strtok_r(nullptr, ":", &save))) {
     char* end = nullptr;
     if (!strncmp(tok, "co", 2)) { v.carve = (int)strtol(tok + 2, &end, 10); }
@@ -119,6 +123,8 @@ static bool template_supported(const Variant& v) {
     case FAM_MERGE: return merge_supported(v);
     case FAM_BCSR3: return bcsr_supported(v);
     case FAM_SELL_TMA: return sell_tma_supported(v);
+    case FAM_DIA: return dia_supported(v);
+    case FAM_DIA_TMA: return dia_tma_supported(v);
   }
   return false;
 }
@@ -136,6 +142,11 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (in.rows % 3 || in.cols % 3 || in.rows == 0) return no("rows/cols not multiples of 3");
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
+  }
+  if (v.fam == FAM_DIA || v.fam == FAM_DIA_TMA) {
+    if (!in.cols_sorted) return no("DIA needs sorted unique columns");
+    if (in.max_row_len > 32 || in.nnz == 0) return no("more than 32 entries in a row: more than 32 diagonals");
+    if (h->dia_state < 0) return no("pattern is not a set of at most 32 (half-full) diagonals");
   }
   if (v.L != 0) {
     if (v.fam != FAM_SELL && v.fam != FAM_SELL_TMA) return no("row splitting is a SELL option");
@@ -178,6 +189,16 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
       if (st == SPMV_OK) h->has_bcsr = true;
       return st;
     }
+    case FAM_DIA_TMA:
+    case FAM_DIA: {
+      if (h->dias.count(v.C)) return SPMV_OK;
+      if (h->dia_state < 0) return SPMV_ERR_UNSUPPORTED;
+      DiaFormat f;
+      spmv_status_t st = build_dia(h->A, v.C, h->al, s, &f);
+      if (st == SPMV_OK) { h->dias[v.C] = f; h->dia_state = 1; }
+      else if (st == SPMV_ERR_UNSUPPORTED) h->dia_state = -1;
+      return st;
+    }
     case FAM_MERGE: {
       const int ti = v.block * v.I;
       if (h->plans.count(ti)) return SPMV_OK;
@@ -200,6 +221,11 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   }
   if (h->has_ell && keep.fam != FAM_ELL) { free_sell(h->ell, h->al); h->has_ell = false; }
   if (h->has_bcsr && keep.fam != FAM_BCSR3) { free_bcsr3(h->bcsr, h->al); h->has_bcsr = false; }
+  for (auto it = h->dias.begin(); it != h->dias.end();) {
+    if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA) && it->first == keep.C) { ++it; continue; }
+    free_dia(it->second, h->al);
+    it = h->dias.erase(it);
+  }
   for (auto it = h->plans.begin(); it != h->plans.end();) {
     if (keep.fam == FAM_MERGE && it->first == keep.block * keep.I) { ++it; continue; }
     free_merge_plan(it->second, h->al);
@@ -226,6 +252,11 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
     case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
+    case FAM_DIA_TMA:
+    case FAM_DIA: {
+      auto it = h->dias.find(v.C);
+      return it == h->dias.end() ? 0 : (int64_t)it->second.nd * it->second.ld * 8 + it->second.ld * 4;
+    }
     case FAM_MERGE: {
       auto it = h->plans.find(v.block * v.I);
       return csr + (it == h->plans.end() ? 0 : it->second.ntiles * 16 + 4);
@@ -254,6 +285,8 @@ static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
     }
     case FAM_MERGE: return merge_func(v);
     case FAM_BCSR3: return bcsr_func(v);
+    case FAM_DIA: return dia_func(v);
+    case FAM_DIA_TMA: return dia_tma_func(v);
   }
   return nullptr;
 }
@@ -270,7 +303,7 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       SPMV_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve));
       g_carve[fn] = v.carve;
     }
-    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA) {
+    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA && v.fam != FAM_DIA_TMA) {
       auto key = std::make_pair(fn, v.block);
       auto oi = g_occ.find(key);
       int occ = 0;
@@ -316,6 +349,14 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       if (!h->has_bcsr) return SPMV_ERR_INTERNAL;
       e = bcsr_launch(v, h->bcsr, a, grid_blocks);
       break;
+    case FAM_DIA_TMA:
+    case FAM_DIA: {
+      auto it = h->dias.find(v.C);
+      if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
+      e = v.fam == FAM_DIA ? dia_launch(v, h->A.rows, it->second, a, grid_blocks)
+                           : dia_tma_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
+      break;
+    }
   }
   if (e != cudaSuccess) {
     set_last_error("launch of %s failed: %s", variant_to_string(v).c_str(), cudaGetErrorString(e));
