@@ -9,6 +9,12 @@
 // Consumers read values/indices from shared memory (conflict-free: consecutive threads,
 // consecutive addresses), gather x through L1 and accumulate in registers.
 //
+// x path: X == 0 gathers x through the read-only/L1 path; X == 2 STAGES THE
+// X WINDOW IN SHARED MEMORY: with every stage the producer also bulk-copies the contiguous run
+// x[lo, lo + C + 2H) around the slice's own rows (lo = s*C - H, clipped) into the stage, and a gather
+// whose column falls inside the window is a shared-memory read; the others (far diagonals of a 3D
+// stencil, unstructured columns) still go through L1.  H is the variant's `h` parameter.
+//
 // Layout and padding semantics are those of kernels_sell.cu (same SellFormat).
 // Work split: CTA b owns slices b, b+gridDim, ...; a slice wider than J steps is streamed
 // as ceil(w/J) stages.  Deterministic: each row is summed by one thread in stored order.
@@ -66,14 +72,16 @@ __global__ void __launch_bounds__(512 + 32)
 sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict__ slice_ptr,
                 const double* __restrict__ sval, const int* __restrict__ scol, const int* __restrict__ perm,
                 double* __restrict__ part, double alpha, const double* __restrict__ x, double beta,
-                double* __restrict__ y) {
+                double* __restrict__ y, int64_t cols, int H) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nconsumers = C / R;
   const size_t val_bytes = (size_t)J * C * sizeof(double);
   const size_t col_bytes = (size_t)J * C * sizeof(int);
+  const int WIN = X == 2 ? C + 2 * H : 0;                                    // x window entries per stage
   double* s_val = reinterpret_cast<double*>(smem_raw);                       // [STAGES][J*C]
-  int* s_col = reinterpret_cast<int*>(smem_raw + STAGES * val_bytes);        // [STAGES][J*C]
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * (val_bytes + col_bytes));
+  double* s_x = s_val + (size_t)STAGES * J * C;                              // [STAGES][WIN]
+  int* s_col = reinterpret_cast<int*>(s_x + (size_t)STAGES * WIN);           // [STAGES][J*C]
+  uint64_t* full = reinterpret_cast<uint64_t*>(s_col + (size_t)STAGES * J * C);
   uint64_t* empty = full + STAGES;
   const int tid = threadIdx.x;
   if (tid == 0) {
@@ -101,9 +109,17 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
           // cfg5, sorted slices) to land under reads that had been ordered before the arrive.
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           const uint32_t vb = (uint32_t)nj * C * sizeof(double), cb = (uint32_t)nj * C * sizeof(int);
-          mbar_expect_tx(&full[stage], vb + cb);
+          uint32_t xb = 0;
+          int64_t lo = 0;
+          if (X == 2) {            // window [lo, lo + n) of x, lo even (16-byte aligned source), n even
+            lo = max((int64_t)0, s * C - H) & ~(int64_t)1;
+            const int64_t n = min((int64_t)WIN, cols - lo) & ~(int64_t)1;
+            xb = n > 0 ? (uint32_t)n * sizeof(double) : 0u;
+          }
+          mbar_expect_tx(&full[stage], vb + cb + xb);
           bulk_g2s(s_val + (size_t)stage * J * C, sval + base + (int64_t)j0 * C, vb, &full[stage]);
           bulk_g2s(s_col + (size_t)stage * J * C, scol + base + (int64_t)j0 * C, cb, &full[stage]);
+          if (xb) bulk_g2s(s_x + (size_t)stage * WIN, x + lo, xb, &full[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -144,16 +160,32 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
           for (int r = 0; r < R; ++r) c[j][r] = -1;
         }
       }
+      double xv[J][R];
+      if (X == 2) {
+        // gathers inside the staged window are shared-memory reads; the stage is released after them
+        const int64_t lo = max((int64_t)0, s * C - H) & ~(int64_t)1;
+        const int64_t n = min((int64_t)WIN, cols - lo) & ~(int64_t)1;
+        const double* xs = s_x + (size_t)stage * WIN;
+#pragma unroll
+        for (int j = 0; j < J; ++j)
+#pragma unroll
+          for (int r = 0; r < R; ++r) {
+            const int cc = max(c[j][r], 0);
+            const int64_t d = (int64_t)cc - lo;
+            xv[j][r] = (d >= 0 && d < n) ? xs[d] : ldx<0>(x, cc);
+          }
+      }
       // The stage is now in registers: hand it back to the producer before the x gathers.
       // The fence orders every lane's shared-memory reads before the arrive.
       asm volatile("fence.acq_rel.cta;" ::: "memory");
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty[stage]);
-      double xv[J][R];
+      if (X != 2) {
 #pragma unroll
-      for (int j = 0; j < J; ++j)
+        for (int j = 0; j < J; ++j)
 #pragma unroll
-        for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, max(c[j][r], 0));
+          for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, max(c[j][r], 0));
+      }
 #pragma unroll
       for (int j = 0; j < J; ++j)
 #pragma unroll
@@ -169,13 +201,17 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
 }
 
 typedef void (*sell_tma_kernel_t)(int64_t, int64_t, int, const int64_t*, const double*, const int*, const int*,
-                                  double*, double, const double*, double, double*);
+                                  double*, double, const double*, double, double*, int64_t, int);
 
 struct TmaEntry { int R, STAGES, J, X; sell_tma_kernel_t k[2]; };
 #define TE(r, st, j) {r, st, j, 0, {sell_tma_kernel<r, st, j, 0, 0>, sell_tma_kernel<r, st, j, 1, 0>}}
 static const TmaEntry g_tma[] = {TE(1, 2, 8), TE(1, 3, 8), TE(1, 4, 8), TE(1, 3, 4), TE(1, 4, 4), TE(1, 6, 4),
                                  TE(2, 2, 8), TE(2, 3, 8), TE(2, 4, 8), TE(2, 3, 4), TE(2, 4, 4), TE(2, 6, 4),
-                                 TE(1, 3, 16), TE(2, 3, 16), TE(1, 2, 16), TE(2, 2, 16)};
+                                 TE(1, 3, 16), TE(2, 3, 16), TE(1, 2, 16), TE(2, 2, 16),
+#define TX(r, st, j) {r, st, j, 2, {sell_tma_kernel<r, st, j, 0, 2>, sell_tma_kernel<r, st, j, 1, 2>}}
+                                 TX(1, 2, 8), TX(1, 3, 8), TX(1, 4, 8), TX(1, 3, 4), TX(1, 4, 4), TX(2, 2, 8), TX(2, 3, 8),
+                                 TX(2, 3, 4), TX(2, 4, 4), TX(1, 2, 16), TX(1, 3, 16), TX(2, 2, 16)};
+#undef TX
 #undef TE
 
 static const TmaEntry* tma_pick(const Variant& v) {
@@ -183,7 +219,10 @@ static const TmaEntry* tma_pick(const Variant& v) {
     if (e.R == v.R && e.STAGES == v.I && e.J == v.U && e.X == v.X) return &e;
   return nullptr;
 }
-static size_t tma_smem(const Variant& v) { return (size_t)v.I * v.U * v.C * 12 + 2 * v.I * 8 + 128; }
+static int tma_win(const Variant& v) { return v.X == 2 ? v.C + 2 * v.H : 0; }
+static size_t tma_smem(const Variant& v) {
+  return (size_t)v.I * v.U * v.C * 12 + (size_t)v.I * tma_win(v) * 8 + 2 * v.I * 8 + 128;
+}
 
 bool sell_tma_supported(const Variant& v) {
   if (!tma_pick(v)) return false;
@@ -191,6 +230,7 @@ bool sell_tma_supported(const Variant& v) {
   if (v.S < 1 || (v.S > 1 && (v.S % v.C != 0 || v.S > 8192 || (v.S & (v.S - 1))))) return false;
   const int consumers = v.C / v.R;
   if (consumers < 32 || consumers > 512 || v.block != consumers + 32) return false;
+  if (v.X == 2 ? (v.H < 8 || v.H > 4096 || v.H % 8) : v.H != 0) return false;
   return tma_smem(v) <= 200 * 1024;
 }
 const void* sell_tma_func(const Variant& v, bool perm) {
@@ -198,7 +238,8 @@ const void* sell_tma_func(const Variant& v, bool perm) {
   return e ? (const void*)e->k[perm ? 1 : 0] : nullptr;
 }
 
-cudaError_t sell_tma_launch(const Variant& v, int64_t rows, const SellFormat& f, const ApplyArgs& a, int sm_count) {
+cudaError_t sell_tma_launch(const Variant& v, int64_t rows, int64_t cols, const SellFormat& f, const ApplyArgs& a,
+                            int sm_count) {
   const TmaEntry* e = tma_pick(v);
   if (!e || f.C != v.C) return cudaErrorInvalidValue;
   if (rows == 0) return cudaSuccess;
@@ -225,8 +266,13 @@ cudaError_t sell_tma_launch(const Variant& v, int64_t rows, const SellFormat& f,
   // persistent: g (default 1) waves of resident CTAs, never more CTAs than slices
   int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;
   if (grid > f.nslices) grid = f.nslices;
+  // x window bulk copies need a 16-byte aligned x; otherwise the window is empty (H = -C/2: every gather
+  // goes through L1) -- same results, the variant just loses its point
+  int H = v.H;
+  int64_t cols_arg = cols;
+  if (v.X == 2 && ((uintptr_t)a.x & 15)) cols_arg = 0;
   k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, f.nslices, f.C, f.slice_ptr, f.val, f.col, f.perm, f.part,
-                                                 a.alpha, a.x, a.beta, a.y);
+                                                 a.alpha, a.x, a.beta, a.y, cols_arg, H);
   return cudaGetLastError();
 }
 

@@ -89,7 +89,8 @@ struct Variant {
   int U = 1;         // u: unroll factor (sell_tma: steps per stage)             (knob 5)
   int R = 1;         // r: rows per thread (csr_scalar, sell)
   int W = 1;         // w: lanes per row (csr_vector), lanes per block row (bcsr3)
-  int X = 0;         // x: 0 read-only path (ld.global.nc), 1 plain ld.global
+  int X = 0;         // x: 0 read-only path (ld.global.nc), 1 plain ld.global, 2 window staged in shared memory
+  int H = 0;         // h: half-width of the shared-memory x window around the slice's rows (x2 only)
   int C = 0;         // c: SELL slice height
   int S = 1;         // s: SELL sorting window sigma
   int I = 0;         // i: merge-path items per thread (sell_tma: pipeline stages)
@@ -129,7 +130,7 @@ cudaError_t sell_launch(const Variant&, int64_t rows, const SellFormat&, const A
 
 bool sell_tma_supported(const Variant&);
 const void* sell_tma_func(const Variant&, bool perm);
-cudaError_t sell_tma_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int sm_count);
+cudaError_t sell_tma_launch(const Variant&, int64_t rows, int64_t cols, const SellFormat&, const ApplyArgs&, int sm_count);
 // adds the segment sums of split rows in a fixed order (after a SELL kernel ran on a split format)
 cudaError_t sell_split_fixup_launch(const SellFormat&, const ApplyArgs&);
 

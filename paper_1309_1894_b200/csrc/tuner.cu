@@ -99,6 +99,9 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
       }
     }
     all.push_back(v);
+    // x window staged in shared memory (a10 ii): only meaningful when the rows of a slice are contiguous
+    if (S == 1 && (J == 4 || J == 8) && ST <= 3)
+      for (int H : {72, 136}) { Variant w = v; w.X = 2; w.H = H; all.push_back(w); }
   }
   for (int C : {128, 256, 512}) for (int R : {1, 2}) for (int J : {4, 7, 8, 9, 14}) for (int ST : {2, 3, 4}) {
     Variant v; v.fam = FAM_DIA_TMA; v.C = C; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;

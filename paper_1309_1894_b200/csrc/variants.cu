@@ -63,6 +63,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
+  if (v.X == 2) add("h", v.H);
   if (v.grid > 0) add("g", v.grid);
   if (v.carve >= 0) add("co", v.carve);
   return std::string(buf);
@@ -105,11 +106,13 @@ bool variant_from_string(const char* s, Variant* out) {
         case 's': v.S = val; break;
         case 'i': v.I = val; break;
         case 'l': v.L = val; break;
+        case 'h': v.H = val; break;
         default: return false;
       }
     }
     if (!end || *end != 0) return false;
   }
+  if (v.X == 2 && v.H == 0) v.H = 136;
   *out = v;
   return true;
 }
@@ -331,7 +334,7 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
     case FAM_SELL_TMA: {
       auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
-      e = sell_tma_launch(v, h->A.rows, it->second, a, h->dev.sm_count);
+      e = sell_tma_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
       if (e == cudaSuccess && it->second.split) e = sell_split_fixup_launch(it->second, a);
       break;
     }
