@@ -23,6 +23,9 @@ __global__ void stats_rows_kernel(int64_t rows, int64_t cols, int64_t nnz, const
                                   const int* __restrict__ ci, RawStats* __restrict__ st) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool ok = i < rows;
+  __shared__ unsigned int s_hist[32];           // per-block histogram: 32 global atomics per block, not one per row
+  if (threadIdx.x < 32) s_hist[threadIdx.x] = 0;
+  __syncthreads();
   unsigned long long bad_rp = 0, bad_col = 0, len_u = 0, len_sq = 0, sig_rp = 0, sig_ci = 0, unsorted = 0;
   long long bw = 0;
   int len = 0, mn = 0x7fffffff, mx = 0;
@@ -55,9 +58,11 @@ __global__ void stats_rows_kernel(int64_t rows, int64_t cols, int64_t nnz, const
       if (!sorted) unsorted = 1;
       int bin = len == 0 ? 0 : (32 - __clz(len));     // 2^(bin-1) <= len < 2^bin
       if (bin > 31) bin = 31;
-      atomicAdd(&st->hist[bin], 1ull);
+      atomicAdd(&s_hist[bin], 1u);
     }
   }
+  __syncthreads();
+  if (threadIdx.x < 32 && s_hist[threadIdx.x]) atomicAdd(&st->hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
   auto add = [](unsigned long long x, unsigned long long y) { return x + y; };
   bad_rp = warp_reduce(bad_rp, add);
   bad_col = warp_reduce(bad_col, add);

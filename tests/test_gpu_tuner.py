@@ -1,0 +1,151 @@
+"""GPU tests of the autotuner ("compare outputs with the
+reference results", north_star (d)): every candidate is verified before it may win, the verifier
+really gates the winner (fault injection), the winner is cached per matrix signature, and the
+stream-count knob is tuned on the batch."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1309_1894_b200 import binding
+from paper_1309_1894_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_ref_on_device(A, alpha, x, beta, y0):
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, alpha, x, beta, y0)
+    return y_ref, scale, H.to_dev(y_ref), H.to_dev(scale)
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 0.25), (3, 0.004), (4, 0.1), (5, 0.2), (1, 1.0)])
+def test_tune_against_the_cpu_oracle_reference(cuda, cfg, scale):
+    """spmv_tune with the ORACLE's y_ref/scale as the reference (north_star (d): 'checks every
+    candidate's output against the oracle before it may win'); the winner then matches the oracle."""
+    prob = W.config(cfg, scale)
+    A = prob.A
+    y_ref, sc, d_ref, d_sc = _oracle_ref_on_device(A, prob.alpha, prob.x, prob.beta, prob.y0)
+    S = binding.SpMV.from_csr(A)
+    dx = H.to_dev(prob.x)
+    dy0 = H.to_dev(prob.y0) if prob.y0 is not None else None
+    rep = S.tune(alpha=prob.alpha, beta=prob.beta, x=dx, y0=dy0, y_ref=d_ref, scale=d_sc, use_cache=2,
+                 reps=2, min_batch_ms=0.05)
+    assert rep["n_rejected"] == 0, [l for l in rep["log"] if l[1] == "rejected"][:5]
+    assert rep["n_timed"] >= 20 and rep["winner"] == S.variant and S.info().tuned == 1
+    assert rep["winner_us"] > 0 and rep["default_us"] > 0
+    assert rep["winner_us"] <= rep["default_us"] * 1.001          # the default is a candidate too
+    # every log line is accounted for
+    kinds = {l[1] for l in rep["log"]}
+    assert kinds <= {"timed", "pruned_slow", "pruned_format", "rejected"}
+    H.check_against_oracle(S, A, prob.alpha, prob.x, prob.beta, prob.y0, what=f"cfg{cfg} winner")
+    S.close()
+
+
+def test_fault_injection_is_rejected_and_cannot_win(cuda):
+    """A candidate whose output is perturbed must be rejected by the verifier and never be the winner."""
+    prob = W.config(2, 0.25)
+    A = prob.A
+    S = binding.SpMV.from_csr(A)
+    clean = S.tune(alpha=1.0, beta=0.5, use_cache=2, reps=2, min_batch_ms=0.05)
+    fam = clean["winner"].split(":")[0]
+    S2 = binding.SpMV.from_csr(A)
+    rep = S2.tune(alpha=1.0, beta=0.5, use_cache=2, reps=2, min_batch_ms=0.05, fault_inject=fam)
+    assert rep["n_rejected"] > 0
+    assert not rep["winner"].startswith(fam + ":"), rep["winner"]
+    rejected = [l for l in rep["log"] if l[1] == "rejected"]
+    assert rejected and all(l[0].startswith(fam) for l in rejected)
+    assert all(float(l[3]) > 1e-12 for l in rejected)             # max err/scale above the tolerance
+    H.check_against_oracle(S2, A, 1.0, prob.x, 0.5, prob.y0, what="winner after fault injection")
+    S.close(); S2.close()
+
+
+def test_all_candidates_faulty_gives_verify_failed(cuda):
+    A = W.laplace2d_5pt(20)
+    S = binding.SpMV.from_csr(A)
+    with pytest.raises(binding.SpmvError) as ei:
+        S.tune(use_cache=2, reps=1, min_batch_ms=0.02, variant_filter="csr_scalar", fault_inject="csr_scalar")
+    assert ei.value.status == 6                                   # SPMV_ERR_VERIFY_FAILED
+    assert S.variant.startswith("csr_scalar:b256:r1:u1:x0") and S.info().tuned == 0
+    S.close()
+
+
+def test_cache_hit_per_signature_and_file_persistence(cuda, tmp_path):
+    """Same structure (different values) -> same signature -> cache hit; different structure -> miss.
+    The cache file written by one tune is honoured after the in-process cache is cleared."""
+    binding.clear_cache()
+    path = str(tmp_path / "tune_cache.txt")
+    A = W.laplace3d_7pt(20)
+    S = binding.SpMV.from_csr(A)
+    r1 = S.tune(use_cache=0, cache_path=path, reps=2, min_batch_ms=0.05)
+    assert not r1["cache_hit"] and os.path.getsize(path) > 0
+    B = W.CSR(A.rows, A.cols, A.row_ptr, A.col_idx, A.val * 3.0 + 1.0)      # same pattern, new values
+    SB = binding.SpMV.from_csr(B)
+    assert SB.info().sig_row_ptr == S.info().sig_row_ptr and SB.info().sig_col_idx == S.info().sig_col_idx
+    r2 = SB.tune(use_cache=0, reps=2, min_batch_ms=0.05)
+    assert r2["cache_hit"] and r2["winner"] == r1["winner"] and r2["tune_seconds"] < r1["tune_seconds"]
+    H.check_against_oracle(SB, B, 1.0, W.uniform(1, B.cols), 0.0, None, what="cache-hit variant")
+    # different structure -> different signature -> no hit
+    Cm = W.laplace3d_7pt(21)
+    SC = binding.SpMV.from_csr(Cm)
+    assert SC.info().sig_col_idx != S.info().sig_col_idx
+    r3 = SC.tune(use_cache=0, reps=1, min_batch_ms=0.02, variant_filter="csr_vector")
+    assert not r3["cache_hit"]
+    # a different beta class (y read or not) is a different key
+    r4 = SB.tune(alpha=1.0, beta=1.0, use_cache=0, reps=1, min_batch_ms=0.02, variant_filter="csr_vector")
+    assert not r4["cache_hit"]
+    # file persistence across a cleared in-process cache
+    binding.clear_cache()
+    S5 = binding.SpMV.from_csr(A)
+    r5 = S5.tune(use_cache=0, cache_path=path, reps=2, min_batch_ms=0.05)
+    assert r5["cache_hit"] and r5["winner"] == r1["winner"]
+    # use_cache=2 bypasses it
+    r6 = S5.tune(use_cache=2, cache_path=path, reps=1, min_batch_ms=0.02, variant_filter="csr_scalar")
+    assert not r6["cache_hit"]
+    for s in (S, SB, SC, S5):
+        s.close()
+    binding.clear_cache()
+
+
+def test_variant_filter_and_candidate_listing(cuda):
+    A = W.fem_block27(5)
+    S = binding.SpMV.from_csr(A)
+    cands = S.variants()
+    fams = {c.split(":")[0] for c in cands}
+    assert {"csr_scalar", "csr_vector", "merge", "bcsr3", "sell", "sell_tma"} <= fams
+    rep = S.tune(use_cache=2, reps=1, min_batch_ms=0.02, variant_filter="bcsr3,merge")
+    names = {l[0].split(":")[0] for l in rep["log"]}
+    assert names <= {"bcsr3", "merge", "csr_scalar"}                # + the default, always timed
+    assert rep["winner"].split(":")[0] in ("bcsr3", "merge", "csr_scalar")
+    # a power-law matrix must not enumerate BCSR / DIA / unsplit sigma=1 SELL, but must enumerate row splitting
+    P = binding.SpMV.from_csr(W.powerlaw(5000, lmax=2000))
+    pc = P.variants()
+    assert not any(c.startswith(("bcsr3", "dia")) for c in pc)
+    assert any(":l32:" in c for c in pc) and any(c.startswith("merge") for c in pc)
+    S.close(); P.close()
+
+
+def test_tune_batch_picks_a_stream_count(cuda):
+    """cfg5 shape at reduced size: 4 handles, stream count in {1, 2, 4} timed on the actual batch."""
+    import torch
+    probs = [W.config(5, 0.25, member=m) for m in range(4)]
+    hs = [binding.SpMV.from_csr(p.A) for p in probs]
+    for h in hs:
+        h.select("sell:b256:c128:s1:r2:u4:x0")
+    xs = [H.to_dev(p.x) for p in probs]
+    ys = [H.to_dev(p.y0).clone() for p in probs]
+    streams = [torch.cuda.current_stream()] + [torch.cuda.Stream() for _ in range(3)]
+    best, times = binding.tune_batch(hs, [1.0] * 4, xs, [1.0] * 4, ys, streams)
+    assert best in (1, 2, 4) and set(times) == {1, 2, 4} and all(t > 0 for t in times.values())
+    assert times[best] == min(times.values())
+    # the batch result equals four single applies (and the oracle)
+    for p, y in zip(probs, ys):
+        y.copy_(H.to_dev(p.y0))
+    binding.apply_batch(hs, [1.0] * 4, xs, [1.0] * 4, ys, streams[:best])
+    torch.cuda.synchronize()
+    for p, y in zip(probs, ys):
+        y_ref, scale = oracle.spmv(p.A.row_ptr, p.A.col_idx, p.A.val, 1.0, p.x, 1.0, p.y0)
+        assert oracle.accept(y.cpu().numpy(), y_ref, scale, H.TOL)[0]
+    for h in hs:
+        h.close()
