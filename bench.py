@@ -46,7 +46,8 @@ def ncu_traffic(variant: str, cfg: int):
     try:
         t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
         e = t.get(f"cfg{cfg}", {})
-        return e.get("dram_bytes_per_launch") if e.get("variant") == variant else e.get("dram_bytes_per_launch")
+        # the capture is of one instantiation of the family; DRAM traffic is a property of the format
+        return e.get("dram_bytes_per_launch") if e.get("variant", "").split(":")[0] == variant.split(":")[0] else None
     except Exception:
         return None
 
@@ -245,7 +246,8 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
         nstreams, stream_times = binding.tune_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams)
     tune_s = time.perf_counter() - t0
     variant = handles[0].variant
-    launches_per_step = members * (2 if variant.startswith("merge") else 1)
+    # merge-path and row-split SELL add one small ordered fix-up kernel per apply
+    launches_per_step = members * (2 if (variant.startswith("merge") or ":l" in variant) else 1)
     for y, y0 in zip(ys, y0s):
         y.copy_(y0)
 
@@ -298,12 +300,18 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
                "h2d_bytes_per_step": 8 * A0.cols + (8 * A0.rows if beta != 0 else 0),
                "d2h_bytes_per_step": 8 * A0.rows}
     info = handles[0].info()
+    peak_meas, _ = measured_peak()
+    eff = nbytes * args.steps / tsum / 1e9
     res = {"cfg": cfg, "workload": probs[0].name if members == 1 else W.CONFIG_NAMES[5],
            "rows": A0.rows, "cols": A0.cols, "nnz": nnz, "members": members,
            "bytes_algorithmic": nbytes, "bytes_format_actual": int(sum(h.info().format_bytes for h in handles[:members])),
            "variant": variant, "nstreams": nstreams, "stream_times_us": stream_times,
            "t_sum_s": tsum, "t_median_us": tmed * 1e6, "t_min_us": tmin * 1e6,
-           "eff_gbs": nbytes * args.steps / tsum / 1e9, "gflops": 2.0 * nnz * args.steps / tsum / 1e9,
+           "eff_gbs": eff, "frac_hbm_nominal_8TBs": eff / NOMINAL_HBM_GBS, "frac_hbm_measured": eff / peak_meas,
+           "format_gbs": float(sum(h.info().format_bytes for h in handles[:members]) +
+                               sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs))
+                         * args.steps / tsum / 1e9,
+           "gathers_per_s": nnz * args.steps / tsum, "gflops": 2.0 * nnz * args.steps / tsum / 1e9,
            "t_default_us": tmed_d * 1e6, "speedup_vs_default": tmed_d / tmed,
            "tune_seconds": tune_s, "tune_reports": [{k: v for k, v in r.items() if k != "log"} for r in reports],
            "launches_per_step": launches_per_step, "timing": {"rotate": f"cold: steps rotate over {copies} device copies of the inputs (footprint > 3x L2), back to back in one event pair",
@@ -385,6 +393,18 @@ def main():
         "tune_seconds": head["tune_seconds"], "deterministic": head["deterministic"],
         "per_config": [{k: v for k, v in r.items() if k not in ("clocks",)} for r in results],
     }
+    if rank == 0:
+        # ceilings measured in the same run with the library's own kernels
+        torch.cuda.synchronize()
+        ceil = {"copy_gbs_1GiB": binding.measure_ceiling(0, 1 << 30, 5),
+                "read_gbs_1GiB": binding.measure_ceiling(1, 1 << 30, 5),
+                "read_gbs_at_headline_size": binding.measure_ceiling(1, max(1 << 20, int(head["bytes_format_actual"])), 5),
+                "empty_launch_us": binding.measure_ceiling(2, 0, 200),
+                "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}
+        line["ceilings"] = ceil
+        for r in line["per_config"]:
+            # unstructured columns: every x gather is its own L1->XBAR request (profiles/r01_cfg3_*.md)
+            r["frac_of_gather_ceiling"] = r["gathers_per_s"] / 1e9 / ceil["random_gather_G_per_s_32MiB_table"]
     if rank == 0 and not args.no_cpu_baseline:
         t = cpu_oracle_times(head_prob)
         nb = W.algorithmic_bytes(head_prob.A.rows, head_prob.A.cols, head_prob.A.nnz, head_prob.beta)

@@ -187,7 +187,8 @@ SPMV_API spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, v
 SPMV_API spmv_status_t spmv_destroy(spmv_handle_t h);
 
 /* Measured ceilings with the library's own kernels, for the bench report:
- * kind 0: device copy GB/s (read+write bytes), 1: read-only streaming sum GB/s,
+ * kind 0: device copy GB/s (read+write bytes) and 1: read-only streaming sum GB/s, `bytes` per launch,
+ * launches back to back over rotating windows (cold);
  * 2: empty-kernel launch latency in microseconds, 3: random 8-byte gathers out of a vector of
  * `bytes` bytes, in giga-gathers per second (the ceiling of the x path when columns are
  * unstructured). */
