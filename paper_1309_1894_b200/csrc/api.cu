@@ -231,10 +231,15 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
     if (!strcmp(name, "brow_ptr")) { src = h->bcsr.brow_ptr; n = sizeof(int32_t) * (h->bcsr.brows + 1); }
     else if (!strcmp(name, "bcol")) { src = h->bcsr.bcol; n = sizeof(int32_t) * h->bcsr.nblocks; }
     else if (!strcmp(name, "bval")) { src = h->bcsr.bval; n = sizeof(double) * 9 * h->bcsr.nblocks; }
-  } else if ((v.fam == FAM_DIA || v.fam == FAM_DIA_TMA) && h->dias.count(v.C)) {
+  } else if ((v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) && h->dias.count(v.C)) {
     const DiaFormat& df = h->dias[v.C];
     if (!strcmp(name, "dia_val")) { src = df.val; n = sizeof(double) * df.nd * df.ld; }
     else if (!strcmp(name, "dia_mask")) { src = df.mask; n = sizeof(unsigned) * df.ld; }
+    else if (!strcmp(name, "dia_coef")) {     // host-resident
+      *bytes = sizeof(double) * df.nd;
+      if (h_buf && cap > 0) memcpy(h_buf, df.coef, *bytes < cap ? *bytes : cap);
+      return SPMV_OK;
+    }
     else if (!strcmp(name, "dia_off")) {      // host-resident: copied directly
       *bytes = sizeof(int) * df.nd;
       if (h_buf && cap > 0) memcpy(h_buf, df.off, *bytes < cap ? *bytes : cap);

@@ -11,6 +11,8 @@
 // mask bit predicates both the x load and the FMA, so NaN/Inf in x reaches exactly the rows CSR
 // semantics say.  x[row + off] is a shifted contiguous stream: coalesced, no gather.
 // Deterministic: one thread sums a row over the diagonals in ascending-offset order.
+#include <string.h>
+
 #include <algorithm>
 
 #include "device_utils.cuh"
@@ -129,6 +131,83 @@ cudaError_t dia_launch(const Variant& v, int64_t rows, const DiaFormat& f, const
   const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
   k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, f.ld, f.C, f.logC, f.nd, dia_offsets(f), f.val, f.mask, a.alpha, a.x,
                                               a.beta, a.y);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ constant-coefficient stencil
+// When every stored entry of a diagonal carries the same value (a constant-coefficient stencil such as
+// cfg2's diag 6 / off -1), the values need not be streamed at all: the kernel reads the mask word
+// (which entries exist near the boundary), x and y only.  Same summation order as dia_kernel, and the
+// coefficients are the stored bit patterns, so the result equals dia_kernel's bit for bit.
+struct DiaCoefs { double c[32]; };
+
+template <int R, int X>
+__global__ void __launch_bounds__(512)
+dia_const_kernel(int64_t rows, int nd, DiaOffsets offs, DiaCoefs coefs, const unsigned* __restrict__ mask,
+                 double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+  const int64_t G = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows; g += G) {
+    const int64_t r0 = g * R;
+    unsigned m[R];
+    double acc[R], yold[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
+      acc[r] = 0.0;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
+    for (int d0 = 0; d0 < nd; d0 += 4) {
+      double xv[4][R];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int d = d0 + u;
+        const int o = offs.off[min(d, nd - 1)];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const bool on = d < nd && ((m[r] >> d) & 1u);
+          xv[u][r] = on ? ldx<X>(x, (int)(r0 + r) + o) : 0.0;
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int d = d0 + u;
+        const double c = coefs.c[min(d, nd - 1)];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const bool on = d < nd && ((m[r] >> d) & 1u);
+          acc[r] = on ? fma(c, xv[u][r], acc[r]) : acc[r];
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  }
+}
+
+typedef void (*dia_const_kernel_t)(int64_t, int, DiaOffsets, DiaCoefs, const unsigned*, double, const double*, double,
+                                   double*);
+static dia_const_kernel_t dia_const_pick(const Variant& v) {
+#define P(r, xx) if (v.R == r && v.X == xx) return dia_const_kernel<r, xx>;
+  P(1, 0) P(2, 0) P(4, 0) P(1, 1) P(2, 1) P(4, 1)
+#undef P
+  return nullptr;
+}
+bool dia_const_supported(const Variant& v) {
+  return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && dia_c_ok(v.C) && dia_const_pick(v) != nullptr;
+}
+const void* dia_const_func(const Variant& v) { return (const void*)dia_const_pick(v); }
+cudaError_t dia_const_launch(const Variant& v, int64_t rows, const DiaFormat& f, const ApplyArgs& a, int grid_blocks) {
+  dia_const_kernel_t k = dia_const_pick(v);
+  if (!k || !f.is_const) return cudaErrorInvalidValue;
+  if (rows == 0) return cudaSuccess;
+  DiaCoefs c;
+  for (int i = 0; i < 32; ++i) c.c[i] = f.coef[i];
+  const int64_t threads = (rows + v.R - 1) / v.R;
+  const int64_t exact = (threads + v.block - 1) / v.block;
+  const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y);
   return cudaGetLastError();
 }
 
@@ -373,6 +452,31 @@ __global__ void dia_fill_kernel(int64_t rows, int64_t ld, int C, int nd, DiaOffs
   mask[r] = m;
 }
 
+// constant-coefficient detection: the first thread to reach a diagonal stores its value as the
+// reference (ref[32+d]); then every stored value is compared with the reference bit for bit
+__global__ void dia_ref_first_kernel(int64_t rows, int C, int nd, const double* __restrict__ dval,
+                                     const unsigned* __restrict__ mask, unsigned long long* __restrict__ ref,
+                                     unsigned* __restrict__ seen) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= rows) return;
+  const unsigned m = mask[r];
+  for (int d = 0; d < nd; ++d)
+    if (((m >> d) & 1u) && atomicCAS(&seen[d], 0u, 1u) == 0u)
+      ref[32 + d] = (unsigned long long)__double_as_longlong(dval[((r / C) * nd + d) * C + r % C]);
+}
+__global__ void dia_cmp_kernel(int64_t rows, int C, int nd, const double* __restrict__ dval,
+                               const unsigned* __restrict__ mask, const unsigned long long* __restrict__ ref,
+                               unsigned* __restrict__ mismatch) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= rows) return;
+  const unsigned m = mask[r];
+  bool bad = false;
+  for (int d = 0; d < nd; ++d)
+    if ((m >> d) & 1u)
+      bad |= (unsigned long long)__double_as_longlong(dval[((r / C) * nd + d) * C + r % C]) != ref[32 + d];
+  if (bad) atomicAdd(mismatch, 1u);
+}
+
 void free_dia(DiaFormat& f, Allocator& al) {
   if (f.val) al.free(f.val, sizeof(double) * std::max<int64_t>((int64_t)f.nd * f.ld, 1));
   if (f.mask) al.free(f.mask, sizeof(unsigned) * std::max<int64_t>(f.ld, 1));
@@ -426,6 +530,33 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
   dia_fill_kernel<<<(unsigned)((f.ld + 255) / 256), 256, 0, s>>>(A.rows, f.ld, C, nd, o, A.row_ptr, A.col_idx, A.val,
                                                              f.val, f.mask);
   SPMV_CUDA_TRY(cudaGetLastError());
+  // constant-coefficient detection
+  {
+    const size_t wbytes = sizeof(unsigned long long) * 64 + sizeof(unsigned) * 40;
+    unsigned long long* d_ref = (unsigned long long*)al.alloc(wbytes, s);
+    if (!d_ref) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+    unsigned* d_seen = (unsigned*)(d_ref + 64);
+    unsigned* d_mis = d_seen + 32;
+    cudaError_t e2 = cudaMemsetAsync(d_ref, 0, wbytes, s);
+    const unsigned g = (unsigned)((A.rows + 255) / 256);
+    if (e2 == cudaSuccess) {
+      dia_ref_first_kernel<<<g, 256, 0, s>>>(A.rows, C, nd, f.val, f.mask, d_ref, d_seen);
+      dia_cmp_kernel<<<g, 256, 0, s>>>(A.rows, C, nd, f.val, f.mask, d_ref, d_mis);
+      e2 = cudaGetLastError();
+    }
+    unsigned long long h_ref[64];
+    unsigned h_mis = 1;
+    if (e2 == cudaSuccess) e2 = cudaMemcpyAsync(h_ref, d_ref, sizeof(h_ref), cudaMemcpyDeviceToHost, s);
+    if (e2 == cudaSuccess) e2 = cudaMemcpyAsync(&h_mis, d_mis, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
+    if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(s);
+    al.free(d_ref, wbytes);
+    if (e2 != cudaSuccess) { free_dia(f, al); set_last_error("build_dia: %s", cudaGetErrorString(e2)); return SPMV_ERR_CUDA; }
+    f.is_const = h_mis == 0;
+    for (int d = 0; d < 32; ++d) {
+      const unsigned long long bits = h_ref[32 + std::min(d, nd - 1)];
+      memcpy(&f.coef[d], &bits, sizeof(double));
+    }
+  }
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
   *out = f;
   return SPMV_OK;

@@ -66,6 +66,10 @@ struct DiaFormat {
   int64_t ld = 0;                // rows rounded up to a multiple of C
   double* val = nullptr;         // [nd * ld], slice-major: ((row / C) * nd + d) * C + row % C
   unsigned* mask = nullptr;      // [ld]
+  // constant-coefficient detection: is_const when every stored entry of each
+  // diagonal holds the same bit pattern; coef[d] is that value.  dia_const then reads no matrix values.
+  bool is_const = false;
+  double coef[32] = {0};
 };
 
 // Merge-path plan: tile t covers merge-path diagonals [t*tile_items, (t+1)*tile_items);
@@ -79,7 +83,7 @@ struct MergePlan {
 };
 
 // ---------------------------------------------------------------- variants
-enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_COUNT };
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_DIA_CONST, FAM_COUNT };
 
 struct Variant {
   int fam = FAM_CSR_SCALAR;
@@ -145,6 +149,9 @@ cudaError_t bcsr_launch(const Variant&, const BcsrFormat&, const ApplyArgs&, int
 bool dia_supported(const Variant&);
 const void* dia_func(const Variant&);
 cudaError_t dia_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+bool dia_const_supported(const Variant&);
+const void* dia_const_func(const Variant&);
+cudaError_t dia_const_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
 bool dia_tma_supported(const Variant&);
 const void* dia_tma_func(const Variant&);
 cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);

@@ -81,6 +81,9 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     for (int R : {1, 2, 4}) for (int U : {2, 4, 8}) {
       Variant v; v.fam = FAM_DIA; v.block = b; v.C = 128; v.R = R; v.U = U; all.push_back(v);
     }
+    for (int R : {1, 2, 4}) {
+      Variant v; v.fam = FAM_DIA_CONST; v.block = b; v.C = 128; v.R = R; all.push_back(v);
+    }
     for (int I : {5, 7, 11}) {
       Variant v; v.fam = FAM_MERGE; v.block = b; v.I = I; all.push_back(v);
     }
@@ -110,7 +113,7 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
   }
   // family, then format key, outermost: formats are then built once per key
   std::stable_sort(all.begin(), all.end(), [](const Variant& a, const Variant& b) {
-    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : v.fam == FAM_DIA_TMA ? (int)FAM_DIA : v.fam; };
+    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : (v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) ? (int)FAM_DIA : v.fam; };
     if (grp(a) != grp(b)) return grp(a) < grp(b);
     if (a.C != b.C) return a.C < b.C;
     if (a.S != b.S) return a.S < b.S;
@@ -415,7 +418,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!budget_left()) break;
     if (variant_to_string(v) == variant_to_string(dflt)) continue;
     // keep device memory bounded: drop formats when the family / format key changes
-    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : q.fam == FAM_DIA_TMA ? (int)FAM_DIA : q.fam; };
+    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : (q.fam == FAM_DIA_TMA || q.fam == FAM_DIA_CONST) ? (int)FAM_DIA : q.fam; };
     if (grp(v) != grp(last_fmt) || v.C != last_fmt.C || v.S != last_fmt.S || v.L != last_fmt.L) {
       Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
       release_formats_except(h, keep);

