@@ -332,6 +332,7 @@ def main():
     ap.add_argument("--configs", default="2", help="comma list; the first is the headline (default cfg2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-all", action="store_true", help="time the CPU oracle on every config of --configs, not only the headline")
     ap.add_argument("--tune-cache", default=None,
                     help="file persisting tuning winners (spmv_tune cache_path); a second run then skips the search")
     args = ap.parse_args()
@@ -363,6 +364,10 @@ def main():
     head_prob = None
     for i, cfg in enumerate(cfgs):
         res, prob = bench_config(cfg, args, torch, binding, W, dist_max, device, primary=(rank == 0))
+        if args.cpu_all and rank == 0 and i > 0:
+            t = cpu_oracle_times(prob, reps=3)
+            res["cpu_oracle"] = {"serial_seconds": t["serial"][0], "parallel_seconds": t["parallel"][0],
+                                 "cores": t["parallel"][1], "sample": "first matrix of the config, median of 3 applies"}
         results.append(res)
         if i == 0:
             head_prob = prob

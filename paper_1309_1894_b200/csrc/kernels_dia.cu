@@ -143,13 +143,18 @@ struct DiaCoefs { double c[32]; };
 
 template <int R, int X>
 __global__ void __launch_bounds__(512)
-dia_const_kernel(int64_t rows, int nd, DiaOffsets offs, DiaCoefs coefs, const unsigned* __restrict__ mask,
-                 double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs coefs,
+                 const unsigned* __restrict__ mask, double alpha, const double* __restrict__ x, double beta,
+                 double* __restrict__ y) {
+  constexpr int U = 8;
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
+  const int xmax = (int)cols - 1;
   for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows; g += G) {
     const int64_t r0 = g * R;
     unsigned m[R];
     double acc[R], yold[R];
+    // mask, old y and the first x loads are independent: one memory round trip, not three.  The x loads
+    // are unpredicated (index clamped into range); an absent entry is loaded but never multiplied (A7).
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
@@ -157,20 +162,16 @@ dia_const_kernel(int64_t rows, int nd, DiaOffsets offs, DiaCoefs coefs, const un
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
-    for (int d0 = 0; d0 < nd; d0 += 4) {
-      double xv[4][R];
+    for (int d0 = 0; d0 < nd; d0 += U) {
+      double xv[U][R];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int d = d0 + u;
-        const int o = offs.off[min(d, nd - 1)];
+      for (int u = 0; u < U; ++u) {
+        const int o = offs.off[min(d0 + u, nd - 1)];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-          const bool on = d < nd && ((m[r] >> d) & 1u);
-          xv[u][r] = on ? ldx<X>(x, (int)(r0 + r) + o) : 0.0;
-        }
+        for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
       }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < U; ++u) {
         const int d = d0 + u;
         const double c = coefs.c[min(d, nd - 1)];
 #pragma unroll
@@ -186,7 +187,7 @@ dia_const_kernel(int64_t rows, int nd, DiaOffsets offs, DiaCoefs coefs, const un
   }
 }
 
-typedef void (*dia_const_kernel_t)(int64_t, int, DiaOffsets, DiaCoefs, const unsigned*, double, const double*, double,
+typedef void (*dia_const_kernel_t)(int64_t, int64_t, int, DiaOffsets, DiaCoefs, const unsigned*, double, const double*, double,
                                    double*);
 static dia_const_kernel_t dia_const_pick(const Variant& v) {
 #define P(r, xx) if (v.R == r && v.X == xx) return dia_const_kernel<r, xx>;
@@ -198,7 +199,8 @@ bool dia_const_supported(const Variant& v) {
   return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && dia_c_ok(v.C) && dia_const_pick(v) != nullptr;
 }
 const void* dia_const_func(const Variant& v) { return (const void*)dia_const_pick(v); }
-cudaError_t dia_const_launch(const Variant& v, int64_t rows, const DiaFormat& f, const ApplyArgs& a, int grid_blocks) {
+cudaError_t dia_const_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
+                             int grid_blocks) {
   dia_const_kernel_t k = dia_const_pick(v);
   if (!k || !f.is_const) return cudaErrorInvalidValue;
   if (rows == 0) return cudaSuccess;
@@ -207,7 +209,7 @@ cudaError_t dia_const_launch(const Variant& v, int64_t rows, const DiaFormat& f,
   const int64_t threads = (rows + v.R - 1) / v.R;
   const int64_t exact = (threads + v.block - 1) / v.block;
   const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y);
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, cols, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y);
   return cudaGetLastError();
 }
 

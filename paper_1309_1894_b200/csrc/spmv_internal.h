@@ -151,7 +151,7 @@ const void* dia_func(const Variant&);
 cudaError_t dia_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
 bool dia_const_supported(const Variant&);
 const void* dia_const_func(const Variant&);
-cudaError_t dia_const_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+cudaError_t dia_const_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int grid_blocks);
 bool dia_tma_supported(const Variant&);
 const void* dia_tma_func(const Variant&);
 cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);

@@ -371,7 +371,7 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
     case FAM_DIA_CONST: {
       auto it = h->dias.find(v.C);
       if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
-      e = dia_const_launch(v, h->A.rows, it->second, a, grid_blocks);
+      e = dia_const_launch(v, h->A.rows, h->A.cols, it->second, a, grid_blocks);
       break;
     }
     case FAM_DIA_TMA:
