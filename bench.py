@@ -238,7 +238,8 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     tsum_d, tmed_d, _ = timed(max(10, args.steps // 10), 3)
     t0 = time.perf_counter()
     reports = [h.tune(alpha=alpha, beta=beta, use_cache=(0 if (i or args.tune_cache) else 2),
-                      cache_path=args.tune_cache, flush_l2=(mode != "warm"), seed=cfg)
+                      cache_path=args.tune_cache, flush_l2=(mode != "warm"), seed=cfg,
+                      variant_filter=args.variant_filter)
                for i, h in enumerate(handles)]
     stream_times = {}
     if members > 1:
@@ -332,6 +333,10 @@ def main():
     ap.add_argument("--configs", default="2", help="comma list; the first is the headline (default cfg2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant-filter", default=None,
+                    help="comma list of descriptor prefixes the tuner may use (spmv_tune variant_filter), e.g. "
+                         "'csr_scalar,csr_vector,sell:,sell_tma,ell,merge,bcsr3,dia:,dia_tma' = everything that still "
+                         "reads the matrix values (no constant-coefficient elision)")
     ap.add_argument("--cpu-all", action="store_true", help="time the CPU oracle on every config of --configs, not only the headline")
     ap.add_argument("--tune-cache", default=None,
                     help="file persisting tuning winners (spmv_tune cache_path); a second run then skips the search")
@@ -380,7 +385,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": head["t_sum_s"] / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": head["workload"], "rows": head["rows"], "nnz": head["nnz"],
-                   "variant": head["variant"], "l2": head["timing"],
+                   "variant": head["variant"], "variant_filter": args.variant_filter, "l2": head["timing"],
                    "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
         "gpu_launches": head["launches_per_step"] * args.steps,
         "clocks": head["clocks"],
