@@ -141,6 +141,31 @@ cudaError_t dia_launch(const Variant& v, int64_t rows, const DiaFormat& f, const
 // coefficients are the stored bit patterns, so the result equals dia_kernel's bit for bit.
 struct DiaCoefs { double c[32]; };
 
+// One grid-stride trip of dia_const: the loads of a trip (mask, old y, first U x values per row) are
+// independent of each other, and the NEXT trip's loads are issued before the current trip's FMAs and
+// store (software pipelining), so two trips' worth of bytes are in flight per thread.
+template <int R, int U, int X>
+struct DiaConstTrip {
+  unsigned m[R];
+  double yold[R];
+  double xv[U][R];
+  __device__ __forceinline__ void load(int64_t r0, int64_t rows, int xmax, const int (&off8)[U],
+                                       const unsigned* __restrict__ mask, const double* __restrict__ x,
+                                       double beta, const double* __restrict__ y) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
+#pragma unroll
+    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int o = off8[u];
+      // unpredicated, index clamped into range: an absent entry is loaded but never multiplied (A7)
+#pragma unroll
+      for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
+    }
+  }
+};
+
 template <int R, int X>
 __global__ void __launch_bounds__(512)
 dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs coefs,
@@ -149,41 +174,57 @@ dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs c
   constexpr int U = 8;
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   const int xmax = (int)cols - 1;
-  for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows; g += G) {
+  int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g * R >= rows) return;
+  int off8[U];
+  double c8[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) { off8[u] = offs.off[u]; c8[u] = coefs.c[u]; }   // entries past nd repeat the last one
+  DiaConstTrip<R, U, X> cur, nxt;
+  cur.load(g * R, rows, xmax, off8, mask, x, beta, y);
+  for (; g * R < rows; g += G) {
     const int64_t r0 = g * R;
-    unsigned m[R];
-    double acc[R], yold[R];
-    // mask, old y and the first x loads are independent: one memory round trip, not three.  The x loads
-    // are unpredicated (index clamped into range); an absent entry is loaded but never multiplied (A7).
+    const bool more = (g + G) * R < rows;
+    if (more) nxt.load((g + G) * R, rows, xmax, off8, mask, x, beta, y);
+    double acc[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
-      acc[r] = 0.0;
+    for (int r = 0; r < R; ++r) acc[r] = 0.0;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const double c = c8[u];
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const bool on = u < nd && ((cur.m[r] >> u) & 1u);
+        acc[r] = on ? fma(c, cur.xv[u][r], acc[r]) : acc[r];
+      }
     }
+    // more than U diagonals: the rest is loaded in place.  Statically unrolled (d0 = 8, 16, 24) so that
+    // the by-value offset/coefficient parameters are never indexed dynamically (no local-memory copy).
 #pragma unroll
-    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
-    for (int d0 = 0; d0 < nd; d0 += U) {
+    for (int d0 = U; d0 < 32; d0 += U) {
+      if (d0 >= nd) break;
       double xv[U][R];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
-        const int o = offs.off[min(d0 + u, nd - 1)];
+        const int o = offs.off[d0 + u];
 #pragma unroll
         for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
       }
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int d = d0 + u;
-        const double c = coefs.c[min(d, nd - 1)];
+        const double c = coefs.c[d];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          const bool on = d < nd && ((m[r] >> d) & 1u);
+          const bool on = d < nd && ((cur.m[r] >> d) & 1u);
           acc[r] = on ? fma(c, xv[u][r], acc[r]) : acc[r];
         }
       }
     }
 #pragma unroll
     for (int r = 0; r < R; ++r)
-      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * cur.yold[r]);
+    if (more) cur = nxt;
   }
 }
 
