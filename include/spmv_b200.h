@@ -171,6 +171,14 @@ SPMV_API spmv_status_t spmv_tune_batch(int32_t n, const spmv_handle_t* hs, const
  * needs.  Errors: INVALID_ARG (unparsable), UNSUPPORTED (not eligible for this matrix). */
 SPMV_API spmv_status_t spmv_select(spmv_handle_t h, const char* variant_descriptor, void* stream);
 
+/* New values on the SAME sparsity pattern (row_ptr / col_idx unchanged; e.g. a time-dependent
+ * coefficient): the handle now borrows d_val, the format of the selected variant is rebuilt from it
+ * and the tuning result (a function of the structure signature) is kept.  If the selected variant
+ * no longer applies to the new values (dia_const on coefficients that stopped being constant) the
+ * handle falls back to the best remaining family it can build (dia_tma, else the default variant)
+ * and *fell_back (may be NULL) is set to 1.  Synchronises `stream`. */
+SPMV_API spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* fell_back, void* stream);
+
 /* Writes the newline-separated descriptors of every candidate the tuner would
  * enumerate for this matrix (after structural pruning) into buf; *len = bytes needed. */
 SPMV_API spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap, size_t* len);

@@ -20,7 +20,7 @@ STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "S
 
 EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_status_string",
+           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache"]
 
 
@@ -95,9 +95,10 @@ def lib():
     L.spmv_format_download.argtypes = [vp, C.c_char_p, vp, C.c_size_t, C.POINTER(C.c_size_t), vp]
     L.spmv_destroy.argtypes = [vp]
     L.spmv_measure_ceiling.argtypes = [i32, C.c_size_t, i32, vp, C.POINTER(dbl)]
+    L.spmv_update_values.argtypes = [vp, vp, C.POINTER(i32), vp]
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling"):
+              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values"):
         getattr(L, n).restype = C.c_int
     L.spmv_status_string.argtypes = [C.c_int]
     L.spmv_status_string.restype = C.c_char_p
@@ -205,6 +206,15 @@ class SpMV:
         _check(lib().spmv_apply(self.h, float(alpha), _dptr(x), float(beta), _dptr(y), _stream_ptr(stream)),
                "spmv_apply")
         return y
+
+    def update_values(self, val, stream=None) -> bool:
+        """New values on the same pattern (CUDA float64 tensor, kept alive here).  Returns True if the
+        selected variant no longer applied and the handle fell back to another one."""
+        assert val.is_cuda and val.is_contiguous() and val.numel() == self.nnz
+        fb = C.c_int32(0)
+        _check(lib().spmv_update_values(self.h, _dptr(val), C.byref(fb), _stream_ptr(stream)), "spmv_update_values")
+        self._keep = (self._keep[0], self._keep[1], val)
+        return bool(fb.value)
 
     def apply_host(self, alpha, x_host, beta, y_host, stream=None):
         """Host-buffer form: x_host/y_host are CPU tensors or numpy arrays (pinned is faster)."""

@@ -150,6 +150,32 @@ spmv_status_t spmv_select(spmv_handle_t h, const char* desc, void* stream) {
   return SPMV_OK;
 }
 
+spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* fell_back, void* stream) {
+  if (!handle_alive(h) || (h->A.nnz > 0 && !d_val)) return SPMV_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));          // no apply may still be reading the old formats
+  h->A.val = d_val;
+  release_all_formats(h);
+  if (h->dia_state > 0) h->dia_state = 0;           // constness must be re-established on the new values
+  if (fell_back) *fell_back = 0;
+  spmv_status_t st = ensure_format(h, h->sel, s);
+  if (st == SPMV_ERR_UNSUPPORTED) {
+    if (fell_back) *fell_back = 1;
+    Variant alt = h->sel;
+    st = SPMV_ERR_UNSUPPORTED;
+    if (h->sel.fam == FAM_DIA_CONST && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
+      std::string why;
+      if (variant_eligible(h, alt, &why)) st = ensure_format(h, alt, s);
+    }
+    if (st != SPMV_OK) { alt = default_variant(); st = SPMV_OK; h->tuned = false; }
+    h->sel = alt;
+    release_formats_except(h, alt);
+  }
+  if (st != SPMV_OK) return st;
+  refresh_info(h);
+  return SPMV_OK;
+}
+
 spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y, void* stream) {
   if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
   if (h->A.rows > 0 && !d_y) return SPMV_ERR_INVALID_ARG;

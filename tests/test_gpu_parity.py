@@ -163,3 +163,32 @@ def test_tma_pipeline_race_regression_full_size(cuda):
             ok, mr, ff, nf = oracle.accept(y.cpu().numpy(), y_ref, scale, H.TOL)
             assert ok, (desc, nf, ff, mr)
     S.close()
+
+
+def test_update_values_keeps_the_variant_and_matches_oracle(cuda):
+    """spmv_update_values: same pattern, new values -> the selected variant's format is rebuilt; a
+    dia_const handle whose coefficients stop being constant falls back to a variant that reads values."""
+    import torch
+    A = W.stencil3d_27pt(9, perturb_stream=50)
+    x, y0 = W.uniform(81, A.cols), W.uniform(82, A.rows)
+    for desc in ("sell:b256:c128:s1:r2:u4:x0", "sell_tma:b288:c256:s1:r1:u8:i3:x0", "dia_tma:b288:c256:r1:u9:i3:x0",
+                 "merge:b256:i7:x0", "csr_vector:b256:w8:u2:x0", "ell:b256:r1:u2:x0"):
+        S = binding.SpMV.from_csr(A)
+        S.select(desc)
+        v2 = W.normal(83, A.nnz)
+        assert S.update_values(torch.from_numpy(v2).cuda()) is False
+        assert S.variant == desc
+        B = W.CSR(A.rows, A.cols, A.row_ptr, A.col_idx, v2)
+        H.check_against_oracle(S, B, 1.0, x, 0.5, y0, what="after update_values")
+        S.close()
+    L = W.laplace3d_7pt(12)
+    S = binding.SpMV.from_csr(L)
+    S.select("dia_const:b256:r2:x0")
+    xl = W.uniform(84, L.cols)
+    v3 = L.val * 2.0                                     # still constant along the diagonals
+    assert S.update_values(torch.from_numpy(v3).cuda()) is False and S.variant.startswith("dia_const")
+    H.check_against_oracle(S, W.CSR(L.rows, L.cols, L.row_ptr, L.col_idx, v3), 1.0, xl, 0.0, None, what="const x2")
+    v4 = W.normal(85, L.nnz)                             # not constant any more
+    assert S.update_values(torch.from_numpy(v4).cuda()) is True and S.variant.startswith("dia_tma")
+    H.check_against_oracle(S, W.CSR(L.rows, L.cols, L.row_ptr, L.col_idx, v4), 1.0, xl, 0.0, None, what="fallback")
+    S.close()
