@@ -273,3 +273,69 @@ def test_accept_rule():
     assert not oracle.accept(t, ref, sc)[0]
     t = ref.copy(); t[5] = np.nan
     assert not oracle.accept(t, ref, sc)[0]
+
+
+# ----------------------------------------------------------------------------
+# CG oracle (oracle_cg.c) -- pins C1..C5
+# ----------------------------------------------------------------------------
+def _dense(A):
+    D = np.zeros((A.rows, A.cols))
+    for i in range(A.rows):
+        for k in range(A.row_ptr[i], A.row_ptr[i + 1]):
+            D[i, A.col_idx[k]] += A.val[k]
+    return D
+
+
+@pytest.mark.parametrize("n", [3, 7, 12])
+def test_c1_cg_matches_dense_solve(n):
+    A = W.laplace2d_5pt(n)
+    D = _dense(A)
+    b = W.uniform(90, A.rows)
+    x, k, rel, hist = oracle.cg(A.row_ptr, A.col_idx, A.val, b, tol=1e-13, max_iters=500)
+    xs = np.linalg.solve(D, b)
+    assert np.abs(x - xs).max() <= 1e-10 * np.abs(xs).max()
+    assert rel <= 1e-13 and k < 500 and hist.size == k + 1
+
+
+def test_c2_identity_converges_in_one_exact_step():
+    n = 50
+    I = W.CSR(n, n, np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32), np.ones(n))
+    b = W.uniform(91, n)
+    x, k, rel, hist = oracle.cg(I.row_ptr, I.col_idx, I.val, b, tol=1e-15, max_iters=10)
+    assert k == 1 and np.array_equal(x, b) and rel == 0.0
+
+
+def test_c3_finite_termination_with_m_distinct_eigenvalues():
+    # diagonal SPD matrix with 4 distinct eigenvalues: CG must converge in <= 4 steps
+    n = 64
+    d = np.array([1.0, 2.0, 5.0, 9.0])[np.arange(n) % 4]
+    Dg = W.CSR(n, n, np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32), d)
+    b = W.uniform(92, n)
+    x, k, rel, _ = oracle.cg(Dg.row_ptr, Dg.col_idx, Dg.val, b, tol=1e-12, max_iters=50)
+    assert k <= 4 and np.abs(x - b / d).max() <= 1e-12
+
+
+def test_c4_recovers_x_true_and_reports_the_true_residual():
+    A = W.laplace2d_5pt(20)
+    xt = W.uniform(93, A.rows)
+    b, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, xt, 0.0)
+    x, k, rel, hist = oracle.cg(A.row_ptr, A.col_idx, A.val, b, tol=1e-12, max_iters=400)
+    assert np.abs(x - xt).max() <= 1e-9
+    Ax, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x, 0.0)
+    true_rel = np.linalg.norm(b - Ax) / np.linalg.norm(b)
+    assert abs(true_rel - rel) <= 1e-12 and rel <= 1e-12
+    assert hist[0] == pytest.approx(np.linalg.norm(b), rel=1e-14)      # x0 = 0: r0 = b
+
+
+def test_c5_zero_iterations_and_initial_guess():
+    A = W.laplace2d_5pt(6)
+    b = W.uniform(94, A.rows)
+    x0 = W.uniform(95, A.rows)
+    x, k, rel, hist = oracle.cg(A.row_ptr, A.col_idx, A.val, b, x0=x0, tol=1e-12, max_iters=0)
+    Ax0, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x0, 0.0)
+    assert k == 0 and np.array_equal(x, x0)
+    assert rel == pytest.approx(np.linalg.norm(b - Ax0) / np.linalg.norm(b), rel=1e-13)
+    # starting at the solution: no iteration needed
+    xs = np.linalg.solve(_dense(A), b)
+    _, k2, rel2, _ = oracle.cg(A.row_ptr, A.col_idx, A.val, b, x0=xs, tol=1e-10, max_iters=100)
+    assert k2 == 0 and rel2 <= 1e-10
