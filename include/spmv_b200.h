@@ -179,6 +179,33 @@ SPMV_API spmv_status_t spmv_select(spmv_handle_t h, const char* variant_descript
  * and *fell_back (may be NULL) is set to 1.  Synchronises `stream`. */
 SPMV_API spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* fell_back, void* stream);
 
+/* Solver loop around apply (the paper's ref [1], is about
+ * iterative solvers): conjugate gradients for a symmetric positive definite A, with the selected
+ * SpMV variant as the matrix product.
+ *   d_b [rows] right-hand side (device, read only); d_x [rows] initial guess in, solution out (device).
+ * Stops first when ||r_k|| <= tol * ||b|| (recurrence residual) or after max_iters iterations, or
+ * when p.Ap <= 0 (A not positive definite: result->breakdown = 1).  Scalars stay on the device;
+ * `check_every` iterations are replayed as one CUDA graph between host polls (plain launches when
+ * `stream` is the legacy default stream, which cannot be captured, or no_graph != 0).
+ * Workspace (3 vectors) comes from the handle's allocator for the duration of the call.
+ * Synchronises `stream`.  Errors: INVALID_ARG (rows != cols, NULL), ALLOC, CUDA. */
+typedef struct {
+  double tol;            /* 0 -> 1e-10 */
+  int32_t max_iters;     /* 0 -> 1000; negative -> 0 iterations (residual of the initial guess only) */
+  int32_t check_every;   /* 0 -> 8 */
+  int32_t no_graph;      /* 1: never use a CUDA graph */
+} spmv_cg_opts_t;
+typedef struct {
+  int32_t iters, converged, breakdown;
+  int32_t iterations_launched;   /* >= iters: iterations issued after convergence are device-side no-ops */
+  int32_t graph_replays;
+  double rel_residual;           /* sqrt(r.r) / ||b||  (sqrt(r.r) when b == 0) */
+  double device_seconds;         /* CUDA events around the whole solve */
+  double wall_seconds;
+} spmv_cg_result_t;
+SPMV_API spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x, const spmv_cg_opts_t* opts,
+                      spmv_cg_result_t* result, void* stream);
+
 /* Writes the newline-separated descriptors of every candidate the tuner would
  * enumerate for this matrix (after structural pruning) into buf; *len = bytes needed. */
 SPMV_API spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap, size_t* len);

@@ -20,7 +20,7 @@ STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "S
 
 EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_status_string",
+           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache"]
 
 
@@ -62,6 +62,16 @@ class TuneOpts(C.Structure):
                 ("seed", C.c_uint64), ("flush_l2", C.c_int32), ("stream", C.c_void_p)]
 
 
+class CgOpts(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_iters", C.c_int32), ("check_every", C.c_int32), ("no_graph", C.c_int32)]
+
+
+class CgResult(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("breakdown", C.c_int32),
+                ("iterations_launched", C.c_int32), ("graph_replays", C.c_int32),
+                ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
+
+
 class TuneReport(C.Structure):
     _fields_ = [("winner", C.c_char * 128), ("winner_us", C.c_double), ("default_us", C.c_double),
                 ("n_enumerated", C.c_int32), ("n_pruned_structural", C.c_int32),
@@ -96,9 +106,10 @@ def lib():
     L.spmv_destroy.argtypes = [vp]
     L.spmv_measure_ceiling.argtypes = [i32, C.c_size_t, i32, vp, C.POINTER(dbl)]
     L.spmv_update_values.argtypes = [vp, vp, C.POINTER(i32), vp]
+    L.spmv_cg.argtypes = [vp, vp, vp, C.POINTER(CgOpts), C.POINTER(CgResult), vp]
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values"):
+              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg"):
         getattr(L, n).restype = C.c_int
     L.spmv_status_string.argtypes = [C.c_int]
     L.spmv_status_string.restype = C.c_char_p
@@ -215,6 +226,14 @@ class SpMV:
         _check(lib().spmv_update_values(self.h, _dptr(val), C.byref(fb), _stream_ptr(stream)), "spmv_update_values")
         self._keep = (self._keep[0], self._keep[1], val)
         return bool(fb.value)
+
+    def cg(self, b, x, *, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, stream=None) -> dict:
+        """Conjugate gradients with the selected variant (spmv_cg).  x: initial guess in, solution out."""
+        assert b.is_cuda and x.is_cuda and b.numel() == self.rows and x.numel() == self.rows
+        o = CgOpts(float(tol), int(max_iters) if max_iters > 0 else -1, int(check_every), int(bool(no_graph)))
+        r = CgResult()
+        _check(lib().spmv_cg(self.h, _dptr(b), _dptr(x), C.byref(o), C.byref(r), _stream_ptr(stream)), "spmv_cg")
+        return {k: getattr(r, k) for k, _ in CgResult._fields_}
 
     def apply_host(self, alpha, x_host, beta, y_host, stream=None):
         """Host-buffer form: x_host/y_host are CPU tensors or numpy arrays (pinned is faster)."""

@@ -1,0 +1,251 @@
+// Solver loop around apply (the paper's ref [1], is about
+// iterative solvers): conjugate gradients with the tuned SpMV variant as its matrix product.
+//
+//   r0 = b - A x0, p0 = r0, rr = r0.r0;  per iteration:  q = A p;  alpha = rr / p.q;
+//   x += alpha p;  r -= alpha q;  rr' = r.r;  beta = rr'/rr;  p = r + beta p.
+//
+// No host round trip inside the loop: alpha, beta, rr, the iteration count and the "done" flag live
+// in device memory, kernels turn into no-ops once done is set, and `check_every` iterations are
+// captured in ONE CUDA graph that is replayed until the host sees done.  Vector updates are fused
+// (x and r update + r.r partials in one pass; p update reads the new partials), reductions are
+// two-level with a fixed shape (per-block partials, then every block re-adds the partials in the same
+// order), so the iterates are bit-identical across runs (reading A20).  No atomics.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <chrono>
+
+#include "handle.h"
+
+namespace spmv {
+
+struct CgState {
+  double rr, bb, pq;
+  int iters, done, converged, breakdown;
+};
+
+constexpr int kCgBlock = 256;
+
+__device__ __forceinline__ double cg_block_sum(double v, double* s_red) {
+  const int tid = threadIdx.x;
+  s_red[tid] = v;
+  __syncthreads();
+#pragma unroll
+  for (int d = kCgBlock / 2; d >= 1; d >>= 1) {
+    if (tid < d) s_red[tid] += s_red[tid + d];
+    __syncthreads();
+  }
+  const double out = s_red[0];
+  __syncthreads();
+  return out;
+}
+// every block adds the nb partials in the same fixed order -> the same value in every block
+__device__ __forceinline__ double cg_sum_partials(const double* __restrict__ part, int nb, double* s_red) {
+  double v = 0.0;
+  for (int i = threadIdx.x; i < nb; i += kCgBlock) v += part[i];
+  return cg_block_sum(v, s_red);
+}
+
+__global__ void __launch_bounds__(kCgBlock)
+cg_init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ q, double* __restrict__ r,
+               double* __restrict__ p, double* __restrict__ part_rr, double* __restrict__ part_bb) {
+  __shared__ double s_red[kCgBlock];
+  double rr = 0.0, bb = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock) {
+    const double bi = b[i], ri = bi - q[i];
+    r[i] = ri;
+    p[i] = ri;
+    rr = fma(ri, ri, rr);
+    bb = fma(bi, bi, bb);
+  }
+  rr = cg_block_sum(rr, s_red);
+  bb = cg_block_sum(bb, s_red);
+  if (threadIdx.x == 0) { part_rr[blockIdx.x] = rr; part_bb[blockIdx.x] = bb; }
+}
+
+__global__ void __launch_bounds__(kCgBlock)
+cg_init_final_kernel(int nb, const double* __restrict__ part_rr, const double* __restrict__ part_bb,
+                     CgState* __restrict__ st, double tol, int max_iters) {
+  __shared__ double s_red[kCgBlock];
+  const double rr = cg_sum_partials(part_rr, nb, s_red);
+  const double bb = cg_sum_partials(part_bb, nb, s_red);
+  if (threadIdx.x == 0) {
+    st->rr = rr; st->bb = bb; st->pq = 0.0;
+    st->iters = 0; st->breakdown = 0;
+    st->converged = sqrt(rr) <= tol * sqrt(bb);
+    st->done = st->converged || max_iters <= 0;
+  }
+}
+
+__global__ void __launch_bounds__(kCgBlock)
+cg_dot_kernel(int64_t n, const double* __restrict__ p, const double* __restrict__ q, double* __restrict__ part,
+              const CgState* __restrict__ st) {
+  __shared__ double s_red[kCgBlock];
+  if (st->done) return;
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock)
+    s = fma(p[i], q[i], s);
+  s = cg_block_sum(s, s_red);
+  if (threadIdx.x == 0) part[blockIdx.x] = s;
+}
+
+// x += alpha p, r -= alpha q, partials of the new r.r  (alpha = rr / p.q from the dot partials)
+__global__ void __launch_bounds__(kCgBlock)
+cg_update_kernel(int64_t n, int nb, const double* __restrict__ part_pq, const CgState* __restrict__ st,
+                 double* __restrict__ x, double* __restrict__ r, const double* __restrict__ p,
+                 const double* __restrict__ q, double* __restrict__ part_rr) {
+  __shared__ double s_red[kCgBlock];
+  if (st->done) return;
+  const double pq = cg_sum_partials(part_pq, nb, s_red);
+  const double alpha = pq > 0.0 ? st->rr / pq : 0.0;      // pq <= 0: not SPD; cg_step_final stops the loop
+  double rr = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock) {
+    x[i] = fma(alpha, p[i], x[i]);
+    const double ri = fma(-alpha, q[i], r[i]);
+    r[i] = ri;
+    rr = fma(ri, ri, rr);
+  }
+  rr = cg_block_sum(rr, s_red);
+  if (threadIdx.x == 0) part_rr[blockIdx.x] = rr;
+}
+
+// p = r + beta p  (beta = rr' / rr, rr' from the partials the update kernel just wrote)
+__global__ void __launch_bounds__(kCgBlock)
+cg_pupdate_kernel(int64_t n, int nb, const double* __restrict__ part_rr, const CgState* __restrict__ st,
+                  const double* __restrict__ r, double* __restrict__ p) {
+  __shared__ double s_red[kCgBlock];
+  if (st->done) return;
+  const double rr_new = cg_sum_partials(part_rr, nb, s_red);
+  const double beta = rr_new / st->rr;
+  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock)
+    p[i] = fma(beta, p[i], r[i]);
+}
+
+// one block, after every other kernel of the iteration has read the old scalars
+__global__ void __launch_bounds__(kCgBlock)
+cg_step_final_kernel(int nb, const double* __restrict__ part_pq, const double* __restrict__ part_rr,
+                     CgState* __restrict__ st, double tol, int max_iters) {
+  __shared__ double s_red[kCgBlock];
+  if (st->done) return;
+  const double pq = cg_sum_partials(part_pq, nb, s_red);
+  const double rr_new = cg_sum_partials(part_rr, nb, s_red);
+  if (threadIdx.x == 0) {
+    st->pq = pq;
+    if (!(pq > 0.0)) { st->breakdown = 1; st->done = 1; return; }
+    st->rr = rr_new;
+    st->iters += 1;
+    st->converged = sqrt(rr_new) <= tol * sqrt(st->bb);
+    st->done = st->converged || st->iters >= max_iters;
+  }
+}
+
+}  // namespace spmv
+
+using namespace spmv;
+
+extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x, const spmv_cg_opts_t* opts,
+                                 spmv_cg_result_t* result, void* stream) {
+  if (!handle_alive(h) || !result) return SPMV_ERR_INVALID_ARG;
+  if (h->A.rows != h->A.cols) { set_last_error("spmv_cg needs a square matrix"); return SPMV_ERR_INVALID_ARG; }
+  const int64_t n = h->A.rows;
+  if (n > 0 && (!d_b || !d_x)) return SPMV_ERR_INVALID_ARG;
+  spmv_cg_opts_t o{};
+  if (opts) o = *opts;
+  const double tol = o.tol > 0 ? o.tol : 1e-10;
+  const int max_iters = o.max_iters > 0 ? o.max_iters : (o.max_iters < 0 ? 0 : 1000);
+  const int check_every = o.check_every > 0 ? o.check_every : 8;
+  const bool use_graph = o.no_graph == 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  memset(result, 0, sizeof(*result));
+  if (n == 0) { result->converged = 1; return SPMV_OK; }
+
+  const int nb = (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * 8);
+  const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + 3 * (size_t)nb) + sizeof(CgState);
+  double* ws = (double*)h->al.alloc(ws_bytes, s);
+  if (!ws) return SPMV_ERR_ALLOC;
+  double *r = ws, *p = r + n, *q = p + n, *part_rr = q + n, *part_bb = part_rr + nb, *part_pq = part_bb + nb;
+  CgState* st = (CgState*)(part_pq + nb);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  auto cleanup = [&]() {
+    if (gexec) cudaGraphExecDestroy(gexec);
+    if (graph) cudaGraphDestroy(graph);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaStreamSynchronize(s);
+    h->al.free(ws, ws_bytes);
+  };
+  auto fail = [&](spmv_status_t code) { cleanup(); return code; };
+  auto iteration = [&]() -> spmv_status_t {
+    ApplyArgs a{1.0, 0.0, p, q, s};
+    spmv_status_t st1 = launch_variant(h, h->sel, a);                       // q = A p
+    if (st1 != SPMV_OK) return st1;
+    cg_dot_kernel<<<nb, kCgBlock, 0, s>>>(n, p, q, part_pq, st);
+    cg_update_kernel<<<nb, kCgBlock, 0, s>>>(n, nb, part_pq, st, d_x, r, p, q, part_rr);
+    cg_pupdate_kernel<<<nb, kCgBlock, 0, s>>>(n, nb, part_rr, st, r, p);
+    cg_step_final_kernel<<<1, kCgBlock, 0, s>>>(nb, part_pq, part_rr, st, tol, max_iters);
+    return cudaGetLastError() == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
+  };
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(SPMV_ERR_CUDA);
+  const auto t0 = std::chrono::steady_clock::now();
+  cudaEventRecord(e0, s);
+  {
+    ApplyArgs a{1.0, 0.0, d_x, q, s};
+    spmv_status_t st1 = launch_variant(h, h->sel, a);                       // q = A x0
+    if (st1 != SPMV_OK) return fail(st1);
+  }
+  cg_init_kernel<<<nb, kCgBlock, 0, s>>>(n, d_b, q, r, p, part_rr, part_bb);
+  cg_init_final_kernel<<<1, kCgBlock, 0, s>>>(nb, part_rr, part_bb, st, tol, max_iters);
+  if (cudaGetLastError() != cudaSuccess) return fail(SPMV_ERR_CUDA);
+  CgState hs{};
+  int launched = 0, graph_replays = 0;
+  auto poll = [&]() -> bool {
+    return cudaMemcpyAsync(&hs, st, sizeof(hs), cudaMemcpyDeviceToHost, s) == cudaSuccess &&
+           cudaStreamSynchronize(s) == cudaSuccess;
+  };
+  if (!poll()) return fail(SPMV_ERR_CUDA);
+  if (!hs.done) {
+    // the first iteration runs un-captured: it settles function attributes and occupancy caches
+    spmv_status_t st1 = iteration();
+    if (st1 != SPMV_OK) return fail(st1);
+    ++launched;
+    if (use_graph && max_iters > 1) {
+      // the legacy default stream cannot be captured: plain launches then
+      if (s != nullptr && cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        for (int k = 0; k < check_every && st1 == SPMV_OK; ++k) st1 = iteration();
+        cudaError_t ce = cudaStreamEndCapture(s, &graph);
+        if (st1 != SPMV_OK || ce != cudaSuccess || !graph) { set_last_error("spmv_cg: graph capture failed"); return fail(SPMV_ERR_CUDA); }
+        if (cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) return fail(SPMV_ERR_CUDA);
+      } else {
+        cudaGetLastError();
+      }
+    }
+    for (;;) {
+      if (!poll()) return fail(SPMV_ERR_CUDA);
+      if (hs.done || launched >= max_iters + check_every) break;
+      if (gexec) {
+        if (cudaGraphLaunch(gexec, s) != cudaSuccess) return fail(SPMV_ERR_CUDA);
+        ++graph_replays;
+      } else {
+        for (int k = 0; k < check_every; ++k) { st1 = iteration(); if (st1 != SPMV_OK) return fail(st1); }
+      }
+      launched += check_every;
+    }
+  }
+  cudaEventRecord(e1, s);
+  cudaEventSynchronize(e1);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  result->iters = hs.iters;
+  result->converged = hs.converged;
+  result->breakdown = hs.breakdown;
+  result->rel_residual = hs.bb > 0.0 ? sqrt(hs.rr) / sqrt(hs.bb) : sqrt(hs.rr);
+  result->device_seconds = (double)ms * 1e-3;
+  result->wall_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+  result->iterations_launched = launched;
+  result->graph_replays = graph_replays;
+  cleanup();
+  return SPMV_OK;
+}
