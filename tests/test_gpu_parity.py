@@ -192,3 +192,31 @@ def test_update_values_keeps_the_variant_and_matches_oracle(cuda):
     assert S.update_values(torch.from_numpy(v4).cuda()) is True and S.variant.startswith("dia_tma")
     H.check_against_oracle(S, W.CSR(L.rows, L.cols, L.row_ptr, L.col_idx, v4), 1.0, xl, 0.0, None, what="fallback")
     S.close()
+
+
+def test_unaligned_vectors_take_the_fallback_paths(cuda):
+    """x / y that are only 8-byte aligned: the bulk-copy (TMA) paths that need 16-byte aligned global
+    addresses (dia_tma old-y stage, sell_tma x2 window) must fall back to plain loads, not fault."""
+    import torch
+    A = W.stencil3d_27pt(9, perturb_stream=51)
+    x, y0 = W.uniform(111, A.cols), W.uniform(112, A.rows)
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x, 0.5, y0)
+    S = binding.SpMV.from_csr(A)
+    for desc in ("dia_tma:b288:c256:r1:u9:i3:x0", "dia_tma:b96:c128:r2:u4:i2:x0", "sell_tma:b288:c256:s1:r1:u8:i3:x2:h136",
+                 "sell_tma:b160:c256:s1:r2:u4:i3:x0", "dia:b256:c128:r2:u4:x0", "sell:b256:c128:s1:r4:u2:x0",
+                 "bcsr3:b256:w8:u1:x0"):
+        if not _select_or_skip(S, desc):
+            continue
+        for xo, yo in ((1, 0), (0, 1), (1, 1)):
+            bx = torch.zeros(A.cols + 2, dtype=torch.float64, device="cuda")
+            by = torch.zeros(A.rows + 2, dtype=torch.float64, device="cuda")
+            dx, dy = bx[xo:xo + A.cols], by[yo:yo + A.rows]
+            assert dx.data_ptr() % 16 == 8 * xo and dy.data_ptr() % 16 == 8 * yo
+            dx.copy_(torch.from_numpy(x)); dy.copy_(torch.from_numpy(y0))
+            S.apply(1.0, dx, 0.5, dy)
+            torch.cuda.synchronize()
+            ok, mr, ff, nf = oracle.accept(dy.cpu().numpy(), y_ref, scale, H.TOL)
+            assert ok, (desc, xo, yo, nf, ff, mr)
+            assert float(by[0]) == 0.0 or yo == 0                 # nothing written before the view
+            assert float(by[yo + A.rows:].abs().sum()) == 0.0     # nor after it
+    S.close()
