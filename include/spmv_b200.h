@@ -123,7 +123,8 @@ typedef struct {
   int32_t cache_hit;
   char runner_up[128];
   double runner_up_us;
-  /* optional per-candidate log: "descriptor status time_us max_err_over_scale\n" */
+  /* optional per-candidate log: "descriptor status time_us max_err_over_scale\n"; status in
+   * {timed, timed1 (one batch only: > 25 % behind the leader), pruned_slow, pruned_format, rejected} */
   char* log_buf;
   size_t log_cap;
   size_t log_len;

@@ -191,7 +191,10 @@ struct Tuner {
   }
 
   // median time per apply over `reps` batches (warm: K applies; cold: K x (flush, apply) - K flushes)
-  spmv_status_t time(const Variant& v, double est_us, double* us) {
+  // Successive halving: after the first timed batch a candidate more than 25 % behind
+  // the current best keeps that single measurement (*quick = true) and the remaining batches are skipped.
+  spmv_status_t time(const Variant& v, double est_us, double best_us, double* us, bool* quick) {
+    *quick = false;
     ApplyArgs a{alpha, beta, x, y, s};
     for (int i = 0; i < warmup; ++i) {
       spmv_status_t st = launch_variant(h, v, a);
@@ -235,6 +238,7 @@ struct Tuner {
         spmv_status_t st = batch(true, &u);
         if (st != SPMV_OK) return st;
         t.push_back(std::max(u - flush_us, 0.01));
+        if (i == 0 && t[0] > 1.25 * best_us) { *quick = true; break; }
       }
     } else {
       int K = (int)(min_batch_ms * 1e3 / std::max(est_us, 1.0)) + 1;
@@ -250,6 +254,7 @@ struct Tuner {
         float ms = 0.f;
         SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
         t.push_back((double)ms * 1e3 / K);
+        if (i == 0 && t[0] > 1.25 * best_us) { *quick = true; break; }
       }
     }
     std::sort(t.begin(), t.end());
@@ -398,10 +403,11 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!pass) { ++n_rej; T.log(d, "rejected", vus, err); return SPMV_OK; }   // can never win
     if (!force_time && vus > 4.0 * best_us + 20.0) { ++n_slow; T.log(d, "pruned_slow", vus, err); return SPMV_OK; }
     double us = 0;
-    s1 = T.time(v, vus, &us);
+    bool quick = false;
+    s1 = T.time(v, vus, force_time ? 1e300 : best_us, &us, &quick);
     if (s1 != SPMV_OK) return s1;
     ++n_timed;
-    T.log(d, "timed", us, err);
+    T.log(d, quick ? "timed1" : "timed", us, err);
     ok.push_back(Scored{v, us});
     if (us < best_us) best_us = us;
     return SPMV_OK;

@@ -38,7 +38,7 @@ def test_tune_against_the_cpu_oracle_reference(cuda, cfg, scale):
     assert rep["winner_us"] <= rep["default_us"] * 1.001          # the default is a candidate too
     # every log line is accounted for
     kinds = {l[1] for l in rep["log"]}
-    assert kinds <= {"timed", "pruned_slow", "pruned_format", "rejected"}
+    assert kinds <= {"timed", "timed1", "pruned_slow", "pruned_format", "rejected"}
     H.check_against_oracle(S, A, prob.alpha, prob.x, prob.beta, prob.y0, what=f"cfg{cfg} winner")
     S.close()
 
