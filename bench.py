@@ -436,6 +436,20 @@ def main():
         for r in line["per_config"]:
             # unstructured columns: every x gather is its own L1->XBAR request (profiles/r01_cfg3_*.md)
             r["frac_of_gather_ceiling"] = r["gathers_per_s"] / 1e9 / ceil["random_gather_G_per_s_32MiB_table"]
+            # what bounds this config's winner and the fraction of that bound
+            if r["cfg"] == 1:
+                r["roofline"] = {"bound": "launch", "achieved": r["t_median_us"], "peak": ceil["empty_launch_us"],
+                                 "unit": "us (lower is better; cold apply vs empty-kernel launch)",
+                                 "frac": ceil["empty_launch_us"] / r["t_median_us"]}
+            elif r["cfg"] == 3:
+                r["roofline"] = {"bound": "l1-xbar gather requests", "achieved": r["gathers_per_s"] / 1e9,
+                                 "peak": ceil["random_gather_G_per_s_32MiB_table"], "unit": "G gathers/s",
+                                 "frac": r["frac_of_gather_ceiling"]}
+            else:
+                r["roofline"] = {"bound": "hbm", "achieved": r["eff_gbs"], "peak": peak, "unit": "GB/s",
+                                 "frac": r["eff_gbs"] / peak, "actual_gbs": r["format_gbs"],
+                                 "frac_actual": r["format_gbs"] / peak,
+                                 "traffic": ncu_traffic(r["variant"], r["cfg"])}
     if rank == 0 and not args.no_cpu_baseline:
         t = cpu_oracle_times(head_prob)
         nb = W.algorithmic_bytes(head_prob.A.rows, head_prob.A.cols, head_prob.A.nnz, head_prob.beta)
