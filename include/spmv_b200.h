@@ -28,6 +28,23 @@
  *     rows == 0 and nnz == 0 are valid.
  *   - There is no CPU fallback: without a CUDA device every compute entry point
  *     returns SPMV_ERR_CUDA.
+ *   - Concurrency: distinct handles are independent.  One handle may have several applies in
+ *     flight on different streams only if its selected variant has no workspace; merge-path
+ *     (tile carries) and row-split SELL (segment sums) own one workspace per handle, so their
+ *     applies must be ordered (same stream, or events).  spmv_cg allocates per call.
+ *
+ * Variant descriptors (spmv_select, tune reports, spmv_list_variants): "family:key<int>:..."
+ *   families  csr_scalar (thread per row), csr_vector (w lanes per row), sell / sell_tma
+ *             (SELL-C-sigma; _tma: matrix stream by cp.async.bulk + mbarrier ring), ell, merge
+ *             (merge-path), bcsr3 (3x3 blocks), dia / dia_tma (diagonals, no column indices),
+ *             dia_const (constant-coefficient stencil: no matrix values read)
+ *   keys      b threads per block | g grid: 0/absent exact cover, k = k waves of resident blocks |
+ *             co shared-memory carve-out percent | u unroll (sell_tma/dia_tma: steps per stage) |
+ *             r rows per thread | w lanes per (block) row | x x path: 0 ld.global.nc, 1 ld.global,
+ *             2 window staged in shared memory (+ h = window half-width) | c slice height |
+ *             s sorting window sigma | l row-split length (rows longer than l become segments) |
+ *             i merge items per thread (sell_tma/dia_tma: pipeline stages)
+ *   "default" = csr_scalar:b256:r1:u1:x0, the fixed default variant.
  */
 #ifndef SPMV_B200_H
 #define SPMV_B200_H
