@@ -236,6 +236,13 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     # ---- default variant, then tune (tuning is setup, outside the timed region)
     streams, nstreams = [torch.cuda.current_stream()], 1
     tsum_d, tmed_d, _ = timed(max(10, args.steps // 10), 3)
+    # second fixed baseline (SURVEY A17 "heuristic default"): sub-warp width = smallest power of two >= mean row length
+    mean_len = handles[0].info().mean_row_len
+    w_h = int(min(32, max(2, 2 ** int(np.ceil(np.log2(max(mean_len, 1.0)))))))
+    heuristic = f"csr_vector:b256:w{w_h}:u1:x0"
+    for h in handles:
+        h.select(heuristic)
+    _, tmed_h, _ = timed(max(10, args.steps // 10), 3)
     t0 = time.perf_counter()
     reports = [h.tune(alpha=alpha, beta=beta, use_cache=(0 if (i or args.tune_cache) else 2),
                       cache_path=args.tune_cache, flush_l2=(mode != "warm"), seed=cfg,
@@ -268,6 +275,20 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
                 one_step()
             torch.cuda.synchronize()
     clocks = sampler.stop() if sampler is not None else None
+
+    # ---- the other cache state: warm (same buffers back to back) for the configs whose headline is cold
+    t_warm_us = None
+    if mode != "warm" and members == 1:
+        for _ in range(5):
+            handles[0].apply(alpha, xs[0], beta, ys[0])
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            handles[0].apply(alpha, xs[0], beta, ys[0])
+        b.record()
+        torch.cuda.synchronize()
+        t_warm_us = a.elapsed_time(b) * 1e3 / args.steps
 
     # ---- parity of what was just timed (sampled rows through the oracle would need the CPU
     # oracle; the full check lives in tests/ -- here: determinism + finite output)
@@ -335,6 +356,9 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
                          * args.steps / tsum / 1e9,
            "gathers_per_s": nnz * args.steps / tsum, "gflops": 2.0 * nnz * args.steps / tsum / 1e9,
            "t_default_us": tmed_d * 1e6, "speedup_vs_default": tmed_d / tmed,
+           "heuristic_variant": heuristic, "t_heuristic_us": tmed_h * 1e6, "speedup_vs_heuristic": tmed_h / tmed,
+           "t_warm_us": t_warm_us if t_warm_us is not None else tmed * 1e6,
+           "t_cold_us": tmed * 1e6 if mode != "warm" else None,
            "tune_seconds": tune_s, "tune_reports": [{k: v for k, v in r.items() if k != "log"} for r in reports],
            "launches_per_step": launches_per_step, "timing": {"rotate": f"cold: steps rotate over {copies} device copies of the inputs (footprint > 3x L2), back to back in one event pair",
                       "flush": "cold: 2xL2 buffer overwritten before every step, per-step events",
@@ -433,6 +457,12 @@ def main():
                 "empty_launch_us": binding.measure_ceiling(2, 0, 200),
                 "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}
         line["ceilings"] = ceil
+        try:
+            cpu_model = [l.split(":", 1)[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")][0]
+        except Exception:
+            cpu_model = "unknown"
+        line["host"] = {"cpu_model": cpu_model, "cores": os.cpu_count(), "cuda": torch.version.cuda,
+                        "driver": torch.cuda.get_device_properties(device).name, "torch": torch.__version__}
         for r in line["per_config"]:
             # unstructured columns: every x gather is its own L1->XBAR request (profiles/r01_cfg3_*.md)
             r["frac_of_gather_ceiling"] = r["gathers_per_s"] / 1e9 / ceil["random_gather_G_per_s_32MiB_table"]

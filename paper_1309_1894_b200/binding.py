@@ -131,6 +131,25 @@ def _stream_ptr(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
+def _raw_current_stream(device_index):
+    """cudaStream_t of torch's current stream as an int (the fast private accessor when torch has it)."""
+    import torch
+    try:
+        return torch._C._cuda_getCurrentRawStream(device_index if device_index is not None else torch.cuda.current_device())
+    except AttributeError:
+        return torch.cuda.current_stream().cuda_stream
+
+
+_apply = None
+
+
+def _apply_fn():
+    global _apply
+    if _apply is None:
+        _apply = lib().spmv_apply
+    return _apply
+
+
 def _dptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
 
@@ -212,10 +231,13 @@ class SpMV:
         return [l for l in buf.value.decode().split("\n") if l]
 
     def apply(self, alpha, x, beta, y, stream=None):
-        """y = alpha*A*x + beta*y on the device, asynchronous on the (current) stream."""
-        assert x.is_cuda and y.is_cuda and x.numel() == self.cols and y.numel() == self.rows
-        _check(lib().spmv_apply(self.h, float(alpha), _dptr(x), float(beta), _dptr(y), _stream_ptr(stream)),
-               "spmv_apply")
+        """y = alpha*A*x + beta*y on the device, asynchronous on the (current) stream.
+        Kept lean: for small matrices the call overhead is what a user sees."""
+        assert x.numel() == self.cols and y.numel() == self.rows and x.is_cuda and y.is_cuda
+        s = _raw_current_stream(x.device.index) if stream is None else stream.cuda_stream
+        st = _apply_fn()(self.h, alpha, x.data_ptr(), beta, y.data_ptr(), s)
+        if st != SPMV_OK:
+            _check(st, "spmv_apply")
         return y
 
     def update_values(self, val, stream=None) -> bool:
