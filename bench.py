@@ -341,7 +341,9 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
         cg = {"iters": best["iters"], "us_per_iteration": best["device_seconds"] / max(best["iters"], 1) * 1e6,
               "eff_gbs": it_bytes * best["iters"] / best["device_seconds"] / 1e9,
               "rel_residual": best["rel_residual"], "graph_replays": best["graph_replays"],
-              "launches_per_iteration": 4 + launches_per_step, "bytes_per_iteration_algorithmic": it_bytes}
+              "fused_single_kernel": bool(best["fused"]),
+              "launches_per_iteration": 0 if best["fused"] else 4 + launches_per_step,
+              "bytes_per_iteration_algorithmic": it_bytes}
     info = handles[0].info()
     peak_meas, _ = measured_peak()
     eff = nbytes * args.steps / tsum / 1e9

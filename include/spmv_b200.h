@@ -212,11 +212,14 @@ typedef struct {
   int32_t max_iters;     /* 0 -> 1000; negative -> 0 iterations (residual of the initial guess only) */
   int32_t check_every;   /* 0 -> 8 */
   int32_t no_graph;      /* 1: never use a CUDA graph */
+  int32_t no_fused;      /* 1: never use the single cooperative kernel that runs the whole solve for small
+                            systems (rows <= 262144, nnz <= 4 Mi): launch-bound otherwise */
 } spmv_cg_opts_t;
 typedef struct {
   int32_t iters, converged, breakdown;
   int32_t iterations_launched;   /* >= iters: iterations issued after convergence are device-side no-ops */
   int32_t graph_replays;
+  int32_t fused;                 /* 1: the whole solve ran in the single cooperative kernel */
   double rel_residual;           /* sqrt(r.r) / ||b||  (sqrt(r.r) when b == 0) */
   double device_seconds;         /* CUDA events around the whole solve */
   double wall_seconds;

@@ -10,6 +10,7 @@
 // (x and r update + r.r partials in one pass; p update reads the new partials), reductions are
 // two-level with a fixed shape (per-block partials, then every block re-adds the partials in the same
 // order), so the iterates are bit-identical across runs (reading A20).  No atomics.
+#include <cooperative_groups.h>
 #include <math.h>
 #include <string.h>
 
@@ -140,6 +141,83 @@ cg_step_final_kernel(int nb, const double* __restrict__ part_pq, const double* _
   }
 }
 
+// ------------------------------------------------------------------ small systems: the whole solve in ONE kernel
+// When every row fits in one resident grid the loop is launch-bound (five graph nodes per iteration cost
+// ~3 us each on a 4096-row system).  This cooperative kernel runs all iterations with three grid-wide
+// barriers per iteration and no launch in between: q = A p straight from the caller's CSR arrays (thread
+// per row, the matrix is cache-resident at this size) with the p.q partial fused into the same pass, then
+// the x/r update with the r.r partial, then the p update.  Same recurrence, same stop rule, fixed
+// reduction shape (deterministic); every block derives the scalars from the partials in the same order.
+__global__ void __launch_bounds__(kCgBlock)
+cg_fused_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci, const double* __restrict__ va,
+                const double* __restrict__ b, double* __restrict__ x, double* __restrict__ r,
+                double* __restrict__ p, double* __restrict__ q, double* __restrict__ part_a,
+                double* __restrict__ part_b, CgState* __restrict__ st, double tol, int max_iters) {
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  __shared__ double s_red[kCgBlock];
+  const int nb = gridDim.x;
+  const int64_t G = (int64_t)nb * kCgBlock, t0 = (int64_t)blockIdx.x * kCgBlock + threadIdx.x;
+  auto row_dot = [&](int64_t i, const double* __restrict__ v) {
+    double s = 0.0;
+    for (int k = rp[i]; k < rp[i + 1]; ++k) s = fma(va[k], v[ci[k]], s);
+    return s;
+  };
+  // r0 = b - A x0, p0 = r0
+  double a = 0.0, c = 0.0;
+  for (int64_t i = t0; i < n; i += G) {
+    const double bi = b[i], ri = bi - row_dot(i, x);
+    r[i] = ri; p[i] = ri;
+    a = fma(ri, ri, a);
+    c = fma(bi, bi, c);
+  }
+  a = cg_block_sum(a, s_red);
+  c = cg_block_sum(c, s_red);
+  if (threadIdx.x == 0) { part_a[blockIdx.x] = a; part_b[blockIdx.x] = c; }
+  grid.sync();
+  double rr = cg_sum_partials(part_a, nb, s_red);
+  const double bb = cg_sum_partials(part_b, nb, s_red);
+  const double stop = tol * sqrt(bb);
+  int k = 0, breakdown = 0;
+  grid.sync();                                   // part_a / part_b are reused below
+  while (!(sqrt(rr) <= stop) && k < max_iters) {
+    double pq = 0.0;
+    for (int64_t i = t0; i < n; i += G) {        // q = A p, fused with the p.q partial
+      const double qi = row_dot(i, p);
+      q[i] = qi;
+      pq = fma(p[i], qi, pq);
+    }
+    pq = cg_block_sum(pq, s_red);
+    if (threadIdx.x == 0) part_a[blockIdx.x] = pq;
+    grid.sync();
+    pq = cg_sum_partials(part_a, nb, s_red);
+    if (!(pq > 0.0)) { breakdown = 1; break; }   // uniform across the grid: every block sees the same pq
+    const double alpha = rr / pq;
+    double rn = 0.0;
+    for (int64_t i = t0; i < n; i += G) {
+      x[i] = fma(alpha, p[i], x[i]);
+      const double ri = fma(-alpha, q[i], r[i]);
+      r[i] = ri;
+      rn = fma(ri, ri, rn);
+    }
+    rn = cg_block_sum(rn, s_red);
+    if (threadIdx.x == 0) part_b[blockIdx.x] = rn;
+    grid.sync();
+    rn = cg_sum_partials(part_b, nb, s_red);
+    const double beta = rn / rr;
+    rr = rn;
+    for (int64_t i = t0; i < n; i += G) p[i] = fma(beta, p[i], r[i]);
+    ++k;
+    grid.sync();                                 // p complete before the next product
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    st->rr = rr; st->bb = bb; st->pq = 0.0;
+    st->iters = k; st->breakdown = breakdown;
+    st->converged = sqrt(rr) <= stop;
+    st->done = 1;
+  }
+}
+
 }  // namespace spmv
 
 using namespace spmv;
@@ -160,7 +238,16 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   memset(result, 0, sizeof(*result));
   if (n == 0) { result->converged = 1; return SPMV_OK; }
 
-  const int nb = (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * 8);
+  // small systems: one cooperative kernel for the whole solve (see cg_fused_kernel)
+  int fused_blocks = 0;
+  if (o.no_fused == 0 && n <= 262144 && h->A.nnz <= 4 * 1024 * 1024) {
+    int occ = 0, coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+    if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)cg_fused_kernel, kCgBlock, 0) == cudaSuccess && occ > 0)
+      fused_blocks = (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * occ);
+  }
+  const int nb = fused_blocks > 0 ? fused_blocks
+                                  : (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * 8);
   const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + 3 * (size_t)nb) + sizeof(CgState);
   double* ws = (double*)h->al.alloc(ws_bytes, s);
   if (!ws) return SPMV_ERR_ALLOC;
@@ -191,6 +278,23 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(SPMV_ERR_CUDA);
   const auto t0 = std::chrono::steady_clock::now();
   cudaEventRecord(e0, s);
+  CgState hs{};
+  int launched = 0, graph_replays = 0;
+  if (fused_blocks > 0) {
+    int64_t n_arg = n;
+    const int *rp = h->A.row_ptr, *ci = h->A.col_idx;
+    const double *va = h->A.val, *bb = d_b;
+    double tol_arg = tol;
+    int mi = max_iters;
+    void* args[] = {&n_arg, &rp, &ci, &va, &bb, &d_x, &r, &p, &q, &part_rr, &part_bb, &st, &tol_arg, &mi};
+    if (cudaLaunchCooperativeKernel((const void*)cg_fused_kernel, dim3(fused_blocks), dim3(kCgBlock), args, 0, s) != cudaSuccess) {
+      set_last_error("spmv_cg: cooperative launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      return fail(SPMV_ERR_CUDA);
+    }
+    if (cudaMemcpyAsync(&hs, st, sizeof(hs), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+      return fail(SPMV_ERR_CUDA);
+    launched = hs.iters;
+  } else {
   {
     ApplyArgs a{1.0, 0.0, d_x, q, s};
     spmv_status_t st1 = launch_variant(h, h->sel, a);                       // q = A x0
@@ -199,8 +303,6 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   cg_init_kernel<<<nb, kCgBlock, 0, s>>>(n, d_b, q, r, p, part_rr, part_bb);
   cg_init_final_kernel<<<1, kCgBlock, 0, s>>>(nb, part_rr, part_bb, st, tol, max_iters);
   if (cudaGetLastError() != cudaSuccess) return fail(SPMV_ERR_CUDA);
-  CgState hs{};
-  int launched = 0, graph_replays = 0;
   auto poll = [&]() -> bool {
     return cudaMemcpyAsync(&hs, st, sizeof(hs), cudaMemcpyDeviceToHost, s) == cudaSuccess &&
            cudaStreamSynchronize(s) == cudaSuccess;
@@ -234,6 +336,7 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
       launched += check_every;
     }
   }
+  }
   cudaEventRecord(e1, s);
   cudaEventSynchronize(e1);
   float ms = 0.f;
@@ -246,6 +349,7 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   result->wall_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
   result->iterations_launched = launched;
   result->graph_replays = graph_replays;
+  result->fused = fused_blocks > 0;
   cleanup();
   return SPMV_OK;
 }

@@ -36,10 +36,10 @@ def test_cg_solves_the_laplacian_like_the_oracle(cuda, desc):
     with torch.cuda.stream(stream):
         db = H.to_dev(b)
         dx = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
-        res = S.cg(db, dx, tol=tol, max_iters=500)
+        res = S.cg(db, dx, tol=tol, max_iters=500, no_fused=True)      # the multi-kernel path (any size)
         stream.synchronize()
         x = dx.cpu().numpy()
-        assert res["converged"] == 1 and res["breakdown"] == 0 and res["graph_replays"] >= 1
+        assert res["converged"] == 1 and res["breakdown"] == 0 and res["graph_replays"] >= 1 and res["fused"] == 0
         assert abs(res["iters"] - k_ref) <= 3, (res, k_ref)
         assert res["rel_residual"] <= tol
         assert _true_rel_res(A, x, b) <= 2 * tol              # recurrence residual ~ true residual
@@ -47,9 +47,9 @@ def test_cg_solves_the_laplacian_like_the_oracle(cuda, desc):
         assert np.abs(x - xt).max() <= 1e-6
         # bit-identical repeat; plain launches equal graph replay bit for bit
         dx2 = torch.zeros_like(dx)
-        res2 = S.cg(db, dx2, tol=tol, max_iters=500)
+        res2 = S.cg(db, dx2, tol=tol, max_iters=500, no_fused=True)
         dx3 = torch.zeros_like(dx)
-        res3 = S.cg(db, dx3, tol=tol, max_iters=500, no_graph=True)
+        res3 = S.cg(db, dx3, tol=tol, max_iters=500, no_graph=True, no_fused=True)
         stream.synchronize()
         assert torch.equal(dx, dx2) and torch.equal(dx, dx3)
         assert res2["iters"] == res["iters"] == res3["iters"] and res3["graph_replays"] == 0
@@ -112,3 +112,31 @@ def test_cg_after_tune_on_cfg1(cuda):
     assert res["converged"] == 1 and abs(res["iters"] - k_ref) <= 5
     assert np.abs(x - prob.x).max() <= 1e-7 and _true_rel_res(A, x, b) <= 2e-11
     S.close()
+
+
+def test_cg_fused_single_kernel_for_small_systems(cuda):
+    """rows <= 262144: the whole solve runs in one cooperative kernel (3 grid barriers per iteration,
+    no launches).  Same recurrence and stop rule as the multi-kernel path and the oracle."""
+    import torch
+    for A, cond in ((W.laplace2d_5pt(64), 1800.0), (W.laplace3d_7pt(40), 700.0)):
+        xt = W.uniform(121, A.rows)
+        b, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, xt, 0.0)
+        tol = 1e-10
+        x_ref, k_ref, _, _ = oracle.cg(A.row_ptr, A.col_idx, A.val, b, tol=tol, max_iters=2000)
+        S = binding.SpMV.from_csr(A)
+        db = H.to_dev(b)
+        dx = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
+        res = S.cg(db, dx, tol=tol, max_iters=2000)
+        x = dx.cpu().numpy()
+        assert res["fused"] == 1 and res["converged"] == 1 and res["graph_replays"] == 0
+        assert abs(res["iters"] - k_ref) <= 5 and res["rel_residual"] <= tol
+        assert _true_rel_res(A, x, b) <= 2 * tol
+        assert np.abs(x - x_ref).max() <= 2 * tol * cond * np.abs(x_ref).max()
+        dx2 = torch.zeros_like(dx)
+        res2 = S.cg(db, dx2, tol=tol, max_iters=2000)
+        assert torch.equal(dx, dx2) and res2["iters"] == res["iters"]          # deterministic
+        dx3 = torch.zeros_like(dx)
+        res3 = S.cg(db, dx3, tol=tol, max_iters=2000, no_fused=True)           # multi-kernel path agrees
+        assert res3["fused"] == 0 and abs(res3["iters"] - res["iters"]) <= 5
+        assert np.abs(dx3.cpu().numpy() - x).max() <= 2 * tol * cond * np.abs(x).max()
+        S.close()
