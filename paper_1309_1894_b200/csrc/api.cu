@@ -163,7 +163,7 @@ spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* 
     if (fell_back) *fell_back = 1;
     Variant alt = h->sel;
     st = SPMV_ERR_UNSUPPORTED;
-    if (h->sel.fam == FAM_DIA_CONST && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
+    if ((h->sel.fam == FAM_DIA_CONST || h->sel.fam == FAM_DIA_CWIN) && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
       std::string why;
       if (variant_eligible(h, alt, &why)) st = ensure_format(h, alt, s);
     }
@@ -257,7 +257,7 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
     if (!strcmp(name, "brow_ptr")) { src = h->bcsr.brow_ptr; n = sizeof(int32_t) * (h->bcsr.brows + 1); }
     else if (!strcmp(name, "bcol")) { src = h->bcsr.bcol; n = sizeof(int32_t) * h->bcsr.nblocks; }
     else if (!strcmp(name, "bval")) { src = h->bcsr.bval; n = sizeof(double) * 9 * h->bcsr.nblocks; }
-  } else if ((v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) && h->dias.count(v.C)) {
+  } else if ((v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) && h->dias.count(v.C)) {
     const DiaFormat& df = h->dias[v.C];
     if (!strcmp(name, "dia_val")) { src = df.val; n = sizeof(double) * df.nd * df.ld; }
     else if (!strcmp(name, "dia_mask")) { src = df.mask; n = sizeof(unsigned) * df.ld; }

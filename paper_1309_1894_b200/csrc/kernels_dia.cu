@@ -564,6 +564,7 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
   f.C = C;
   f.logC = C == 128 ? 7 : C == 256 ? 8 : 9;
   f.ld = ((A.rows + C - 1) / C) * C;
+  dia_compute_windows(f);
   f.val = (double*)al.alloc(sizeof(double) * nd * f.ld, s);
   f.mask = (unsigned*)al.alloc(sizeof(unsigned) * f.ld, s);
   if (!f.val || !f.mask) { free_dia(f, al); return SPMV_ERR_ALLOC; }

@@ -70,6 +70,13 @@ struct DiaFormat {
   // diagonal holds the same bit pattern; coef[d] is that value.  dia_const then reads no matrix values.
   bool is_const = false;
   double coef[32] = {0};
+  // x windows for the dia_win kernels (kernels_dia_win.cu): groups of near-consecutive offsets share one
+  // contiguous window of x per slice
+  int ng = 0, win_total = 0;     // groups; total window entries per slice
+  int g_lo[32] = {0};            // window start relative to the slice's first row (even)
+  int g_len[32] = {0};           // window length (even)
+  int g_dst[32] = {0};           // offset of the window inside the stage's window area
+  int d_xoff[32] = {0};          // per diagonal: index of x[s*C + off[d]] inside the window area
 };
 
 // Merge-path plan: tile t covers merge-path diagonals [t*tile_items, (t+1)*tile_items);
@@ -83,7 +90,7 @@ struct MergePlan {
 };
 
 // ---------------------------------------------------------------- variants
-enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_DIA_CONST, FAM_COUNT };
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_DIA_CONST, FAM_DIA_WIN, FAM_DIA_CWIN, FAM_COUNT };
 
 struct Variant {
   int fam = FAM_CSR_SCALAR;
@@ -152,6 +159,11 @@ cudaError_t dia_launch(const Variant&, int64_t rows, const DiaFormat&, const App
 bool dia_const_supported(const Variant&);
 const void* dia_const_func(const Variant&);
 cudaError_t dia_const_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+bool dia_win_supported(const Variant&);
+const void* dia_win_func(const Variant&);
+bool dia_win_fits(const Variant&, const DiaFormat&);
+cudaError_t dia_win_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);
+void dia_compute_windows(DiaFormat& f);
 bool dia_tma_supported(const Variant&);
 const void* dia_tma_func(const Variant&);
 cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);

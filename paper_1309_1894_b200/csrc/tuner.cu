@@ -111,9 +111,13 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     if (in.max_row_len > 0 && J > in.max_row_len + 1 && J != 4) { ++*n_pruned; continue; }   // stage deeper than the row
     all.push_back(v);
   }
+  for (int fam : {(int)FAM_DIA_WIN, (int)FAM_DIA_CWIN}) for (int C : {128, 256, 512}) for (int R : {1, 2}) for (int ST : {2, 3}) {
+    Variant v; v.fam = fam; v.C = C; v.R = R; v.I = ST; v.block = C / R + 32;
+    all.push_back(v);
+  }
   // family, then format key, outermost: formats are then built once per key
   std::stable_sort(all.begin(), all.end(), [](const Variant& a, const Variant& b) {
-    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : (v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) ? (int)FAM_DIA : v.fam; };
+    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : (v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : v.fam; };
     if (grp(a) != grp(b)) return grp(a) < grp(b);
     if (a.C != b.C) return a.C < b.C;
     if (a.S != b.S) return a.S < b.S;
@@ -424,7 +428,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!budget_left()) break;
     if (variant_to_string(v) == variant_to_string(dflt)) continue;
     // keep device memory bounded: drop formats when the family / format key changes
-    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : (q.fam == FAM_DIA_TMA || q.fam == FAM_DIA_CONST) ? (int)FAM_DIA : q.fam; };
+    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : (q.fam == FAM_DIA_TMA || q.fam == FAM_DIA_CONST || q.fam == FAM_DIA_WIN || q.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : q.fam; };
     if (grp(v) != grp(last_fmt) || v.C != last_fmt.C || v.S != last_fmt.S || v.L != last_fmt.L) {
       Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
       release_formats_except(h, keep);
@@ -444,7 +448,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     for (int g : {0, 1, 2, 4, 8}) for (int co : carves) {
       if (g == 0 && co == -1) continue;
       if (L.fam == FAM_MERGE && g != 0) continue;
-      if ((L.fam == FAM_SELL_TMA || L.fam == FAM_DIA_TMA) && (g == 0 || g == 8)) continue;   // persistent: g = waves of resident CTAs
+      if ((L.fam == FAM_SELL_TMA || L.fam == FAM_DIA_TMA || L.fam == FAM_DIA_WIN || L.fam == FAM_DIA_CWIN) && (g == 0 || g == 8)) continue;   // persistent: g = waves of resident CTAs
       if (!budget_left()) break;
       Variant v = L; v.grid = g; v.carve = co;
       if (!filter_match(o.variant_filter, variant_to_string(v))) continue;

@@ -43,7 +43,7 @@ void Allocator::free(void* p, size_t bytes) {
 }
 
 // ------------------------------------------------------------------ descriptors
-static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma", "dia_const"};
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma", "dia_const", "dia_win", "dia_cwin"};
 
 Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
 
@@ -61,6 +61,8 @@ std::string variant_to_string(const Variant& v) {
     case FAM_DIA: add("c", v.C); add("r", v.R); add("u", v.U); break;
     case FAM_DIA_TMA: add("c", v.C); add("r", v.R); add("u", v.U); add("i", v.I); break;
     case FAM_DIA_CONST: add("r", v.R); break;
+    case FAM_DIA_WIN:
+    case FAM_DIA_CWIN: add("c", v.C); add("r", v.R); add("i", v.I); break;
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
@@ -91,6 +93,7 @@ bool variant_from_string(const char* s, Variant* out) {
   if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
   if (fam == FAM_DIA || fam == FAM_DIA_CONST) v.C = 128;
   if (fam == FAM_DIA_TMA) { v.C = 256; v.U = 8; v.I = 3; v.block = 288; }
+  if (fam == FAM_DIA_WIN || fam == FAM_DIA_CWIN) { v.C = 256; v.I = 2; v.block = 288; }
   while ((tok = strtok_r(nullptr, ":", &save))) {
     char* end = nullptr;
     if (!strncmp(tok, "co", 2)) { v.carve = (int)strtol(tok + 2, &end, 10); }
@@ -130,6 +133,8 @@ static bool template_supported(const Variant& v) {
     case FAM_DIA: return dia_supported(v);
     case FAM_DIA_TMA: return dia_tma_supported(v);
     case FAM_DIA_CONST: return dia_const_supported(v);
+    case FAM_DIA_WIN:
+    case FAM_DIA_CWIN: return dia_win_supported(v);
   }
   return false;
 }
@@ -148,8 +153,9 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
   }
-  if (v.fam == FAM_DIA_CONST && h->dia_state == 2) return no("coefficients are not constant along the diagonals");
-  if (v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST) {
+  if ((v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_CWIN) && h->dia_state == 2)
+    return no("coefficients are not constant along the diagonals");
+  if (v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) {
     if (!in.cols_sorted) return no("DIA needs sorted unique columns");
     if (in.max_row_len > 32 || in.nnz == 0) return no("more than 32 entries in a row: more than 32 diagonals");
     if (h->dia_state < 0) return no("pattern is not a set of at most 32 (half-full) diagonals");
@@ -195,11 +201,16 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
       if (st == SPMV_OK) h->has_bcsr = true;
       return st;
     }
+    case FAM_DIA_WIN:
+    case FAM_DIA_CWIN:
     case FAM_DIA_CONST:
     case FAM_DIA_TMA:
     case FAM_DIA: {
+      const bool need_const = v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_CWIN;
+      const bool is_win = v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN;
       if (h->dias.count(v.C)) {
-        if (v.fam == FAM_DIA_CONST && !h->dias[v.C].is_const) return SPMV_ERR_UNSUPPORTED;
+        if (need_const && !h->dias[v.C].is_const) return SPMV_ERR_UNSUPPORTED;
+        if (is_win && !dia_win_fits(v, h->dias[v.C])) { set_last_error("dia_win: a slice does not fit in shared memory"); return SPMV_ERR_UNSUPPORTED; }
         return SPMV_OK;
       }
       if (h->dia_state < 0) return SPMV_ERR_UNSUPPORTED;
@@ -208,7 +219,8 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
       if (st == SPMV_OK) {
         h->dias[v.C] = f;
         h->dia_state = f.is_const ? 1 : 2;       // 2: diagonal pattern, but values vary along the diagonals
-        if (v.fam == FAM_DIA_CONST && !f.is_const) return SPMV_ERR_UNSUPPORTED;
+        if (need_const && !f.is_const) return SPMV_ERR_UNSUPPORTED;
+        if (is_win && !dia_win_fits(v, f)) { set_last_error("dia_win: a slice does not fit in shared memory"); return SPMV_ERR_UNSUPPORTED; }
       }
       else if (st == SPMV_ERR_UNSUPPORTED) h->dia_state = -1;
       return st;
@@ -236,7 +248,8 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   if (h->has_ell && keep.fam != FAM_ELL) { free_sell(h->ell, h->al); h->has_ell = false; }
   if (h->has_bcsr && keep.fam != FAM_BCSR3) { free_bcsr3(h->bcsr, h->al); h->has_bcsr = false; }
   for (auto it = h->dias.begin(); it != h->dias.end();) {
-    if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST) && it->first == keep.C) { ++it; continue; }
+    if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST || keep.fam == FAM_DIA_WIN ||
+         keep.fam == FAM_DIA_CWIN) && it->first == keep.C) { ++it; continue; }
     free_dia(it->second, h->al);
     it = h->dias.erase(it);
   }
@@ -266,10 +279,12 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
     case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
+    case FAM_DIA_CWIN:
     case FAM_DIA_CONST: {
       auto it = h->dias.find(v.C);
       return it == h->dias.end() ? 0 : A.rows * 4;       // the mask words are all that is read of the matrix
     }
+    case FAM_DIA_WIN:
     case FAM_DIA_TMA:
     case FAM_DIA: {
       auto it = h->dias.find(v.C);
@@ -306,6 +321,8 @@ static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
     case FAM_DIA: return dia_func(v);
     case FAM_DIA_TMA: return dia_tma_func(v);
     case FAM_DIA_CONST: return dia_const_func(v);
+    case FAM_DIA_WIN:
+    case FAM_DIA_CWIN: return dia_win_func(v);
   }
   return nullptr;
 }
@@ -322,7 +339,8 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       SPMV_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve));
       g_carve[fn] = v.carve;
     }
-    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA && v.fam != FAM_DIA_TMA) {
+    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA && v.fam != FAM_DIA_TMA && v.fam != FAM_DIA_WIN &&
+        v.fam != FAM_DIA_CWIN) {
       auto key = std::make_pair(fn, v.block);
       auto oi = g_occ.find(key);
       int occ = 0;
@@ -368,6 +386,13 @@ spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs
       if (!h->has_bcsr) return SPMV_ERR_INTERNAL;
       e = bcsr_launch(v, h->bcsr, a, grid_blocks);
       break;
+    case FAM_DIA_WIN:
+    case FAM_DIA_CWIN: {
+      auto it = h->dias.find(v.C);
+      if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
+      e = dia_win_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
+      break;
+    }
     case FAM_DIA_CONST: {
       auto it = h->dias.find(v.C);
       if (it == h->dias.end()) return SPMV_ERR_INTERNAL;

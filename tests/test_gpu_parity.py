@@ -204,7 +204,7 @@ def test_unaligned_vectors_take_the_fallback_paths(cuda):
     S = binding.SpMV.from_csr(A)
     for desc in ("dia_tma:b288:c256:r1:u9:i3:x0", "dia_tma:b96:c128:r2:u4:i2:x0", "sell_tma:b288:c256:s1:r1:u8:i3:x2:h136",
                  "sell_tma:b160:c256:s1:r2:u4:i3:x0", "dia:b256:c128:r2:u4:x0", "sell:b256:c128:s1:r4:u2:x0",
-                 "bcsr3:b256:w8:u1:x0"):
+                 "dia_win:b288:c256:r1:i2:x0", "dia_win:b96:c128:r2:i3:x0", "bcsr3:b256:w8:u1:x0"):
         if not _select_or_skip(S, desc):
             continue
         for xo, yo in ((1, 0), (0, 1), (1, 1)):
