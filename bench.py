@@ -353,6 +353,8 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
            "variant": variant, "nstreams": nstreams, "stream_times_us": stream_times,
            "t_sum_s": tsum, "t_median_us": tmed * 1e6, "t_min_us": tmin * 1e6,
            "eff_gbs": eff, "frac_hbm_nominal_8TBs": eff / NOMINAL_HBM_GBS, "frac_hbm_measured": eff / peak_meas,
+           "bytes_actual": int(sum(h.info().format_bytes for h in handles[:members]) +
+                               sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs)),
            "format_gbs": float(sum(h.info().format_bytes for h in handles[:members]) +
                                sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs))
                          * args.steps / tsum / 1e9,
@@ -455,7 +457,7 @@ def main():
         torch.cuda.synchronize()
         ceil = {"copy_gbs_1GiB": binding.measure_ceiling(0, 1 << 30, 5),
                 "read_gbs_1GiB": binding.measure_ceiling(1, 1 << 30, 5),
-                "read_gbs_at_headline_size": binding.measure_ceiling(1, max(1 << 20, int(head["bytes_format_actual"])), 5),
+                "read_gbs_at_headline_size": binding.measure_ceiling(1, max(1 << 20, int(head["bytes_actual"])), 5),
                 "empty_launch_us": binding.measure_ceiling(2, 0, 200),
                 "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}
         line["ceilings"] = ceil
