@@ -75,8 +75,6 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
                 double* __restrict__ y, int64_t cols, int H) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nconsumers = C / R;
-  const size_t val_bytes = (size_t)J * C * sizeof(double);
-  const size_t col_bytes = (size_t)J * C * sizeof(int);
   const int WIN = X == 2 ? C + 2 * H : 0;                                    // x window entries per stage
   double* s_val = reinterpret_cast<double*>(smem_raw);                       // [STAGES][J*C]
   double* s_x = s_val + (size_t)STAGES * J * C;                              // [STAGES][WIN]
