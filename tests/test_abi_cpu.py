@@ -62,3 +62,17 @@ def test_struct_sizes_match_header():
     # guards the ctypes mirrors against drift from include/spmv_b200.h (x86-64 layout)
     assert ctypes.sizeof(binding.Info) == 3 * 8 + 2 * 4 + 2 * 8 + 32 * 8 + 8 + 2 * 4 + 8 + 2 * 8 + 2 * 4 + 3 * 8 + 128 + 64
     assert ctypes.sizeof(binding.Allocator) == 24
+
+
+def test_sizes_over_the_int32_limits_are_unsupported(L):
+    """Limits (include/spmv_b200.h): rows, cols, nnz <= 2^31-1 -> SPMV_ERR_UNSUPPORTED, checked before any
+    device work (so it can be asserted without a GPU); negative sizes -> INVALID_ARG."""
+    import ctypes as C
+    h = C.c_void_p(0)
+    dummy = (C.c_int32 * 4)()
+    big = 1 << 31
+    for rows, cols, nnz in ((big, 10, 10), (10, big, 10), (10, 10, big)):
+        st = L.spmv_create(C.byref(h), C.c_int64(rows), C.c_int64(cols), C.c_int64(nnz), dummy, dummy, dummy, None, None)
+        assert st == 3 and not h.value
+    st = L.spmv_create(C.byref(h), C.c_int64(-1), C.c_int64(10), C.c_int64(10), dummy, dummy, dummy, None, None)
+    assert st == 1 and not h.value
