@@ -220,3 +220,40 @@ def test_unaligned_vectors_take_the_fallback_paths(cuda):
             assert float(by[0]) == 0.0 or yo == 0                 # nothing written before the view
             assert float(by[yo + A.rows:].abs().sum()) == 0.0     # nor after it
     S.close()
+
+
+def test_fuzz_random_matrices_random_variants(cuda):
+    """Seeded fuzz: random shapes / row-length laws / orderings x random candidates of the tuner's own
+    enumeration (plus the representative list) x random scalars, each against the oracle."""
+    rng = np.random.default_rng(2024)
+    n_checked = 0
+    for trial in range(24):
+        rows = int(rng.integers(1, 2500))
+        cols = int(rng.integers(1, 2500))
+        law = trial % 4
+        if law == 0:
+            lengths = rng.integers(0, min(cols, 12) + 1, rows)
+        elif law == 1:                                               # skewed: a few heavy rows
+            lengths = np.minimum((rng.pareto(1.2, rows) * 2).astype(np.int64), cols)
+        elif law == 2:                                               # many empty rows
+            lengths = np.where(rng.random(rows) < 0.7, 0, rng.integers(1, min(cols, 40) + 1, rows))
+        else:                                                        # constant length
+            lengths = np.full(rows, int(rng.integers(1, min(cols, 9) + 1)))
+        A = W.csr_from_lengths(lengths, cols, 200 + trial, sort=bool(trial % 3))
+        x = W.uniform(300 + trial, cols)
+        y0 = W.uniform(400 + trial, rows)
+        alpha, beta = float(rng.normal()), float(rng.choice([0.0, 1.0, -0.75]))
+        y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, alpha, x, beta, y0 if beta != 0.0 else None)
+        S = binding.SpMV.from_csr(A)
+        cands = S.variants()
+        pick = list(rng.choice(cands, size=min(10, len(cands)), replace=False)) + \
+            list(rng.choice(H.REPRESENTATIVE_VARIANTS, size=6, replace=False))
+        for desc in pick:
+            if not _select_or_skip(S, str(desc)):
+                continue
+            y = H.gpu_apply(S, alpha, x, beta, y0 if beta != 0.0 else None)
+            ok, mr, ff, nf = oracle.accept(y, y_ref, scale, H.TOL)
+            assert ok, (trial, rows, cols, law, str(desc), nf, ff, mr)
+            n_checked += 1
+        S.close()
+    assert n_checked > 200
