@@ -504,7 +504,7 @@ __global__ void dia_ref_first_kernel(int64_t rows, int C, int nd, const double* 
   if (r >= rows) return;
   const unsigned m = mask[r];
   for (int d = 0; d < nd; ++d)
-    if (((m >> d) & 1u) && atomicCAS(&seen[d], 0u, 1u) == 0u)
+    if (((m >> d) & 1u) && *(volatile unsigned*)&seen[d] == 0u && atomicCAS(&seen[d], 0u, 1u) == 0u)   // plain test first: no atomic storm
       ref[32 + d] = (unsigned long long)__double_as_longlong(dval[((r / C) * nd + d) * C + r % C]);
 }
 __global__ void dia_cmp_kernel(int64_t rows, int C, int nd, const double* __restrict__ dval,
