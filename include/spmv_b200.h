@@ -128,6 +128,12 @@ typedef struct {
                                  is perturbed before verification                       */
   uint64_t seed;
   int32_t flush_l2;           /* 1: overwrite a > L2-sized buffer before each timed launch */
+  int32_t search;             /* 0: exhaustive (every eligible candidate, the paper's loop);
+                                 1: feature-guided: only the families the structure
+                                 statistics predict -- diagonal pattern -> dia*, dense 3x3 blocks -> bcsr3,
+                                 skewed row lengths -> row-split sell + merge, otherwise sell_tma / sell /
+                                 csr_vector -- plus sell_tma and csr_vector as the fallback.  Every candidate
+                                 that is run is still verified before it may win. */
   void* stream;
 } spmv_tune_opts_t;
 

@@ -59,7 +59,7 @@ class TuneOpts(C.Structure):
                 ("min_batch_ms", C.c_double), ("time_budget_s", C.c_double),
                 ("variant_filter", C.c_char_p), ("n_carveouts", C.c_int32), ("carveouts", C.c_int32 * 8),
                 ("use_cache", C.c_int32), ("cache_path", C.c_char_p), ("fault_inject", C.c_char_p),
-                ("seed", C.c_uint64), ("flush_l2", C.c_int32), ("stream", C.c_void_p)]
+                ("seed", C.c_uint64), ("flush_l2", C.c_int32), ("search", C.c_int32), ("stream", C.c_void_p)]
 
 
 class CgOpts(C.Structure):
@@ -270,7 +270,7 @@ class SpMV:
     def tune(self, *, alpha=1.0, beta=0.0, x=None, y0=None, y_ref=None, scale=None, tolerance=0.0,
              warmup=0, reps=0, min_batch_ms=0.0, time_budget_s=0.0, variant_filter=None,
              carveouts=None, use_cache=0, cache_path=None, fault_inject=None, seed=0, flush_l2=False,
-             stream=None, log_bytes=1 << 20) -> dict:
+             stream=None, log_bytes=1 << 20, search=0) -> dict:
         o = TuneOpts()
         o.has_scalars, o.alpha, o.beta = 1, float(alpha), float(beta)
         o.d_x_probe, o.d_y0_probe = _dptr(x), _dptr(y0)
@@ -286,6 +286,7 @@ class SpMV:
         o.cache_path = cache_path.encode() if cache_path else None
         o.fault_inject = fault_inject.encode() if fault_inject else None
         o.seed, o.flush_l2, o.stream = int(seed), int(bool(flush_l2)), _stream_ptr(stream)
+        o.search = int(search)
         rep = TuneReport()
         logbuf = C.create_string_buffer(log_bytes) if log_bytes else None
         if logbuf is not None:

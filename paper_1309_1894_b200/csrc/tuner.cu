@@ -388,6 +388,24 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
   // ---- phase 1: every candidate, verify then time
   int n_pruned = 0;
   std::vector<Variant> cand = enumerate_candidates(h, o.variant_filter, &n_pruned);
+  if (o.search == 1) {
+    // feature-guided cut: keep the families the statistics point at, plus a generic fallback
+    const spmv_info_t& in = h->info;
+    const bool skew = in.var_row_len > 0.0 && (double)in.max_row_len > 4.0 * in.mean_row_len + 8.0;
+    const bool maybe_dia = in.cols_sorted && in.max_row_len <= 32 && in.nnz > 0 && h->dia_state >= 0;
+    auto keep = [&](const Variant& v) {
+      if (v.fam == FAM_SELL_TMA && v.L == 0 && v.X == 0) return !skew;                     // fallback (regular rows)
+      if (v.fam == FAM_CSR_VECTOR) return true;                                            // fallback (any matrix)
+      if (maybe_dia) return v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_CWIN;
+      if (in.block3_full) return v.fam == FAM_BCSR3;
+      if (skew) return v.fam == FAM_MERGE || ((v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) && v.L > 0);
+      return v.fam == FAM_SELL && v.S == 1;
+    };
+    std::vector<Variant> cut;
+    for (const Variant& v : cand)
+      if (keep(v)) cut.push_back(v); else ++n_pruned;
+    cand.swap(cut);
+  }
   const Variant dflt = default_variant();
   std::vector<Scored> ok;
   double best_us = 1e300, default_us = 0.0;

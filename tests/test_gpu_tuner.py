@@ -149,3 +149,21 @@ def test_tune_batch_picks_a_stream_count(cuda):
         assert oracle.accept(y.cpu().numpy(), y_ref, scale, H.TOL)[0]
     for h in hs:
         h.close()
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 0.5), (3, 0.03), (4, 0.25), (5, 0.5)])
+def test_feature_guided_search_finds_the_same_class_of_winner(cuda, cfg, scale):
+    """search=1: far fewer candidates, every one still verified, and the winner is as
+    fast as the exhaustive winner (same family; time within 15 %)."""
+    prob = W.config(cfg, scale)
+    A = prob.A
+    S = binding.SpMV.from_csr(A)
+    full = S.tune(alpha=prob.alpha, beta=prob.beta, use_cache=2, reps=3)
+    S2 = binding.SpMV.from_csr(A)
+    quick = S2.tune(alpha=prob.alpha, beta=prob.beta, use_cache=2, reps=3, search=1)
+    assert quick["n_rejected"] == 0 and quick["n_timed"] >= 5
+    assert quick["n_enumerated"] < 0.9 * full["n_enumerated"]
+    assert quick["tune_seconds"] < full["tune_seconds"]
+    assert quick["winner_us"] <= 1.15 * full["winner_us"], (quick["winner"], full["winner"])
+    H.check_against_oracle(S2, A, prob.alpha, prob.x, prob.beta, prob.y0, what=f"cfg{cfg} guided winner")
+    S.close(); S2.close()
