@@ -165,7 +165,7 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (v.L < 4 || v.L > 65536) return no("split length out of range");
     if (v.S <= 1) return no("row splitting needs a sorting window (s > 1)");
   }
-  if (v.fam == FAM_SELL || v.fam == FAM_ELL || v.fam == FAM_MERGE || v.fam == FAM_SELL_TMA) {
+  if (v.fam == FAM_MERGE) {      // the merge path has rows + nnz items and is indexed with int32
     if (in.rows + in.nnz > 0x7ffffff0ll) return no("rows+nnz over int32");
   }
   return true;

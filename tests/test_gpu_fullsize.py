@@ -75,3 +75,54 @@ def test_full_size_cfg5_batch_over_streams(cuda):
     print(f"cfg5: winner {hs[0].variant}, streams {best}, batch times {times}")
     for h in hs:
         h.close()
+
+
+def test_nnz_near_the_int32_limit(cuda):
+    """Maximum sizes: 16 777 216 rows x 127 entries = 2 130 706 432 non-zeros (99.2 % of 2^31-1), built on
+    the device from a closed-form pattern.  Values and x are small integers, so every variant must agree
+    BITWISE with the oracle, which is evaluated on sampled rows (the same pattern, rebuilt on the host).
+    Exercises 64-bit offsets in the kernels and converters; merge-path (rows + nnz over int32) must be refused."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90 * 2**30:
+        pytest.skip("needs ~80 GB of free device memory")
+    rows = cols = 1 << 24
+    L = 127
+    stride = cols // L
+    dev = "cuda:0"
+    rp = (torch.arange(rows + 1, dtype=torch.int64, device=dev) * L).to(torch.int32)
+    i32 = torch.arange(rows, dtype=torch.int32, device=dev)
+    j32 = torch.arange(L, dtype=torch.int32, device=dev)
+    ci = (j32[None, :] * stride + (i32 % stride)[:, None]).reshape(-1).contiguous()
+    val = (((i32[:, None] + j32[None, :]) % 7) - 3).to(torch.float64).reshape(-1).contiguous()
+    assert ci.numel() == rows * L == 2130706432 and int(rp[-1]) == rows * L
+    x = ((torch.arange(cols, dtype=torch.int32, device=dev) % 5) - 2).to(torch.float64)
+    # oracle on sampled rows: the same closed form on the host, as a small CSR of its own
+    rng = np.random.default_rng(7)
+    sample = np.unique(np.r_[np.arange(5), rows - 1 - np.arange(5), rng.integers(0, rows, 2000),
+                             (np.arange(1, 128) * (1 << 17)) - 1])          # incl. rows around 2^31-byte boundaries
+    j = np.arange(L, dtype=np.int64)
+    s_ci = (j[None, :] * stride + (sample % stride)[:, None]).astype(np.int32).reshape(-1)
+    s_val = (((sample[:, None] + j[None, :]) % 7) - 3).astype(np.float64).reshape(-1)
+    s_rp = (np.arange(sample.size + 1) * L).astype(np.int32)
+    xh = ((np.arange(cols) % 5) - 2).astype(np.float64)
+    y0_s = (sample % 3).astype(np.float64)
+    y_ref, _ = oracle.spmv(s_rp, s_ci, s_val, 2.0, xh, -1.0, y0_s)
+    assert np.array_equal(ci[torch.from_numpy(sample[:3] * L).to(dev)].cpu().numpy(), s_ci[::L][:3])
+    S = binding.SpMV(rows, cols, rp, ci, val)
+    info = S.info()
+    assert info.nnz == rows * L and info.min_row_len == info.max_row_len == L and info.cols_sorted == 1
+    with pytest.raises(binding.SpmvError) as e:
+        S.select("merge:b256:i7:x0")
+    assert e.value.status == 3
+    y0 = (torch.arange(rows, dtype=torch.int32, device=dev) % 3).to(torch.float64)
+    idx = torch.from_numpy(sample).to(dev)
+    for desc in ("default", "csr_vector:b256:w32:u4:x0", "sell:b256:c128:s1:r2:u4:x0", "sell_tma:b288:c256:s1:r1:u16:i2:x0"):
+        S.select(desc)
+        y = y0.clone()
+        S.apply(2.0, x, -1.0, y)
+        torch.cuda.synchronize()
+        got = y[idx].cpu().numpy()
+        assert np.array_equal(got, y_ref), (desc, np.flatnonzero(got != y_ref)[:5])
+        assert bool(torch.isfinite(y).all()) and float(y.abs().max()) <= 2.0 * 6 * L + 2
+    S.close()
