@@ -151,11 +151,22 @@ struct DiaConstTrip {
   double xv[U][R];
   __device__ __forceinline__ void load(int64_t r0, int64_t rows, int xmax, const int (&off8)[U],
                                        const unsigned* __restrict__ mask, const double* __restrict__ x,
-                                       double beta, const double* __restrict__ y) {
+                                       double beta, const double* __restrict__ y, bool yvec) {
+    if (R == 2 && yvec && r0 + 1 < rows) {          // 64-/128-bit loads of the two adjacent rows
+      const uint2 mm = __ldg(reinterpret_cast<const uint2*>(mask + r0));
+      m[0] = mm.x; m[R - 1] = mm.y;
+      if (beta != 0.0) {
+        const double2 yy = *reinterpret_cast<const double2*>(y + r0);
+        yold[0] = yy.x; yold[R - 1] = yy.y;
+      } else {
+        yold[0] = 0.0; yold[R - 1] = 0.0;
+      }
+    } else {
 #pragma unroll
-    for (int r = 0; r < R; ++r) m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
+      for (int r = 0; r < R; ++r) m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
 #pragma unroll
-    for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
+      for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
+    }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int o = off8[u];
@@ -170,7 +181,7 @@ template <int R, int X>
 __global__ void __launch_bounds__(512)
 dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs coefs,
                  const unsigned* __restrict__ mask, double alpha, const double* __restrict__ x, double beta,
-                 double* __restrict__ y) {
+                 double* __restrict__ y, int yvec) {
   constexpr int U = 8;
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   const int xmax = (int)cols - 1;
@@ -181,11 +192,11 @@ dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs c
 #pragma unroll
   for (int u = 0; u < U; ++u) { off8[u] = offs.off[u]; c8[u] = coefs.c[u]; }   // entries past nd repeat the last one
   DiaConstTrip<R, U, X> cur, nxt;
-  cur.load(g * R, rows, xmax, off8, mask, x, beta, y);
+  cur.load(g * R, rows, xmax, off8, mask, x, beta, y, yvec != 0);
   for (; g * R < rows; g += G) {
     const int64_t r0 = g * R;
     const bool more = (g + G) * R < rows;
-    if (more) nxt.load((g + G) * R, rows, xmax, off8, mask, x, beta, y);
+    if (more) nxt.load((g + G) * R, rows, xmax, off8, mask, x, beta, y, yvec != 0);
     double acc[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0;
@@ -221,15 +232,22 @@ dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs c
         }
       }
     }
+    if (R == 2 && yvec && r0 + 1 < rows) {
+      double2 out;
+      out.x = (beta == 0.0) ? alpha * acc[0] : fma(alpha, acc[0], beta * cur.yold[0]);
+      out.y = (beta == 0.0) ? alpha * acc[R - 1] : fma(alpha, acc[R - 1], beta * cur.yold[R - 1]);
+      *reinterpret_cast<double2*>(y + r0) = out;
+    } else {
 #pragma unroll
-    for (int r = 0; r < R; ++r)
-      if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * cur.yold[r]);
+      for (int r = 0; r < R; ++r)
+        if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * cur.yold[r]);
+    }
     if (more) cur = nxt;
   }
 }
 
 typedef void (*dia_const_kernel_t)(int64_t, int64_t, int, DiaOffsets, DiaCoefs, const unsigned*, double, const double*, double,
-                                   double*);
+                                   double*, int);
 static dia_const_kernel_t dia_const_pick(const Variant& v) {
 #define P(r, xx) if (v.R == r && v.X == xx) return dia_const_kernel<r, xx>;
   P(1, 0) P(2, 0) P(4, 0) P(1, 1) P(2, 1) P(4, 1)
@@ -250,7 +268,8 @@ cudaError_t dia_const_launch(const Variant& v, int64_t rows, int64_t cols, const
   const int64_t threads = (rows + v.R - 1) / v.R;
   const int64_t exact = (threads + v.block - 1) / v.block;
   const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, cols, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y);
+  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, cols, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y,
+                                              (int)(((uintptr_t)a.y & 15) == 0));
   return cudaGetLastError();
 }
 
