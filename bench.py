@@ -1,17 +1,30 @@
 #!/usr/bin/env python
 """bench.py -- fp64 SpMV effective GB/s & fraction of B200 HBM peak (autotuned vs default).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--configs 2[,1,3,4,5]] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--configs 4,1,2,3,5] [--impl reference]
+    python bench.py --profile-one CFG [--variant DESC|tuned] [--iters 5]      (ncu / sanitizer driver)
 
-One "step" is one pass of the hot path, y = alpha*A*x + beta*y through spmv_apply with the
-autotuned variant, on BASELINE.json:configs[1] (cfg2: 3D 7-point Laplacian 128^3, alpha=1,
-beta=0.5), inputs resident in HBM.  Cold-cache protocol: the steps rotate over several device
-copies of the inputs (combined footprint > 3x the 126 MB L2), run back to back and are bracketed
-by one CUDA event pair on the launching stream (cfg1 is too small for that: L2 flush per step).  `value` = algorithmic bytes (nnz*12 + (rows+1)*4 + 8*cols + 8*rows
-[+ 8*rows if beta != 0]) / time, whole job.  `e2e` is the same metric through spmv_apply_host
-with pinned HOST vectors (H2D of x and y, apply, D2H of y inside the timed region).
-N > 1: N independent replicas (the path is single-GPU; "replicas only"),
-barrier + max over ranks, no data-path collective.
+One "step" is one pass of the hot path, y = alpha*A*x + beta*y through spmv_apply with the autotuned
+variant (cfg5: the batch of four applies through spmv_apply_batch), inputs resident in HBM.  Every
+config of --configs is tuned, checked against the oracle and timed; the FIRST one is the headline of
+the JSON line (default cfg4, the largest single matrix: 2.58 GB as CSR), the rest sit in `per_config`.
+
+Three numbers per config, never conflated:
+  eff_gbs       algorithmic bytes of the CSR byte model (nnz*12 + (rows+1)*4 + 8*cols + 8*rows
+                [+ 8*rows if beta != 0]) / time -- the metric's own definition, `value`;
+  roofline      bytes the WINNING format must move (its matrix arrays + x + y, `bytes_actual`) / time
+                against MEASURED_PEAKS.json:hbm_gbs -- a real roofline fraction (<= ~1.1);
+  traffic       DRAM bytes per launch measured by ncu (profiles/traffic.json), when captured.
+
+Timing: W warm-up steps, then batches of K steps; a batch is bracketed by one CUDA event pair on the
+launching stream (per-step pairs in `flush` mode) and batches repeat until the timed region lasts
+>= --min-ms (50 ms), the reported time per step is the MEDIAN batch / K, max over ranks.  Cache
+state: `warm` when the winner's bytes are >= 4x L2 (cfg3-5: every apply streams from HBM anyway),
+`rotate` over enough device copies that the rotated footprint exceeds 3x L2 (cfg2), `flush` (a 2x L2
+buffer overwritten before every step) when even that would need too many copies (cfg1).
+`e2e` is the same metric through spmv_apply_host with pinned HOST vectors (H2D of x and y, apply,
+D2H of y inside the timed region).  N > 1: N independent replicas (the path is
+single-GPU; "replicas only"), barrier + max over ranks, no data-path collective.
 """
 from __future__ import annotations
 
@@ -31,6 +44,8 @@ sys.path.insert(0, ROOT)
 METRIC = "fp64 SpMV effective GB/s & fraction of B200 HBM peak (autotuned vs default)"
 NOMINAL_HBM_GBS = 8000.0      # BASELINE.json:north_star "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
+DEFAULT_CONFIGS = "4,1,2,3,5"
+ORACLE_SAMPLE_ROWS = 16384
 
 
 def measured_peak():
@@ -100,118 +115,147 @@ class ClockSampler:
         return out
 
 
-def cpu_oracle_times(prob, reps=5):
-    """The oracle as it stands on the host cores: serial and row-parallel (bit-identical)."""
+# ------------------------------------------------------------------------------------------------
+# the oracle on the host cores: ONE protocol for the cpu_baseline leg and for --impl reference
+# ------------------------------------------------------------------------------------------------
+def oracle_time(prob, warmup: int, steps: int, parallel: bool = True):
+    """`warmup` untimed then `steps` timed applies of the oracle as it stands, back to back and in
+    place on one y vector (no allocation inside the timed region).  Returns (mean seconds per
+    apply, threads used)."""
     import oracle
     A = prob.A
     rp = np.ascontiguousarray(A.row_ptr, dtype=np.int32)
     ci = np.ascontiguousarray(A.col_idx, dtype=np.int32)
     va = np.ascontiguousarray(A.val, dtype=np.float64)
     x = np.ascontiguousarray(prob.x)
-    y0 = prob.y0 if prob.y0 is not None else np.zeros(A.rows)
+    y = (prob.y0 if prob.y0 is not None else np.zeros(A.rows)).copy()
     scale = np.empty(A.rows)
-    out = {}
-    for par in (False, True):
-        ts, threads = [], 1
-        for i in range(reps + 1):
-            y = y0.copy()
-            t0 = time.perf_counter()
-            threads = oracle.spmv_inplace(rp, ci, va, prob.alpha, x, prob.beta, y, scale, parallel=par)
-            ts.append(time.perf_counter() - t0)
-        out["parallel" if par else "serial"] = (float(np.median(ts[1:])), int(threads))
-    return out
+    threads = 1
+    for _ in range(warmup):
+        threads = oracle.spmv_inplace(rp, ci, va, prob.alpha, x, prob.beta, y, scale, parallel=parallel)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        threads = oracle.spmv_inplace(rp, ci, va, prob.alpha, x, prob.beta, y, scale, parallel=parallel)
+    return (time.perf_counter() - t0) / max(steps, 1), int(threads)
+
+
+def cpu_baseline(prob, W, steps_parallel=5, steps_serial=2):
+    """cpu_baseline object for one config: the oracle's row-parallel form (bit-identical to the
+    serial loop) on every host core, plus the serial figure."""
+    nb = W.algorithmic_bytes(prob.A.rows, prob.A.cols, prob.A.nnz, prob.beta)
+    tp, threads = oracle_time(prob, 1, steps_parallel, parallel=True)
+    ts, _ = oracle_time(prob, 1, steps_serial, parallel=False)
+    return {"value": nb / tp / 1e9, "unit": "GB/s", "cores": threads, "kind": "oracle",
+            "sample": f"whole matrix of {prob.name} ({prob.A.nnz} nnz): 1 warm-up + {steps_parallel} applies "
+                      "back to back, in place, mean",
+            "parallel_seconds": tp, "serial_seconds": ts, "serial_value": nb / ts / 1e9,
+            "gflops": 2.0 * prob.A.nnz / tp / 1e9}
+
+
+def oracle_check(prob, y_gpu: np.ndarray, n_sample: int = ORACLE_SAMPLE_ROWS, tol: float = 1e-12):
+    """Sampled-row parity of what was timed: the oracle (oracle/, plain CPU row loop) recomputes
+    `n_sample` seeded rows (+ the first and last 64) from the same inputs; acceptance rule and
+    tolerance are north_star's (1e-12 relative to scale_i).  Returns a small report dict."""
+    import oracle
+    A = prob.A
+    rows = A.rows
+    rng = np.random.default_rng(12345)
+    pick = np.unique(np.concatenate([rng.integers(0, rows, size=min(n_sample, rows)),
+                                     np.arange(min(64, rows)), np.arange(max(rows - 64, 0), rows)]))
+    rp = A.row_ptr.astype(np.int64)
+    lens = (rp[pick + 1] - rp[pick])
+    sub_rp = np.zeros(pick.size + 1, dtype=np.int64)
+    np.cumsum(lens, out=sub_rp[1:])
+    idx = np.repeat(rp[pick] - sub_rp[:-1], lens) + np.arange(int(sub_rp[-1]), dtype=np.int64)
+    y0 = prob.y0[pick] if prob.y0 is not None else None
+    y_ref, scale = oracle.spmv(sub_rp.astype(np.int32), A.col_idx[idx], A.val[idx], prob.alpha, prob.x, prob.beta, y0)
+    ok, mr, ff, nf = oracle.accept(y_gpu[pick], y_ref, scale, tol)
+    return {"rows_checked": int(pick.size), "ok": bool(ok), "max_err_over_scale": float(mr), "n_fail": int(nf),
+            "first_fail_row": int(pick[ff]) if nf else -1, "tolerance": tol}
 
 
 def run_reference(args, W):
-    """--impl reference: the oracle (row-parallel form of the same loop) on the host cores."""
+    """--impl reference: the oracle (row-parallel form of the same loop) on the host cores, on the
+    product arm's headline config, --warmup W and --steps K honoured as given."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle
     cfg = int(args.configs.split(",")[0])
     prob = W.config(cfg)
     A = prob.A
-    nbytes = W.algorithmic_bytes(A.rows, A.cols, A.nnz, prob.beta)
-    rp, ci, va = (np.ascontiguousarray(A.row_ptr), np.ascontiguousarray(A.col_idx), np.ascontiguousarray(A.val))
-    y0 = prob.y0 if prob.y0 is not None else np.zeros(A.rows)
-    scale = np.empty(A.rows)
-    y = y0.copy()
-    threads = 1
-    steps = min(args.steps, 50)          # bounded sample: at most 50 full applies
-    for _ in range(min(args.warmup, 3)):
-        threads = oracle.spmv_inplace(rp, ci, va, prob.alpha, prob.x, prob.beta, y, scale, parallel=True)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        threads = oracle.spmv_inplace(rp, ci, va, prob.alpha, prob.x, prob.beta, y, scale, parallel=True)
-    dt = (time.perf_counter() - t0) / steps
+    nbytes = W.algorithmic_bytes(A.rows, A.cols, A.nnz, prob.beta) * (4 if cfg == 5 else 1)
+    nnz = A.nnz * (4 if cfg == 5 else 1)
+    dt, threads = oracle_time(prob, args.warmup, args.steps, parallel=True)
+    if cfg == 5:
+        dt *= 4           # a step of cfg5 is four applies; the four matrices share one pattern
     gbs = nbytes / dt / 1e9
-    sample = f"{steps} full applies of {prob.name} (whole matrix, {A.nnz} nnz)"
+    sample = (f"{args.steps} applies of the whole matrix of {prob.name} ({A.nnz} nnz), in place, back to back"
+              + ("; a step = 4 x that time" if cfg == 5 else ""))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
-        "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": prob.name, "rows": A.rows, "nnz": A.nnz},
+        "config": headline_config(W, cfg, A.rows, nnz),
         "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gflops": 2.0 * A.nnz / dt / 1e9,
+        "gflops": 2.0 * nnz / dt / 1e9,
     }))
 
 
+def headline_config(W, cfg, rows, nnz):
+    """The `config` object: identical in both arms (workload only; what was selected is `selection`)."""
+    return {"workload": W.CONFIG_NAMES[cfg], "rows": int(rows), "nnz": int(nnz)}
+
+
+# ------------------------------------------------------------------------------------------------
+# one config on this rank
+# ------------------------------------------------------------------------------------------------
 def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
-    """Tune + time one config on this rank; returns a result dict."""
     members = 4 if cfg == 5 else 1
     probs = [W.config(cfg, member=m) for m in range(members)]
     A0 = probs[0].A
     alpha, beta = probs[0].alpha, probs[0].beta
     nbytes = sum(W.algorithmic_bytes(p.A.rows, p.A.cols, p.A.nnz, p.beta) for p in probs)
     nnz = sum(p.A.nnz for p in probs)
+    vec_bytes = sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs)
     l2 = torch.cuda.get_device_properties(device).L2_cache_size
-    # Cold-cache protocol (timing rules: "flush L2 or use inputs larger than L2"):
-    #  rotate: the step cycles through `copies` independent device copies of the inputs whose
-    #          combined footprint exceeds 3x L2, so every apply streams its matrix from HBM and
-    #          the K steps run back to back inside ONE event pair;
-    #  flush : (cfg1, 0.3 MB) a 2xL2 buffer is overwritten before every step, per-step events.
-    #  warm  : working set >> L2 already (cfg3-5), K steps back to back.
-    if nbytes >= 4 * l2:
-        mode, copies = "warm", 1
-    elif nbytes * 16 >= 3 * l2:
-        mode, copies = "rotate", int(np.ceil(3 * l2 / nbytes)) + 1
-    else:
-        mode, copies = "flush", 1
+
     handles, xs, ys, y0s = [], [], [], []
-    for c in range(copies):
+
+    def add_copy():
         for p in probs:
             handles.append(binding.SpMV.from_csr(p.A, device=device))
             xs.append(torch.from_numpy(p.x).to(device))
             y0 = p.y0 if p.y0 is not None else np.zeros(p.A.rows)
             y0s.append(torch.from_numpy(y0).to(device))
             ys.append(y0s[-1].clone())
-    flush = torch.empty(int(2 * l2 // 8), dtype=torch.float64, device=device) if mode == "flush" else None
-    step_no = [0]
+
+    add_copy()
+    state = {"copies": 1, "mode": "warm", "step": 0, "nstreams": 1}
+    streams = [torch.cuda.current_stream()]
+    flush = None
 
     def one_step():
         if members == 1:
-            i = step_no[0] % copies
-            step_no[0] += 1
+            i = state["step"] % state["copies"]
+            state["step"] += 1
             handles[i].apply(alpha, xs[i], beta, ys[i])
         else:
-            binding.apply_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams[:nstreams])
+            binding.apply_batch(handles[:members], [alpha] * members, xs[:members], [beta] * members, ys[:members],
+                                streams[:state["nstreams"]])
 
     def fork_join_step(ev):
-        for s in streams[1:nstreams]:
+        for s in streams[1:state["nstreams"]]:
             s.wait_event(ev)
         one_step()
-        for s in streams[1:nstreams]:
+        for s in streams[1:state["nstreams"]]:
             j = torch.cuda.Event()
             j.record(s)
             torch.cuda.current_stream().wait_event(j)
 
-    def timed(steps, warmup):
-        """returns (total seconds, median seconds per step, min seconds per step)"""
-        for _ in range(warmup):
-            one_step()
-        torch.cuda.synchronize()
-        if mode == "flush":
+    def batch(steps):
+        """K steps; returns seconds per step of this batch (device time, CUDA events on the launching stream)."""
+        if state["mode"] == "flush":
             evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
             for a, b in evs:
                 flush.fill_(1.0)
@@ -219,8 +263,7 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
                 one_step()
                 b.record()
             torch.cuda.synchronize()
-            ts = np.array([a.elapsed_time(b) for a, b in evs]) * 1e-3
-            return float(ts.sum()), float(np.median(ts)), float(ts.min())
+            return float(np.sum([a.elapsed_time(b) for a, b in evs])) * 1e-3 / steps
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         for _ in range(steps):
@@ -230,97 +273,154 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
                 one_step()
         b.record()
         torch.cuda.synchronize()
-        t = a.elapsed_time(b) * 1e-3
-        return t, t / steps, t / steps
+        return a.elapsed_time(b) * 1e-3 / steps
 
-    # ---- default variant, then tune (tuning is setup, outside the timed region)
-    streams, nstreams = [torch.cuda.current_stream()], 1
-    tsum_d, tmed_d, _ = timed(max(10, args.steps // 10), 3)
-    # second fixed baseline (SURVEY A17 "heuristic default"): sub-warp width = smallest power of two >= mean row length
-    mean_len = handles[0].info().mean_row_len
-    w_h = int(min(32, max(2, 2 ** int(np.ceil(np.log2(max(mean_len, 1.0)))))))
-    heuristic = f"csr_vector:b256:w{w_h}:u1:x0"
-    for h in handles:
-        h.select(heuristic)
-    _, tmed_h, _ = timed(max(10, args.steps // 10), 3)
-    t0 = time.perf_counter()
-    reports = [h.tune(alpha=alpha, beta=beta, use_cache=(0 if (i or args.tune_cache) else 2),
-                      cache_path=args.tune_cache, flush_l2=(mode != "warm"), seed=cfg,
+    def timed(steps, warmup, min_ms, max_batches=400):
+        """returns (list of per-step seconds, one entry per batch)"""
+        for _ in range(warmup):
+            one_step()
+        torch.cuda.synchronize()
+        ts = [batch(steps)]
+        while sum(ts) * steps * 1e3 < min_ms and len(ts) < max_batches:
+            ts.append(batch(steps))
+        return ts
+
+    # ---- tune first (setup, outside the timed region); the two fixed baselines are timed below under the
+    # same cache protocol as the winner
+    def tune(h, first):
+        # the cold protocol applies when the CSR-model footprint is below 4x L2 (decided before the winner is known)
+        return h.tune(alpha=alpha, beta=beta, use_cache=(0 if (not first or args.tune_cache) else 2),
+                      cache_path=args.tune_cache, flush_l2=(nbytes < 4 * l2), seed=cfg,
                       variant_filter=args.variant_filter)
-               for i, h in enumerate(handles)]
+    t0 = time.perf_counter()
+    reports = [tune(h, i == 0) for i, h in enumerate(handles)]
     stream_times = {}
     if members > 1:
         streams = [torch.cuda.current_stream()] + [torch.cuda.Stream(device=device) for _ in range(3)]
-        nstreams, stream_times = binding.tune_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams)
+        state["nstreams"], stream_times = binding.tune_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams)
     tune_s = time.perf_counter() - t0
     variant = handles[0].variant
+    fmt_bytes = int(sum(h.info().format_bytes for h in handles[:members]))
+    bytes_actual = fmt_bytes + vec_bytes
     # merge-path and row-split SELL add one small ordered fix-up kernel per apply
     launches_per_step = members * (2 if (variant.startswith("merge") or ":l" in variant) else 1)
+
+    # ---- cache protocol, sized from what the WINNER streams (not from the CSR byte model)
+    if bytes_actual >= 4 * l2:
+        state["mode"] = "warm"
+    else:
+        copies = int(np.ceil(3.0 * l2 / bytes_actual)) + 1
+        if members == 1 and copies <= 16:
+            state["mode"] = "rotate"
+            for _ in range(copies - 1):
+                add_copy()
+                tune(handles[-1], False)          # in-process cache hit: same variant
+            state["copies"] = copies
+        else:
+            state["mode"] = "flush"
+            flush = torch.empty(int(2 * l2 // 8), dtype=torch.float64, device=device)
+    # ---- the two fixed baselines, same cache protocol (default: SURVEY A17; heuristic: sub-warp width = smallest
+    # power of two >= the mean row length), then back to the tuned variant
+    mean_len = handles[0].info().mean_row_len
+    w_h = int(min(32, max(2, 2 ** int(np.ceil(np.log2(max(mean_len, 1.0)))))))
+    heuristic = f"csr_vector:b256:w{w_h}:u1:x0"
+    k_base = max(5, args.steps // 4)
+    base_t = {}
+    for name in ("default", heuristic):
+        for h in handles:
+            h.select(name)
+        base_t[name] = float(np.median(timed(k_base, 3, 5.0, max_batches=20)))
+    t_default, t_heur = base_t["default"], base_t[heuristic]
+    for h in handles:
+        h.select(variant)
+    assert all(h.variant == variant for h in handles), "copies must run the tuned variant"
     for y, y0 in zip(ys, y0s):
         y.copy_(y0)
+    timing_note = {
+        "rotate": f"cold: steps rotate over {state['copies']} device copies of the inputs ({state['copies']} x "
+                  f"{bytes_actual / 1e6:.1f} MB streamed by the winner > 3x L2), back to back in one event pair per batch",
+        "flush": "cold: 2xL2 buffer overwritten before every step, per-step event pairs",
+        "warm": f"winner streams {bytes_actual / 1e6:.0f} MB per step >= 4x L2: steps back to back in one event pair per batch",
+    }[state["mode"]]
 
-    # ---- the timed region: barrier + sync on both sides, max over ranks
+    # ---- the timed region: barrier + sync on both sides, median batch, max over ranks
     sampler = ClockSampler(torch.cuda.current_device()) if primary else None
     for _ in range(args.warmup):
         one_step()
     torch.cuda.synchronize()
     dist_max(0.0)                               # barrier
-    tsum, tmed, tmin = timed(args.steps, 0)
-    tsum = dist_max(tsum)
-    # keep the GPU under the same load a little longer so the clock sampler sees it
-    if sampler is not None:
-        t_end = time.time() + 0.6
+    ts = timed(args.steps, 0, args.min_ms)
+    t_step = dist_max(float(np.median(ts)))
+    n_batches = len(ts)
+    if sampler is not None:                     # keep the same load a little longer so the sampler sees it
+        t_end = time.time() + 0.5
         while time.time() < t_end:
-            for _ in range(50):
+            for _ in range(20):
                 one_step()
             torch.cuda.synchronize()
     clocks = sampler.stop() if sampler is not None else None
 
-    # ---- the other cache state: warm (same buffers back to back) for the configs whose headline is cold
-    t_warm_us = None
-    if mode != "warm" and members == 1:
-        for _ in range(5):
-            handles[0].apply(alpha, xs[0], beta, ys[0])
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(args.steps):
-            handles[0].apply(alpha, xs[0], beta, ys[0])
-        b.record()
-        torch.cuda.synchronize()
-        t_warm_us = a.elapsed_time(b) * 1e3 / args.steps
+    # ---- the other cache state: warm (same buffers back to back) where the headline is cold
+    t_warm = t_step
+    if state["mode"] != "warm" and members == 1:
+        keep = (state["mode"], state["copies"])
+        state["mode"], state["copies"] = "warm", 1
+        t_warm = float(np.median(timed(args.steps, 5, 5.0)))
+        state["mode"], state["copies"] = keep
 
-    # ---- parity of what was just timed (sampled rows through the oracle would need the CPU
-    # oracle; the full check lives in tests/ -- here: determinism + finite output)
+    # ---- host cost of one spmv_apply call: wall clock of n enqueues on an idle stream / n
+    torch.cuda.synchronize()
+    n_host = 256                                 # below the launch-queue depth even for two-launch variants
+    h0, x0d, y0d = handles[0], xs[0], ys[0]
+    t1 = time.perf_counter()
+    for _ in range(n_host):
+        h0.apply(alpha, x0d, beta, y0d)
+    host_us = (time.perf_counter() - t1) / n_host * 1e6
+    torch.cuda.synchronize()
+
+    # ---- parity of what was timed: determinism, and the oracle on sampled rows
     def first_members():
         for y, y0 in zip(ys[:members], y0s[:members]):
             y.copy_(y0)
         if members == 1:
             handles[0].apply(alpha, xs[0], beta, ys[0])
         else:
-            binding.apply_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams[:1])
+            binding.apply_batch(handles[:members], [alpha] * members, xs[:members], [beta] * members, ys[:members],
+                                streams[:state["nstreams"]])
         torch.cuda.synchronize()
         return [y.clone() for y in ys[:members]]
     first = first_members()
     deterministic = all(torch.equal(a, b) for a, b in zip(first, first_members()))
-    finite = all(bool(torch.isfinite(y).all()) for y in ys)
+    parity = None
+    if primary and not args.no_oracle_check:
+        checks = [oracle_check(p, y.cpu().numpy()) for p, y in zip(probs, first)]
+        parity = {"ok": all(c["ok"] for c in checks), "rows_checked": sum(c["rows_checked"] for c in checks),
+                  "max_err_over_scale": max(c["max_err_over_scale"] for c in checks),
+                  "n_fail": sum(c["n_fail"] for c in checks), "tolerance": 1e-12,
+                  "what": "one apply of the timed variant from y0 vs oracle/ on seeded sample rows"}
+        if not parity["ok"]:
+            raise SystemExit(f"bench: cfg{cfg} {variant} FAILED the oracle check: {checks}")
 
-    # ---- e2e through spmv_apply_host with pinned host vectors
-    e2e = None
-    if members == 1:
-        xh = torch.from_numpy(probs[0].x).pin_memory()
-        yh = torch.from_numpy((probs[0].y0 if probs[0].y0 is not None else np.zeros(A0.rows)).copy()).pin_memory()
-        for _ in range(3):
-            handles[0].apply_host(alpha, xh, beta, yh)
-        n_e2e = max(5, min(args.steps, 50))
-        torch.cuda.synchronize(); dist_max(0.0)
-        t1 = time.perf_counter()
-        for _ in range(n_e2e):
-            handles[0].apply_host(alpha, xh, beta, yh)      # synchronises the stream itself
-        te = dist_max((time.perf_counter() - t1) / n_e2e)
-        e2e = {"value": nbytes / te / 1e9, "unit": "GB/s", "ms_per_step": te * 1e3, "steps": n_e2e,
-               "h2d_bytes_per_step": 8 * A0.cols + (8 * A0.rows if beta != 0 else 0),
-               "d2h_bytes_per_step": 8 * A0.rows}
+    # ---- e2e through spmv_apply_host with pinned host vectors (every member, one after the other)
+    xh = [torch.from_numpy(p.x).pin_memory() for p in probs]
+    yh = [torch.from_numpy((p.y0 if p.y0 is not None else np.zeros(p.A.rows)).copy()).pin_memory() for p in probs]
+
+    def e2e_step():
+        for m in range(members):
+            handles[m].apply_host(alpha, xh[m], beta, yh[m])     # synchronises the stream itself
+    for _ in range(3):
+        e2e_step()
+    n_e2e = max(5, min(args.steps, 50))
+    torch.cuda.synchronize()
+    dist_max(0.0)
+    t1 = time.perf_counter()
+    for _ in range(n_e2e):
+        e2e_step()
+    te = dist_max((time.perf_counter() - t1) / n_e2e)
+    e2e = {"value": nbytes / te / 1e9, "unit": "GB/s", "ms_per_step": te * 1e3, "steps": n_e2e,
+           "h2d_bytes_per_step": int(sum(8 * p.A.cols + (8 * p.A.rows if p.beta != 0 else 0) for p in probs)),
+           "d2h_bytes_per_step": int(sum(8 * p.A.rows for p in probs))}
+
     # ---- solver loop around apply (SURVEY 8(f) rank 3): fixed-count CG on the SPD configs
     cg = None
     if cfg in (1, 2) and members == 1:
@@ -342,53 +442,110 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
               "eff_gbs": it_bytes * best["iters"] / best["device_seconds"] / 1e9,
               "rel_residual": best["rel_residual"], "graph_replays": best["graph_replays"],
               "fused_single_kernel": bool(best["fused"]),
-              "launches_per_iteration": 0 if best["fused"] else 4 + launches_per_step,
               "bytes_per_iteration_algorithmic": it_bytes}
+
+    # ---- K applies replayed as one CUDA graph (launch-bound configs; a clearly labelled extra line)
+    graph = None
+    if members == 1 and hasattr(handles[0], "graph_time") and cfg in (1, 2):
+        graph = handles[0].graph_time(alpha, xs[0], beta, ys[0], k=50, reps=20)
+
     info = handles[0].info()
     peak_meas, _ = measured_peak()
-    eff = nbytes * args.steps / tsum / 1e9
-    res = {"cfg": cfg, "workload": probs[0].name if members == 1 else W.CONFIG_NAMES[5],
-           "rows": A0.rows, "cols": A0.cols, "nnz": nnz, "members": members,
-           "bytes_algorithmic": nbytes, "bytes_format_actual": int(sum(h.info().format_bytes for h in handles[:members])),
-           "variant": variant, "nstreams": nstreams, "stream_times_us": stream_times,
-           "t_sum_s": tsum, "t_median_us": tmed * 1e6, "t_min_us": tmin * 1e6,
-           "eff_gbs": eff, "frac_hbm_nominal_8TBs": eff / NOMINAL_HBM_GBS, "frac_hbm_measured": eff / peak_meas,
-           "bytes_actual": int(sum(h.info().format_bytes for h in handles[:members]) +
-                               sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs)),
-           "format_gbs": float(sum(h.info().format_bytes for h in handles[:members]) +
-                               sum(8 * p.A.cols + 8 * p.A.rows * (2 if p.beta != 0 else 1) for p in probs))
-                         * args.steps / tsum / 1e9,
-           "gathers_per_s": nnz * args.steps / tsum, "gflops": 2.0 * nnz * args.steps / tsum / 1e9,
-           "t_default_us": tmed_d * 1e6, "speedup_vs_default": tmed_d / tmed,
-           "heuristic_variant": heuristic, "t_heuristic_us": tmed_h * 1e6, "speedup_vs_heuristic": tmed_h / tmed,
-           "t_warm_us": t_warm_us if t_warm_us is not None else tmed * 1e6,
-           "t_cold_us": tmed * 1e6 if mode != "warm" else None,
-           "tune_seconds": tune_s, "tune_reports": [{k: v for k, v in r.items() if k != "log"} for r in reports],
-           "launches_per_step": launches_per_step, "timing": {"rotate": f"cold: steps rotate over {copies} device copies of the inputs (footprint > 3x L2), back to back in one event pair",
-                      "flush": "cold: 2xL2 buffer overwritten before every step, per-step events",
-                      "warm": "working set >= 4x L2, steps back to back in one event pair"}[mode],
-           "deterministic": deterministic, "finite": finite, "e2e": e2e, "clocks": clocks, "cg": cg,
-           "sm_count": info.sm_count, "l2_bytes": info.l2_bytes, "device": info.device_name.decode()}
+    res = {"cfg": cfg, "workload": W.CONFIG_NAMES[cfg], "rows": A0.rows, "cols": A0.cols, "nnz": nnz, "members": members,
+           "variant": variant, "nstreams": state["nstreams"], "stream_times_us": stream_times,
+           "bytes_algorithmic": nbytes, "bytes_format_actual": fmt_bytes, "bytes_actual": bytes_actual,
+           "t_step_us": t_step * 1e6, "t_batches_us": {"n": n_batches, "min": float(np.min(ts)) * 1e6,
+                                                      "median": float(np.median(ts)) * 1e6, "max": float(np.max(ts)) * 1e6},
+           "timed_region_ms": float(np.sum(ts)) * args.steps * 1e3,
+           "eff_gbs": nbytes / t_step / 1e9, "actual_gbs": bytes_actual / t_step / 1e9,
+           "frac_effective_of_8TBs": nbytes / t_step / 1e9 / NOMINAL_HBM_GBS,
+           "frac_effective_of_measured": nbytes / t_step / 1e9 / peak_meas,
+           "frac_actual_of_measured": bytes_actual / t_step / 1e9 / peak_meas,
+           "gathers_per_s": nnz / t_step, "gflops": 2.0 * nnz / t_step / 1e9,
+           "t_default_us": t_default * 1e6, "speedup_vs_default": t_default / t_step,
+           "heuristic_variant": heuristic, "t_heuristic_us": t_heur * 1e6, "speedup_vs_heuristic": t_heur / t_step,
+           "t_warm_us": t_warm * 1e6, "t_cold_us": t_step * 1e6 if state["mode"] != "warm" else None,
+           "host_us_per_apply": host_us, "gpu_launches": launches_per_step * args.steps * n_batches,
+           "tune_seconds": tune_s, "tune_reports": [{k: v for k, v in r.items() if k != "log"} for r in reports[:members]],
+           "launches_per_step": launches_per_step, "timing": timing_note, "cache_mode": state["mode"],
+           "deterministic": deterministic, "parity": parity, "e2e": e2e, "clocks": clocks, "cg": cg,
+           "graph_replay": graph, "sm_count": info.sm_count, "l2_bytes": info.l2_bytes,
+           "device": info.device_name.decode()}
     for h in handles:
         h.close()
     return res, probs[0]
 
 
+def config_roofline(r, peak, ceil):
+    """What bounds this config's winner and the fraction of that bound."""
+    if r["cfg"] == 1:       # 0.1 MB per apply: launch-latency-bound (SURVEY sec. 8(d))
+        return {"bound": "launch", "achieved": r["t_step_us"], "peak": ceil["empty_launch_us"],
+                "unit": "us (lower is better; cold apply vs empty-kernel launch)",
+                "frac": ceil["empty_launch_us"] / r["t_step_us"],
+                "actual_gbs": r["actual_gbs"], "frac_hbm_actual": r["frac_actual_of_measured"]}
+    if r["cfg"] == 3:       # unstructured columns: every x gather is its own L1->XBAR request
+        g = r["gathers_per_s"] / 1e9
+        return {"bound": "l1-xbar gather requests", "achieved": g, "peak": ceil["random_gather_G_per_s_32MiB_table"],
+                "unit": "G gathers/s", "frac": g / ceil["random_gather_G_per_s_32MiB_table"],
+                "actual_gbs": r["actual_gbs"], "frac_hbm_actual": r["frac_actual_of_measured"],
+                "traffic": ncu_traffic(r["variant"], r["cfg"])}
+    return {"bound": "hbm", "achieved": r["actual_gbs"], "peak": peak, "unit": "GB/s",
+            "frac": r["frac_actual_of_measured"], "bytes_per_launch": r["bytes_actual"],
+            "effective_gbs": r["eff_gbs"], "frac_effective": r["frac_effective_of_measured"],
+            "traffic": ncu_traffic(r["variant"], r["cfg"]),
+            "note": "achieved = bytes the winning format must move (its arrays + x + y) / time; effective_* uses the "
+                    "CSR byte model of the metric and exceeds 1 when the format streams fewer bytes than CSR"}
+
+
+def profile_one(args, torch, binding, W):
+    """A few applies of one variant on one config: the command the ncu captures under profiles/ run."""
+    cfg = args.profile_one
+    prob = W.config(cfg)
+    A = prob.A
+    S = binding.SpMV.from_csr(A)
+    x = torch.from_numpy(prob.x).cuda()
+    y = torch.from_numpy(prob.y0 if prob.y0 is not None else np.zeros(A.rows)).cuda()
+    if args.variant in (None, "tuned"):
+        rep = S.tune(alpha=prob.alpha, beta=prob.beta, use_cache=2, flush_l2=True, variant_filter=args.variant_filter)
+        print("tuned:", rep["winner"], f"{rep['winner_us']:.2f} us; default {rep['default_us']:.2f} us")
+    else:
+        S.select(args.variant)
+    flush = torch.empty(int(2 * S.info().l2_bytes // 8), dtype=torch.float64, device="cuda")
+    ts = []
+    for _ in range(args.iters):
+        flush.fill_(1.0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        S.apply(prob.alpha, x, prob.beta, y)
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e3)
+    nb = W.algorithmic_bytes(A.rows, A.cols, A.nnz, prob.beta)
+    t = float(np.median(ts))
+    print(f"{prob.name} | {S.variant} | {t:.2f} us/apply (cold, single launches) | {nb / t / 1e3:.1f} GB/s effective | "
+          f"format bytes {S.info().format_bytes}")
+    S.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--configs", default="2", help="comma list; the first is the headline (default cfg2)")
+    ap.add_argument("--configs", default=DEFAULT_CONFIGS, help="comma list; the first is the headline (default cfg4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--min-ms", type=float, default=50.0, help="batches of --steps repeat until the timed region lasts this long")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-oracle-check", action="store_true")
     ap.add_argument("--variant-filter", default=None,
                     help="comma list of descriptor prefixes the tuner may use (spmv_tune variant_filter), e.g. "
                          "'csr_scalar,csr_vector,sell:,sell_tma,ell,merge,bcsr3,dia:,dia_tma' = everything that still "
                          "reads the matrix values (no constant-coefficient elision)")
-    ap.add_argument("--cpu-all", action="store_true", help="time the CPU oracle on every config of --configs, not only the headline")
     ap.add_argument("--tune-cache", default=None,
                     help="file persisting tuning winners (spmv_tune cache_path); a second run then skips the search")
+    ap.add_argument("--profile-one", type=int, default=0, metavar="CFG", help="ncu / sanitizer driver: a few cold applies of one variant")
+    ap.add_argument("--variant", default=None, help="--profile-one: descriptor to force ('tuned' or absent: tune)")
+    ap.add_argument("--iters", type=int, default=5)
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
 
@@ -402,6 +559,9 @@ def main():
     binding.lib()                               # fail loudly if the CUDA library is missing
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    if args.profile_one:
+        profile_one(args, torch, binding, W)
+        return
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -415,53 +575,41 @@ def main():
 
     cfgs = [int(c) for c in args.configs.split(",")]
     results = []
-    head_prob = None
-    for i, cfg in enumerate(cfgs):
+    for cfg in cfgs:
         res, prob = bench_config(cfg, args, torch, binding, W, dist_max, device, primary=(rank == 0))
-        if args.cpu_all and rank == 0 and i > 0:
-            t = cpu_oracle_times(prob, reps=3)
-            res["cpu_oracle"] = {"serial_seconds": t["serial"][0], "parallel_seconds": t["parallel"][0],
-                                 "cores": t["parallel"][1], "sample": "first matrix of the config, median of 3 applies"}
+        if rank == 0 and not args.no_cpu_baseline:
+            res["cpu_baseline"] = cpu_baseline(prob, W)
+            if res["members"] > 1:
+                res["cpu_baseline"]["sample"] += f" (first of the {res['members']} matrices; GB/s per matrix is the batch's GB/s)"
         results.append(res)
-        if i == 0:
-            head_prob = prob
+        del prob
     head = results[0]
     peak, peak_src = measured_peak()
-    # whole job: every rank ran the same work; time is the max over ranks
-    value = head["eff_gbs"] * world
     line = {
-        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": head["t_sum_s"] / args.steps * 1e3, "higher_is_better": True,
+        "metric": METRIC, "value": head["eff_gbs"] * world, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": head["t_step_us"] * 1e-3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": head["workload"], "rows": head["rows"], "nnz": head["nnz"],
-                   "variant": head["variant"], "variant_filter": args.variant_filter, "l2": head["timing"],
-                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
-        "gpu_launches": head["launches_per_step"] * args.steps,
+        "config": headline_config(W, head["cfg"], head["rows"], head["nnz"]),
+        "selection": {"variant": head["variant"], "nstreams": head["nstreams"], "variant_filter": args.variant_filter,
+                      "l2": head["timing"],
+                      "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
+        "timed_batches": head["t_batches_us"]["n"], "timed_region_ms": head["timed_region_ms"],
+        "gpu_launches": head["gpu_launches"],
         "clocks": head["clocks"],
-        "e2e": ({"value": head["e2e"]["value"] * world, "unit": "GB/s",
-                 "h2d_bytes_per_step": head["e2e"]["h2d_bytes_per_step"],
-                 "d2h_bytes_per_step": head["e2e"]["d2h_bytes_per_step"],
-                 "ms_per_step": head["e2e"]["ms_per_step"]} if head["e2e"] else None),
-        "roofline": {"bound": "hbm", "achieved": head["eff_gbs"], "peak": peak, "unit": "GB/s",
-                     "frac": head["eff_gbs"] / peak, "peak_source": peak_src,
-                     "frac_of_nominal_8TBs": head["eff_gbs"] / NOMINAL_HBM_GBS,
-                     "traffic": ncu_traffic(head["variant"], head["cfg"]),
-                     "actual_gbs": head["format_gbs"], "frac_actual": head["format_gbs"] / peak,
-                     "actual_bytes_per_launch": head["bytes_actual"],
-                     "note": "achieved = algorithmic (CSR byte model) bytes / time, as the metric defines it; the winning "
-                             "format streams fewer bytes (actual_*), so frac can exceed 1",
-                     "kernel": head["variant"], "algorithmic_bytes_per_launch": head["bytes_algorithmic"],
-                     "format_bytes_per_launch": head["bytes_format_actual"]},
+        "e2e": {"value": head["e2e"]["value"] * world, "unit": "GB/s",
+                "h2d_bytes_per_step": head["e2e"]["h2d_bytes_per_step"],
+                "d2h_bytes_per_step": head["e2e"]["d2h_bytes_per_step"],
+                "ms_per_step": head["e2e"]["ms_per_step"]},
         "gflops": head["gflops"] * world, "speedup_vs_default": head["speedup_vs_default"],
-        "tune_seconds": head["tune_seconds"], "deterministic": head["deterministic"], "cg": head["cg"],
-        "per_config": [{k: v for k, v in r.items() if k not in ("clocks",)} for r in results],
+        "tune_seconds": head["tune_seconds"], "deterministic": head["deterministic"], "parity": head["parity"],
+        "host_us_per_apply": head["host_us_per_apply"],
+        "per_config": results,
     }
     if rank == 0:
         # ceilings measured in the same run with the library's own kernels
         torch.cuda.synchronize()
         ceil = {"copy_gbs_1GiB": binding.measure_ceiling(0, 1 << 30, 5),
                 "read_gbs_1GiB": binding.measure_ceiling(1, 1 << 30, 5),
-                "read_gbs_at_headline_size": binding.measure_ceiling(1, max(1 << 20, int(head["bytes_actual"])), 5),
                 "empty_launch_us": binding.measure_ceiling(2, 0, 200),
                 "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}
         line["ceilings"] = ceil
@@ -470,32 +618,13 @@ def main():
         except Exception:
             cpu_model = "unknown"
         line["host"] = {"cpu_model": cpu_model, "cores": os.cpu_count(), "cuda": torch.version.cuda,
-                        "driver": torch.cuda.get_device_properties(device).name, "torch": torch.__version__}
-        for r in line["per_config"]:
-            # unstructured columns: every x gather is its own L1->XBAR request (profiles/r01_cfg3_*.md)
-            r["frac_of_gather_ceiling"] = r["gathers_per_s"] / 1e9 / ceil["random_gather_G_per_s_32MiB_table"]
-            # what bounds this config's winner and the fraction of that bound
-            if r["cfg"] == 1:
-                r["roofline"] = {"bound": "launch", "achieved": r["t_median_us"], "peak": ceil["empty_launch_us"],
-                                 "unit": "us (lower is better; cold apply vs empty-kernel launch)",
-                                 "frac": ceil["empty_launch_us"] / r["t_median_us"]}
-            elif r["cfg"] == 3:
-                r["roofline"] = {"bound": "l1-xbar gather requests", "achieved": r["gathers_per_s"] / 1e9,
-                                 "peak": ceil["random_gather_G_per_s_32MiB_table"], "unit": "G gathers/s",
-                                 "frac": r["frac_of_gather_ceiling"]}
-            else:
-                r["roofline"] = {"bound": "hbm", "achieved": r["eff_gbs"], "peak": peak, "unit": "GB/s",
-                                 "frac": r["eff_gbs"] / peak, "actual_gbs": r["format_gbs"],
-                                 "frac_actual": r["format_gbs"] / peak,
-                                 "traffic": ncu_traffic(r["variant"], r["cfg"])}
-    if rank == 0 and not args.no_cpu_baseline:
-        t = cpu_oracle_times(head_prob)
-        nb = W.algorithmic_bytes(head_prob.A.rows, head_prob.A.cols, head_prob.A.nnz, head_prob.beta)
-        line["cpu_baseline"] = {"value": nb / t["parallel"][0] / 1e9, "unit": "GB/s", "cores": t["parallel"][1],
-                                "kind": "oracle", "sample": f"whole {head_prob.name} matrix, median of 5 applies",
-                                "serial_value": nb / t["serial"][0] / 1e9, "serial_seconds": t["serial"][0],
-                                "parallel_seconds": t["parallel"][0]}
-    if rank == 0:
+                        "gpu": torch.cuda.get_device_properties(device).name, "torch": torch.__version__}
+        for r in results:
+            r["roofline"] = config_roofline(r, peak, ceil)
+            r["roofline"]["peak_source"] = peak_src if r["roofline"]["bound"] == "hbm" else "measured in this run (spmv_measure_ceiling)"
+        line["roofline"] = dict(head["roofline"], kernel=head["variant"])
+        line["cpu_baseline"] = head.get("cpu_baseline")
+        line["cg"] = next((r["cg"] for r in results if r["cg"]), None)
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist
