@@ -261,6 +261,7 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
     const DiaFormat& df = h->dias[v.C];
     if (!strcmp(name, "dia_val")) { src = df.val; n = sizeof(double) * df.nd * df.ld; }
     else if (!strcmp(name, "dia_mask")) { src = df.mask; n = sizeof(unsigned) * df.ld; }
+    else if (!strcmp(name, "dia_mask_small") && df.mask_small) { src = df.mask_small; n = (size_t)df.mask_elem * df.ld; }
     else if (!strcmp(name, "dia_coef")) {     // host-resident
       *bytes = sizeof(double) * df.nd;
       if (h_buf && cap > 0) memcpy(h_buf, df.coef, *bytes < cap ? *bytes : cap);

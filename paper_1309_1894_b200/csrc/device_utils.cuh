@@ -47,6 +47,12 @@ __device__ __forceinline__ int4 ld_stream4(const int* p) {         // 16-byte al
 // dependent use placed between two loads would delay every load behind it.
 __device__ __forceinline__ void phase_fence() { asm volatile("" ::: "memory"); }
 
+// Programmatic dependent launch (sm_90+): launch_dependents lets the next kernel of the stream begin its
+// prologue while this grid is still running; wait blocks until every prerequisite grid has completed and its
+// memory is visible.  Both are no-ops for a kernel launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // BLAS-style epilogue (reading A1): y is not read when beta == 0.
 __device__ __forceinline__ void store_y(double* __restrict__ y, int64_t i, double alpha, double s, double beta) {
   y[i] = (beta == 0.0) ? alpha * s : fma(alpha, s, beta * y[i]);

@@ -139,138 +139,219 @@ cudaError_t dia_launch(const Variant& v, int64_t rows, const DiaFormat& f, const
 // cfg2's diag 6 / off -1), the values need not be streamed at all: the kernel reads the mask word
 // (which entries exist near the boundary), x and y only.  Same summation order as dia_kernel, and the
 // coefficients are the stored bit patterns, so the result equals dia_kernel's bit for bit.
+//
+// Shape (round 2; measured on cfg2 with _work/stencil_probe.cu): one trip per thread over an EXACT grid
+// -- the hardware block scheduler keeps every SM's load queue full, a persistent grid-stride loop with
+// software pipelining (round 1: 124 registers, 21 us) does not -- a thread owns R adjacent rows and reads
+// x[r0 + off .. r0 + off + R) as aligned 16-byte pairs; for an odd offset the pair is taken one element
+// to the left and the missing right neighbour comes from the next lane by shuffle (lane 31 loads it).
+// The mask is stored in the narrowest type that holds nd bits (1 byte per row for nd <= 8).  The kernel
+// is a programmatic dependent launch: it signals its own dependents at once, loads its mask words
+// (immutable, owned by the handle) and only then waits for the previous kernel of the stream, so the
+// launch latency and the first memory round trip of apply k+1 overlap the tail of apply k.
 struct DiaCoefs { double c[32]; };
 
-// One grid-stride trip of dia_const: the loads of a trip (mask, old y, first U x values per row) are
-// independent of each other, and the NEXT trip's loads are issued before the current trip's FMAs and
-// store (software pipelining), so two trips' worth of bytes are in flight per thread.
-template <int R, int U, int X>
-struct DiaConstTrip {
-  unsigned m[R];
-  double yold[R];
-  double xv[U][R];
-  __device__ __forceinline__ void load(int64_t r0, int64_t rows, int xmax, const int (&off8)[U],
-                                       const unsigned* __restrict__ mask, const double* __restrict__ x,
-                                       double beta, const double* __restrict__ y, bool yvec) {
-    if (R == 2 && yvec && r0 + 1 < rows) {          // 64-/128-bit loads of the two adjacent rows
-      const uint2 mm = __ldg(reinterpret_cast<const uint2*>(mask + r0));
-      m[0] = mm.x; m[R - 1] = mm.y;
-      if (beta != 0.0) {
-        const double2 yy = *reinterpret_cast<const double2*>(y + r0);
-        yold[0] = yy.x; yold[R - 1] = yy.y;
-      } else {
-        yold[0] = 0.0; yold[R - 1] = 0.0;
-      }
-    } else {
-#pragma unroll
-      for (int r = 0; r < R; ++r) m[r] = r0 + r < rows ? __ldg(mask + r0 + r) : 0u;
-#pragma unroll
-      for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && r0 + r < rows) ? y[r0 + r] : 0.0;
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int o = off8[u];
-      // unpredicated, index clamped into range: an absent entry is loaded but never multiplied (A7)
-#pragma unroll
-      for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
-    }
-  }
-};
+template <int X>
+__device__ __forceinline__ double2 ldx2(const double* __restrict__ x, int i) {     // 16-byte aligned
+  if (X == 0) return __ldg(reinterpret_cast<const double2*>(x + i));
+  double2 v;
+  asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(x + i));
+  return v;
+}
 
+// R > 1 (needs cols % 2 == 0 and 16-byte aligned x): e[r] = x[b + r], r < R, b even, as aligned pairs.  A pair
+// lies either completely inside [0, cols) or completely outside; an outside pair is read at a clamped
+// (still aligned) index and never multiplied (its mask bits are off: such entries cannot be stored).
 template <int R, int X>
-__global__ void __launch_bounds__(512)
-dia_const_kernel(int64_t rows, int64_t cols, int nd, DiaOffsets offs, DiaCoefs coefs,
-                 const unsigned* __restrict__ mask, double alpha, const double* __restrict__ x, double beta,
-                 double* __restrict__ y, int yvec) {
-  constexpr int U = 8;
-  const int64_t G = (int64_t)gridDim.x * blockDim.x;
-  const int xmax = (int)cols - 1;
-  int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (g * R >= rows) return;
-  int off8[U];
-  double c8[U];
+__device__ __forceinline__ void dia_load_pairs(const double* __restrict__ x, int b, int cols, double (&e)[R]) {
 #pragma unroll
-  for (int u = 0; u < U; ++u) { off8[u] = offs.off[u]; c8[u] = coefs.c[u]; }   // entries past nd repeat the last one
-  DiaConstTrip<R, U, X> cur, nxt;
-  cur.load(g * R, rows, xmax, off8, mask, x, beta, y, yvec != 0);
-  for (; g * R < rows; g += G) {
-    const int64_t r0 = g * R;
-    const bool more = (g + G) * R < rows;
-    if (more) nxt.load((g + G) * R, rows, xmax, off8, mask, x, beta, y, yvec != 0);
-    double acc[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) acc[r] = 0.0;
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const double c = c8[u];
-#pragma unroll
-      for (int r = 0; r < R; ++r) {
-        const bool on = u < nd && ((cur.m[r] >> u) & 1u);
-        acc[r] = on ? fma(c, cur.xv[u][r], acc[r]) : acc[r];
-      }
-    }
-    // more than U diagonals: the rest is loaded in place.  Statically unrolled (d0 = 8, 16, 24) so that
-    // the by-value offset/coefficient parameters are never indexed dynamically (no local-memory copy).
-#pragma unroll
-    for (int d0 = U; d0 < 32; d0 += U) {
-      if (d0 >= nd) break;
-      double xv[U][R];
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const int o = offs.off[d0 + u];
-#pragma unroll
-        for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
-      }
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const int d = d0 + u;
-        const double c = coefs.c[d];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-          const bool on = d < nd && ((cur.m[r] >> d) & 1u);
-          acc[r] = on ? fma(c, xv[u][r], acc[r]) : acc[r];
-        }
-      }
-    }
-    if (R == 2 && yvec && r0 + 1 < rows) {
-      double2 out;
-      out.x = (beta == 0.0) ? alpha * acc[0] : fma(alpha, acc[0], beta * cur.yold[0]);
-      out.y = (beta == 0.0) ? alpha * acc[R - 1] : fma(alpha, acc[R - 1], beta * cur.yold[R - 1]);
-      *reinterpret_cast<double2*>(y + r0) = out;
-    } else {
-#pragma unroll
-      for (int r = 0; r < R; ++r)
-        if (r0 + r < rows) y[r0 + r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * cur.yold[r]);
-    }
-    if (more) cur = nxt;
+  for (int r = 0; r < R; r += 2) {
+    const double2 p = ldx2<X>(x, min(max(b + r, 0), cols - 2));
+    e[r] = p.x; e[r + 1] = p.y;
   }
 }
 
-typedef void (*dia_const_kernel_t)(int64_t, int64_t, int, DiaOffsets, DiaCoefs, const unsigned*, double, const double*, double,
-                                   double*, int);
-static dia_const_kernel_t dia_const_pick(const Variant& v) {
-#define P(r, xx) if (v.R == r && v.X == xx) return dia_const_kernel<r, xx>;
+template <typename MT> struct DiaMaskVec;
+template <> struct DiaMaskVec<unsigned char> { typedef uchar2 V2; typedef uchar4 V4; };
+template <> struct DiaMaskVec<unsigned short> { typedef ushort2 V2; typedef ushort4 V4; };
+template <> struct DiaMaskVec<unsigned> { typedef uint2 V2; typedef uint4 V4; };
+
+// ND > 0: exactly ND diagonals, fully unrolled, no run-time diagonal count (5-, 7-, 9-, 27-point stencils);
+// ND == 0: any nd <= 32, chunks of 8 with warp-uniform guards.  Registers decide this kernel's speed (one
+// memory round trip per thread: occupancy IS the memory-level parallelism; measured 21 us at 59 registers,
+// 12.7 us at 23 on cfg2), hence the exact instantiations and the min-blocks launch bound.
+constexpr int dia_const_min_blocks(int R, int ND) { return (ND == 0 || ND > 9) ? (R == 4 ? 1 : 2) : (R == 1 ? 4 : R == 2 ? 2 : 1); }
+
+template <int R, int ND, int X, typename MT>
+__device__ __forceinline__ void
+dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
+               double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+  pdl_launch_dependents();
+  constexpr int NDC = ND == 0 ? 8 : (ND % 9 == 0 ? 9 : (ND <= 8 ? ND : 8));     // diagonals per chunk
+  constexpr int DMAX = ND == 0 ? 32 : ND;
+  const int nd = ND == 0 ? nd_rt : ND;
+  // 32-bit indices: build_dia admits the pattern only when rows + cols < 2^31.  Exact grid, one trip per
+  // thread.  Lanes past the end stay for the shuffles (R > 1) on the virtual rows after the last one: their
+  // x indices are clamped, their mask words exist (the mask array is padded to a multiple of the slice
+  // height >= 32*R), nothing is stored.
+  const int r0 = (blockIdx.x * blockDim.x + threadIdx.x) * R;
+  if (R == 1 && r0 >= rows) return;
+  unsigned m[R];
+  if constexpr (R == 2) {
+    const typename DiaMaskVec<MT>::V2 mm = *reinterpret_cast<const typename DiaMaskVec<MT>::V2*>(mask + r0);
+    m[0] = mm.x; m[1] = mm.y;
+  } else if constexpr (R == 4) {
+    const typename DiaMaskVec<MT>::V4 mm = *reinterpret_cast<const typename DiaMaskVec<MT>::V4*>(mask + r0);
+    m[0] = mm.x; m[1] = mm.y; m[2] = mm.z; m[3] = mm.w;
+  } else {
+    m[0] = mask[r0];
+  }
+  pdl_wait();                                                // x and y may be the previous kernel's output
+  const bool full = r0 + R <= rows;
+  double yold[R], acc[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) { yold[r] = 0.0; acc[r] = 0.0; }
+  if (beta != 0.0) {
+    if constexpr (R > 1) {
+      if (full) {
+#pragma unroll
+        for (int r = 0; r < R; r += 2) {
+          const double2 p = *reinterpret_cast<const double2*>(y + r0 + r);
+          yold[r] = p.x; yold[r + 1] = p.y;
+        }
+      } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r) if (r0 + r < rows) yold[r] = y[r0 + r];
+      }
+    } else {
+      yold[0] = y[r0];
+    }
+  }
+  // statically unrolled over the chunks so that the by-value offset / coefficient parameters are never
+  // indexed dynamically
+#pragma unroll
+  for (int d0 = 0; d0 < DMAX; d0 += NDC) {
+    if (ND == 0 && d0 >= nd) break;
+    double xv[NDC][R];
+#pragma unroll
+    for (int u = 0; u < NDC; ++u) {
+      const int d = d0 + u;
+      if (d < DMAX && (ND != 0 || d < nd)) {                 // warp-uniform
+        const int o = offs.off[d < 32 ? d : 31];
+        if constexpr (R == 1) {
+          xv[u][0] = ldx<X>(x, min(max(r0 + o, 0), cols - 1));
+        } else {
+          // branch-free for either parity of the offset (p is warp-uniform: r0 is even): the run starts at
+          // the even index b = r0 + o - p; for p = 1 it is shifted left by one element and the right
+          // neighbour x[b + R] comes from the next lane's first element (lane 31 loads it)
+          const int p = o & 1;
+          const int b = r0 + o - p;
+          double e[R];
+          dia_load_pairs<R, X>(x, b, cols, e);
+          double nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
+          if (p && (threadIdx.x & 31) == 31) nxt = ldx<X>(x, min(max(b + R, 0), cols - 1));
+#pragma unroll
+          for (int r = 0; r + 1 < R; ++r) xv[u][r] = p ? e[r + 1] : e[r];
+          xv[u][R - 1] = p ? nxt : e[R - 1];
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < NDC; ++u) {
+      const int d = d0 + u;
+      if (d < DMAX && (ND != 0 || d < nd)) {
+        const double c = coefs.c[d < 32 ? d : 31];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = ((m[r] >> d) & 1u) ? fma(c, xv[u][r], acc[r]) : acc[r];
+      }
+    }
+  }
+  double out[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) out[r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  if constexpr (R > 1) {
+    if (full) {
+#pragma unroll
+      for (int r = 0; r < R; r += 2) *reinterpret_cast<double2*>(y + r0 + r) = make_double2(out[r], out[r + 1]);
+      return;
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    if (r0 + r < rows) y[r0 + r] = out[r];
+}
+
+template <int R, int ND, int X, typename MT>
+__global__ void __launch_bounds__(512, dia_const_min_blocks(R, ND))
+dia_const_kernel(int rows, int cols, int nd_rt, const __grid_constant__ DiaOffsets offs,
+                 const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
+                 const double* __restrict__ x, double beta, double* __restrict__ y) {
+  dia_const_body<R, ND, X, MT>(rows, cols, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+}
+// two rows per thread on a small stencil: 48 registers keep 1280 threads per SM resident without spilling
+template <int ND, int X, typename MT>
+__global__ void __maxnreg__(48)
+dia_const_kernel_r2(int rows, int cols, int nd_rt, const __grid_constant__ DiaOffsets offs,
+                    const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
+                    const double* __restrict__ x, double beta, double* __restrict__ y) {
+  dia_const_body<2, ND, X, MT>(rows, cols, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+}
+
+template <int R, int X, typename MT>
+static const void* dia_const_pick_nd(int nd) {
+  if constexpr (R == 2) {
+    switch (nd) {
+      case 3: return (const void*)dia_const_kernel_r2<3, X, MT>;
+      case 5: return (const void*)dia_const_kernel_r2<5, X, MT>;
+      case 7: return (const void*)dia_const_kernel_r2<7, X, MT>;
+      case 9: return (const void*)dia_const_kernel_r2<9, X, MT>;
+      default: break;
+    }
+  }
+  switch (nd) {
+    case 3: return (const void*)dia_const_kernel<R, 3, X, MT>;
+    case 5: return (const void*)dia_const_kernel<R, 5, X, MT>;
+    case 7: return (const void*)dia_const_kernel<R, 7, X, MT>;
+    case 9: return (const void*)dia_const_kernel<R, 9, X, MT>;
+    case 27: return (const void*)dia_const_kernel<R, 27, X, MT>;
+    default: return (const void*)dia_const_kernel<R, 0, X, MT>;
+  }
+}
+template <int R, int X>
+static const void* dia_const_pick_mt(int mask_elem, int nd) {
+  return mask_elem == 1 ? dia_const_pick_nd<R, X, unsigned char>(nd)
+       : mask_elem == 2 ? dia_const_pick_nd<R, X, unsigned short>(nd) : dia_const_pick_nd<R, X, unsigned>(nd);
+}
+static const void* dia_const_pick(int R, int X, int mask_elem, int nd) {
+#define P(r, xx) if (R == r && X == xx) return dia_const_pick_mt<r, xx>(mask_elem, nd);
   P(1, 0) P(2, 0) P(4, 0) P(1, 1) P(2, 1) P(4, 1)
 #undef P
   return nullptr;
 }
-bool dia_const_supported(const Variant& v) {
-  return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && dia_c_ok(v.C) && dia_const_pick(v) != nullptr;
+bool dia_const_supported(const Variant& v) {      // exact grid only (no g key): one trip per thread
+  return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && v.grid == 0 && dia_c_ok(v.C) &&
+         dia_const_pick(v.R, v.X, 4, 0) != nullptr;
 }
-const void* dia_const_func(const Variant& v) { return (const void*)dia_const_pick(v); }
+const void* dia_const_func(const Variant& v) { return dia_const_pick(v.R, v.X, 4, 0); }
 cudaError_t dia_const_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
                              int grid_blocks) {
-  dia_const_kernel_t k = dia_const_pick(v);
-  if (!k || !f.is_const) return cudaErrorInvalidValue;
+  if (!f.is_const) return cudaErrorInvalidValue;
   if (rows == 0) return cudaSuccess;
+  // 16-byte pair accesses need aligned vectors and an even column count (a pair is then never half inside
+  // [0, cols)): anything else runs the one-row-per-thread instantiation
+  const int R = ((((uintptr_t)a.x | (uintptr_t)a.y) & 15) == 0 && cols % 2 == 0) ? v.R : 1;
+  const void* mask = f.mask_small ? f.mask_small : (const void*)f.mask;
+  const void* k = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd);
+  if (!k) return cudaErrorInvalidValue;
   DiaCoefs c;
   for (int i = 0; i < 32; ++i) c.c[i] = f.coef[i];
-  const int64_t threads = (rows + v.R - 1) / v.R;
-  const int64_t exact = (threads + v.block - 1) / v.block;
-  const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, cols, f.nd, dia_offsets(f), c, f.mask, a.alpha, a.x, a.beta, a.y,
-                                              (int)(((uintptr_t)a.y & 15) == 0));
-  return cudaGetLastError();
+  DiaOffsets o = dia_offsets(f);
+  const int64_t threads = (rows + R - 1) / R;
+  const int64_t grid = (threads + v.block - 1) / v.block;
+  (void)grid_blocks;
+  int nd = f.nd, rows32 = (int)rows, cols32 = (int)cols;
+  void* args[] = {&rows32, &cols32, &nd, &o, &c, &mask, (void*)&a.alpha, (void*)&a.x, (void*)&a.beta, (void*)&a.y};
+  return launch_kernel_pdl(k, (unsigned)grid, v.block, 0, a.stream, args);
 }
 
 // ------------------------------------------------------------------ DIA with the value stream on the TMA engine
@@ -539,7 +620,15 @@ __global__ void dia_cmp_kernel(int64_t rows, int C, int nd, const double* __rest
   if (bad) atomicAdd(mismatch, 1u);
 }
 
+// narrow copy of the mask words for dia_const (1 byte per row when nd <= 8, 2 when nd <= 16)
+template <typename MT>
+__global__ void dia_mask_narrow_kernel(int64_t ld, const unsigned* __restrict__ mask, MT* __restrict__ out) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r < ld) out[r] = (MT)mask[r];
+}
+
 void free_dia(DiaFormat& f, Allocator& al) {
+  if (f.mask_small) al.free(f.mask_small, (size_t)f.mask_elem * std::max<int64_t>(f.ld, 1));
   if (f.val) al.free(f.val, sizeof(double) * std::max<int64_t>((int64_t)f.nd * f.ld, 1));
   if (f.mask) al.free(f.mask, sizeof(unsigned) * std::max<int64_t>(f.ld, 1));
   f = DiaFormat();
@@ -618,6 +707,16 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
     for (int d = 0; d < 32; ++d) {
       const unsigned long long bits = h_ref[32 + std::min(d, nd - 1)];
       memcpy(&f.coef[d], &bits, sizeof(double));
+    }
+    if (f.is_const && nd <= 16) {
+      f.mask_elem = nd <= 8 ? 1 : 2;
+      f.mask_small = al.alloc((size_t)f.mask_elem * f.ld, s);
+      if (!f.mask_small) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+      const unsigned gm = (unsigned)((f.ld + 255) / 256);
+      if (f.mask_elem == 1) dia_mask_narrow_kernel<unsigned char><<<gm, 256, 0, s>>>(f.ld, f.mask, (unsigned char*)f.mask_small);
+      else dia_mask_narrow_kernel<unsigned short><<<gm, 256, 0, s>>>(f.ld, f.mask, (unsigned short*)f.mask_small);
+      cudaError_t e3 = cudaGetLastError();
+      if (e3 != cudaSuccess) { free_dia(f, al); set_last_error("build_dia: %s", cudaGetErrorString(e3)); return SPMV_ERR_CUDA; }
     }
   }
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));

@@ -70,6 +70,8 @@ struct DiaFormat {
   // diagonal holds the same bit pattern; coef[d] is that value.  dia_const then reads no matrix values.
   bool is_const = false;
   double coef[32] = {0};
+  void* mask_small = nullptr;    // is_const && nd <= 16: the mask words narrowed to mask_elem bytes per row
+  int mask_elem = 4;
   // x windows for the dia_win kernels (kernels_dia_win.cu): groups of near-consecutive offsets share one
   // contiguous window of x per slice
   int ng = 0, win_total = 0;     // groups; total window entries per slice
@@ -167,6 +169,25 @@ void dia_compute_windows(DiaFormat& f);
 bool dia_tma_supported(const Variant&);
 const void* dia_tma_func(const Variant&);
 cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);
+
+// Launch through cudaLaunchKernelExC; pdl = true marks the launch as a programmatic dependent launch
+// (cudaLaunchAttributeProgrammaticStreamSerialization): the kernel may start while the previous kernel of
+// the stream drains, and MUST execute griddepcontrol.wait (device_utils.cuh: pdl_wait) before it touches
+// anything a previous kernel may write or still read.
+inline cudaError_t launch_kernel_pdl(const void* k, unsigned grid, unsigned block, size_t smem, cudaStream_t s,
+                                     void** args, bool pdl = true) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid, 1, 1);
+  cfg.blockDim = dim3(block, 1, 1);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelExC(&cfg, k, args);
+}
 
 // y = beta*y (or 0): the alpha == 0 path (reading A2)
 cudaError_t scale_y_launch(int64_t rows, double beta, double* y, cudaStream_t s);

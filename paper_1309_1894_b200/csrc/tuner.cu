@@ -470,6 +470,8 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
       if (!budget_left()) break;
       Variant v = L; v.grid = g; v.carve = co;
       if (!filter_match(o.variant_filter, variant_to_string(v))) continue;
+      std::string why;
+      if (!variant_eligible(h, v, &why)) continue;      // e.g. dia_const has no grid key (exact grid only)
       ++n_enum;
       st = try_candidate(v, false);
       if (st != SPMV_OK) return fail(st);

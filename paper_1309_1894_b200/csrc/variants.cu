@@ -282,7 +282,8 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
     case FAM_DIA_CWIN:
     case FAM_DIA_CONST: {
       auto it = h->dias.find(v.C);
-      return it == h->dias.end() ? 0 : A.rows * 4;       // the mask words are all that is read of the matrix
+      if (it == h->dias.end()) return 0;                 // the mask words are all that is read of the matrix
+      return A.rows * (v.fam == FAM_DIA_CONST && it->second.mask_small ? it->second.mask_elem : 4);
     }
     case FAM_DIA_WIN:
     case FAM_DIA_TMA:

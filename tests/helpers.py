@@ -53,7 +53,7 @@ REPRESENTATIVE_VARIANTS = [
     "sell:b256:c128:s8192:l16:r2:u2:x0", "sell:b128:c512:s1024:l64:r1:u4:x0", "sell:b256:c128:s256:l4:r1:u2:x1",
     "sell_tma:b160:c128:s8192:l32:r1:u4:i3:x0", "sell_tma:b160:c256:s2048:l128:r2:u8:i2:x0",
     "dia:b256:c128:r1:u4:x0", "dia:b128:c256:r2:u8:x0", "dia:b256:c512:r4:u2:x1", "dia:b512:c128:r1:u1:x0:g2",
-    "dia_const:b256:r1:x0", "dia_const:b128:r2:x1", "dia_const:b512:r4:x0:g2",
+    "dia_const:b256:r1:x0", "dia_const:b128:r2:x1", "dia_const:b512:r4:x0",
     "dia_win:b288:c256:r1:i2:x0", "dia_win:b96:c128:r2:i3:x0", "dia_win:b160:c128:r1:i4:x0:g2",
     "dia_cwin:b288:c256:r1:i3:x0", "dia_cwin:b288:c512:r2:i2:x0", "dia_cwin:b544:c512:r1:i4:x0",
     "dia_tma:b288:c256:r1:u8:i3:x0", "dia_tma:b96:c128:r2:u4:i2:x0", "dia_tma:b544:c512:r1:u7:i4:x0", "dia_tma:b160:c256:r2:u9:i2:x0:g2",
