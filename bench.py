@@ -446,8 +446,25 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
 
     # ---- K applies replayed as one CUDA graph (launch-bound configs; a clearly labelled extra line)
     graph = None
-    if members == 1 and hasattr(handles[0], "graph_time") and cfg in (1, 2):
-        graph = handles[0].graph_time(alpha, xs[0], beta, ys[0], k=50, reps=20)
+    if members == 1 and cfg in (1, 2):
+        kg = 50
+        g = handles[0].graph(alpha, xs[0], beta, ys[0], kg)
+        for _ in range(3):
+            g.launch()
+        torch.cuda.synchronize()
+        tg = []
+        for _ in range(20):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            g.launch()
+            b.record()
+            torch.cuda.synchronize()
+            tg.append(a.elapsed_time(b) * 1e3 / kg)
+        g.close()
+        graph = {"applies_per_graph": kg, "us_per_apply": float(np.median(tg)),
+                 "eff_gbs": nbytes / float(np.median(tg)) / 1e3,
+                 "note": "ADDITIONAL line, not the headline: spmv_graph_create captures 50 back-to-back applies on ONE "
+                         "set of buffers (warm caches), one cudaGraphLaunch replays them; launch cost amortised"}
 
     info = handles[0].info()
     peak_meas, _ = measured_peak()

@@ -177,6 +177,17 @@ SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d
 SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
                               double* h_y, void* stream);
 
+/* k back-to-back applies y <- alpha*A*x + beta*y of the selected variant captured into ONE CUDA graph (SURVEY.md
+ * sec. 8(d): "a CUDA-graph replay of K applies may be reported as an additional, clearly labelled line"
+ * lists the launch configuration among the tuned parameters -- for a launch-bound matrix the launch itself is the
+ * cost).  Pointers, scalars and the variant are baked in: re-create the graph after spmv_select / spmv_tune /
+ * spmv_update_values.  spmv_graph_launch replays it on `stream` (asynchronous).  Errors: INVALID_ARG, CUDA. */
+typedef struct spmv_graph_s* spmv_graph_t;
+SPMV_API spmv_status_t spmv_graph_create(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y,
+                                int32_t k, spmv_graph_t* out);
+SPMV_API spmv_status_t spmv_graph_launch(spmv_graph_t g, void* stream);
+SPMV_API spmv_status_t spmv_graph_destroy(spmv_graph_t g);
+
 /* n independent applies, handle i on streams[i % nstreams] ("number of
  * asynchronous streams").  No synchronisation. */
 SPMV_API spmv_status_t spmv_apply_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,

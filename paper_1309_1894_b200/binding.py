@@ -21,7 +21,8 @@ STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "S
 EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
            "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_status_string",
-           "spmv_last_error", "spmv_version", "spmv_clear_cache"]
+           "spmv_last_error", "spmv_version", "spmv_clear_cache", "spmv_graph_create", "spmv_graph_launch",
+           "spmv_graph_destroy"]
 
 
 class SpmvError(RuntimeError):
@@ -108,9 +109,13 @@ def lib():
     L.spmv_measure_ceiling.argtypes = [i32, C.c_size_t, i32, vp, C.POINTER(dbl)]
     L.spmv_update_values.argtypes = [vp, vp, C.POINTER(i32), vp]
     L.spmv_cg.argtypes = [vp, vp, vp, C.POINTER(CgOpts), C.POINTER(CgResult), vp]
+    L.spmv_graph_create.argtypes = [vp, dbl, vp, dbl, vp, i32, C.POINTER(vp)]
+    L.spmv_graph_launch.argtypes = [vp, vp]
+    L.spmv_graph_destroy.argtypes = [vp]
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg"):
+              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg",
+              "spmv_graph_create", "spmv_graph_launch", "spmv_graph_destroy"):
         getattr(L, n).restype = C.c_int
     L.spmv_status_string.argtypes = [C.c_int]
     L.spmv_status_string.restype = C.c_char_p
@@ -132,23 +137,13 @@ def _stream_ptr(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
-def _raw_current_stream(device_index):
+def _getraw(device_index):
     """cudaStream_t of torch's current stream as an int (the fast private accessor when torch has it)."""
     import torch
     try:
-        return torch._C._cuda_getCurrentRawStream(device_index if device_index is not None else torch.cuda.current_device())
+        return torch._C._cuda_getCurrentRawStream(device_index)
     except AttributeError:
-        return torch.cuda.current_stream().cuda_stream
-
-
-_apply = None
-
-
-def _apply_fn():
-    global _apply
-    if _apply is None:
-        _apply = lib().spmv_apply
-    return _apply
+        return torch.cuda.current_stream(device_index).cuda_stream
 
 
 def _dptr(t):
@@ -191,6 +186,8 @@ class SpMV:
                                C.byref(self._alloc) if self._alloc is not None else None, _stream_ptr(stream))
         _check(st, "spmv_create")
         self.h = h
+        self._apply = lib().spmv_apply
+        self._dev = row_ptr.device.index
 
     @classmethod
     def from_csr(cls, A, device="cuda:0", **kw):
@@ -233,10 +230,12 @@ class SpMV:
 
     def apply(self, alpha, x, beta, y, stream=None):
         """y = alpha*A*x + beta*y on the device, asynchronous on the (current) stream.
-        Kept lean: for small matrices the call overhead is what a user sees."""
-        assert x.numel() == self.cols and y.numel() == self.rows and x.is_cuda and y.is_cuda
-        s = _raw_current_stream(x.device.index) if stream is None else stream.cuda_stream
-        st = _apply_fn()(self.h, alpha, x.data_ptr(), beta, y.data_ptr(), s)
+        Kept lean: for small matrices the call overhead is what a user sees (a ctypes call costs ~0.7 us,
+        the CUDA launch ~2 us; spmv_graph_create amortises both over k applies)."""
+        if x.numel() != self.cols or y.numel() != self.rows or not (x.is_cuda and y.is_cuda):
+            raise ValueError("spmv_apply: x must hold cols and y rows CUDA float64 entries")
+        s = _getraw(self._dev) if stream is None else stream.cuda_stream
+        st = self._apply(self.h, alpha, x.data_ptr(), beta, y.data_ptr(), s)
         if st != SPMV_OK:
             _check(st, "spmv_apply")
         return y
@@ -258,6 +257,14 @@ class SpMV:
         r = CgResult()
         _check(lib().spmv_cg(self.h, _dptr(b), _dptr(x), C.byref(o), C.byref(r), _stream_ptr(stream)), "spmv_cg")
         return {k: getattr(r, k) for k, _ in CgResult._fields_}
+
+    def graph(self, alpha, x, beta, y, k: int) -> "Graph":
+        """k back-to-back applies captured into one CUDA graph (spmv_graph_create); x, y are baked in."""
+        assert x.is_cuda and y.is_cuda and x.numel() == self.cols and y.numel() == self.rows
+        g = C.c_void_p(0)
+        _check(lib().spmv_graph_create(self.h, float(alpha), _dptr(x), float(beta), _dptr(y), int(k), C.byref(g)),
+               "spmv_graph_create")
+        return Graph(g, k, (x, y, self))
 
     def apply_host(self, alpha, x_host, beta, y_host, stream=None):
         """Host-buffer form: x_host/y_host are CPU tensors or numpy arrays (pinned is faster)."""
@@ -315,6 +322,27 @@ class SpMV:
             _check(lib().spmv_format_download(self.h, name.encode(), C.c_void_p(out.ctypes.data), n.value,
                                               C.byref(n), _stream_ptr()), f"spmv_format_download({name})")
         return out
+
+
+class Graph:
+    """spmv_graph_t wrapper; keeps the vectors and the handle it was captured from alive."""
+
+    def __init__(self, g, k, keep):
+        self.g, self.k, self._keep = g, k, keep
+
+    def launch(self, stream=None):
+        _check(lib().spmv_graph_launch(self.g, _stream_ptr(stream)), "spmv_graph_launch")
+
+    def close(self):
+        if self.g is not None and self.g.value:
+            _check(lib().spmv_graph_destroy(self.g), "spmv_graph_destroy")
+            self.g = C.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def apply_batch(handles, alphas, xs, betas, ys, streams):

@@ -29,6 +29,19 @@ static void refresh_info(spmv_handle_s* h) {
 }
 void handle_refresh_info(spmv_handle_s* h) { refresh_info(h); }
 
+spmv_status_t adopt_variant(spmv_handle_s* h, const Variant& v, cudaStream_t s) {
+  spmv_status_t st = ensure_format(h, v, s);
+  if (st != SPMV_OK) return st;
+  LaunchPlan p;
+  st = build_plan(h, v, &p);
+  if (st != SPMV_OK) return st;
+  h->sel = v;
+  h->plan = p;
+  release_formats_except(h, v);
+  refresh_info(h);
+  return SPMV_OK;
+}
+
 }  // namespace spmv
 
 using namespace spmv;
@@ -105,8 +118,7 @@ spmv_status_t spmv_create(spmv_handle_t* out, int64_t rows, int64_t cols, int64_
   in.sm_count = h->dev.sm_count;
   in.l2_bytes = h->dev.l2_bytes;
   strncpy(in.device_name, h->dev.name, sizeof(in.device_name) - 1);
-  h->sel = default_variant();
-  refresh_info(h);
+  if (adopt_variant(h, default_variant(), s) != SPMV_OK) { delete h; return SPMV_ERR_CUDA; }
   {
     std::lock_guard<std::mutex> lk(g_live_mu);
     g_live.insert((void*)h);
@@ -121,6 +133,7 @@ spmv_status_t spmv_destroy(spmv_handle_t h) {
     std::lock_guard<std::mutex> lk(g_live_mu);
     g_live.erase((void*)h);
   }
+  cudaDeviceSynchronize();          // no apply may still be using the formats or the staging vectors
   release_all_formats(h);
   if (h->d_x_stage) h->al.free(h->d_x_stage, sizeof(double) * h->A.cols);
   if (h->d_y_stage) h->al.free(h->d_y_stage, sizeof(double) * h->A.rows);
@@ -142,42 +155,40 @@ spmv_status_t spmv_select(spmv_handle_t h, const char* desc, void* stream) {
   if (!variant_from_string(desc, &v)) { set_last_error("cannot parse variant '%s'", desc); return SPMV_ERR_INVALID_ARG; }
   std::string why;
   if (!variant_eligible(h, v, &why)) { set_last_error("variant %s not eligible: %s", desc, why.c_str()); return SPMV_ERR_UNSUPPORTED; }
-  spmv_status_t st = ensure_format(h, v, (cudaStream_t)stream);
+  spmv_status_t st = adopt_variant(h, v, (cudaStream_t)stream);
   if (st != SPMV_OK) return st;
-  h->sel = v;
-  release_formats_except(h, v);
-  refresh_info(h);
+  SPMV_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   return SPMV_OK;
 }
 
 spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* fell_back, void* stream) {
   if (!handle_alive(h) || (h->A.nnz > 0 && !d_val)) return SPMV_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  SPMV_CUDA_TRY(cudaStreamSynchronize(s));          // no apply may still be reading the old formats
+  SPMV_CUDA_TRY(cudaDeviceSynchronize());           // no apply on any stream may still be reading the old formats
   h->A.val = d_val;
   release_all_formats(h);
   if (h->dia_state > 0) h->dia_state = 0;           // constness must be re-established on the new values
   if (fell_back) *fell_back = 0;
-  spmv_status_t st = ensure_format(h, h->sel, s);
+  spmv_status_t st = adopt_variant(h, h->sel, s);
   if (st == SPMV_ERR_UNSUPPORTED) {
     if (fell_back) *fell_back = 1;
     Variant alt = h->sel;
     st = SPMV_ERR_UNSUPPORTED;
     if ((h->sel.fam == FAM_DIA_CONST || h->sel.fam == FAM_DIA_CWIN) && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
       std::string why;
-      if (variant_eligible(h, alt, &why)) st = ensure_format(h, alt, s);
+      if (variant_eligible(h, alt, &why)) st = adopt_variant(h, alt, s);
     }
-    if (st != SPMV_OK) { alt = default_variant(); st = SPMV_OK; h->tuned = false; }
-    h->sel = alt;
-    release_formats_except(h, alt);
+    if (st != SPMV_OK) { h->tuned = false; st = adopt_variant(h, default_variant(), s); }
   }
   if (st != SPMV_OK) return st;
-  refresh_info(h);
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
   return SPMV_OK;
 }
 
+// The apply path: argument checks, then one (two for merge-path / row-split SELL) kernel launch from the
+// plan resolved at select / tune time.  No locks, no lookups, no CUDA attribute or occupancy calls.
 spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y, void* stream) {
-  if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
+  if (!h || h->magic != kHandleMagic) return SPMV_ERR_INVALID_ARG;
   if (h->A.rows > 0 && !d_y) return SPMV_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
   if (alpha == 0.0 || h->A.rows == 0) {           // reading A2: A and x are not referenced
@@ -187,7 +198,53 @@ spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, doubl
   }
   if (h->A.cols > 0 && !d_x) return SPMV_ERR_INVALID_ARG;
   ApplyArgs a{alpha, beta, d_x, d_y, s};
-  return launch_variant(h, h->sel, a);
+  return launch_plan(h->plan, a);
+}
+
+struct spmv_graph_s {
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  int k = 0;
+};
+
+spmv_status_t spmv_graph_create(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y, int32_t k,
+                                spmv_graph_t* out) {
+  if (!handle_alive(h) || !out || k < 1) return SPMV_ERR_INVALID_ARG;
+  cudaStream_t cs = nullptr;
+  SPMV_CUDA_TRY(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+  spmv_graph_s* g = new (std::nothrow) spmv_graph_s();
+  if (!g) { cudaStreamDestroy(cs); return SPMV_ERR_ALLOC; }
+  g->k = k;
+  cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+  spmv_status_t st = SPMV_OK;
+  for (int i = 0; i < k && e == cudaSuccess && st == SPMV_OK; ++i) st = spmv_apply(h, alpha, d_x, beta, d_y, cs);
+  cudaError_t e2 = cudaStreamEndCapture(cs, &g->graph);         // always end the capture, also after a failure
+  if (e == cudaSuccess) e = e2;
+  if (e == cudaSuccess && st == SPMV_OK) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+  cudaStreamDestroy(cs);
+  if (e != cudaSuccess || st != SPMV_OK) {
+    if (e != cudaSuccess) set_last_error("spmv_graph_create: %s", cudaGetErrorString(e));
+    if (g->graph) cudaGraphDestroy(g->graph);
+    delete g;
+    cudaGetLastError();
+    return st != SPMV_OK ? st : SPMV_ERR_CUDA;
+  }
+  *out = g;
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_graph_launch(spmv_graph_t g, void* stream) {
+  if (!g || !g->exec) return SPMV_ERR_INVALID_ARG;
+  SPMV_CUDA_TRY(cudaGraphLaunch(g->exec, (cudaStream_t)stream));
+  return SPMV_OK;
+}
+
+spmv_status_t spmv_graph_destroy(spmv_graph_t g) {
+  if (!g) return SPMV_ERR_INVALID_ARG;
+  if (g->exec) cudaGraphExecDestroy(g->exec);
+  if (g->graph) cudaGraphDestroy(g->graph);
+  delete g;
+  return SPMV_OK;
 }
 
 spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,

@@ -15,6 +15,7 @@ struct spmv_handle_s {
   int device = 0;
   spmv_info_t info{};
   spmv::Variant sel;
+  spmv::LaunchPlan plan;          // resolved launch of `sel` (rebuilt by select / tune / update_values)
   bool tuned = false;
 
   // owned formats, built on demand
@@ -46,8 +47,12 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
 // Builds (or finds) the format the variant needs.  UNSUPPORTED if the built format turns
 // out too padded to be worth keeping.
 spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s);
-// Launches the variant (format must exist).  Resolves grid size and carve-out.
-spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs& a);
+// Resolves kernel, grid, shared memory, carve-out and the argument block of `v` (format must exist).
+spmv_status_t build_plan(spmv_handle_s* h, const Variant& v, LaunchPlan* out);
+// Launches a resolved plan: patch alpha / x / beta / y, one or two kernel launches, nothing else.
+spmv_status_t launch_plan(const LaunchPlan& p, const ApplyArgs& a);
+// Makes `v` the selected variant: format, plan, info.  Waits for the device first when formats are freed.
+spmv_status_t adopt_variant(spmv_handle_s* h, const Variant& v, cudaStream_t s);
 // Bytes of matrix data the variant streams per apply (format-actual, not algorithmic).
 int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v);
 // Frees every owned format the given variant does not need.

@@ -77,18 +77,22 @@ static bcsr_kernel_t pick(const Variant& v) {
 bool bcsr_supported(const Variant& v) {
   return v.block >= 32 && v.block <= 1024 && v.block % 32 == 0 && pick(v) != nullptr;
 }
-const void* bcsr_func(const Variant& v) { return (const void*)pick(v); }
-
-cudaError_t bcsr_launch(const Variant& v, const BcsrFormat& f, const ApplyArgs& a, int grid_blocks) {
+cudaError_t bcsr_plan(const Variant& v, const BcsrFormat& f, int sm_count, LaunchPlan* out) {
   bcsr_kernel_t k = pick(v);
   if (!k) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (f.brows == 0) return cudaSuccess;
-  int64_t per_block = v.block / v.W;
-  int64_t exact = (f.brows + per_block - 1) / per_block;
-  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>((int)f.brows, f.brow_ptr, f.bcol, f.bval, a.alpha, a.x, a.beta,
-                                              a.y);
-  return cudaGetLastError();
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)k;
+  c.block = v.block;
+  const int64_t per_block = v.block / v.W;
+  const int64_t exact = (f.brows + per_block - 1) / per_block;
+  cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
+  if (e != cudaSuccess) return e;
+  c.add((int)f.brows); c.add((const int*)f.brow_ptr); c.add((const int*)f.bcol); c.add((const double*)f.bval);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  out->n = 1;
+  return cudaSuccess;
 }
 
 }  // namespace spmv

@@ -18,14 +18,15 @@ csr_scalar_kernel(int rows, const int* __restrict__ rp, const int* __restrict__ 
                   double beta, double* __restrict__ y) {
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < rows; g += G * R) {
-    int k[R], e[R];
+    // unsigned: k + U can pass 2^31 - 1 when nnz is near the int32 limit (positions stay below 2^32)
+    unsigned k[R], e[R];
     double s[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       int64_t row = g + (int64_t)r * G;
       bool ok = row < rows;
-      k[r] = ok ? __ldg(rp + row) : 0;
-      e[r] = ok ? __ldg(rp + row + 1) : 0;
+      k[r] = ok ? (unsigned)__ldg(rp + row) : 0u;
+      e[r] = ok ? (unsigned)__ldg(rp + row + 1) : 0u;
       s[r] = 0.0;
     }
     bool more = true;
@@ -69,15 +70,15 @@ csr_vector_kernel(int rows, const int* __restrict__ rp, const int* __restrict__ 
   for (int64_t base = warp_first; base < rows; base += nsub) {
     const int64_t row = base + (threadIdx.x & 31) / W;
     const bool ok = row < rows;
-    const int start = ok ? __ldg(rp + row) : 0;
-    const int end = ok ? __ldg(rp + row + 1) : 0;
+    const unsigned start = ok ? (unsigned)__ldg(rp + row) : 0u;     // unsigned: k + u*W may pass 2^31 - 1
+    const unsigned end = ok ? (unsigned)__ldg(rp + row + 1) : 0u;
     double s = 0.0;
-    for (int k = start + lane; k < end; k += W * U) {
+    for (unsigned k = start + lane; k < end; k += W * U) {
       double v[U];
       int c[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
-        int kk = k + u * W;
+        const unsigned kk = k + u * W;
         bool in = kk < end;
         v[u] = in ? __ldg(va + kk) : 0.0;
         c[u] = in ? __ldg(ci + kk) : -1;
@@ -132,30 +133,42 @@ static csr_kernel_t vector_pick(const Variant& v) {
 static bool block_ok(int b) { return b >= 32 && b <= 1024 && (b % 32) == 0; }
 
 bool csr_scalar_supported(const Variant& v) { return block_ok(v.block) && scalar_pick(v) != nullptr; }
-const void* csr_scalar_func(const Variant& v) { return (const void*)scalar_pick(v); }
-cudaError_t csr_scalar_launch(const Variant& v, const CsrView& A, const ApplyArgs& a, int grid_blocks) {
+static void csr_args(KernelCall& c, const CsrView& A) {
+  c.add((int)A.rows); c.add(A.row_ptr); c.add(A.col_idx); c.add(A.val);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+}
+cudaError_t csr_scalar_plan(const Variant& v, const CsrView& A, int sm_count, LaunchPlan* out) {
   csr_kernel_t k = scalar_pick(v);
   if (!k) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (A.rows == 0) return cudaSuccess;
-  int64_t exact = (A.rows + (int64_t)v.block * v.R - 1) / ((int64_t)v.block * v.R);
-  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>((int)A.rows, A.row_ptr, A.col_idx, A.val, a.alpha, a.x,
-                                              a.beta, a.y);
-  return cudaGetLastError();
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)k;
+  c.block = v.block;
+  const int64_t exact = (A.rows + (int64_t)v.block * v.R - 1) / ((int64_t)v.block * v.R);
+  cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
+  if (e != cudaSuccess) return e;
+  csr_args(c, A);
+  out->n = 1;
+  return cudaSuccess;
 }
 
 bool csr_vector_supported(const Variant& v) { return block_ok(v.block) && vector_pick(v) != nullptr; }
-const void* csr_vector_func(const Variant& v) { return (const void*)vector_pick(v); }
-cudaError_t csr_vector_launch(const Variant& v, const CsrView& A, const ApplyArgs& a, int grid_blocks) {
+cudaError_t csr_vector_plan(const Variant& v, const CsrView& A, int sm_count, LaunchPlan* out) {
   csr_kernel_t k = vector_pick(v);
   if (!k) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (A.rows == 0) return cudaSuccess;
-  int64_t rows_per_block = v.block / v.W;
-  int64_t exact = (A.rows + rows_per_block - 1) / rows_per_block;
-  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>((int)A.rows, A.row_ptr, A.col_idx, A.val, a.alpha, a.x,
-                                              a.beta, a.y);
-  return cudaGetLastError();
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)k;
+  c.block = v.block;
+  const int64_t rows_per_block = v.block / v.W;
+  const int64_t exact = (A.rows + rows_per_block - 1) / rows_per_block;
+  cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
+  if (e != cudaSuccess) return e;
+  csr_args(c, A);
+  out->n = 1;
+  return cudaSuccess;
 }
 
 }  // namespace spmv

@@ -114,24 +114,29 @@ static bool dia_c_ok(int C) { return C == 128 || C == 256 || C == 512; }
 bool dia_supported(const Variant& v) {
   return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && dia_c_ok(v.C) && dia_pick(v) != nullptr;
 }
-const void* dia_func(const Variant& v) { return (const void*)dia_pick(v); }
-
 static DiaOffsets dia_offsets(const DiaFormat& f) {
   DiaOffsets o;
   for (int i = 0; i < 32; ++i) o.off[i] = f.off[i];
   return o;
 }
 
-cudaError_t dia_launch(const Variant& v, int64_t rows, const DiaFormat& f, const ApplyArgs& a, int grid_blocks) {
+cudaError_t dia_plan(const Variant& v, int64_t rows, const DiaFormat& f, int sm_count, LaunchPlan* out) {
   dia_kernel_t k = dia_pick(v);
   if (!k || f.C != v.C) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)k;
+  c.block = v.block;
   const int64_t threads = (f.ld + v.R - 1) / v.R;
   const int64_t exact = (threads + v.block - 1) / v.block;
-  const int64_t grid = grid_blocks > 0 ? std::min<int64_t>(grid_blocks, exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, f.ld, f.C, f.logC, f.nd, dia_offsets(f), f.val, f.mask, a.alpha, a.x,
-                                              a.beta, a.y);
-  return cudaGetLastError();
+  cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
+  if (e != cudaSuccess) return e;
+  c.add(rows); c.add((int64_t)f.ld); c.add(f.C); c.add(f.logC); c.add(f.nd); c.add(dia_offsets(f));
+  c.add((const double*)f.val); c.add((const unsigned*)f.mask);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  out->n = 1;
+  return cudaSuccess;
 }
 
 // ------------------------------------------------------------------ constant-coefficient stencil
@@ -332,26 +337,30 @@ bool dia_const_supported(const Variant& v) {      // exact grid only (no g key):
   return v.block >= 32 && v.block <= 512 && v.block % 32 == 0 && v.grid == 0 && dia_c_ok(v.C) &&
          dia_const_pick(v.R, v.X, 4, 0) != nullptr;
 }
-const void* dia_const_func(const Variant& v) { return dia_const_pick(v.R, v.X, 4, 0); }
-cudaError_t dia_const_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
-                             int grid_blocks) {
-  if (!f.is_const) return cudaErrorInvalidValue;
-  if (rows == 0) return cudaSuccess;
-  // 16-byte pair accesses need aligned vectors and an even column count (a pair is then never half inside
-  // [0, cols)): anything else runs the one-row-per-thread instantiation
-  const int R = ((((uintptr_t)a.x | (uintptr_t)a.y) & 15) == 0 && cols % 2 == 0) ? v.R : 1;
-  const void* mask = f.mask_small ? f.mask_small : (const void*)f.mask;
-  const void* k = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd);
-  if (!k) return cudaErrorInvalidValue;
-  DiaCoefs c;
-  for (int i = 0; i < 32; ++i) c.c[i] = f.coef[i];
-  DiaOffsets o = dia_offsets(f);
+static void dia_const_call(KernelCall& c, int R, const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f) {
+  c = KernelCall();
+  c.fn = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd);
+  c.block = v.block;
   const int64_t threads = (rows + R - 1) / R;
-  const int64_t grid = (threads + v.block - 1) / v.block;
-  (void)grid_blocks;
-  int nd = f.nd, rows32 = (int)rows, cols32 = (int)cols;
-  void* args[] = {&rows32, &cols32, &nd, &o, &c, &mask, (void*)&a.alpha, (void*)&a.x, (void*)&a.beta, (void*)&a.y};
-  return launch_kernel_pdl(k, (unsigned)grid, v.block, 0, a.stream, args);
+  c.grid = (unsigned)((threads + v.block - 1) / v.block);
+  c.pdl = true;
+  DiaCoefs co;
+  for (int i = 0; i < 32; ++i) co.c[i] = f.coef[i];
+  c.add((int)rows); c.add((int)cols); c.add(f.nd); c.add(dia_offsets(f)); c.add(co);
+  c.add(f.mask_small ? (const void*)f.mask_small : (const void*)f.mask);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+}
+cudaError_t dia_const_plan(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, LaunchPlan* out) {
+  if (!f.is_const || !dia_const_pick(v.R, v.X, 4, 0)) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
+  if (rows == 0) return cudaSuccess;
+  // 16-byte pair accesses need an even column count (a pair is then never half inside [0, cols)) and aligned
+  // vectors: the one-row-per-thread instantiation is the alternative taken per apply when x or y is not
+  const int R = cols % 2 == 0 ? v.R : 1;
+  dia_const_call(out->k[0], R, v, rows, cols, f);
+  if (R > 1) { dia_const_call(out->alt, 1, v, rows, cols, f); out->has_alt = true; }
+  out->n = 1;
+  return cudaSuccess;
 }
 
 // ------------------------------------------------------------------ DIA with the value stream on the TMA engine
@@ -525,36 +534,27 @@ bool dia_tma_supported(const Variant& v) {
   if (consumers < 32 || consumers > 512 || v.block != consumers + 32) return false;
   return dia_tma_smem(v) <= 200 * 1024;
 }
-const void* dia_tma_func(const Variant& v) {
-  const DiaTmaEntry* e = dia_tma_pick(v);
-  return e ? (const void*)e->k : nullptr;
-}
-
-cudaError_t dia_tma_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
-                           int sm_count) {
+cudaError_t dia_tma_plan(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, int sm_count,
+                         LaunchPlan* out) {
   const DiaTmaEntry* e = dia_tma_pick(v);
   if (!e || f.C != v.C) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
-  const size_t smem = dia_tma_smem(v);
-  static thread_local const void* attr_k = nullptr;
-  static thread_local size_t attr_smem = 0;
-  static thread_local int occ = 1;
-  if (attr_k != (const void*)e->k || attr_smem != smem) {
-    cudaError_t err = cudaFuncSetAttribute((const void*)e->k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)e->k, v.block, smem);
-    if (err != cudaSuccess) return err;
-    if (occ < 1) occ = 1;
-    attr_k = (const void*)e->k;
-    attr_smem = smem;
-  }
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)e->k;
+  c.block = v.block;
+  c.smem = (unsigned)dia_tma_smem(v);
+  cudaError_t err = allow_smem(c.fn, c.smem);
+  if (err != cudaSuccess) return err;
   const int64_t nslices = f.ld / f.C;
-  int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;   // persistent: g waves of resident CTAs
-  if (grid > nslices) grid = nslices;
-  const int y_bulk = ((uintptr_t)a.y & 15) == 0;     // cp.async.bulk needs 16-byte aligned global addresses
-  e->k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, cols, nslices, f.C, f.nd, dia_offsets(f), f.val, f.mask, a.alpha,
-                                                   a.x, a.beta, a.y, y_bulk);
-  return cudaGetLastError();
+  err = resolve_grid(v.grid > 0 ? v.grid : 1, c.fn, v.block, c.smem, sm_count, nslices, &c.grid);   // persistent
+  if (err != cudaSuccess) return err;
+  c.add(rows); c.add(cols); c.add(nslices); c.add(f.C); c.add(f.nd); c.add(dia_offsets(f));
+  c.add((const double*)f.val); c.add((const unsigned*)f.mask);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.add_flag(1);                 // y_bulk: cp.async.bulk needs 16-byte aligned global addresses
+  out->n = 1;
+  return cudaSuccess;
 }
 
 // ------------------------------------------------------------------ converter

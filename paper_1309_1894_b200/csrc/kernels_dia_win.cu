@@ -170,11 +170,6 @@ bool dia_win_supported(const Variant& v) {
   const int consumers = v.C / v.R;
   return consumers >= 32 && consumers <= 512 && v.block == consumers + 32;
 }
-const void* dia_win_func(const Variant& v) {
-  const DiaWinEntry* e = dia_win_pick(v);
-  return e ? (const void*)e->k : nullptr;
-}
-
 static size_t dia_win_smem(const Variant& v, const DiaFormat& f) {
   const size_t vals_d = v.fam == FAM_DIA_CWIN ? 0 : (size_t)f.nd * f.C;
   const size_t stage_d = vals_d + f.C + f.win_total + f.C / 2;
@@ -182,25 +177,23 @@ static size_t dia_win_smem(const Variant& v, const DiaFormat& f) {
 }
 bool dia_win_fits(const Variant& v, const DiaFormat& f) { return dia_win_smem(v, f) <= 200 * 1024; }
 
-cudaError_t dia_win_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, const ApplyArgs& a,
-                           int sm_count) {
+cudaError_t dia_win_plan(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, int sm_count,
+                         LaunchPlan* out) {
   const DiaWinEntry* e = dia_win_pick(v);
   if (!e || f.C != v.C || (e->CONST && !f.is_const)) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
+  KernelCall& c = out->k[0];
   const size_t smem = dia_win_smem(v, f);
   if (smem > 200 * 1024) return cudaErrorInvalidValue;
-  static thread_local const void* attr_k = nullptr;
-  static thread_local size_t attr_smem = 0;
-  static thread_local int occ = 1;
-  if (attr_k != (const void*)e->k || attr_smem != smem) {
-    cudaError_t err = cudaFuncSetAttribute((const void*)e->k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)e->k, v.block, smem);
-    if (err != cudaSuccess) return err;
-    if (occ < 1) occ = 1;
-    attr_k = (const void*)e->k;
-    attr_smem = smem;
-  }
+  c.fn = (const void*)e->k;
+  c.block = v.block;
+  c.smem = (unsigned)smem;
+  cudaError_t err = allow_smem(c.fn, c.smem);
+  if (err != cudaSuccess) return err;
+  const int64_t nslices = f.ld / f.C;
+  err = resolve_grid(v.grid > 0 ? v.grid : 1, c.fn, v.block, c.smem, sm_count, nslices, &c.grid);   // persistent
+  if (err != cudaSuccess) return err;
   DiaWinMeta m;
   for (int i = 0; i < 32; ++i) {
     m.off[i] = f.off[i]; m.xoff[i] = f.d_xoff[i]; m.coef[i] = f.coef[i];
@@ -208,13 +201,13 @@ cudaError_t dia_win_launch(const Variant& v, int64_t rows, int64_t cols, const D
   }
   m.ng = f.ng;
   m.win_total = f.win_total;
-  const int64_t nslices = f.ld / f.C;
-  int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;
-  if (grid > nslices) grid = nslices;
-  const int y_bulk = ((uintptr_t)a.y & 15) == 0, x_bulk = ((uintptr_t)a.x & 15) == 0;
-  e->k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, cols, nslices, f.C, f.nd, m, f.val, f.mask, a.alpha, a.x, a.beta,
-                                                   a.y, y_bulk, x_bulk);
-  return cudaGetLastError();
+  c.add(rows); c.add(cols); c.add(nslices); c.add(f.C); c.add(f.nd); c.add(m);
+  c.add((const double*)f.val); c.add((const unsigned*)f.mask);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.add_flag(1);                 // y_bulk
+  c.add_flag(2);                 // x_bulk
+  out->n = 1;
+  return cudaSuccess;
 }
 
 // Offset groups for a slice height C (host; called by build_dia): consecutive offsets whose spread stays

@@ -186,29 +186,29 @@ static const MergeEntry* merge_pick(const Variant& v) {
 }
 
 bool merge_supported(const Variant& v) { return merge_pick(v) != nullptr; }
-const void* merge_func(const Variant& v) {
-  const MergeEntry* e = merge_pick(v);
-  return e ? (const void*)e->k : nullptr;
-}
-
-cudaError_t merge_launch(const Variant& v, const CsrView& A, const MergePlan& p, const ApplyArgs& a) {
+cudaError_t merge_plan(const Variant& v, const CsrView& A, const MergePlan& p, LaunchPlan* out) {
   const MergeEntry* e = merge_pick(v);
   if (!e || p.tile_items != v.block * v.I) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (A.rows == 0) return cudaSuccess;
-  static thread_local const void* last_attr = nullptr;
-  if (e->smem > 48 * 1024 && last_attr != (const void*)e->k) {
-    cudaError_t err = cudaFuncSetAttribute((const void*)e->k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem);
-    if (err != cudaSuccess) return err;
-    last_attr = (const void*)e->k;
-  }
-  e->k<<<(unsigned)p.ntiles, e->B, e->smem, a.stream>>>((int)A.rows, (int)A.nnz, A.row_ptr, A.col_idx, A.val,
-                                                       p.tile_row, p.carry_row, p.carry_val, a.alpha, a.x,
-                                                       a.beta, a.y);
-  cudaError_t err = cudaGetLastError();
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)e->k;
+  c.grid = (unsigned)p.ntiles;
+  c.block = e->B;
+  c.smem = (unsigned)e->smem;
+  cudaError_t err = allow_smem(c.fn, c.smem);
   if (err != cudaSuccess) return err;
-  merge_fixup_kernel<<<(unsigned)((p.ntiles + 255) / 256), 256, 0, a.stream>>>(p.ntiles, p.carry_row,
-                                                                            p.carry_val, a.alpha, a.y);
-  return cudaGetLastError();
+  c.add((int)A.rows); c.add((int)A.nnz); c.add(A.row_ptr); c.add(A.col_idx); c.add(A.val);
+  c.add((const int*)p.tile_row); c.add(p.carry_row); c.add(p.carry_val);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  KernelCall& f = out->k[1];
+  f.fn = (const void*)merge_fixup_kernel;
+  f.grid = (unsigned)((p.ntiles + 255) / 256);
+  f.block = 256;
+  f.add((int64_t)p.ntiles); f.add((const int*)p.carry_row); f.add((const double*)p.carry_val);
+  f.add_alpha(); f.add_y();
+  out->n = 2;
+  return cudaSuccess;
 }
 
 spmv_status_t build_merge_plan(const CsrView& A, int tile_items, Allocator& al, cudaStream_t s,

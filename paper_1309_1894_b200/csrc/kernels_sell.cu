@@ -128,11 +128,13 @@ __global__ void sell_split_fixup_kernel(int64_t nsplit, const int* __restrict__ 
   if (lane == 0) store_y(y, __ldg(srow + w), alpha, s, beta);
 }
 
-cudaError_t sell_split_fixup_launch(const SellFormat& f, const ApplyArgs& a) {
-  if (!f.split || f.nsplit == 0) return cudaSuccess;
-  sell_split_fixup_kernel<<<(unsigned)((f.nsplit * 32 + 255) / 256), 256, 0, a.stream>>>(f.nsplit, f.srow, f.sptr, f.part,
-                                                                                      a.alpha, a.beta, a.y);
-  return cudaGetLastError();
+void sell_split_fixup_call(const SellFormat& f, KernelCall* c) {
+  *c = KernelCall();
+  c->fn = (const void*)sell_split_fixup_kernel;
+  c->grid = (unsigned)((f.nsplit * 32 + 255) / 256);
+  c->block = 256;
+  c->add((int64_t)f.nsplit); c->add((const int*)f.srow); c->add((const int*)f.sptr); c->add((const double*)f.part);
+  c->add_alpha(); c->add_beta(); c->add_y();
 }
 
 typedef void (*sell_kernel_t)(int64_t, int64_t, int, int, const int64_t*, const double*, const int*,
@@ -161,21 +163,26 @@ bool sell_supported(const Variant& v) {
   }
   return true;
 }
-const void* sell_func(const Variant& v, bool perm) { return (const void*)pick(v, perm); }
-
-cudaError_t sell_launch(const Variant& v, int64_t rows, const SellFormat& f, const ApplyArgs& a,
-                        int grid_blocks) {
+cudaError_t sell_plan(const Variant& v, int64_t rows, const SellFormat& f, int sm_count, LaunchPlan* out) {
   const bool perm = f.perm != nullptr;
   sell_kernel_t k = pick(v, perm);
   if (!k) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)k;
+  c.block = v.block;
   const int64_t rows_padded = f.nslices * (int64_t)f.C;
   const int64_t threads = (rows_padded + v.R - 1) / v.R;
-  int64_t exact = (threads + v.block - 1) / v.block;
-  int64_t grid = grid_blocks > 0 ? (grid_blocks < exact ? grid_blocks : exact) : exact;
-  k<<<(unsigned)grid, v.block, 0, a.stream>>>(rows, rows_padded, f.C, f.logC, f.slice_ptr, f.val, f.col,
-                                              f.perm, f.part, a.alpha, a.x, a.beta, a.y);
-  return cudaGetLastError();
+  const int64_t exact = (threads + v.block - 1) / v.block;
+  cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
+  if (e != cudaSuccess) return e;
+  c.add(rows); c.add(rows_padded); c.add(f.C); c.add(f.logC); c.add((const int64_t*)f.slice_ptr);
+  c.add((const double*)f.val); c.add((const int*)f.col); c.add((const int*)f.perm); c.add(f.part);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  out->n = 1;
+  if (f.split && f.nsplit > 0) { sell_split_fixup_call(f, &out->k[1]); out->n = 2; }
+  return cudaSuccess;
 }
 
 }  // namespace spmv

@@ -231,47 +231,31 @@ bool sell_tma_supported(const Variant& v) {
   if (v.X == 2 ? (v.H < 8 || v.H > 4096 || v.H % 8) : v.H != 0) return false;
   return tma_smem(v) <= 200 * 1024;
 }
-const void* sell_tma_func(const Variant& v, bool perm) {
-  const TmaEntry* e = tma_pick(v);
-  return e ? (const void*)e->k[perm ? 1 : 0] : nullptr;
-}
-
-cudaError_t sell_tma_launch(const Variant& v, int64_t rows, int64_t cols, const SellFormat& f, const ApplyArgs& a,
-                            int sm_count) {
+cudaError_t sell_tma_plan(const Variant& v, int64_t rows, int64_t cols, const SellFormat& f, int sm_count,
+                          LaunchPlan* out) {
   const TmaEntry* e = tma_pick(v);
   if (!e || f.C != v.C) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
-  sell_tma_kernel_t k = e->k[f.perm ? 1 : 0];
-  const size_t smem = tma_smem(v);
-  static thread_local const void* last_attr = nullptr;
-  static thread_local size_t last_smem = 0;
-  if (last_attr != (const void*)k || last_smem != smem) {
-    cudaError_t err = cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    last_attr = (const void*)k;
-    last_smem = smem;
-  }
-  static thread_local int occ = 1;
-  static thread_local const void* occ_k = nullptr;
-  static thread_local size_t occ_smem = 0;
-  if (occ_k != (const void*)k || occ_smem != smem) {
-    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)k, v.block, smem);
-    if (err != cudaSuccess) return err;
-    if (occ < 1) occ = 1;
-    occ_k = (const void*)k;
-    occ_smem = smem;
-  }
+  KernelCall& c = out->k[0];
+  c.fn = (const void*)e->k[f.perm ? 1 : 0];
+  c.block = v.block;
+  c.smem = (unsigned)tma_smem(v);
+  cudaError_t err = allow_smem(c.fn, c.smem);
+  if (err != cudaSuccess) return err;
   // persistent: g (default 1) waves of resident CTAs, never more CTAs than slices
-  int64_t grid = (int64_t)(v.grid > 0 ? v.grid : 1) * sm_count * occ;
-  if (grid > f.nslices) grid = f.nslices;
-  // x window bulk copies need a 16-byte aligned x; otherwise the window is empty (H = -C/2: every gather
+  err = resolve_grid(v.grid > 0 ? v.grid : 1, c.fn, v.block, c.smem, sm_count, f.nslices, &c.grid);
+  if (err != cudaSuccess) return err;
+  c.add(rows); c.add((int64_t)f.nslices); c.add(f.C); c.add((const int64_t*)f.slice_ptr); c.add((const double*)f.val);
+  c.add((const int*)f.col); c.add((const int*)f.perm); c.add(f.part);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  // x window bulk copies need a 16-byte aligned x; otherwise the window is empty (cols = 0: every gather
   // goes through L1) -- same results, the variant just loses its point
-  int H = v.H;
-  int64_t cols_arg = cols;
-  if (v.X == 2 && ((uintptr_t)a.x & 15)) cols_arg = 0;
-  k<<<(unsigned)grid, v.block, smem, a.stream>>>(rows, f.nslices, f.C, f.slice_ptr, f.val, f.col, f.perm, f.part,
-                                                 a.alpha, a.x, a.beta, a.y, cols_arg, H);
-  return cudaGetLastError();
+  if (v.X == 2) c.add_flag(3, cols); else c.add(cols);
+  c.add((int)v.H);
+  out->n = 1;
+  if (f.split && f.nsplit > 0) { sell_split_fixup_call(f, &out->k[1]); out->n = 2; }
+  return cudaSuccess;
 }
 
 }  // namespace spmv

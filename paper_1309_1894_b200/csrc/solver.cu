@@ -267,7 +267,7 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   auto fail = [&](spmv_status_t code) { cleanup(); return code; };
   auto iteration = [&]() -> spmv_status_t {
     ApplyArgs a{1.0, 0.0, p, q, s};
-    spmv_status_t st1 = launch_variant(h, h->sel, a);                       // q = A p
+    spmv_status_t st1 = launch_plan(h->plan, a);                       // q = A p
     if (st1 != SPMV_OK) return st1;
     cg_dot_kernel<<<nb, kCgBlock, 0, s>>>(n, p, q, part_pq, st);
     cg_update_kernel<<<nb, kCgBlock, 0, s>>>(n, nb, part_pq, st, d_x, r, p, q, part_rr);
@@ -297,7 +297,7 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   } else {
   {
     ApplyArgs a{1.0, 0.0, d_x, q, s};
-    spmv_status_t st1 = launch_variant(h, h->sel, a);                       // q = A x0
+    spmv_status_t st1 = launch_plan(h->plan, a);                       // q = A x0
     if (st1 != SPMV_OK) return fail(st1);
   }
   cg_init_kernel<<<nb, kCgBlock, 0, s>>>(n, d_b, q, r, p, part_rr, part_bb);

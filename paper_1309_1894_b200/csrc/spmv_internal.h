@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include <string>
 #include <vector>
@@ -127,48 +128,81 @@ struct DeviceProps {
   char name[64] = {0};
 };
 
+// ---------------------------------------------------------------- launch plans
+// Everything a launch needs, resolved ONCE (spmv_select / spmv_tune / per tuner candidate): kernel, grid,
+// block, dynamic shared memory, and the marshalled argument block.  spmv_apply copies the block, patches
+// alpha / x / beta / y (and the few alignment-dependent arguments) and launches: no map lookups, no
+// occupancy queries, no attribute calls and no locks on the apply path.
+struct KernelCall {
+  const void* fn = nullptr;
+  unsigned grid = 0, block = 0, smem = 0;
+  bool pdl = false;              // programmatic dependent launch (the kernel executes griddepcontrol.wait)
+  int nargs = 0, used = 0;
+  int off[20] = {0};
+  int i_alpha = -1, i_x = -1, i_beta = -1, i_y = -1;
+  // arguments that depend on the vectors' alignment: kind 1: int = (y 16-byte aligned), 2: int = (x 16-byte
+  // aligned), 3: int64 = flag_val if x is 16-byte aligned else 0
+  int flag_idx[2] = {-1, -1}, flag_kind[2] = {0, 0};
+  int64_t flag_val = 0;
+  alignas(16) unsigned char store[1280];
+  template <typename T>
+  int add(const T& v) {
+    used = (int)((used + alignof(T) - 1) / alignof(T) * alignof(T));
+    memcpy(store + used, &v, sizeof(T));
+    off[nargs] = used;
+    used += (int)sizeof(T);
+    return nargs++;
+  }
+  void add_alpha() { i_alpha = add(0.0); }
+  void add_beta() { i_beta = add(0.0); }
+  void add_x() { i_x = add((const double*)nullptr); }
+  void add_y() { i_y = add((double*)nullptr); }
+  void add_flag(int kind, int64_t val = 0) {
+    const int slot = flag_idx[0] < 0 ? 0 : 1;
+    flag_kind[slot] = kind;
+    flag_val = val;
+    flag_idx[slot] = kind == 3 ? add((int64_t)0) : add((int)0);
+  }
+};
+struct LaunchPlan {
+  int n = 0;                     // kernel launches per apply (0: nothing to do)
+  KernelCall k[2];               // [1]: the ordered fix-up of merge-path / row-split SELL
+  bool has_alt = false;          // alt replaces k[0] when x or y is not 16-byte aligned (dia_const pairs)
+  KernelCall alt;
+};
+cudaError_t run_plan(const LaunchPlan& p, const ApplyArgs& a);
+// grid for "g waves of resident blocks" (Variant::grid > 0), capped at the exact cover; sets nothing
+cudaError_t resolve_grid(int g, const void* fn, int block, size_t smem, int sm_count, int64_t exact, unsigned* grid);
+// cudaFuncAttributeMaxDynamicSharedMemorySize (per device and function: set at every plan build)
+cudaError_t allow_smem(const void* fn, size_t smem);
+
 // Per-family entry points (kernels_*.cu).  `supported` checks template-parameter
-// availability only; structural eligibility is decided by the tuner / select.
+// availability only; structural eligibility is decided by the tuner / select.  `plan` fills the
+// launch plan for a built format.
 bool csr_scalar_supported(const Variant&);
-const void* csr_scalar_func(const Variant&);
-cudaError_t csr_scalar_launch(const Variant&, const CsrView&, const ApplyArgs&, int grid_blocks);
-
+cudaError_t csr_scalar_plan(const Variant&, const CsrView&, int sm_count, LaunchPlan*);
 bool csr_vector_supported(const Variant&);
-const void* csr_vector_func(const Variant&);
-cudaError_t csr_vector_launch(const Variant&, const CsrView&, const ApplyArgs&, int grid_blocks);
-
+cudaError_t csr_vector_plan(const Variant&, const CsrView&, int sm_count, LaunchPlan*);
 bool sell_supported(const Variant&);
-const void* sell_func(const Variant&, bool perm);
-cudaError_t sell_launch(const Variant&, int64_t rows, const SellFormat&, const ApplyArgs&, int grid_blocks);
-
+cudaError_t sell_plan(const Variant&, int64_t rows, const SellFormat&, int sm_count, LaunchPlan*);
 bool sell_tma_supported(const Variant&);
-const void* sell_tma_func(const Variant&, bool perm);
-cudaError_t sell_tma_launch(const Variant&, int64_t rows, int64_t cols, const SellFormat&, const ApplyArgs&, int sm_count);
+cudaError_t sell_tma_plan(const Variant&, int64_t rows, int64_t cols, const SellFormat&, int sm_count, LaunchPlan*);
 // adds the segment sums of split rows in a fixed order (after a SELL kernel ran on a split format)
-cudaError_t sell_split_fixup_launch(const SellFormat&, const ApplyArgs&);
-
+void sell_split_fixup_call(const SellFormat&, KernelCall*);
 bool merge_supported(const Variant&);
-const void* merge_func(const Variant&);
-cudaError_t merge_launch(const Variant&, const CsrView&, const MergePlan&, const ApplyArgs&);
-
+cudaError_t merge_plan(const Variant&, const CsrView&, const MergePlan&, LaunchPlan*);
 bool bcsr_supported(const Variant&);
-const void* bcsr_func(const Variant&);
-cudaError_t bcsr_launch(const Variant&, const BcsrFormat&, const ApplyArgs&, int grid_blocks);
-
+cudaError_t bcsr_plan(const Variant&, const BcsrFormat&, int sm_count, LaunchPlan*);
 bool dia_supported(const Variant&);
-const void* dia_func(const Variant&);
-cudaError_t dia_launch(const Variant&, int64_t rows, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+cudaError_t dia_plan(const Variant&, int64_t rows, const DiaFormat&, int sm_count, LaunchPlan*);
 bool dia_const_supported(const Variant&);
-const void* dia_const_func(const Variant&);
-cudaError_t dia_const_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int grid_blocks);
+cudaError_t dia_const_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, LaunchPlan*);
 bool dia_win_supported(const Variant&);
-const void* dia_win_func(const Variant&);
 bool dia_win_fits(const Variant&, const DiaFormat&);
-cudaError_t dia_win_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);
+cudaError_t dia_win_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, int sm_count, LaunchPlan*);
 void dia_compute_windows(DiaFormat& f);
 bool dia_tma_supported(const Variant&);
-const void* dia_tma_func(const Variant&);
-cudaError_t dia_tma_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, const ApplyArgs&, int sm_count);
+cudaError_t dia_tma_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, int sm_count, LaunchPlan*);
 
 // Launch through cudaLaunchKernelExC; pdl = true marks the launch as a programmatic dependent launch
 // (cudaLaunchAttributeProgrammaticStreamSerialization): the kernel may start while the previous kernel of

@@ -168,13 +168,19 @@ struct Tuner {
     return SPMV_OK;
   }
 
-  // one launch from y0, compared with the reference; returns pass/fail and the launch time
-  spmv_status_t verify(const Variant& v, bool* pass, double* err, double* us) {
+  // One launch from y0, compared with the reference; returns pass/fail and a launch time.  The candidate's
+  // very first launch (lazy module load, first-touch of its format) is untimed; the timed one is a second
+  // launch from y0, so the slow-candidate gate sees kernel time, not host latency.
+  spmv_status_t verify(const Variant& v, const LaunchPlan& plan, bool* pass, double* err, double* us) {
+    ApplyArgs a{alpha, beta, x, y, s};
     spmv_status_t st = reset_y();
     if (st != SPMV_OK) return st;
-    ApplyArgs a{alpha, beta, x, y, s};
+    st = launch_plan(plan, a);
+    if (st != SPMV_OK) return st;
+    st = reset_y();
+    if (st != SPMV_OK) return st;
     SPMV_CUDA_TRY(cudaEventRecord(e0, s));
-    st = launch_variant(h, v, a);
+    st = launch_plan(plan, a);
     if (st != SPMV_OK) return st;
     SPMV_CUDA_TRY(cudaEventRecord(e1, s));
     if (fault && *fault && variant_to_string(v).compare(0, strlen(fault), fault) == 0) {
@@ -197,11 +203,11 @@ struct Tuner {
   // median time per apply over `reps` batches (warm: K applies; cold: K x (flush, apply) - K flushes)
   // Successive halving: after the first timed batch a candidate more than 25 % behind
   // the current best keeps that single measurement (*quick = true) and the remaining batches are skipped.
-  spmv_status_t time(const Variant& v, double est_us, double best_us, double* us, bool* quick) {
+  spmv_status_t time(const LaunchPlan& plan, double est_us, double best_us, double* us, bool* quick) {
     *quick = false;
     ApplyArgs a{alpha, beta, x, y, s};
     for (int i = 0; i < warmup; ++i) {
-      spmv_status_t st = launch_variant(h, v, a);
+      spmv_status_t st = launch_plan(plan, a);
       if (st != SPMV_OK) return st;
     }
     std::vector<double> t;
@@ -215,7 +221,7 @@ struct Tuner {
         for (int k = 0; k < K; ++k) {
           if (flush_l2_launch(flushbuf, flush_n, s) != cudaSuccess) return SPMV_ERR_CUDA;
           if (with_apply) {
-            spmv_status_t st = launch_variant(h, v, a);
+            spmv_status_t st = launch_plan(plan, a);
             if (st != SPMV_OK) return st;
           }
         }
@@ -250,7 +256,7 @@ struct Tuner {
       for (int i = 0; i < reps; ++i) {
         SPMV_CUDA_TRY(cudaEventRecord(e0, s));
         for (int k = 0; k < K; ++k) {
-          spmv_status_t st = launch_variant(h, v, a);
+          spmv_status_t st = launch_plan(plan, a);
           if (st != SPMV_OK) return st;
         }
         SPMV_CUDA_TRY(cudaEventRecord(e1, s));
@@ -340,10 +346,8 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
       Variant v;
       std::string why;
       if (variant_from_string(it->second.variant.c_str(), &v) && variant_eligible(h, v, &why) &&
-          ensure_format(h, v, T.s) == SPMV_OK) {
-        h->sel = v;
+          adopt_variant(h, v, T.s) == SPMV_OK) {
         h->tuned = true;
-        release_formats_except(h, v);
         handle_refresh_info(h);
         if (report) {
           strncpy(report->winner, it->second.variant.c_str(), sizeof(report->winner) - 1);
@@ -419,14 +423,17 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     spmv_status_t s1 = ensure_format(h, v, T.s);
     if (s1 == SPMV_ERR_UNSUPPORTED) { ++n_pruned; T.log(d, "pruned_format", 0, 0); return SPMV_OK; }
     if (s1 != SPMV_OK) return s1;
+    LaunchPlan plan;
+    s1 = build_plan(h, v, &plan);
+    if (s1 != SPMV_OK) return s1;
     bool pass = false; double err = 0, vus = 0;
-    s1 = T.verify(v, &pass, &err, &vus);
+    s1 = T.verify(v, plan, &pass, &err, &vus);
     if (s1 != SPMV_OK) return s1;
     if (!pass) { ++n_rej; T.log(d, "rejected", vus, err); return SPMV_OK; }   // can never win
     if (!force_time && vus > 4.0 * best_us + 20.0) { ++n_slow; T.log(d, "pruned_slow", vus, err); return SPMV_OK; }
     double us = 0;
     bool quick = false;
-    s1 = T.time(v, vus, force_time ? 1e300 : best_us, &us, &quick);
+    s1 = T.time(plan, vus, force_time ? 1e300 : best_us, &us, &quick);
     if (s1 != SPMV_OK) return s1;
     ++n_timed;
     T.log(d, quick ? "timed1" : "timed", us, err);
@@ -489,20 +496,17 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
   }
   if (ok.empty()) {
     T.cleanup();
-    release_all_formats(h);
-    h->sel = dflt;
+    adopt_variant(h, dflt, T.s);
     h->tuned = false;
     handle_refresh_info(h);
     if (report) report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     set_last_error("spmv_tune: no candidate matched the reference result");
     return SPMV_ERR_VERIFY_FAILED;
   }
-  const Scored& win = ok[0];
-  st = ensure_format(h, win.v, T.s);
+  const Scored win = ok[0];
+  st = adopt_variant(h, win.v, T.s);
   if (st != SPMV_OK) return fail(st);
-  h->sel = win.v;
   h->tuned = true;
-  release_formats_except(h, win.v);
   T.cleanup();
   handle_refresh_info(h);
   const std::string wd = variant_to_string(win.v);

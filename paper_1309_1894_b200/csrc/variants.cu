@@ -4,7 +4,7 @@
 #include <stdlib.h>
 #include <string.h>
 
-#include <mutex>
+#include <algorithm>
 
 #include "handle.h"
 
@@ -240,6 +240,17 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
 }
 
 void release_formats_except(spmv_handle_s* h, const Variant& keep) {
+  // An apply launched on ANY stream may still be reading a format that is about to be freed (and a
+  // stream-ordered allocator behind the callbacks would recycle the memory at once): wait for the device
+  // before the first free.  Slow path only (select / tune / update_values / destroy).
+  const bool keeps_sell = keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA;
+  const bool keeps_dia = keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST ||
+                         keep.fam == FAM_DIA_WIN || keep.fam == FAM_DIA_CWIN;
+  size_t n_free = (h->has_ell && keep.fam != FAM_ELL) + (h->has_bcsr && keep.fam != FAM_BCSR3);
+  for (const auto& kv : h->sells) n_free += !(keeps_sell && kv.first == sell_key(keep));
+  for (const auto& kv : h->dias) n_free += !(keeps_dia && kv.first == keep.C);
+  for (const auto& kv : h->plans) n_free += !(keep.fam == FAM_MERGE && kv.first == keep.block * keep.I);
+  if (n_free) cudaDeviceSynchronize();
   for (auto it = h->sells.begin(); it != h->sells.end();) {
     if ((keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA) && it->first == sell_key(keep)) { ++it; continue; }
     free_sell(it->second, h->al);
@@ -299,118 +310,122 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
   }
 }
 
-// ------------------------------------------------------------------ launch
-static std::mutex g_attr_mu;
-static std::map<const void*, int> g_carve;                          // current carve-out per kernel
-static std::map<std::pair<const void*, int>, int> g_occ;            // resident blocks per SM
-
-static const void* variant_func(const spmv_handle_s* h, const Variant& v) {
-  switch (v.fam) {
-    case FAM_CSR_SCALAR: return csr_scalar_func(v);
-    case FAM_CSR_VECTOR: return csr_vector_func(v);
-    case FAM_SELL: {
-      auto it = h->sells.find(sell_key(v));
-      return sell_func(v, it != h->sells.end() && it->second.perm != nullptr);
-    }
-    case FAM_ELL: return sell_func(v, false);
-    case FAM_SELL_TMA: {
-      auto it = h->sells.find(sell_key(v));
-      return sell_tma_func(v, it != h->sells.end() && it->second.perm != nullptr);
-    }
-    case FAM_MERGE: return merge_func(v);
-    case FAM_BCSR3: return bcsr_func(v);
-    case FAM_DIA: return dia_func(v);
-    case FAM_DIA_TMA: return dia_tma_func(v);
-    case FAM_DIA_CONST: return dia_const_func(v);
-    case FAM_DIA_WIN:
-    case FAM_DIA_CWIN: return dia_win_func(v);
+// ------------------------------------------------------------------ launch plans
+cudaError_t resolve_grid(int g, const void* fn, int block, size_t smem, int sm_count, int64_t exact, unsigned* grid) {
+  int64_t n = exact;
+  if (g > 0) {
+    int occ = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, block, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    n = std::min<int64_t>(exact, (int64_t)g * sm_count * occ);
   }
-  return nullptr;
+  if (n < 1) n = 1;
+  if (n > 0x7fffffffll) return cudaErrorInvalidConfiguration;
+  *grid = (unsigned)n;
+  return cudaSuccess;
 }
 
-spmv_status_t launch_variant(spmv_handle_s* h, const Variant& v, const ApplyArgs& a) {
-  const void* fn = variant_func(h, v);
-  if (!fn) { set_last_error("variant %s has no kernel", variant_to_string(v).c_str()); return SPMV_ERR_INTERNAL; }
-  int grid_blocks = 0;
-  {
-    std::lock_guard<std::mutex> lk(g_attr_mu);
-    auto ci = g_carve.find(fn);
-    const int cur = ci == g_carve.end() ? -1 : ci->second;
-    if (cur != v.carve) {   // PAPER.md:23 "size of L1 cache" -> shared-memory carve-out hint
-      SPMV_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve));
-      g_carve[fn] = v.carve;
-    }
-    if (v.grid > 0 && v.fam != FAM_MERGE && v.fam != FAM_SELL_TMA && v.fam != FAM_DIA_TMA && v.fam != FAM_DIA_WIN &&
-        v.fam != FAM_DIA_CWIN) {
-      auto key = std::make_pair(fn, v.block);
-      auto oi = g_occ.find(key);
-      int occ = 0;
-      if (oi == g_occ.end()) {
-        SPMV_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, v.block, 0));
-        if (occ < 1) occ = 1;
-        g_occ[key] = occ;
-      } else {
-        occ = oi->second;
-      }
-      grid_blocks = v.grid * h->dev.sm_count * occ;
+cudaError_t allow_smem(const void* fn, size_t smem) {
+  if (smem <= 48 * 1024) return cudaSuccess;
+  return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+static inline cudaError_t run_call(const KernelCall& c, const ApplyArgs& a) {
+  // private copy of the argument block: concurrent applies of one handle never share mutable state
+  alignas(16) unsigned char buf[sizeof(c.store)];
+  memcpy(buf, c.store, (size_t)c.used);
+  if (c.i_alpha >= 0) memcpy(buf + c.off[c.i_alpha], &a.alpha, sizeof(double));
+  if (c.i_beta >= 0) memcpy(buf + c.off[c.i_beta], &a.beta, sizeof(double));
+  if (c.i_x >= 0) memcpy(buf + c.off[c.i_x], &a.x, sizeof(void*));
+  if (c.i_y >= 0) memcpy(buf + c.off[c.i_y], &a.y, sizeof(void*));
+  for (int f = 0; f < 2; ++f) {
+    if (c.flag_idx[f] < 0) continue;
+    if (c.flag_kind[f] == 3) {
+      const int64_t v = ((uintptr_t)a.x & 15) == 0 ? c.flag_val : 0;
+      memcpy(buf + c.off[c.flag_idx[f]], &v, sizeof(v));
+    } else {
+      const int v = (((uintptr_t)(c.flag_kind[f] == 1 ? (const void*)a.y : (const void*)a.x)) & 15) == 0;
+      memcpy(buf + c.off[c.flag_idx[f]], &v, sizeof(v));
     }
   }
-  cudaError_t e = cudaSuccess;
+  void* argp[20];
+  for (int i = 0; i < c.nargs; ++i) argp[i] = buf + c.off[i];
+  return launch_kernel_pdl(c.fn, c.grid, c.block, c.smem, a.stream, argp, c.pdl);
+}
+
+cudaError_t run_plan(const LaunchPlan& p, const ApplyArgs& a) {
+  if (p.n == 0) return cudaSuccess;
+  const bool aligned = p.has_alt ? ((((uintptr_t)a.x | (uintptr_t)a.y) & 15) == 0) : true;
+  cudaError_t e = run_call(aligned ? p.k[0] : p.alt, a);
+  if (e == cudaSuccess && p.n > 1) e = run_call(p.k[1], a);
+  return e;
+}
+
+// Resolves everything a launch of `v` on this handle needs (the format must exist).  The carve-out
+// ("size of L1 cache") is a per-function, per-process attribute: it is (re)set here, at select /
+// tune time, never on the apply path; two handles that select the SAME kernel with DIFFERENT co values share
+// the one set last.
+spmv_status_t build_plan(spmv_handle_s* h, const Variant& v, LaunchPlan* out) {
+  cudaError_t e = cudaErrorInvalidValue;
+  const int sms = h->dev.sm_count;
   switch (v.fam) {
-    case FAM_CSR_SCALAR: e = csr_scalar_launch(v, h->A, a, grid_blocks); break;
-    case FAM_CSR_VECTOR: e = csr_vector_launch(v, h->A, a, grid_blocks); break;
-    case FAM_SELL: {
-      auto it = h->sells.find(sell_key(v));
-      if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
-      e = sell_launch(v, h->A.rows, it->second, a, grid_blocks);
-      if (e == cudaSuccess && it->second.split) e = sell_split_fixup_launch(it->second, a);
-      break;
-    }
+    case FAM_CSR_SCALAR: e = csr_scalar_plan(v, h->A, sms, out); break;
+    case FAM_CSR_VECTOR: e = csr_vector_plan(v, h->A, sms, out); break;
+    case FAM_SELL:
     case FAM_SELL_TMA: {
       auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
-      e = sell_tma_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
-      if (e == cudaSuccess && it->second.split) e = sell_split_fixup_launch(it->second, a);
+      e = v.fam == FAM_SELL ? sell_plan(v, h->A.rows, it->second, sms, out)
+                            : sell_tma_plan(v, h->A.rows, h->A.cols, it->second, sms, out);
       break;
     }
     case FAM_ELL:
       if (!h->has_ell) return SPMV_ERR_INTERNAL;
-      e = sell_launch(v, h->A.rows, h->ell, a, grid_blocks);
+      e = sell_plan(v, h->A.rows, h->ell, sms, out);
       break;
     case FAM_MERGE: {
       auto it = h->plans.find(v.block * v.I);
       if (it == h->plans.end()) return SPMV_ERR_INTERNAL;
-      e = merge_launch(v, h->A, it->second, a);
+      e = merge_plan(v, h->A, it->second, out);
       break;
     }
     case FAM_BCSR3:
       if (!h->has_bcsr) return SPMV_ERR_INTERNAL;
-      e = bcsr_launch(v, h->bcsr, a, grid_blocks);
+      e = bcsr_plan(v, h->bcsr, sms, out);
       break;
+    case FAM_DIA:
+    case FAM_DIA_TMA:
+    case FAM_DIA_CONST:
     case FAM_DIA_WIN:
     case FAM_DIA_CWIN: {
       auto it = h->dias.find(v.C);
       if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
-      e = dia_win_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
-      break;
-    }
-    case FAM_DIA_CONST: {
-      auto it = h->dias.find(v.C);
-      if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
-      e = dia_const_launch(v, h->A.rows, h->A.cols, it->second, a, grid_blocks);
-      break;
-    }
-    case FAM_DIA_TMA:
-    case FAM_DIA: {
-      auto it = h->dias.find(v.C);
-      if (it == h->dias.end()) return SPMV_ERR_INTERNAL;
-      e = v.fam == FAM_DIA ? dia_launch(v, h->A.rows, it->second, a, grid_blocks)
-                           : dia_tma_launch(v, h->A.rows, h->A.cols, it->second, a, h->dev.sm_count);
+      const DiaFormat& f = it->second;
+      e = v.fam == FAM_DIA ? dia_plan(v, h->A.rows, f, sms, out)
+        : v.fam == FAM_DIA_TMA ? dia_tma_plan(v, h->A.rows, h->A.cols, f, sms, out)
+        : v.fam == FAM_DIA_CONST ? dia_const_plan(v, h->A.rows, h->A.cols, f, out)
+                                 : dia_win_plan(v, h->A.rows, h->A.cols, f, sms, out);
       break;
     }
   }
+  if (e == cudaSuccess && out->n > 0) {
+    e = cudaFuncSetAttribute(out->k[0].fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve);
+    if (e == cudaSuccess && out->has_alt)
+      e = cudaFuncSetAttribute(out->alt.fn, cudaFuncAttributePreferredSharedMemoryCarveout, v.carve);
+  }
   if (e != cudaSuccess) {
-    set_last_error("launch of %s failed: %s", variant_to_string(v).c_str(), cudaGetErrorString(e));
+    cudaGetLastError();
+    set_last_error("cannot prepare the launch of %s: %s", variant_to_string(v).c_str(), cudaGetErrorString(e));
+    return SPMV_ERR_CUDA;
+  }
+  return SPMV_OK;
+}
+
+spmv_status_t launch_plan(const LaunchPlan& p, const ApplyArgs& a) {
+  cudaError_t e = run_plan(p, a);
+  if (e != cudaSuccess) {
+    set_last_error("kernel launch failed: %s", cudaGetErrorString(e));
     return SPMV_ERR_CUDA;
   }
   return SPMV_OK;
