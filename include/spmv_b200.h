@@ -37,7 +37,9 @@
  *   families  csr_scalar (thread per row), csr_vector (w lanes per row), sell / sell_tma
  *             (SELL-C-sigma; _tma: matrix stream by cp.async.bulk + mbarrier ring), ell, merge
  *             (merge-path), bcsr3 (3x3 blocks), dia / dia_tma (diagonals, no column indices),
- *             dia_const (constant-coefficient stencil: no matrix values read)
+ *             dia_const (constant-coefficient stencil: no matrix values read), sell16 / sell16_tma (SELL with 16-bit
+ *             delta-encoded column indices per slice: 10 bytes per entry, banded patterns whose slices span
+ *             fewer than 65535 columns)
  *   keys      b threads per block | g grid: 0/absent exact cover, k = k waves of resident blocks |
  *             co shared-memory carve-out percent | u unroll (sell_tma/dia_tma: steps per stage) |
  *             r rows per thread | w lanes per (block) row | x x path: 0 ld.global.nc, 1 ld.global,
@@ -251,7 +253,8 @@ SPMV_API spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap
 SPMV_API spmv_status_t spmv_get_info(spmv_handle_t h, spmv_info_t* out);
 
 /* Inspection (tests): copy an owned array of the selected variant's format to the host.
- * name in {"slice_ptr","sval","scol","perm","brow_ptr","bcol","bval","tile_row"};
+ * name in {"slice_ptr","sval","scol","scol16","sbase","perm","brow_ptr","bcol","bval","tile_row","dia_val",
+ * "dia_mask","dia_mask_small","dia_off","dia_coef"};
  * *bytes receives the array size; copies min(cap, size) bytes when h_buf != NULL. */
 SPMV_API spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_buf,
                                    size_t cap, size_t* bytes, void* stream);

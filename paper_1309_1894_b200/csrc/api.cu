@@ -299,7 +299,7 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
   const void* src = nullptr;
   size_t n = 0;
   const SellFormat* sf = nullptr;
-  if (v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) {
+  if (is_sell_family(v)) {
     auto it = h->sells.find(sell_key(v));
     if (it != h->sells.end()) sf = &it->second;
   } else if (v.fam == FAM_ELL && h->has_ell) {
@@ -308,7 +308,9 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
   if (sf) {
     if (!strcmp(name, "slice_ptr")) { src = sf->slice_ptr; n = sizeof(int64_t) * (sf->nslices + 1); }
     else if (!strcmp(name, "sval")) { src = sf->val; n = sizeof(double) * sf->padded; }
-    else if (!strcmp(name, "scol")) { src = sf->col; n = sizeof(int32_t) * sf->padded; }
+    else if (!strcmp(name, "scol") && sf->col) { src = sf->col; n = sizeof(int32_t) * sf->padded; }
+    else if (!strcmp(name, "scol16") && sf->col16) { src = sf->col16; n = sizeof(uint16_t) * sf->padded; }
+    else if (!strcmp(name, "sbase") && sf->sbase) { src = sf->sbase; n = sizeof(int32_t) * sf->nslices; }
     else if (!strcmp(name, "perm") && sf->perm) { src = sf->perm; n = sizeof(int32_t) * sf->nslices * sf->C; }
   } else if (v.fam == FAM_BCSR3 && h->has_bcsr) {
     if (!strcmp(name, "brow_ptr")) { src = h->bcsr.brow_ptr; n = sizeof(int32_t) * (h->bcsr.brows + 1); }

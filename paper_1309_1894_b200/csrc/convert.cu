@@ -172,7 +172,81 @@ __global__ void split_compose_kernel(int64_t rows_padded, const int* __restrict_
   perm[p] = v >= 0 ? vtarget[v] : -1;
 }
 
+// ---- 16-bit delta-encoded column indices
+// one warp per slice: smallest and largest stored column; bad[0] counts slices spanning >= 65535 columns
+__global__ void sell_span_kernel(int64_t nslices, const int64_t* __restrict__ slice_ptr, const int* __restrict__ scol,
+                                 int* __restrict__ sbase, unsigned* __restrict__ bad) {
+  const int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (s >= nslices) return;
+  int lo = 0x7fffffff, hi = -1;
+  for (int64_t q = slice_ptr[s] + lane; q < slice_ptr[s + 1]; q += 32) {
+    const int c = scol[q];
+    if (c >= 0) { lo = min(lo, c); hi = max(hi, c); }
+  }
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
+    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, d));
+  }
+  if (lane == 0) {
+    sbase[s] = hi < 0 ? 0 : lo;
+    if (hi >= 0 && hi - lo >= 0xFFFF) atomicAdd(bad, 1u);
+  }
+}
+__global__ void sell_narrow_kernel(int64_t nslices, const int64_t* __restrict__ slice_ptr, const int* __restrict__ scol,
+                                   const int* __restrict__ sbase, unsigned short* __restrict__ col16) {
+  const int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (s >= nslices) return;
+  const int base = sbase[s];
+  for (int64_t q = slice_ptr[s] + lane; q < slice_ptr[s + 1]; q += 32) {
+    const int c = scol[q];
+    col16[q] = c < 0 ? (unsigned short)0xFFFFu : (unsigned short)(c - base);
+  }
+}
+
+spmv_status_t sell_narrow_indices(SellFormat& f, Allocator& al, cudaStream_t s) {
+  if (f.col16 || !f.col || f.split) return SPMV_ERR_UNSUPPORTED;
+  int32_t* sbase = (int32_t*)al.alloc(sizeof(int32_t) * (f.nslices + 1), s);      // [nslices] + the bad-slice counter
+  if (!sbase) return SPMV_ERR_ALLOC;
+  unsigned* bad = (unsigned*)(sbase + f.nslices);
+  unsigned h_bad = 1;
+  const unsigned grid = (unsigned)((f.nslices * 32 + 255) / 256);
+  cudaError_t e = cudaMemsetAsync(bad, 0, sizeof(unsigned), s);
+  if (e == cudaSuccess) {
+    sell_span_kernel<<<grid, 256, 0, s>>>(f.nslices, f.slice_ptr, f.col, sbase, bad);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h_bad, bad, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess || h_bad) {
+    al.free(sbase, sizeof(int32_t) * (f.nslices + 1));
+    if (e != cudaSuccess) { set_last_error("sell_narrow_indices: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+    set_last_error("sell16: %u slices span 65535 columns or more", h_bad);
+    return SPMV_ERR_UNSUPPORTED;
+  }
+  uint16_t* c16 = (uint16_t*)al.alloc(sizeof(uint16_t) * f.padded, s);
+  if (!c16) { al.free(sbase, sizeof(int32_t) * (f.nslices + 1)); return SPMV_ERR_ALLOC; }
+  sell_narrow_kernel<<<grid, 256, 0, s>>>(f.nslices, f.slice_ptr, f.col, sbase, c16);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) {
+    al.free(sbase, sizeof(int32_t) * (f.nslices + 1));
+    al.free(c16, sizeof(uint16_t) * f.padded);
+    set_last_error("sell_narrow_indices: %s", cudaGetErrorString(e));
+    return SPMV_ERR_CUDA;
+  }
+  al.free(f.col, sizeof(int32_t) * f.padded);
+  f.col = nullptr;
+  f.col16 = c16;
+  f.sbase = sbase;
+  return SPMV_OK;
+}
+
 void free_sell(SellFormat& f, Allocator& al) {
+  if (f.col16) al.free(f.col16, sizeof(uint16_t) * f.padded);
+  if (f.sbase) al.free(f.sbase, sizeof(int32_t) * (f.nslices + 1));
   if (f.slice_ptr) al.free(f.slice_ptr, sizeof(int64_t) * (f.nslices + 1));
   if (f.val) al.free(f.val, sizeof(double) * f.padded);
   if (f.col) al.free(f.col, sizeof(int32_t) * f.padded);

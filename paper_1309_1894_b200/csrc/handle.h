@@ -19,7 +19,7 @@ struct spmv_handle_s {
   bool tuned = false;
 
   // owned formats, built on demand
-  std::map<std::tuple<int, int, int>, spmv::SellFormat> sells;   // key (C, sigma, split)
+  std::map<std::tuple<int, int, int, int>, spmv::SellFormat> sells;   // key (C, sigma, split, 16-bit indices)
   spmv::SellFormat ell;
   bool has_ell = false;
   spmv::BcsrFormat bcsr;
@@ -35,7 +35,9 @@ struct spmv_handle_s {
 
 namespace spmv {
 
-inline std::tuple<int, int, int> sell_key(const Variant& v) { return std::make_tuple(v.C, v.S, v.L); }
+inline bool is_sell16(const Variant& v) { return v.fam == FAM_SELL16 || v.fam == FAM_SELL16_TMA; }
+inline bool is_sell_family(const Variant& v) { return v.fam == FAM_SELL || v.fam == FAM_SELL_TMA || is_sell16(v); }
+inline std::tuple<int, int, int, int> sell_key(const Variant& v) { return std::make_tuple(v.C, v.S, v.L, is_sell16(v) ? 1 : 0); }
 
 constexpr uint64_t kHandleMagic = 0x53504D5642323030ull;   // "SPMVB200"
 constexpr const char* kVersion = "0.1.0";

@@ -7,48 +7,89 @@
 // R=4: 2 x double2 + int4), fully coalesced across the warp, with no width padding.
 // Padding entries have col = -1 and are skipped, never multiplied (reading A7), so a
 // NaN/Inf in x cannot leak into a row that CSR would leave clean.
+//
+// 16-bit form (sell16, SURVEY sec. 8(f) rank 1 "16-bit delta-encoded column indices inside SELL slices"):
+// the column of an entry is sbase[slice] + a 16-bit delta (0xFFFF = padding), 10 bytes per stored entry
+// instead of 12, for banded matrices that DIA refuses (more than 32 diagonals, fill below one half).
 #include "device_utils.cuh"
 #include "spmv_internal.h"
 
 namespace spmv {
 
+__device__ __forceinline__ unsigned short ld_stream_u16(const unsigned short* p) {
+  unsigned short v;
+  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ unsigned ld_stream_u32(const void* p) {     // 4-byte aligned
+  unsigned v;
+  asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint2 ld_stream_u32x2(const void* p) {      // 8-byte aligned
+  uint2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ int col_of_delta(unsigned d, int base) { return d == 0xFFFFu ? -1 : base + (int)d; }
+
 template <int R>
 struct VecLoad;
 template <>
 struct VecLoad<1> {
-  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, int, double* v, int* c) {
     v[0] = ld_stream(pv);
     c[0] = ld_stream(pc);
+  }
+  static __device__ __forceinline__ void load(const double* pv, const unsigned short* pc, int base, double* v, int* c) {
+    v[0] = ld_stream(pv);
+    c[0] = col_of_delta(ld_stream_u16(pc), base);
   }
 };
 template <>
 struct VecLoad<2> {
-  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, int, double* v, int* c) {
     double2 a = ld_stream2(pv);
     int2 b = ld_stream2(pc);
     v[0] = a.x; v[1] = a.y; c[0] = b.x; c[1] = b.y;
   }
+  static __device__ __forceinline__ void load(const double* pv, const unsigned short* pc, int base, double* v, int* c) {
+    double2 a = ld_stream2(pv);
+    const unsigned b = ld_stream_u32(pc);
+    v[0] = a.x; v[1] = a.y;
+    c[0] = col_of_delta(b & 0xFFFFu, base); c[1] = col_of_delta(b >> 16, base);
+  }
 };
 template <>
 struct VecLoad<4> {
-  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, int, double* v, int* c) {
     double2 a0 = ld_stream2(pv);
     double2 a1 = ld_stream2(pv + 2);
     int4 b = ld_stream4(pc);
     v[0] = a0.x; v[1] = a0.y; v[2] = a1.x; v[3] = a1.y;
     c[0] = b.x; c[1] = b.y; c[2] = b.z; c[3] = b.w;
   }
+  static __device__ __forceinline__ void load(const double* pv, const unsigned short* pc, int base, double* v, int* c) {
+    double2 a0 = ld_stream2(pv);
+    double2 a1 = ld_stream2(pv + 2);
+    const uint2 b = ld_stream_u32x2(pc);
+    v[0] = a0.x; v[1] = a0.y; v[2] = a1.x; v[3] = a1.y;
+    c[0] = col_of_delta(b.x & 0xFFFFu, base); c[1] = col_of_delta(b.x >> 16, base);
+    c[2] = col_of_delta(b.y & 0xFFFFu, base); c[3] = col_of_delta(b.y >> 16, base);
+  }
 };
 
 // heavier instantiations trade occupancy for registers (loads in flight per thread)
 constexpr int sell_max_block(int R, int U) { return R * U >= 16 ? 256 : 512; }
 
-template <int R, int U, int PERM, int X>
+// IT = int: 32-bit column indices; IT = unsigned short: 16-bit deltas against sbase[slice]
+template <int R, int U, int PERM, int X, typename IT>
 __global__ void __launch_bounds__(sell_max_block(R, U))
 sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
             const int64_t* __restrict__ slice_ptr, const double* __restrict__ sval,
-            const int* __restrict__ scol, const int* __restrict__ perm, double* __restrict__ part, double alpha,
-            const double* __restrict__ x, double beta, double* __restrict__ y) {
+            const IT* __restrict__ scol, const int* __restrict__ sbase, const int* __restrict__ perm,
+            double* __restrict__ part, double alpha, const double* __restrict__ x, double beta,
+            double* __restrict__ y) {
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows_padded; g += G) {
     const int64_t r0 = g * R;
@@ -56,8 +97,9 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
     const int off = (int)(r0 - s * C);
     const int64_t base = __ldg(slice_ptr + s);
     const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
+    const int cbase = sizeof(IT) == 2 ? __ldg(sbase + s) : 0;
     const double* pv = sval + base + off;
-    const int* pc = scol + base + off;
+    const IT* pc = scol + base + off;
     double acc[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0;
@@ -84,7 +126,7 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
         // steps past the slice width re-read the last valid step (in bounds, L2-resident) and
         // are masked afterwards: unconditional loads let the compiler batch all U of them
         const int jj = min(j + u, w - 1);
-        VecLoad<R>::load(pv + (int64_t)jj * C, pc + (int64_t)jj * C, v[u], c[u]);
+        VecLoad<R>::load(pv + (int64_t)jj * C, pc + (int64_t)jj * C, cbase, v[u], c[u]);
       }
 #pragma unroll
       for (int u = 0; u < U; ++u)
@@ -137,26 +179,27 @@ void sell_split_fixup_call(const SellFormat& f, KernelCall* c) {
   c->add_alpha(); c->add_beta(); c->add_y();
 }
 
-typedef void (*sell_kernel_t)(int64_t, int64_t, int, int, const int64_t*, const double*, const int*,
-                              const int*, double*, double, const double*, double, double*);
-
-template <int PERM, int X>
-static sell_kernel_t pick_ru(int R, int U) {
-#define P(r, u) if (R == r && U == u) return sell_kernel<r, u, PERM, X>;
+template <int PERM, int X, typename IT>
+static const void* pick_ru(int R, int U) {
+#define P(r, u) if (R == r && U == u) return (const void*)sell_kernel<r, u, PERM, X, IT>;
   P(1, 1) P(1, 2) P(1, 4) P(1, 8) P(2, 1) P(2, 2) P(2, 4) P(2, 8) P(4, 1) P(4, 2) P(4, 4) P(4, 8)
 #undef P
   return nullptr;
 }
-static sell_kernel_t pick(const Variant& v, bool perm) {
-  if (v.X == 0) return perm ? pick_ru<1, 0>(v.R, v.U) : pick_ru<0, 0>(v.R, v.U);
-  if (v.X == 1) return perm ? pick_ru<1, 1>(v.R, v.U) : pick_ru<0, 1>(v.R, v.U);
+template <typename IT>
+static const void* pick_it(const Variant& v, bool perm) {
+  if (v.X == 0) return perm ? pick_ru<1, 0, IT>(v.R, v.U) : pick_ru<0, 0, IT>(v.R, v.U);
+  if (v.X == 1) return perm ? pick_ru<1, 1, IT>(v.R, v.U) : pick_ru<0, 1, IT>(v.R, v.U);
   return nullptr;
+}
+static const void* pick(const Variant& v, bool perm) {
+  return v.fam == FAM_SELL16 ? pick_it<unsigned short>(v, perm) : pick_it<int>(v, perm);
 }
 
 bool sell_supported(const Variant& v) {
   if (pick(v, false) == nullptr) return false;
   if (v.block < 32 || v.block > sell_max_block(v.R, v.U) || v.block % 32) return false;
-  if (v.fam == FAM_SELL) {
+  if (v.fam == FAM_SELL || v.fam == FAM_SELL16) {
     if (v.C < 128 || v.C > 4096 || (v.C & (v.C - 1))) return false;   // power of two, multiple of 32*Rmax
     if (v.S < 1) return false;
     if (v.S > 1 && (v.S % v.C != 0 || v.S > 8192 || (v.S & (v.S - 1)))) return false;
@@ -165,12 +208,12 @@ bool sell_supported(const Variant& v) {
 }
 cudaError_t sell_plan(const Variant& v, int64_t rows, const SellFormat& f, int sm_count, LaunchPlan* out) {
   const bool perm = f.perm != nullptr;
-  sell_kernel_t k = pick(v, perm);
-  if (!k) return cudaErrorInvalidValue;
+  const void* k = pick(v, perm);
+  if (!k || (v.fam == FAM_SELL16) != (f.col16 != nullptr)) return cudaErrorInvalidValue;
   *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
   KernelCall& c = out->k[0];
-  c.fn = (const void*)k;
+  c.fn = k;
   c.block = v.block;
   const int64_t rows_padded = f.nslices * (int64_t)f.C;
   const int64_t threads = (rows_padded + v.R - 1) / v.R;
@@ -178,7 +221,8 @@ cudaError_t sell_plan(const Variant& v, int64_t rows, const SellFormat& f, int s
   cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
   if (e != cudaSuccess) return e;
   c.add(rows); c.add(rows_padded); c.add(f.C); c.add(f.logC); c.add((const int64_t*)f.slice_ptr);
-  c.add((const double*)f.val); c.add((const int*)f.col); c.add((const int*)f.perm); c.add(f.part);
+  c.add((const double*)f.val); c.add(f.col16 ? (const void*)f.col16 : (const void*)f.col); c.add((const int*)f.sbase);
+  c.add((const int*)f.perm); c.add(f.part);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
   out->n = 1;
   if (f.split && f.nsplit > 0) { sell_split_fixup_call(f, &out->k[1]); out->n = 2; }

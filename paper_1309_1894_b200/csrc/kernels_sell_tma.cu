@@ -20,75 +20,66 @@
 // as ceil(w/J) stages.  Deterministic: each row is summed by one thread in stored order.
 #include "device_utils.cuh"
 #include "spmv_internal.h"
+#include "tma_utils.cuh"
 
 namespace spmv {
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra WAIT_DONE;\n"
-      "bra WAIT_LOOP;\n"
-      "WAIT_DONE:\n"
-      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
+using tma::bar_arrive;
+using tma::bar_expect_tx;
+using tma::bar_init;
+using tma::bar_wait;
+using tma::bulk_g2s;
+
+__device__ __forceinline__ int tma_col_of_delta(unsigned d, int base) { return d == 0xFFFFu ? -1 : base + (int)d; }
 
 template <int R>
 struct SmemVec;
 template <>
 struct SmemVec<1> {
-  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) { v[0] = *pv; c[0] = *pc; }
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, int, double* v, int* c) { v[0] = *pv; c[0] = *pc; }
+  static __device__ __forceinline__ void load(const double* pv, const unsigned short* pc, int base, double* v, int* c) {
+    v[0] = *pv; c[0] = tma_col_of_delta(*pc, base);
+  }
 };
 template <>
 struct SmemVec<2> {
-  static __device__ __forceinline__ void load(const double* pv, const int* pc, double* v, int* c) {
+  static __device__ __forceinline__ void load(const double* pv, const int* pc, int, double* v, int* c) {
     double2 a = *reinterpret_cast<const double2*>(pv);
     int2 b = *reinterpret_cast<const int2*>(pc);
     v[0] = a.x; v[1] = a.y; c[0] = b.x; c[1] = b.y;
   }
+  static __device__ __forceinline__ void load(const double* pv, const unsigned short* pc, int base, double* v, int* c) {
+    double2 a = *reinterpret_cast<const double2*>(pv);
+    const unsigned b = *reinterpret_cast<const unsigned*>(pc);
+    v[0] = a.x; v[1] = a.y;
+    c[0] = tma_col_of_delta(b & 0xFFFFu, base); c[1] = tma_col_of_delta(b >> 16, base);
+  }
 };
 
 // blockDim.x = C/R consumer threads + 32 (warp C/R/32 is the producer warp)
-template <int R, int STAGES, int J, int PERM, int X>
+// IT = int: 32-bit column indices; IT = unsigned short: 16-bit deltas against sbase[slice] (sell16_tma)
+template <int R, int STAGES, int J, int PERM, int X, typename IT>
 __global__ void __launch_bounds__(512 + 32)
 sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict__ slice_ptr,
-                const double* __restrict__ sval, const int* __restrict__ scol, const int* __restrict__ perm,
-                double* __restrict__ part, double alpha, const double* __restrict__ x, double beta,
-                double* __restrict__ y, int64_t cols, int H) {
+                const double* __restrict__ sval, const IT* __restrict__ scol, const int* __restrict__ sbase,
+                const int* __restrict__ perm, double* __restrict__ part, double alpha,
+                const double* __restrict__ x, double beta, double* __restrict__ y, int64_t cols, int H) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nconsumers = C / R;
   const int WIN = X == 2 ? C + 2 * H : 0;                                    // x window entries per stage
   double* s_val = reinterpret_cast<double*>(smem_raw);                       // [STAGES][J*C]
   double* s_x = s_val + (size_t)STAGES * J * C;                              // [STAGES][WIN]
-  int* s_col = reinterpret_cast<int*>(s_x + (size_t)STAGES * WIN);           // [STAGES][J*C]
-  uint64_t* full = reinterpret_cast<uint64_t*>(s_col + (size_t)STAGES * J * C);
+  IT* s_col = reinterpret_cast<IT*>(s_x + (size_t)STAGES * WIN);             // [STAGES][J*C]
+  uint64_t* full = reinterpret_cast<uint64_t*>(s_col + (size_t)STAGES * J * C);   // J*C*sizeof(IT) is a multiple of 256
   uint64_t* empty = full + STAGES;
   const int tid = threadIdx.x;
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], nconsumers / 32);
+      bar_init(&full[s], 1);
+      bar_init(&empty[s], nconsumers / 32);
     }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    tma::bar_init_fence();
   }
   __syncthreads();
 
@@ -101,12 +92,12 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
         const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
         for (int j0 = 0; j0 < w; j0 += J) {
           const int nj = min(J, w - j0);
-          mbar_wait(&empty[stage], phase ^ 1);
+          bar_wait(&empty[stage], phase ^ 1);
           // The consumers read this stage through the generic proxy; the refill is an async-proxy
           // write.  Without this cross-proxy fence the refill was observed (B200, full-size
           // cfg5, sorted slices) to land under reads that had been ordered before the arrive.
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          const uint32_t vb = (uint32_t)nj * C * sizeof(double), cb = (uint32_t)nj * C * sizeof(int);
+          tma::fence_proxy_async();
+          const uint32_t vb = (uint32_t)nj * C * sizeof(double), cb = (uint32_t)nj * C * sizeof(IT);
           uint32_t xb = 0;
           int64_t lo = 0;
           if (X == 2) {            // window [lo, lo + n) of x, lo even (16-byte aligned source), n even
@@ -114,7 +105,7 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
             const int64_t n = min((int64_t)WIN, cols - lo) & ~(int64_t)1;
             xb = n > 0 ? (uint32_t)n * sizeof(double) : 0u;
           }
-          mbar_expect_tx(&full[stage], vb + cb + xb);
+          bar_expect_tx(&full[stage], vb + cb + xb);
           bulk_g2s(s_val + (size_t)stage * J * C, sval + base + (int64_t)j0 * C, vb, &full[stage]);
           bulk_g2s(s_col + (size_t)stage * J * C, scol + base + (int64_t)j0 * C, cb, &full[stage]);
           if (xb) bulk_g2s(s_x + (size_t)stage * WIN, x + lo, xb, &full[stage]);
@@ -132,6 +123,7 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
     const int64_t base = __ldg(slice_ptr + s);
     const int w = (int)((__ldg(slice_ptr + s + 1) - base) / C);
     const int64_t r0 = s * C + (int64_t)tid * R;
+    const int cbase = sizeof(IT) == 2 ? __ldg(sbase + s) : 0;
     int64_t orow[R];
     double yold[R], acc[R];
 #pragma unroll
@@ -145,14 +137,14 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
     for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && orow[r] >= 0) ? y[orow[r]] : 0.0;
     for (int j0 = 0; j0 < w; j0 += J) {
       const int nj = min(J, w - j0);
-      mbar_wait(&full[stage], phase);
+      bar_wait(&full[stage], phase);
       const double* pv = s_val + (size_t)stage * J * C + tid * R;
-      const int* pc = s_col + (size_t)stage * J * C + tid * R;
+      const IT* pc = s_col + (size_t)stage * J * C + tid * R;
       double v[J][R];
       int c[J][R];
 #pragma unroll
       for (int j = 0; j < J; ++j) {
-        SmemVec<R>::load(pv + j * C, pc + j * C, v[j], c[j]);
+        SmemVec<R>::load(pv + j * C, pc + j * C, cbase, v[j], c[j]);
         if (j >= nj) {          // beyond this stage's steps: stale shared memory, masked off
 #pragma unroll
           for (int r = 0; r < R; ++r) c[j][r] = -1;
@@ -177,7 +169,7 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
       // The fence orders every lane's shared-memory reads before the arrive.
       asm volatile("fence.acq_rel.cta;" ::: "memory");
       __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[stage]);
+      if (lane == 0) bar_arrive(&empty[stage]);
       if (X != 2) {
 #pragma unroll
         for (int j = 0; j < J; ++j)
@@ -198,28 +190,31 @@ sell_tma_kernel(int64_t rows, int64_t nslices, int C, const int64_t* __restrict_
   }
 }
 
-typedef void (*sell_tma_kernel_t)(int64_t, int64_t, int, const int64_t*, const double*, const int*, const int*,
-                                  double*, double, const double*, double, double*, int64_t, int);
-
-struct TmaEntry { int R, STAGES, J, X; sell_tma_kernel_t k[2]; };
-#define TE(r, st, j) {r, st, j, 0, {sell_tma_kernel<r, st, j, 0, 0>, sell_tma_kernel<r, st, j, 1, 0>}}
+struct TmaEntry { int R, STAGES, J, X, I16; const void* k[2]; };
+#define TE(r, st, j) {r, st, j, 0, 0, {(const void*)sell_tma_kernel<r, st, j, 0, 0, int>, (const void*)sell_tma_kernel<r, st, j, 1, 0, int>}}
+#define TX(r, st, j) {r, st, j, 2, 0, {(const void*)sell_tma_kernel<r, st, j, 0, 2, int>, (const void*)sell_tma_kernel<r, st, j, 1, 2, int>}}
+#define TS(r, st, j) {r, st, j, 0, 1, {(const void*)sell_tma_kernel<r, st, j, 0, 0, unsigned short>, (const void*)sell_tma_kernel<r, st, j, 1, 0, unsigned short>}}
 static const TmaEntry g_tma[] = {TE(1, 2, 8), TE(1, 3, 8), TE(1, 4, 8), TE(1, 3, 4), TE(1, 4, 4), TE(1, 6, 4),
                                  TE(2, 2, 8), TE(2, 3, 8), TE(2, 4, 8), TE(2, 3, 4), TE(2, 4, 4), TE(2, 6, 4),
                                  TE(1, 3, 16), TE(2, 3, 16), TE(1, 2, 16), TE(2, 2, 16),
-#define TX(r, st, j) {r, st, j, 2, {sell_tma_kernel<r, st, j, 0, 2>, sell_tma_kernel<r, st, j, 1, 2>}}
                                  TX(1, 2, 8), TX(1, 3, 8), TX(1, 4, 8), TX(1, 3, 4), TX(1, 4, 4), TX(2, 2, 8), TX(2, 3, 8),
-                                 TX(2, 3, 4), TX(2, 4, 4), TX(1, 2, 16), TX(1, 3, 16), TX(2, 2, 16)};
+                                 TX(2, 3, 4), TX(2, 4, 4), TX(1, 2, 16), TX(1, 3, 16), TX(2, 2, 16),
+                                 TS(1, 3, 8), TS(1, 4, 8), TS(1, 4, 4), TS(1, 6, 4), TS(1, 2, 16), TS(1, 3, 16),
+                                 TS(2, 3, 8), TS(2, 4, 8), TS(2, 4, 4), TS(2, 6, 4), TS(2, 2, 16), TS(2, 3, 16)};
+#undef TS
 #undef TX
 #undef TE
 
 static const TmaEntry* tma_pick(const Variant& v) {
+  const int i16 = v.fam == FAM_SELL16_TMA ? 1 : 0;
   for (const auto& e : g_tma)
-    if (e.R == v.R && e.STAGES == v.I && e.J == v.U && e.X == v.X) return &e;
+    if (e.R == v.R && e.STAGES == v.I && e.J == v.U && e.X == v.X && e.I16 == i16) return &e;
   return nullptr;
 }
 static int tma_win(const Variant& v) { return v.X == 2 ? v.C + 2 * v.H : 0; }
 static size_t tma_smem(const Variant& v) {
-  return (size_t)v.I * v.U * v.C * 12 + (size_t)v.I * tma_win(v) * 8 + 2 * v.I * 8 + 128;
+  const size_t entry = v.fam == FAM_SELL16_TMA ? 10 : 12;
+  return (size_t)v.I * v.U * v.C * entry + (size_t)v.I * tma_win(v) * 8 + 2 * v.I * 8 + 128;
 }
 
 bool sell_tma_supported(const Variant& v) {
@@ -234,11 +229,11 @@ bool sell_tma_supported(const Variant& v) {
 cudaError_t sell_tma_plan(const Variant& v, int64_t rows, int64_t cols, const SellFormat& f, int sm_count,
                           LaunchPlan* out) {
   const TmaEntry* e = tma_pick(v);
-  if (!e || f.C != v.C) return cudaErrorInvalidValue;
+  if (!e || f.C != v.C || (v.fam == FAM_SELL16_TMA) != (f.col16 != nullptr)) return cudaErrorInvalidValue;
   *out = LaunchPlan();
   if (rows == 0) return cudaSuccess;
   KernelCall& c = out->k[0];
-  c.fn = (const void*)e->k[f.perm ? 1 : 0];
+  c.fn = e->k[f.perm ? 1 : 0];
   c.block = v.block;
   c.smem = (unsigned)tma_smem(v);
   cudaError_t err = allow_smem(c.fn, c.smem);
@@ -247,7 +242,8 @@ cudaError_t sell_tma_plan(const Variant& v, int64_t rows, int64_t cols, const Se
   err = resolve_grid(v.grid > 0 ? v.grid : 1, c.fn, v.block, c.smem, sm_count, f.nslices, &c.grid);
   if (err != cudaSuccess) return err;
   c.add(rows); c.add((int64_t)f.nslices); c.add(f.C); c.add((const int64_t*)f.slice_ptr); c.add((const double*)f.val);
-  c.add((const int*)f.col); c.add((const int*)f.perm); c.add(f.part);
+  c.add(f.col16 ? (const void*)f.col16 : (const void*)f.col); c.add((const int*)f.sbase); c.add((const int*)f.perm);
+  c.add(f.part);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
   // x window bulk copies need a 16-byte aligned x; otherwise the window is empty (cols = 0: every gather
   // goes through L1) -- same results, the variant just loses its point

@@ -31,7 +31,11 @@ struct SellFormat {
   int64_t padded = 0;        // stored entries including padding
   int64_t* slice_ptr = nullptr;   // [nslices+1]
   double* val = nullptr;          // [padded]
-  int32_t* col = nullptr;         // [padded]
+  int32_t* col = nullptr;         // [padded]  (null in the 16-bit form)
+  // 16-bit delta-encoded column indices: col = sbase[slice] + col16, col16 == 0xFFFF
+  // marks padding; built only when every slice spans fewer than 65535 columns.  10 bytes per entry.
+  uint16_t* col16 = nullptr;      // [padded]
+  int32_t* sbase = nullptr;       // [nslices] smallest column of the slice
   int32_t* perm = nullptr;        // [nslices*C] sell row -> original row (or -1); null if sigma==1
   bool is_ell = false;
   // Row splitting (split = L > 0): a row longer than L is cut into ceil(len/L) segments of at most L
@@ -93,7 +97,7 @@ struct MergePlan {
 };
 
 // ---------------------------------------------------------------- variants
-enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_DIA_CONST, FAM_DIA_WIN, FAM_DIA_CWIN, FAM_COUNT };
+enum Family { FAM_CSR_SCALAR = 0, FAM_CSR_VECTOR, FAM_SELL, FAM_ELL, FAM_MERGE, FAM_BCSR3, FAM_SELL_TMA, FAM_DIA, FAM_DIA_TMA, FAM_DIA_CONST, FAM_DIA_WIN, FAM_DIA_CWIN, FAM_SELL16, FAM_SELL16_TMA, FAM_COUNT };
 
 struct Variant {
   int fam = FAM_CSR_SCALAR;
@@ -251,6 +255,8 @@ cudaError_t compute_stats(const CsrView& A, RawStats* h_out, cudaStream_t s);
 
 spmv_status_t build_sell(const CsrView& A, int C, int sigma, bool ell, int split, Allocator& al,
                          cudaStream_t s, SellFormat* out);
+// replaces f.col by (sbase, col16); UNSUPPORTED (f left as it was) when a slice spans 65535 columns or more
+spmv_status_t sell_narrow_indices(SellFormat& f, Allocator& al, cudaStream_t s);
 void free_sell(SellFormat& f, Allocator& al);
 spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out);
 void free_bcsr3(BcsrFormat& f, Allocator& al);

@@ -75,6 +75,13 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
       }
       all.push_back(v);
     }
+    // 16-bit delta indices (8(f) rank 1): banded patterns only (eligibility: 2*bandwidth + max(C, S) < 65535)
+    for (int C : {128, 512}) for (int S : {1, 8192}) for (int R : {1, 2, 4}) for (int U : {2, 4, 8}) {
+      Variant v; v.fam = FAM_SELL16; v.block = b; v.C = C; v.S = S; v.R = R; v.U = U;
+      if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
+      if (S == 1 && skewed) { ++*n_pruned; continue; }
+      all.push_back(v);
+    }
     for (int R : {1, 2, 4}) for (int U : {1, 2, 4, 8}) {
       Variant v; v.fam = FAM_ELL; v.block = b; v.R = R; v.U = U; all.push_back(v);
     }
@@ -106,6 +113,12 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     if (S == 1 && (J == 4 || J == 8) && ST <= 3)
       for (int H : {72, 136}) { Variant w = v; w.X = 2; w.H = H; all.push_back(w); }
   }
+  for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
+    Variant v; v.fam = FAM_SELL16_TMA; v.C = C; v.S = S; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;
+    if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
+    if (S == 1 && skewed) { ++*n_pruned; continue; }
+    all.push_back(v);
+  }
   for (int C : {128, 256, 512}) for (int R : {1, 2}) for (int J : {4, 7, 8, 9, 14}) for (int ST : {2, 3, 4}) {
     Variant v; v.fam = FAM_DIA_TMA; v.C = C; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;
     if (in.max_row_len > 0 && J > in.max_row_len + 1 && J != 4) { ++*n_pruned; continue; }   // stage deeper than the row
@@ -117,7 +130,7 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
   }
   // family, then format key, outermost: formats are then built once per key
   std::stable_sort(all.begin(), all.end(), [](const Variant& a, const Variant& b) {
-    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : (v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : v.fam; };
+    auto grp = [](const Variant& v) { return v.fam == FAM_SELL_TMA ? (int)FAM_SELL : v.fam == FAM_SELL16_TMA ? (int)FAM_SELL16 : (v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : v.fam; };
     if (grp(a) != grp(b)) return grp(a) < grp(b);
     if (a.C != b.C) return a.C < b.C;
     if (a.S != b.S) return a.S < b.S;
@@ -403,6 +416,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
       if (maybe_dia) return v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_CWIN;
       if (in.block3_full) return v.fam == FAM_BCSR3;
       if (skew) return v.fam == FAM_MERGE || ((v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) && v.L > 0);
+      if (is_sell16(v)) return true;                                                       // banded, not diagonal: 10 B per entry
       return v.fam == FAM_SELL && v.S == 1;
     };
     std::vector<Variant> cut;
@@ -453,7 +467,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     if (!budget_left()) break;
     if (variant_to_string(v) == variant_to_string(dflt)) continue;
     // keep device memory bounded: drop formats when the family / format key changes
-    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : (q.fam == FAM_DIA_TMA || q.fam == FAM_DIA_CONST || q.fam == FAM_DIA_WIN || q.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : q.fam; };
+    auto grp = [](const Variant& q) { return q.fam == FAM_SELL_TMA ? (int)FAM_SELL : q.fam == FAM_SELL16_TMA ? (int)FAM_SELL16 : (q.fam == FAM_DIA_TMA || q.fam == FAM_DIA_CONST || q.fam == FAM_DIA_WIN || q.fam == FAM_DIA_CWIN) ? (int)FAM_DIA : q.fam; };
     if (grp(v) != grp(last_fmt) || v.C != last_fmt.C || v.S != last_fmt.S || v.L != last_fmt.L) {
       Variant keep = ok.empty() ? dflt : std::min_element(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; })->v;
       release_formats_except(h, keep);
@@ -473,7 +487,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     for (int g : {0, 1, 2, 4, 8}) for (int co : carves) {
       if (g == 0 && co == -1) continue;
       if (L.fam == FAM_MERGE && g != 0) continue;
-      if ((L.fam == FAM_SELL_TMA || L.fam == FAM_DIA_TMA || L.fam == FAM_DIA_WIN || L.fam == FAM_DIA_CWIN) && (g == 0 || g == 8)) continue;   // persistent: g = waves of resident CTAs
+      if ((L.fam == FAM_SELL_TMA || L.fam == FAM_SELL16_TMA || L.fam == FAM_DIA_TMA || L.fam == FAM_DIA_WIN || L.fam == FAM_DIA_CWIN) && (g == 0 || g == 8)) continue;   // persistent: g = waves of resident CTAs
       if (!budget_left()) break;
       Variant v = L; v.grid = g; v.carve = co;
       if (!filter_match(o.variant_filter, variant_to_string(v))) continue;

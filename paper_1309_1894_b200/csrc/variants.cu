@@ -43,7 +43,7 @@ void Allocator::free(void* p, size_t bytes) {
 }
 
 // ------------------------------------------------------------------ descriptors
-static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma", "dia_const", "dia_win", "dia_cwin"};
+static const char* kFamName[FAM_COUNT] = {"csr_scalar", "csr_vector", "sell", "ell", "merge", "bcsr3", "sell_tma", "dia", "dia_tma", "dia_const", "dia_win", "dia_cwin", "sell16", "sell16_tma"};
 
 Variant default_variant() { return Variant(); }   // csr_scalar:b256:r1:u1:x0 (reading A17)
 
@@ -54,6 +54,7 @@ std::string variant_to_string(const Variant& v) {
   switch (v.fam) {
     case FAM_CSR_SCALAR: add("r", v.R); add("u", v.U); break;
     case FAM_CSR_VECTOR: add("w", v.W); add("u", v.U); break;
+    case FAM_SELL16:
     case FAM_SELL: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); break;
     case FAM_ELL: add("r", v.R); add("u", v.U); break;
     case FAM_MERGE: add("i", v.I); break;
@@ -63,6 +64,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_DIA_CONST: add("r", v.R); break;
     case FAM_DIA_WIN:
     case FAM_DIA_CWIN: add("c", v.C); add("r", v.R); add("i", v.I); break;
+    case FAM_SELL16_TMA:
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
@@ -88,8 +90,8 @@ bool variant_from_string(const char* s, Variant* out) {
   if (fam < 0) return false;
   v.fam = fam;
   if (fam == FAM_MERGE) v.I = 7;
-  if (fam == FAM_SELL) { v.C = 128; v.S = 1; }
-  if (fam == FAM_SELL_TMA) { v.C = 256; v.S = 1; v.U = 8; v.I = 3; v.block = 288; }
+  if (fam == FAM_SELL || fam == FAM_SELL16) { v.C = 128; v.S = 1; }
+  if (fam == FAM_SELL_TMA || fam == FAM_SELL16_TMA) { v.C = 256; v.S = 1; v.U = 8; v.I = 3; v.block = 288; }
   if (fam == FAM_CSR_VECTOR || fam == FAM_BCSR3) v.W = 8;
   if (fam == FAM_DIA || fam == FAM_DIA_CONST) v.C = 128;
   if (fam == FAM_DIA_TMA) { v.C = 256; v.U = 8; v.I = 3; v.block = 288; }
@@ -126,9 +128,11 @@ static bool template_supported(const Variant& v) {
     case FAM_CSR_SCALAR: return csr_scalar_supported(v);
     case FAM_CSR_VECTOR: return csr_vector_supported(v);
     case FAM_SELL:
+    case FAM_SELL16:
     case FAM_ELL: return sell_supported(v);
     case FAM_MERGE: return merge_supported(v);
     case FAM_BCSR3: return bcsr_supported(v);
+    case FAM_SELL16_TMA:
     case FAM_SELL_TMA: return sell_tma_supported(v);
     case FAM_DIA: return dia_supported(v);
     case FAM_DIA_TMA: return dia_tma_supported(v);
@@ -160,6 +164,12 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (in.max_row_len > 32 || in.nnz == 0) return no("more than 32 entries in a row: more than 32 diagonals");
     if (h->dia_state < 0) return no("pattern is not a set of at most 32 (half-full) diagonals");
   }
+  if (is_sell16(v)) {
+    // a slice of C rows inside a sorting window of S rows touches columns within bandwidth of its rows
+    if (v.L != 0) return no("sell16 has no row splitting");
+    if (2 * in.bandwidth + std::max(v.C, v.S) >= 0xFFFF && in.rows > 0)
+      return no("column span of a slice can reach 65535: 16-bit deltas do not fit");
+  }
   if (v.L != 0) {
     if (v.fam != FAM_SELL && v.fam != FAM_SELL_TMA) return no("row splitting is a SELL option");
     if (v.L < 4 || v.L > 65536) return no("split length out of range");
@@ -174,6 +184,8 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
 // ------------------------------------------------------------------ formats
 spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) {
   switch (v.fam) {
+    case FAM_SELL16:
+    case FAM_SELL16_TMA:
     case FAM_SELL_TMA:
     case FAM_SELL: {
       auto key = sell_key(v);
@@ -185,6 +197,10 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
         free_sell(f, h->al);
         set_last_error("SELL c%d s%d: padding over 2x nnz", v.C, v.S);
         return SPMV_ERR_UNSUPPORTED;
+      }
+      if (is_sell16(v)) {
+        st = sell_narrow_indices(f, h->al, s);
+        if (st != SPMV_OK) { free_sell(f, h->al); return st; }
       }
       h->sells[key] = f;
       return SPMV_OK;
@@ -243,7 +259,7 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   // An apply launched on ANY stream may still be reading a format that is about to be freed (and a
   // stream-ordered allocator behind the callbacks would recycle the memory at once): wait for the device
   // before the first free.  Slow path only (select / tune / update_values / destroy).
-  const bool keeps_sell = keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA;
+  const bool keeps_sell = is_sell_family(keep);
   const bool keeps_dia = keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST ||
                          keep.fam == FAM_DIA_WIN || keep.fam == FAM_DIA_CWIN;
   size_t n_free = (h->has_ell && keep.fam != FAM_ELL) + (h->has_bcsr && keep.fam != FAM_BCSR3);
@@ -252,7 +268,7 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   for (const auto& kv : h->plans) n_free += !(keep.fam == FAM_MERGE && kv.first == keep.block * keep.I);
   if (n_free) cudaDeviceSynchronize();
   for (auto it = h->sells.begin(); it != h->sells.end();) {
-    if ((keep.fam == FAM_SELL || keep.fam == FAM_SELL_TMA) && it->first == sell_key(keep)) { ++it; continue; }
+    if (keeps_sell && it->first == sell_key(keep)) { ++it; continue; }
     free_sell(it->second, h->al);
     it = h->sells.erase(it);
   }
@@ -280,13 +296,15 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
   const CsrView& A = h->A;
   const int64_t csr = A.nnz * 12 + (A.rows + 1) * 4;
   switch (v.fam) {
+    case FAM_SELL16:
+    case FAM_SELL16_TMA:
     case FAM_SELL_TMA:
     case FAM_SELL: {
       auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return 0;
       const SellFormat& f = it->second;
-      return f.padded * 12 + (f.nslices + 1) * 8 + (f.perm ? f.nslices * (int64_t)f.C * 4 : 0) +
-             f.nparts * 16 + f.nsplit * 8;
+      return f.padded * (f.col16 ? 10 : 12) + (f.nslices + 1) * 8 + (f.col16 ? f.nslices * 4 : 0) +
+             (f.perm ? f.nslices * (int64_t)f.C * 4 : 0) + f.nparts * 16 + f.nsplit * 8;
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
     case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
@@ -373,10 +391,12 @@ spmv_status_t build_plan(spmv_handle_s* h, const Variant& v, LaunchPlan* out) {
     case FAM_CSR_SCALAR: e = csr_scalar_plan(v, h->A, sms, out); break;
     case FAM_CSR_VECTOR: e = csr_vector_plan(v, h->A, sms, out); break;
     case FAM_SELL:
+    case FAM_SELL16:
+    case FAM_SELL16_TMA:
     case FAM_SELL_TMA: {
       auto it = h->sells.find(sell_key(v));
       if (it == h->sells.end()) return SPMV_ERR_INTERNAL;
-      e = v.fam == FAM_SELL ? sell_plan(v, h->A.rows, it->second, sms, out)
+      e = (v.fam == FAM_SELL || v.fam == FAM_SELL16) ? sell_plan(v, h->A.rows, it->second, sms, out)
                             : sell_tma_plan(v, h->A.rows, h->A.cols, it->second, sms, out);
       break;
     }

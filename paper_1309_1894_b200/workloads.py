@@ -114,8 +114,9 @@ def csr_from_lengths(lengths, cols: int, stream: int, *, sort=True, values="norm
     return CSR(rows, cols, row_ptr.astype(np.int32), col_idx.astype(np.int32), val)
 
 
-def _distinct_columns(row_ptr: np.ndarray, cols: int, stream: int) -> np.ndarray:
-    """Per row: uniform draws from [0, cols), duplicates rejected and redrawn, sorted.
+def _distinct_columns(row_ptr: np.ndarray, cols: int, stream: int, lo=None, span=None) -> np.ndarray:
+    """Per row: uniform draws from [0, cols) -- or from [lo[row], lo[row] + span[row]) when given --
+    duplicates rejected and redrawn, sorted.
     (BASELINE.json:configs[2] "columns uniform random without replacement ... sorted")."""
     rows = row_ptr.size - 1
     nnz = int(row_ptr[-1])
@@ -125,6 +126,25 @@ def _distinct_columns(row_ptr: np.ndarray, cols: int, stream: int) -> np.ndarray
     rid = np.repeat(np.arange(rows, dtype=_U64), lengths)
     shift = _U64(32)
     key = np.empty(nnz, dtype=_U64)
+    if lo is not None:
+        assert (2 * lengths <= span).all(), "windowed draws need rows at most half as long as their window"
+        e_lo = np.repeat(np.asarray(lo, dtype=_U64), lengths)
+        e_span = np.repeat(np.asarray(span, dtype=_U64), lengths)
+        draw = lambda strm, idx, sel: e_lo[sel] + mix64(strm, idx) % e_span[sel]
+        key[:] = (rid << shift) | draw(stream, np.arange(nnz, dtype=_U64), slice(None))
+        attempt = 0
+        while True:
+            key.sort()
+            dup = np.flatnonzero(key[1:] == key[:-1]) + 1
+            if dup.size == 0:
+                break
+            attempt += 1
+            assert attempt < 1000, "column rejection sampling did not converge"
+            # after sorting, entry `dup` still belongs to row key >> 32: redraw inside that row's window
+            r = (key[dup] >> shift).astype(np.int64)
+            lo_a, span_a = np.asarray(lo, dtype=_U64), np.asarray(span, dtype=_U64)
+            key[dup] = (key[dup] & ~_U64(0xFFFFFFFF)) | (lo_a[r] + mix64(stream + 1000 * attempt, dup.astype(_U64)) % span_a[r])
+        return (key & _U64(0xFFFFFFFF)).astype(np.int64)
     for a in range(0, nnz, _CHUNK):
         b = min(nnz, a + _CHUNK)
         key[a:b] = (rid[a:b] << shift) | (mix64(stream, np.arange(a, b, dtype=_U64)) % _U64(cols))
@@ -285,6 +305,23 @@ def powerlaw(rows: int, cols: int | None = None, s: float = 1.8, lmax: int = 200
     col_idx = _distinct_columns(row_ptr, cols, col_stream)
     val = normal(val_stream, nnz)
     return CSR(rows, cols, row_ptr.astype(np.int32), col_idx.astype(np.int32), val)
+
+
+def banded_random(rows: int, per_row: int = 24, half_band: int = 12000, stream: int = 80) -> CSR:
+    """Square banded matrix with UNSTRUCTURED columns inside the band (a finite-element matrix on an
+    irregular mesh after bandwidth-reducing reordering): every row holds `per_row` distinct columns drawn
+    uniformly from [i - half_band, i + half_band] (clipped to the matrix), sorted; values N(0,1).
+    Thousands of distinct diagonals, so the DIA family refuses it, while every SELL slice spans fewer than
+    65535 columns: the workload of the 16-bit delta-index variants."""
+    i = np.arange(rows, dtype=np.int64)
+    lo = np.maximum(i - half_band, 0)
+    hi = np.minimum(i + half_band, rows - 1)
+    span = hi - lo + 1
+    lengths = np.minimum(per_row, span // 2).astype(np.int64)
+    row_ptr = np.zeros(rows + 1, dtype=np.int64)
+    np.cumsum(lengths, out=row_ptr[1:])
+    col_idx = _distinct_columns(row_ptr, rows, stream, lo=lo, span=span)
+    return CSR(rows, rows, row_ptr.astype(np.int32), col_idx.astype(np.int32), normal(stream + 1, int(row_ptr[-1])))
 
 
 # ----------------------------------------------------------------------------

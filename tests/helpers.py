@@ -52,6 +52,9 @@ REPRESENTATIVE_VARIANTS = [
     # long rows cut into segments of l entries (virtual rows) + ordered fix-up
     "sell:b256:c128:s8192:l16:r2:u2:x0", "sell:b128:c512:s1024:l64:r1:u4:x0", "sell:b256:c128:s256:l4:r1:u2:x1",
     "sell_tma:b160:c128:s8192:l32:r1:u4:i3:x0", "sell_tma:b160:c256:s2048:l128:r2:u8:i2:x0",
+    # 16-bit delta-encoded column indices (banded patterns only)
+    "sell16:b256:c128:s1:r1:u2:x0", "sell16:b128:c128:s1:r2:u4:x0", "sell16:b256:c512:s512:r4:u2:x1", "sell16:b256:c128:s8192:r2:u8:x0:g2",
+    "sell16_tma:b288:c256:s1:r1:u8:i3:x0", "sell16_tma:b160:c256:s1:r2:u4:i4:x0", "sell16_tma:b160:c128:s1024:r1:u16:i2:x0",
     "dia:b256:c128:r1:u4:x0", "dia:b128:c256:r2:u8:x0", "dia:b256:c512:r4:u2:x1", "dia:b512:c128:r1:u1:x0:g2",
     "dia_const:b256:r1:x0", "dia_const:b128:r2:x1", "dia_const:b512:r4:x0",
     "dia_win:b288:c256:r1:i2:x0", "dia_win:b96:c128:r2:i3:x0", "dia_win:b160:c128:r1:i4:x0:g2",
@@ -84,5 +87,6 @@ def zoo():
     out.append(("st27_9", W.stencil3d_27pt(9, perturb_stream=50)))
     out.append(("fem_5", W.fem_block27(5)))
     out.append(("powerlaw_3k", W.powerlaw(3000, lmax=2500)))
+    out.append(("banded_4k", W.banded_random(4000, 12, 900, stream=81)))
     out.append(("rows_129", W.csr_from_lengths(np.random.default_rng(10).integers(1, 20, 129), 129, 10)))
     return out

