@@ -432,7 +432,7 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
             best = None
             for _ in range(3):
                 xg = torch.zeros(A0.rows, dtype=torch.float64, device=device)
-                r = handles[0].cg(bvec, xg, tol=1e-300, max_iters=n_it, check_every=25)
+                r = handles[0].cg(bvec, xg, tol=1e-300, max_iters=n_it, check_every=25, tune_loop=True)
                 if best is None or r["device_seconds"] < best["device_seconds"]:
                     best = r
             st.synchronize()
@@ -441,8 +441,11 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
         cg = {"iters": best["iters"], "us_per_iteration": best["device_seconds"] / max(best["iters"], 1) * 1e6,
               "eff_gbs": it_bytes * best["iters"] / best["device_seconds"] / 1e9,
               "rel_residual": best["rel_residual"], "graph_replays": best["graph_replays"],
-              "fused_single_kernel": bool(best["fused"]),
+              "fused_single_kernel": bool(best["fused"]), "fused_dot": bool(best["fused_dot"]),
+              "kernels_per_iteration": best["kernels_per_iteration"], "loop_variant": best["loop_variant"],
               "bytes_per_iteration_algorithmic": it_bytes}
+        for h in handles:                      # tune_loop may have adopted another leader: back to the apply winner
+            h.select(variant)
 
     # ---- K applies replayed as one CUDA graph (launch-bound configs; a clearly labelled extra line)
     graph = None
@@ -491,6 +494,35 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     for h in handles:
         h.close()
     return res, probs[0]
+
+
+def bench_banded(args, torch, binding, W, device):
+    """Extra line: a banded matrix with unstructured columns inside the band (2^21 rows, 24
+    entries per row within +-2000 of the diagonal: ~4000 distinct diagonals, DIA refuses it).  Tuned twice: over
+    everything, and over the 32-bit-index families only; both winners are checked against the oracle."""
+    A = W.banded_random(1 << 21, 24, 2000)
+    x = W.uniform(90, A.cols)
+    prob = W.Problem("banded-random 2^21 rows, 24/row within +-2000", A, x, None, 1.0, 0.0)
+    nb = W.algorithmic_bytes(A.rows, A.cols, A.nnz, 0.0)
+    S = binding.SpMV.from_csr(A, device=device)
+    dx = torch.from_numpy(x).to(device)
+    dy = torch.zeros(A.rows, dtype=torch.float64, device=device)
+    out = {"workload": prob.name, "rows": A.rows, "nnz": A.nnz, "bytes_algorithmic": nb}
+    for key, flt in (("idx32_only", "csr_scalar,csr_vector,sell:,sell_tma,ell,merge"), ("all", None)):
+        rep = S.tune(alpha=1.0, beta=0.0, use_cache=2, variant_filter=flt, seed=7)
+        S.apply(1.0, dx, 0.0, dy)
+        torch.cuda.synchronize()
+        chk = oracle_check(prob, dy.cpu().numpy())
+        if not chk["ok"]:
+            raise SystemExit(f"bench: banded {rep['winner']} FAILED the oracle check: {chk}")
+        fb = int(S.info().format_bytes)
+        out[key] = {"variant": rep["winner"], "us": rep["winner_us"], "eff_gbs": nb / rep["winner_us"] / 1e3,
+                    "format_bytes": fb, "actual_gbs": (fb + 16 * A.rows) / rep["winner_us"] / 1e3,
+                    "max_err_over_scale": chk["max_err_over_scale"], "tune_seconds": rep["tune_seconds"]}
+    out["speedup_16bit_over_32bit"] = out["idx32_only"]["us"] / out["all"]["us"]
+    out["timing"] = "spmv_tune's own protocol: median of 5 batches of back-to-back applies (603 MB CSR: warm = streaming)"
+    S.close()
+    return out
 
 
 def config_roofline(r, peak, ceil):
@@ -554,6 +586,7 @@ def main():
     ap.add_argument("--min-ms", type=float, default=50.0, help="batches of --steps repeat until the timed region lasts this long")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-oracle-check", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the banded-matrix line (16-bit vs 32-bit column indices)")
     ap.add_argument("--variant-filter", default=None,
                     help="comma list of descriptor prefixes the tuner may use (spmv_tune variant_filter), e.g. "
                          "'csr_scalar,csr_vector,sell:,sell_tma,ell,merge,bcsr3,dia:,dia_tma' = everything that still "
@@ -642,6 +675,8 @@ def main():
         line["roofline"] = dict(head["roofline"], kernel=head["variant"])
         line["cpu_baseline"] = head.get("cpu_baseline")
         line["cg"] = next((r["cg"] for r in results if r["cg"]), None)
+        if not args.no_extras:
+            line["banded"] = bench_banded(args, torch, binding, W, device)
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist

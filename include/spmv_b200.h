@@ -233,12 +233,20 @@ typedef struct {
   int32_t no_graph;      /* 1: never use a CUDA graph */
   int32_t no_fused;      /* 1: never use the single cooperative kernel that runs the whole solve for small
                             systems (rows <= 262144, nnz <= 4 Mi): launch-bound otherwise */
+  int32_t no_fused_dot;  /* 1: never fuse p.q into the SpMV kernel's epilogue (large systems; available for the
+                            dia_const family): a dot kernel then makes a second pass over p and q */
+  int32_t tune_loop;     /* 1: before solving, time a few iterations of the loop with each of the leaders of the
+                            last spmv_tune of this handle and adopt the fastest (SURVEY 8(f) rank 3 "tune for the
+                            loop rather than the single apply"); no-op when the handle was not tuned in this process */
 } spmv_cg_opts_t;
 typedef struct {
   int32_t iters, converged, breakdown;
   int32_t iterations_launched;   /* >= iters: iterations issued after convergence are device-side no-ops */
   int32_t graph_replays;
   int32_t fused;                 /* 1: the whole solve ran in the single cooperative kernel */
+  int32_t fused_dot;             /* 1: p.q came out of the SpMV kernel's epilogue */
+  int32_t kernels_per_iteration; /* launches per iteration (0 when fused) */
+  char loop_variant[128];        /* the variant the loop ran with (differs from the apply winner after tune_loop) */
   double rel_residual;           /* sqrt(r.r) / ||b||  (sqrt(r.r) when b == 0) */
   double device_seconds;         /* CUDA events around the whole solve */
   double wall_seconds;

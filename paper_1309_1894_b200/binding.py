@@ -65,12 +65,13 @@ class TuneOpts(C.Structure):
 
 class CgOpts(C.Structure):
     _fields_ = [("tol", C.c_double), ("max_iters", C.c_int32), ("check_every", C.c_int32), ("no_graph", C.c_int32),
-                ("no_fused", C.c_int32)]
+                ("no_fused", C.c_int32), ("no_fused_dot", C.c_int32), ("tune_loop", C.c_int32)]
 
 
 class CgResult(C.Structure):
     _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("breakdown", C.c_int32),
                 ("iterations_launched", C.c_int32), ("graph_replays", C.c_int32), ("fused", C.c_int32),
+                ("fused_dot", C.c_int32), ("kernels_per_iteration", C.c_int32), ("loop_variant", C.c_char * 128),
                 ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
 
 
@@ -249,14 +250,17 @@ class SpMV:
         self._keep = (self._keep[0], self._keep[1], val)
         return bool(fb.value)
 
-    def cg(self, b, x, *, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, no_fused=False, stream=None) -> dict:
+    def cg(self, b, x, *, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, no_fused=False,
+           no_fused_dot=False, tune_loop=False, stream=None) -> dict:
         """Conjugate gradients with the selected variant (spmv_cg).  x: initial guess in, solution out."""
         assert b.is_cuda and x.is_cuda and b.numel() == self.rows and x.numel() == self.rows
         o = CgOpts(float(tol), int(max_iters) if max_iters > 0 else -1, int(check_every), int(bool(no_graph)),
-                   int(bool(no_fused)))
+                   int(bool(no_fused)), int(bool(no_fused_dot)), int(bool(tune_loop)))
         r = CgResult()
         _check(lib().spmv_cg(self.h, _dptr(b), _dptr(x), C.byref(o), C.byref(r), _stream_ptr(stream)), "spmv_cg")
-        return {k: getattr(r, k) for k, _ in CgResult._fields_}
+        out = {k: getattr(r, k) for k, _ in CgResult._fields_}
+        out["loop_variant"] = out["loop_variant"].decode()
+        return out
 
     def graph(self, alpha, x, beta, y, k: int) -> "Graph":
         """k back-to-back applies captured into one CUDA graph (spmv_graph_create); x, y are baked in."""

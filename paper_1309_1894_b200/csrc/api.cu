@@ -1,8 +1,10 @@
 // C ABI entry points (include/spmv_b200.h) except spmv_tune / spmv_tune_batch (tuner.cu)
 // and spmv_measure_ceiling (verify.cu).
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <mutex>
 #include <set>
 
@@ -137,6 +139,8 @@ spmv_status_t spmv_destroy(spmv_handle_t h) {
   release_all_formats(h);
   if (h->d_x_stage) h->al.free(h->d_x_stage, sizeof(double) * h->A.cols);
   if (h->d_y_stage) h->al.free(h->d_y_stage, sizeof(double) * h->A.rows);
+  for (cudaEvent_t e : h->hs_events) cudaEventDestroy(e);
+  if (h->hs_up) { cudaStreamDestroy(h->hs_up); cudaStreamDestroy(h->hs_up2); cudaStreamDestroy(h->hs_run); cudaStreamDestroy(h->hs_down); }
   h->magic = 0;
   delete h;
   return SPMV_OK;
@@ -247,21 +251,88 @@ spmv_status_t spmv_graph_destroy(spmv_graph_t g) {
   return SPMV_OK;
 }
 
+// Host-vector apply.  Where the selected variant has a row-range form (plan_for_rows) the call is a pipeline over
+// chunks of rows on three internal streams: upload (x as far as the chunk's rows reach -- its rows plus the
+// matrix bandwidth -- and the chunk of y when beta != 0) | kernel on the chunk | download of the chunk of y.
+// PCIe is full duplex, so the download of chunk k-1 overlaps the upload of chunk k+1 and the kernel of chunk k;
+// for a banded matrix the first kernel starts long before x is complete.  Results are bit-identical to the
+// one-launch form: a row is summed by the same kernel code in the same order.
 spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
                               void* stream) {
   if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
   if ((h->A.rows > 0 && !h_y) || (h->A.cols > 0 && !h_x)) return SPMV_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  if (!h->d_x_stage) h->d_x_stage = (double*)h->al.alloc(sizeof(double) * h->A.cols, s);
-  if (!h->d_y_stage) h->d_y_stage = (double*)h->al.alloc(sizeof(double) * h->A.rows, s);
+  const int64_t rows = h->A.rows, cols = h->A.cols;
+  if (!h->d_x_stage) h->d_x_stage = (double*)h->al.alloc(sizeof(double) * cols, s);
+  if (!h->d_y_stage) h->d_y_stage = (double*)h->al.alloc(sizeof(double) * rows, s);
   if (!h->d_x_stage || !h->d_y_stage) return SPMV_ERR_ALLOC;
-  if (h->A.cols) SPMV_CUDA_TRY(cudaMemcpyAsync(h->d_x_stage, h_x, sizeof(double) * h->A.cols, cudaMemcpyHostToDevice, s));
-  if (beta != 0.0 && h->A.rows)
-    SPMV_CUDA_TRY(cudaMemcpyAsync(h->d_y_stage, h_y, sizeof(double) * h->A.rows, cudaMemcpyHostToDevice, s));
-  spmv_status_t st = spmv_apply(h, alpha, h->d_x_stage, beta, h->d_y_stage, stream);
-  if (st != SPMV_OK) return st;
-  if (h->A.rows) SPMV_CUDA_TRY(cudaMemcpyAsync(h_y, h->d_y_stage, sizeof(double) * h->A.rows, cudaMemcpyDeviceToHost, s));
+  double *dx = h->d_x_stage, *dy = h->d_y_stage;
+
+  // chunks of ~3 MB of y (smaller: the fixed cost of a PCIe copy shows; larger: less overlap), boundaries on the
+  // variant's range alignment
+  const int64_t align = h->plan.range_align > 0 ? h->plan.range_align : 1;
+  static const double chunk_mb = getenv("SPMV_HOST_CHUNK_MB") ? atof(getenv("SPMV_HOST_CHUNK_MB")) : 3.0;   // measured: 2-4 MB of y per chunk is the flat optimum
+  int64_t nchunks = std::min<int64_t>(32, (int64_t)(rows * 8 / (chunk_mb * 1048576.0)));
+  int64_t chunk = nchunks > 1 ? ((rows + nchunks - 1) / nchunks + align - 1) / align * align : rows;
+  const bool pipelined = alpha != 0.0 && nchunks > 1 && chunk < rows && h->plan.n == 1 && h->plan.range_kind != RANGE_NONE;
+  if (!pipelined) {
+    if (cols) SPMV_CUDA_TRY(cudaMemcpyAsync(dx, h_x, sizeof(double) * cols, cudaMemcpyHostToDevice, s));
+    if (beta != 0.0 && rows) SPMV_CUDA_TRY(cudaMemcpyAsync(dy, h_y, sizeof(double) * rows, cudaMemcpyHostToDevice, s));
+    spmv_status_t st = spmv_apply(h, alpha, dx, beta, dy, stream);
+    if (st != SPMV_OK) return st;
+    if (rows) SPMV_CUDA_TRY(cudaMemcpyAsync(h_y, dy, sizeof(double) * rows, cudaMemcpyDeviceToHost, s));
+    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+    return SPMV_OK;
+  }
+  nchunks = (rows + chunk - 1) / chunk;
+  if (!h->hs_up) {
+    SPMV_CUDA_TRY(cudaStreamCreateWithFlags(&h->hs_up, cudaStreamNonBlocking));
+    SPMV_CUDA_TRY(cudaStreamCreateWithFlags(&h->hs_up2, cudaStreamNonBlocking));
+    SPMV_CUDA_TRY(cudaStreamCreateWithFlags(&h->hs_run, cudaStreamNonBlocking));
+    SPMV_CUDA_TRY(cudaStreamCreateWithFlags(&h->hs_down, cudaStreamNonBlocking));
+  }
+  while ((int64_t)h->hs_events.size() < 3 * nchunks + 2) {
+    cudaEvent_t e;
+    SPMV_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    h->hs_events.push_back(e);
+  }
+  cudaEvent_t* ev = h->hs_events.data();
+  // work already queued on the caller's stream comes first
+  SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks], s));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up, ev[3 * nchunks], 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up2, ev[3 * nchunks], 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * nchunks], 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_down, ev[3 * nchunks], 0));
+  const bool aligned = true;                 // the staging vectors come from the allocator: 16-byte aligned
+  const int64_t bw = h->info.bandwidth;
+  int64_t x_up = 0;                          // x[0, x_up) is queued for upload
+  for (int64_t c = 0; c < nchunks; ++c) {
+    const int64_t a = c * chunk, b = std::min(rows, a + chunk);
+    const int64_t need = std::min(cols, b + bw + 1);          // rows < b reference columns < b + bandwidth + 1
+    if (need > x_up) {
+      SPMV_CUDA_TRY(cudaMemcpyAsync(dx + x_up, h_x + x_up, sizeof(double) * (need - x_up), cudaMemcpyHostToDevice, h->hs_up));
+      x_up = need;
+    }
+    SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c], h->hs_up));
+    SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * c], 0));
+    if (beta != 0.0) {       // y on its own upload stream: the fixed latencies of the two small copies overlap
+      SPMV_CUDA_TRY(cudaMemcpyAsync(dy + a, h_y + a, sizeof(double) * (b - a), cudaMemcpyHostToDevice, h->hs_up2));
+      SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c + 2], h->hs_up2));
+      SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * c + 2], 0));
+    }
+    KernelCall kc;
+    if (!plan_for_rows(h->plan, rows, cols, a, b, aligned, &kc)) { set_last_error("apply_host: range launch refused"); return SPMV_ERR_INTERNAL; }
+    ApplyArgs args{alpha, beta, dx, dy, h->hs_run};
+    cudaError_t e = run_call(kc, args);
+    if (e != cudaSuccess) { set_last_error("apply_host: chunk launch failed: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+    SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c + 1], h->hs_run));
+    SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_down, ev[3 * c + 1], 0));
+    SPMV_CUDA_TRY(cudaMemcpyAsync(h_y + a, dy + a, sizeof(double) * (b - a), cudaMemcpyDeviceToHost, h->hs_down));
+  }
+  SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks + 1], h->hs_down));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(s, ev[3 * nchunks + 1], 0));
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  SPMV_CUDA_TRY(cudaStreamSynchronize(h->hs_up));       // (nothing pending: every upload precedes a kernel that has finished)
   return SPMV_OK;
 }
 

@@ -17,6 +17,7 @@ struct spmv_handle_s {
   spmv::Variant sel;
   spmv::LaunchPlan plan;          // resolved launch of `sel` (rebuilt by select / tune / update_values)
   bool tuned = false;
+  std::vector<std::string> leaders;   // best three distinct candidates of the last spmv_tune (spmv_cg tune_loop)
 
   // owned formats, built on demand
   std::map<std::tuple<int, int, int, int>, spmv::SellFormat> sells;   // key (C, sigma, split, 16-bit indices)
@@ -28,9 +29,11 @@ struct spmv_handle_s {
   std::map<int, spmv::DiaFormat> dias;                     // key C
   int dia_state = 0;                                       // 0 not tried, 1 built once, -1 pattern is not diagonal
 
-  // staging for spmv_apply_host
+  // staging for spmv_apply_host, and the three internal streams + events of its chunk pipeline
   double* d_x_stage = nullptr;
   double* d_y_stage = nullptr;
+  cudaStream_t hs_up = nullptr, hs_up2 = nullptr, hs_run = nullptr, hs_down = nullptr;
+  std::vector<cudaEvent_t> hs_events;
 };
 
 namespace spmv {
@@ -51,6 +54,8 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
 spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s);
 // Resolves kernel, grid, shared memory, carve-out and the argument block of `v` (format must exist).
 spmv_status_t build_plan(spmv_handle_s* h, const Variant& v, LaunchPlan* out);
+// q = A x with x.q fused into the kernel (solver loop); UNSUPPORTED when the selected family has no such form.
+spmv_status_t build_dot_plan(spmv_handle_s* h, double* part, int* n_part, LaunchPlan* out);
 // Launches a resolved plan: patch alpha / x / beta / y, one or two kernel launches, nothing else.
 spmv_status_t launch_plan(const LaunchPlan& p, const ApplyArgs& a);
 // Makes `v` the selected variant: format, plan, info.  Waits for the device first when formats are freed.

@@ -91,7 +91,10 @@ cudaError_t bcsr_plan(const Variant& v, const BcsrFormat& f, int sm_count, Launc
   if (e != cudaSuccess) return e;
   c.add((int)f.brows); c.add((const int*)f.brow_ptr); c.add((const int*)f.bcol); c.add((const double*)f.bval);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.per_block = per_block;       // block rows
   out->n = 1;
+  out->range_kind = RANGE_BCSR;
+  out->range_align = 3;
   return cudaSuccess;
 }
 

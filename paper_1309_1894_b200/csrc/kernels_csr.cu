@@ -149,7 +149,9 @@ cudaError_t csr_scalar_plan(const Variant& v, const CsrView& A, int sm_count, La
   cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
   if (e != cudaSuccess) return e;
   csr_args(c, A);
+  c.per_block = (int64_t)v.block * v.R;
   out->n = 1;
+  out->range_kind = RANGE_CSR;
   return cudaSuccess;
 }
 
@@ -167,7 +169,9 @@ cudaError_t csr_vector_plan(const Variant& v, const CsrView& A, int sm_count, La
   cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
   if (e != cudaSuccess) return e;
   csr_args(c, A);
+  c.per_block = rows_per_block;
   out->n = 1;
+  out->range_kind = RANGE_CSR;
   return cudaSuccess;
 }
 

@@ -15,6 +15,7 @@
 
 #include <algorithm>
 
+#include "cg_reduce.cuh"
 #include "device_utils.cuh"
 #include "spmv_internal.h"
 
@@ -135,7 +136,11 @@ cudaError_t dia_plan(const Variant& v, int64_t rows, const DiaFormat& f, int sm_
   c.add(rows); c.add((int64_t)f.ld); c.add(f.C); c.add(f.logC); c.add(f.nd); c.add(dia_offsets(f));
   c.add((const double*)f.val); c.add((const unsigned*)f.mask);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.per_block = (int64_t)v.block * v.R;
   out->n = 1;
+  out->range_kind = RANGE_DIA;
+  out->range_align = f.C;
+  out->range_elem = f.nd;
   return cudaSuccess;
 }
 
@@ -164,14 +169,16 @@ __device__ __forceinline__ double2 ldx2(const double* __restrict__ x, int i) {  
   return v;
 }
 
-// R > 1 (needs cols % 2 == 0 and 16-byte aligned x): e[r] = x[b + r], r < R, b even, as aligned pairs.  A pair
-// lies either completely inside [0, cols) or completely outside; an outside pair is read at a clamped
+// x indices are relative to the x pointer the kernel was given and valid in [xlo, xhi] (the whole vector:
+// [0, cols - 1]; a row range [a, b) launched by spmv_apply_host: x + a, [-a, cols - 1 - a]).
+// R > 1 (needs cols % 2 == 0, xlo even and a 16-byte aligned x): e[r] = x[b + r], r < R, b even, as aligned pairs.
+// A pair lies either completely inside [xlo, xhi] or completely outside; an outside pair is read at a clamped
 // (still aligned) index and never multiplied (its mask bits are off: such entries cannot be stored).
 template <int R, int X>
-__device__ __forceinline__ void dia_load_pairs(const double* __restrict__ x, int b, int cols, double (&e)[R]) {
+__device__ __forceinline__ void dia_load_pairs(const double* __restrict__ x, int b, int xlo, int xhi, double (&e)[R]) {
 #pragma unroll
   for (int r = 0; r < R; r += 2) {
-    const double2 p = ldx2<X>(x, min(max(b + r, 0), cols - 2));
+    const double2 p = ldx2<X>(x, min(max(b + r, xlo), xhi - 1));
     e[r] = p.x; e[r + 1] = p.y;
   }
 }
@@ -187,10 +194,14 @@ template <> struct DiaMaskVec<unsigned> { typedef uint2 V2; typedef uint4 V4; };
 // 12.7 us at 23 on cfg2), hence the exact instantiations and the min-blocks launch bound.
 constexpr int dia_const_min_blocks(int R, int ND) { return (ND == 0 || ND > 9) ? (R == 4 ? 1 : 2) : (R == 1 ? 4 : R == 2 ? 2 : 1); }
 
-template <int R, int ND, int X, typename MT>
+// DOT (R == 1 only; the solver loop, solver.cu): the kernel also writes its block's share of sum_i x_i * y_i
+// (square matrix) to dot_part[blockIdx.x]; the caller adds the gridDim.x partials in index order.  No
+// arrival counter here: a fence + atomic at the tail of 8192 short blocks costs more than the dot pass saved.
+template <int R, int ND, int X, typename MT, bool DOT = false>
 __device__ __forceinline__ void
-dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
-               double alpha, const double* __restrict__ x, double beta, double* __restrict__ y) {
+dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
+               double alpha, const double* __restrict__ x, double beta, double* __restrict__ y,
+               double* __restrict__ dot_part = nullptr) {
   pdl_launch_dependents();
   constexpr int NDC = ND == 0 ? 8 : (ND % 9 == 0 ? 9 : (ND <= 8 ? ND : 8));     // diagonals per chunk
   constexpr int DMAX = ND == 0 ? 32 : ND;
@@ -200,7 +211,7 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
   // x indices are clamped, their mask words exist (the mask array is padded to a multiple of the slice
   // height >= 32*R), nothing is stored.
   const int r0 = (blockIdx.x * blockDim.x + threadIdx.x) * R;
-  if (R == 1 && r0 >= rows) return;
+  if (R == 1 && !DOT && r0 >= rows) return;
   unsigned m[R];
   if constexpr (R == 2) {
     const typename DiaMaskVec<MT>::V2 mm = *reinterpret_cast<const typename DiaMaskVec<MT>::V2*>(mask + r0);
@@ -229,7 +240,7 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
         for (int r = 0; r < R; ++r) if (r0 + r < rows) yold[r] = y[r0 + r];
       }
     } else {
-      yold[0] = y[r0];
+      if (!DOT || r0 < rows) yold[0] = y[r0];
     }
   }
   // statically unrolled over the chunks so that the by-value offset / coefficient parameters are never
@@ -244,7 +255,7 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
       if (d < DMAX && (ND != 0 || d < nd)) {                 // warp-uniform
         const int o = offs.off[d < 32 ? d : 31];
         if constexpr (R == 1) {
-          xv[u][0] = ldx<X>(x, min(max(r0 + o, 0), cols - 1));
+          xv[u][0] = ldx<X>(x, min(max(r0 + o, xlo), xhi));
         } else {
           // branch-free for either parity of the offset (p is warp-uniform: r0 is even): the run starts at
           // the even index b = r0 + o - p; for p = 1 it is shifted left by one element and the right
@@ -252,9 +263,9 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
           const int p = o & 1;
           const int b = r0 + o - p;
           double e[R];
-          dia_load_pairs<R, X>(x, b, cols, e);
+          dia_load_pairs<R, X>(x, b, xlo, xhi, e);
           double nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
-          if (p && (threadIdx.x & 31) == 31) nxt = ldx<X>(x, min(max(b + R, 0), cols - 1));
+          if (p && (threadIdx.x & 31) == 31) nxt = ldx<X>(x, min(max(b + R, xlo), xhi));
 #pragma unroll
           for (int r = 0; r + 1 < R; ++r) xv[u][r] = p ? e[r + 1] : e[r];
           xv[u][R - 1] = p ? nxt : e[R - 1];
@@ -274,6 +285,14 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
   double out[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) out[r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  if constexpr (DOT) {
+    __shared__ double s_warp[33];
+    const bool live = r0 < rows;
+    if (live) y[r0] = out[0];
+    const double mine = block_sum_fixed(live ? ldx<X>(x, r0) * out[0] : 0.0, s_warp);
+    if (threadIdx.x == 0) dot_part[blockIdx.x] = mine;
+    return;
+  }
   if constexpr (R > 1) {
     if (full) {
 #pragma unroll
@@ -288,18 +307,36 @@ dia_const_body(int rows, int cols, int nd_rt, const DiaOffsets& offs, const DiaC
 
 template <int R, int ND, int X, typename MT>
 __global__ void __launch_bounds__(512, dia_const_min_blocks(R, ND))
-dia_const_kernel(int rows, int cols, int nd_rt, const __grid_constant__ DiaOffsets offs,
+dia_const_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                  const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                  const double* __restrict__ x, double beta, double* __restrict__ y) {
-  dia_const_body<R, ND, X, MT>(rows, cols, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+  dia_const_body<R, ND, X, MT>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y);
 }
 // two rows per thread on a small stencil: 48 registers keep 1280 threads per SM resident without spilling
 template <int ND, int X, typename MT>
 __global__ void __maxnreg__(48)
-dia_const_kernel_r2(int rows, int cols, int nd_rt, const __grid_constant__ DiaOffsets offs,
+dia_const_kernel_r2(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                     const double* __restrict__ x, double beta, double* __restrict__ y) {
-  dia_const_body<2, ND, X, MT>(rows, cols, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+  dia_const_body<2, ND, X, MT>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+}
+
+// one row per thread with the fused dot product (the solver loop)
+template <int ND, typename MT>
+__global__ void __launch_bounds__(512, 2)
+dia_const_dot_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
+                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
+                     const double* __restrict__ x, double beta, double* __restrict__ y, double* __restrict__ dot_part) {
+  dia_const_body<1, ND, 0, MT, true>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y, dot_part);
+}
+template <typename MT>
+static const void* dia_const_dot_pick_nd(int nd) {
+  switch (nd) {
+    case 5: return (const void*)dia_const_dot_kernel<5, MT>;
+    case 7: return (const void*)dia_const_dot_kernel<7, MT>;
+    case 27: return (const void*)dia_const_dot_kernel<27, MT>;
+    default: return (const void*)dia_const_dot_kernel<0, MT>;
+  }
 }
 
 template <int R, int X, typename MT>
@@ -346,10 +383,33 @@ static void dia_const_call(KernelCall& c, int R, const Variant& v, int64_t rows,
   c.pdl = true;
   DiaCoefs co;
   for (int i = 0; i < 32; ++i) co.c[i] = f.coef[i];
-  c.add((int)rows); c.add((int)cols); c.add(f.nd); c.add(dia_offsets(f)); c.add(co);
+  c.add((int)rows); c.add((int)0); c.add((int)cols - 1); c.add(f.nd); c.add(dia_offsets(f)); c.add(co);
   c.add(f.mask_small ? (const void*)f.mask_small : (const void*)f.mask);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.per_block = (int64_t)v.block * R;
 }
+cudaError_t dia_const_dot_plan(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, double* part,
+                               int* n_part, LaunchPlan* out) {
+  if (!f.is_const || rows != cols || rows == 0) return cudaErrorInvalidValue;
+  *out = LaunchPlan();
+  KernelCall& c = out->k[0];
+  const int me = f.mask_small ? f.mask_elem : 4;
+  c.fn = me == 1 ? dia_const_dot_pick_nd<unsigned char>(f.nd)
+       : me == 2 ? dia_const_dot_pick_nd<unsigned short>(f.nd) : dia_const_dot_pick_nd<unsigned>(f.nd);
+  c.block = v.block;
+  c.grid = (unsigned)((rows + v.block - 1) / v.block);
+  c.pdl = true;
+  DiaCoefs co;
+  for (int i = 0; i < 32; ++i) co.c[i] = f.coef[i];
+  c.add((int)rows); c.add((int)0); c.add((int)cols - 1); c.add(f.nd); c.add(dia_offsets(f)); c.add(co);
+  c.add(f.mask_small ? (const void*)f.mask_small : (const void*)f.mask);
+  c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.add(part);
+  *n_part = (int)c.grid;
+  out->n = 1;
+  return cudaSuccess;
+}
+
 cudaError_t dia_const_plan(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, LaunchPlan* out) {
   if (!f.is_const || !dia_const_pick(v.R, v.X, 4, 0)) return cudaErrorInvalidValue;
   *out = LaunchPlan();
@@ -360,6 +420,9 @@ cudaError_t dia_const_plan(const Variant& v, int64_t rows, int64_t cols, const D
   dia_const_call(out->k[0], R, v, rows, cols, f);
   if (R > 1) { dia_const_call(out->alt, 1, v, rows, cols, f); out->has_alt = true; }
   out->n = 1;
+  out->range_kind = RANGE_DIA_CONST;
+  out->range_align = f.C;
+  out->range_elem = f.mask_small ? f.mask_elem : 4;
   return cudaSuccess;
 }
 
@@ -402,7 +465,7 @@ __device__ __forceinline__ void dbulk_g2s(void* dst, const void* src, uint32_t b
 // before the stage wait, everything else arrives through the ring.
 template <int R, int STAGES, int J, int X>
 __global__ void __launch_bounds__(512 + 32)
-dia_tma_kernel(int64_t rows, int64_t cols, int64_t nslices, int C, int nd, DiaOffsets offs,
+dia_tma_kernel(int64_t rows, int64_t xlo, int64_t xhi, int64_t nslices, int C, int nd, DiaOffsets offs,
                const double* __restrict__ dval, const unsigned* __restrict__ mask, double alpha,
                const double* __restrict__ x, double beta, double* __restrict__ y, int y_bulk) {
   extern __shared__ __align__(128) unsigned char dia_smem[];
@@ -451,7 +514,7 @@ dia_tma_kernel(int64_t rows, int64_t cols, int64_t nslices, int C, int nd, DiaOf
 
   uint32_t stage = 0, phase = 0;
   const int lane = tid & 31;
-  const int xmax = (int)cols - 1;
+  const int xmin = (int)xlo, xmax = (int)xhi;      // valid x indices relative to the x pointer given
   for (int64_t s = blockIdx.x; s < nslices; s += gridDim.x) {
     const int64_t r0 = s * C + (int64_t)tid * R;
     const bool ybulk = want_y && (s + 1) * C <= rows;
@@ -469,7 +532,7 @@ dia_tma_kernel(int64_t rows, int64_t cols, int64_t nslices, int C, int nd, DiaOf
       for (int j = 0; j < J; ++j) {
         const int o = offs.off[min(d0 + j, nd - 1)];
 #pragma unroll
-        for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, min(max((int)(r0 + r) + o, 0), xmax));
+        for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, min(max((int)(r0 + r) + o, xmin), xmax));
       }
       dbar_wait(&full[stage], phase);
       if (d0 == 0) {
@@ -511,7 +574,7 @@ dia_tma_kernel(int64_t rows, int64_t cols, int64_t nslices, int C, int nd, DiaOf
   }
 }
 
-typedef void (*dia_tma_kernel_t)(int64_t, int64_t, int64_t, int, int, DiaOffsets, const double*, const unsigned*, double,
+typedef void (*dia_tma_kernel_t)(int64_t, int64_t, int64_t, int64_t, int, int, DiaOffsets, const double*, const unsigned*, double,
                                  const double*, double, double*, int);
 struct DiaTmaEntry { int R, STAGES, J; dia_tma_kernel_t k; };
 #define DE(r, st, j) {r, st, j, dia_tma_kernel<r, st, j, 0>}
@@ -549,11 +612,15 @@ cudaError_t dia_tma_plan(const Variant& v, int64_t rows, int64_t cols, const Dia
   const int64_t nslices = f.ld / f.C;
   err = resolve_grid(v.grid > 0 ? v.grid : 1, c.fn, v.block, c.smem, sm_count, nslices, &c.grid);   // persistent
   if (err != cudaSuccess) return err;
-  c.add(rows); c.add(cols); c.add(nslices); c.add(f.C); c.add(f.nd); c.add(dia_offsets(f));
+  c.add(rows); c.add((int64_t)0); c.add(cols - 1); c.add(nslices); c.add(f.C); c.add(f.nd); c.add(dia_offsets(f));
   c.add((const double*)f.val); c.add((const unsigned*)f.mask);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
   c.add_flag(1);                 // y_bulk: cp.async.bulk needs 16-byte aligned global addresses
+  c.per_block = f.C;             // one slice per CTA trip; the grid is capped at the persistent size
   out->n = 1;
+  out->range_kind = RANGE_DIA_TMA;
+  out->range_align = f.C;
+  out->range_elem = f.nd;
   return cudaSuccess;
 }
 

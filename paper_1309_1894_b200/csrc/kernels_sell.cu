@@ -11,6 +11,8 @@
 // 16-bit form (sell16, SURVEY sec. 8(f) rank 1 "16-bit delta-encoded column indices inside SELL slices"):
 // the column of an entry is sbase[slice] + a 16-bit delta (0xFFFF = padding), 10 bytes per stored entry
 // instead of 12, for banded matrices that DIA refuses (more than 32 diagonals, fill below one half).
+#include <algorithm>
+
 #include "device_utils.cuh"
 #include "spmv_internal.h"
 
@@ -224,8 +226,14 @@ cudaError_t sell_plan(const Variant& v, int64_t rows, const SellFormat& f, int s
   c.add((const double*)f.val); c.add(f.col16 ? (const void*)f.col16 : (const void*)f.col); c.add((const int*)f.sbase);
   c.add((const int*)f.perm); c.add(f.part);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.per_block = (int64_t)v.block * v.R;
   out->n = 1;
   if (f.split && f.nsplit > 0) { sell_split_fixup_call(f, &out->k[1]); out->n = 2; }
+  else if (!f.is_ell && !f.split) {       // slices [s0, s1): the rows of a sorting window stay inside it
+    out->range_kind = RANGE_SELL;
+    out->range_align = std::max(f.C, f.sigma);
+    out->range_elem = f.C;
+  }
   return cudaSuccess;
 }
 

@@ -18,6 +18,8 @@
 // Layout and padding semantics are those of kernels_sell.cu (same SellFormat).
 // Work split: CTA b owns slices b, b+gridDim, ...; a slice wider than J steps is streamed
 // as ceil(w/J) stages.  Deterministic: each row is summed by one thread in stored order.
+#include <algorithm>
+
 #include "device_utils.cuh"
 #include "spmv_internal.h"
 #include "tma_utils.cuh"
@@ -249,8 +251,14 @@ cudaError_t sell_tma_plan(const Variant& v, int64_t rows, int64_t cols, const Se
   // goes through L1) -- same results, the variant just loses its point
   if (v.X == 2) c.add_flag(3, cols); else c.add(cols);
   c.add((int)v.H);
+  c.per_block = 1;               // slices per CTA trip; the grid is capped at the persistent size
   out->n = 1;
   if (f.split && f.nsplit > 0) { sell_split_fixup_call(f, &out->k[1]); out->n = 2; }
+  else if (v.X != 2) {
+    out->range_kind = RANGE_SELL_TMA;
+    out->range_align = std::max(f.C, f.sigma);
+    out->range_elem = f.C;
+  }
   return cudaSuccess;
 }
 

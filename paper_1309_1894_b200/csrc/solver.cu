@@ -17,14 +17,10 @@
 #include <algorithm>
 #include <chrono>
 
+#include "cg_reduce.cuh"
 #include "handle.h"
 
 namespace spmv {
-
-struct CgState {
-  double rr, bb, pq;
-  int iters, done, converged, breakdown;
-};
 
 constexpr int kCgBlock = 256;
 
@@ -48,10 +44,17 @@ __device__ __forceinline__ double cg_sum_partials(const double* __restrict__ par
   return cg_block_sum(v, s_red);
 }
 
+// Large systems: three or four kernels per iteration, every reduction finished by the last block to arrive
+// (cg_reduce.cuh), so no kernel exists only to add partials and no block re-adds them:
+//   q = A p, then st->pq = p.q: cg_dot_kernel, or -- when the SpMV kernel has the fused dot and wrote its block
+//                                partials -- the one-block cg_pq_kernel (no second pass over p and q)
+//   cg_update_kernel : x += alpha p, r -= alpha q, r.r; its last block also advances the scalars
+//   cg_pupdate_kernel: p = r + beta p
 __global__ void __launch_bounds__(kCgBlock)
 cg_init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ q, double* __restrict__ r,
-               double* __restrict__ p, double* __restrict__ part_rr, double* __restrict__ part_bb) {
-  __shared__ double s_red[kCgBlock];
+               double* __restrict__ p, double* __restrict__ part_rr, double* __restrict__ part_bb,
+               CgState* __restrict__ st, double tol, int max_iters) {
+  __shared__ double s_warp[33];
   double rr = 0.0, bb = 0.0;
   for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock) {
     const double bi = b[i], ri = bi - q[i];
@@ -60,84 +63,92 @@ cg_init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict
     rr = fma(ri, ri, rr);
     bb = fma(bi, bi, bb);
   }
-  rr = cg_block_sum(rr, s_red);
-  bb = cg_block_sum(bb, s_red);
-  if (threadIdx.x == 0) { part_rr[blockIdx.x] = rr; part_bb[blockIdx.x] = bb; }
-}
-
-__global__ void __launch_bounds__(kCgBlock)
-cg_init_final_kernel(int nb, const double* __restrict__ part_rr, const double* __restrict__ part_bb,
-                     CgState* __restrict__ st, double tol, int max_iters) {
-  __shared__ double s_red[kCgBlock];
-  const double rr = cg_sum_partials(part_rr, nb, s_red);
-  const double bb = cg_sum_partials(part_bb, nb, s_red);
-  if (threadIdx.x == 0) {
-    st->rr = rr; st->bb = bb; st->pq = 0.0;
-    st->iters = 0; st->breakdown = 0;
-    st->converged = sqrt(rr) <= tol * sqrt(bb);
-    st->done = st->converged || max_iters <= 0;
+  rr = block_sum_fixed(rr, s_warp);
+  bb = block_sum_fixed(bb, s_warp);
+  if (threadIdx.x == 0) part_bb[blockIdx.x] = bb;      // published by the fence inside grid_sum_last_block
+  double rr_all = 0.0;
+  if (grid_sum_last_block(rr, part_rr, &st->cnt_rr, s_warp, &rr_all)) {
+    double v = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) v += __ldcg(part_bb + i);
+    const double bb_all = block_sum_fixed(v, s_warp);
+    if (threadIdx.x == 0) {
+      st->rr = rr_all; st->rr_prev = rr_all; st->bb = bb_all; st->pq = 0.0;
+      st->iters = 0; st->breakdown = 0;
+      st->converged = sqrt(rr_all) <= tol * sqrt(bb_all);
+      st->done = st->converged || max_iters <= 0;
+    }
   }
 }
 
 __global__ void __launch_bounds__(kCgBlock)
 cg_dot_kernel(int64_t n, const double* __restrict__ p, const double* __restrict__ q, double* __restrict__ part,
-              const CgState* __restrict__ st) {
-  __shared__ double s_red[kCgBlock];
+              CgState* __restrict__ st) {
+  __shared__ double s_warp[33];
   if (st->done) return;
   double s = 0.0;
   for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock)
     s = fma(p[i], q[i], s);
-  s = cg_block_sum(s, s_red);
-  if (threadIdx.x == 0) part[blockIdx.x] = s;
+  s = block_sum_fixed(s, s_warp);
+  double all = 0.0;
+  if (grid_sum_last_block(s, part, &st->cnt_pq, s_warp, &all) && threadIdx.x == 0) st->pq = all;
 }
 
-// x += alpha p, r -= alpha q, partials of the new r.r  (alpha = rr / p.q from the dot partials)
-__global__ void __launch_bounds__(kCgBlock)
-cg_update_kernel(int64_t n, int nb, const double* __restrict__ part_pq, const CgState* __restrict__ st,
-                 double* __restrict__ x, double* __restrict__ r, const double* __restrict__ p,
-                 const double* __restrict__ q, double* __restrict__ part_rr) {
-  __shared__ double s_red[kCgBlock];
+// st->pq = sum of the SpMV kernel's block partials (fused dot), one block, index order
+__global__ void __launch_bounds__(1024)
+cg_pq_kernel(int n_part, const double* __restrict__ part, CgState* __restrict__ st) {
+  __shared__ double s_warp[33];
   if (st->done) return;
-  const double pq = cg_sum_partials(part_pq, nb, s_red);
-  const double alpha = pq > 0.0 ? st->rr / pq : 0.0;      // pq <= 0: not SPD; cg_step_final stops the loop
+  double v = 0.0;
+  for (int i = threadIdx.x; i < n_part; i += blockDim.x) v += part[i];
+  v = block_sum_fixed(v, s_warp);
+  if (threadIdx.x == 0) st->pq = v;
+}
+
+// r -= alpha q and the new r.r; alpha = rr / p.q.  The last block to arrive advances the scalars: every other
+// block has read the old ones by then.  x += alpha p is left to cg_pupdate_kernel, which reads p anyway
+// (p is then read once per iteration instead of twice).
+__global__ void __launch_bounds__(kCgBlock)
+cg_update_kernel(int64_t n, CgState* __restrict__ st, double* __restrict__ r, const double* __restrict__ q,
+                 double* __restrict__ part_rr, double tol, int max_iters) {
+  __shared__ double s_warp[33];
+  if (st->done) {                                         // no step this iteration: nothing for cg_pupdate_kernel either
+    if (blockIdx.x == 0 && threadIdx.x == 0) st->x_pending = 0;
+    return;
+  }
+  const double pq = st->pq;
+  const double alpha = pq > 0.0 ? st->rr / pq : 0.0;      // pq <= 0: not SPD; the loop stops below
   double rr = 0.0;
   for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock) {
-    x[i] = fma(alpha, p[i], x[i]);
     const double ri = fma(-alpha, q[i], r[i]);
     r[i] = ri;
     rr = fma(ri, ri, rr);
   }
-  rr = cg_block_sum(rr, s_red);
-  if (threadIdx.x == 0) part_rr[blockIdx.x] = rr;
-}
-
-// p = r + beta p  (beta = rr' / rr, rr' from the partials the update kernel just wrote)
-__global__ void __launch_bounds__(kCgBlock)
-cg_pupdate_kernel(int64_t n, int nb, const double* __restrict__ part_rr, const CgState* __restrict__ st,
-                  const double* __restrict__ r, double* __restrict__ p) {
-  __shared__ double s_red[kCgBlock];
-  if (st->done) return;
-  const double rr_new = cg_sum_partials(part_rr, nb, s_red);
-  const double beta = rr_new / st->rr;
-  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock)
-    p[i] = fma(beta, p[i], r[i]);
-}
-
-// one block, after every other kernel of the iteration has read the old scalars
-__global__ void __launch_bounds__(kCgBlock)
-cg_step_final_kernel(int nb, const double* __restrict__ part_pq, const double* __restrict__ part_rr,
-                     CgState* __restrict__ st, double tol, int max_iters) {
-  __shared__ double s_red[kCgBlock];
-  if (st->done) return;
-  const double pq = cg_sum_partials(part_pq, nb, s_red);
-  const double rr_new = cg_sum_partials(part_rr, nb, s_red);
-  if (threadIdx.x == 0) {
-    st->pq = pq;
-    if (!(pq > 0.0)) { st->breakdown = 1; st->done = 1; return; }
+  rr = block_sum_fixed(rr, s_warp);
+  double rr_new = 0.0;
+  if (grid_sum_last_block(rr, part_rr, &st->cnt_rr, s_warp, &rr_new) && threadIdx.x == 0) {
+    if (!(pq > 0.0)) { st->breakdown = 1; st->done = 1; st->x_pending = 0; return; }
+    st->rr_prev = st->rr;
     st->rr = rr_new;
     st->iters += 1;
+    st->x_pending = 1;
     st->converged = sqrt(rr_new) <= tol * sqrt(st->bb);
     st->done = st->converged || st->iters >= max_iters;
+  }
+}
+
+// x += alpha p (alpha = rr_old / p.q, the step cg_update_kernel took) and, unless the loop just finished,
+// p = r + beta p with beta = rr_new / rr_old
+__global__ void __launch_bounds__(kCgBlock)
+cg_pupdate_kernel(int64_t n, const CgState* __restrict__ st, double* __restrict__ x, const double* __restrict__ r,
+                  double* __restrict__ p) {
+  if (!st->x_pending) return;
+  const double alpha = st->rr_prev / st->pq;
+  const double beta = st->rr / st->rr_prev;
+  const bool more = !st->done;
+  for (int64_t i = (int64_t)blockIdx.x * kCgBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kCgBlock) {
+    const double pi = p[i];
+    x[i] = fma(alpha, pi, x[i]);
+    if (more) p[i] = fma(beta, pi, r[i]);
   }
 }
 
@@ -211,7 +222,7 @@ cg_fused_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ c
     grid.sync();                                 // p complete before the next product
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
-    st->rr = rr; st->bb = bb; st->pq = 0.0;
+    st->rr = rr; st->rr_prev = rr; st->bb = bb; st->pq = 0.0;
     st->iters = k; st->breakdown = breakdown;
     st->converged = sqrt(rr) <= stop;
     st->done = 1;
@@ -238,6 +249,39 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   memset(result, 0, sizeof(*result));
   if (n == 0) { result->converged = 1; return SPMV_OK; }
 
+  // Tune for the loop: the single-apply ranking is measured cold, the loop runs with its
+  // five vectors resident in L2 and a dot product attached to the product.  Each leader of the last spmv_tune
+  // runs a few iterations of THIS loop on a scratch solution vector; the fastest is adopted.
+  if (o.tune_loop && h->leaders.size() > 1) {
+    double* xs = (double*)h->al.alloc(sizeof(double) * (size_t)n, s);
+    if (!xs) return SPMV_ERR_ALLOC;
+    spmv_cg_opts_t po = o;
+    po.tune_loop = 0; po.tol = 1e-300; po.max_iters = 24; po.check_every = 8;
+    std::string best;
+    double best_s = 1e300;
+    const std::vector<std::string> leaders = h->leaders;
+    for (const std::string& d : leaders) {
+      Variant v;
+      std::string why;
+      if (!variant_from_string(d.c_str(), &v) || !variant_eligible(h, v, &why) || adopt_variant(h, v, s) != SPMV_OK) continue;
+      spmv_cg_result_t pr;
+      double t = 1e300;
+      for (int rep = 0; rep < 2; ++rep) {                    // the second run is the measurement
+        if (cudaMemsetAsync(xs, 0, sizeof(double) * (size_t)n, s) != cudaSuccess) break;
+        if (spmv_cg(h, d_b, xs, &po, &pr, stream) != SPMV_OK) break;
+        if (rep == 1 && pr.iters > 0) t = pr.device_seconds / pr.iters;
+      }
+      if (t < best_s) { best_s = t; best = d; }
+    }
+    cudaStreamSynchronize(s);
+    h->al.free(xs, sizeof(double) * (size_t)n);
+    Variant v;
+    if (!best.empty() && variant_from_string(best.c_str(), &v)) {
+      spmv_status_t st = adopt_variant(h, v, s);
+      if (st != SPMV_OK) return st;
+    }
+  }
+
   // small systems: one cooperative kernel for the whole solve (see cg_fused_kernel)
   int fused_blocks = 0;
   if (o.no_fused == 0 && n <= 262144 && h->A.nnz <= 4 * 1024 * 1024) {
@@ -246,13 +290,24 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
     if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)cg_fused_kernel, kCgBlock, 0) == cudaSuccess && occ > 0)
       fused_blocks = (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * occ);
   }
+  // one wave of fat blocks, grid-stride: the fence + arrival at the tail of a reducing kernel is paid per block,
+  // and with the five vectors mostly L2-resident an exact grid measured slower for the p/x update too
   const int nb = fused_blocks > 0 ? fused_blocks
                                   : (int)std::min<int64_t>((n + kCgBlock - 1) / kCgBlock, (int64_t)h->dev.sm_count * 8);
-  const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + 3 * (size_t)nb) + sizeof(CgState);
+  // partial arrays: one slot per block of whichever kernel writes them (the SpMV kernel with the fused dot
+  // runs an exact grid of >= 32 rows per block)
+  const size_t npart = std::max<size_t>((size_t)nb, (size_t)((n + 31) / 32));    // (fused: nb is the cooperative grid)
+  const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + 3 * npart) + sizeof(CgState);
   double* ws = (double*)h->al.alloc(ws_bytes, s);
   if (!ws) return SPMV_ERR_ALLOC;
-  double *r = ws, *p = r + n, *q = p + n, *part_rr = q + n, *part_bb = part_rr + nb, *part_pq = part_bb + nb;
-  CgState* st = (CgState*)(part_pq + nb);
+  double *r = ws, *p = r + n, *q = p + n, *part_rr = q + n, *part_bb = part_rr + npart, *part_pq = part_bb + npart;
+  CgState* st = (CgState*)(part_pq + npart);
+  if (cudaMemsetAsync(st, 0, sizeof(CgState), s) != cudaSuccess) { h->al.free(ws, ws_bytes); return SPMV_ERR_CUDA; }
+  // q = A p with p.q fused into the SpMV kernel's epilogue where the selected family has that form
+  LaunchPlan dot_plan;
+  int n_dot_part = 0;
+  const bool fused_dot = o.no_fused_dot == 0 && fused_blocks == 0 &&
+                         build_dot_plan(h, part_pq, &n_dot_part, &dot_plan) == SPMV_OK && (size_t)n_dot_part <= npart;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t gexec = nullptr;
@@ -267,12 +322,12 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   auto fail = [&](spmv_status_t code) { cleanup(); return code; };
   auto iteration = [&]() -> spmv_status_t {
     ApplyArgs a{1.0, 0.0, p, q, s};
-    spmv_status_t st1 = launch_plan(h->plan, a);                       // q = A p
+    spmv_status_t st1 = launch_plan(fused_dot ? dot_plan : h->plan, a);      // q = A p  [+ st->pq = p.q]
     if (st1 != SPMV_OK) return st1;
-    cg_dot_kernel<<<nb, kCgBlock, 0, s>>>(n, p, q, part_pq, st);
-    cg_update_kernel<<<nb, kCgBlock, 0, s>>>(n, nb, part_pq, st, d_x, r, p, q, part_rr);
-    cg_pupdate_kernel<<<nb, kCgBlock, 0, s>>>(n, nb, part_rr, st, r, p);
-    cg_step_final_kernel<<<1, kCgBlock, 0, s>>>(nb, part_pq, part_rr, st, tol, max_iters);
+    if (fused_dot) cg_pq_kernel<<<1, 1024, 0, s>>>(n_dot_part, part_pq, st);
+    else cg_dot_kernel<<<nb, kCgBlock, 0, s>>>(n, p, q, part_pq, st);
+    cg_update_kernel<<<nb, kCgBlock, 0, s>>>(n, st, r, q, part_rr, tol, max_iters);
+    cg_pupdate_kernel<<<nb, kCgBlock, 0, s>>>(n, st, d_x, r, p);     // (measured: programmatic dependent launches gain nothing here)
     return cudaGetLastError() == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
   };
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(SPMV_ERR_CUDA);
@@ -300,8 +355,7 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
     spmv_status_t st1 = launch_plan(h->plan, a);                       // q = A x0
     if (st1 != SPMV_OK) return fail(st1);
   }
-  cg_init_kernel<<<nb, kCgBlock, 0, s>>>(n, d_b, q, r, p, part_rr, part_bb);
-  cg_init_final_kernel<<<1, kCgBlock, 0, s>>>(nb, part_rr, part_bb, st, tol, max_iters);
+  cg_init_kernel<<<nb, kCgBlock, 0, s>>>(n, d_b, q, r, p, part_rr, part_bb, st, tol, max_iters);
   if (cudaGetLastError() != cudaSuccess) return fail(SPMV_ERR_CUDA);
   auto poll = [&]() -> bool {
     return cudaMemcpyAsync(&hs, st, sizeof(hs), cudaMemcpyDeviceToHost, s) == cudaSuccess &&
@@ -349,7 +403,10 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   result->wall_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
   result->iterations_launched = launched;
   result->graph_replays = graph_replays;
+  strncpy(result->loop_variant, variant_to_string(h->sel).c_str(), sizeof(result->loop_variant) - 1);
   result->fused = fused_blocks > 0;
+  result->fused_dot = fused_dot ? 1 : 0;
+  result->kernels_per_iteration = fused_blocks > 0 ? 0 : 4 + (h->plan.n > 1 ? h->plan.n - 1 : 0);
   cleanup();
   return SPMV_OK;
 }

@@ -148,7 +148,14 @@ struct KernelCall {
   // aligned), 3: int64 = flag_val if x is 16-byte aligned else 0
   int flag_idx[2] = {-1, -1}, flag_kind[2] = {0, 0};
   int64_t flag_val = 0;
+  // row-range launches (spmv_apply_host pipelines chunks of rows): element offsets added to x / y when the
+  // pointers are patched, and the rows (slices, block rows) one block covers, to size a range's grid
+  int64_t x_off = 0, y_off = 0, per_block = 0;
   alignas(16) unsigned char store[1280];
+  template <typename T>
+  void set(int i, const T& v) { memcpy(store + off[i], &v, sizeof(T)); }
+  template <typename T>
+  T get(int i) const { T v; memcpy(&v, store + off[i], sizeof(T)); return v; }
   template <typename T>
   int add(const T& v) {
     used = (int)((used + alignof(T) - 1) / alignof(T) * alignof(T));
@@ -168,13 +175,22 @@ struct KernelCall {
     flag_idx[slot] = kind == 3 ? add((int64_t)0) : add((int)0);
   }
 };
+// how (whether) a plan can be re-aimed at a range of rows: which arguments shift (variants.cu: plan_for_rows)
+enum RangeKind { RANGE_NONE = 0, RANGE_CSR, RANGE_BCSR, RANGE_SELL, RANGE_SELL_TMA, RANGE_DIA, RANGE_DIA_TMA, RANGE_DIA_CONST };
 struct LaunchPlan {
+  int range_kind = RANGE_NONE;
+  int range_align = 1;           // range boundaries are multiples of this many rows
+  int range_elem = 0;            // kind-specific (DIA: diagonals; dia_const: bytes per mask word)
   int n = 0;                     // kernel launches per apply (0: nothing to do)
   KernelCall k[2];               // [1]: the ordered fix-up of merge-path / row-split SELL
   bool has_alt = false;          // alt replaces k[0] when x or y is not 16-byte aligned (dia_const pairs)
   KernelCall alt;
 };
 cudaError_t run_plan(const LaunchPlan& p, const ApplyArgs& a);
+cudaError_t run_call(const KernelCall& c, const ApplyArgs& a);
+// the plan's kernel call re-aimed at rows [a, b) (a a multiple of range_align; b too, or b == rows); the x / y
+// pointers passed at run time stay those of the WHOLE vectors.  false: this plan has no range form.
+bool plan_for_rows(const LaunchPlan& p, int64_t rows, int64_t cols, int64_t a, int64_t b, bool aligned, KernelCall* out);
 // grid for "g waves of resident blocks" (Variant::grid > 0), capped at the exact cover; sets nothing
 cudaError_t resolve_grid(int g, const void* fn, int block, size_t smem, int sm_count, int64_t exact, unsigned* grid);
 // cudaFuncAttributeMaxDynamicSharedMemorySize (per device and function: set at every plan build)
@@ -201,6 +217,9 @@ bool dia_supported(const Variant&);
 cudaError_t dia_plan(const Variant&, int64_t rows, const DiaFormat&, int sm_count, LaunchPlan*);
 bool dia_const_supported(const Variant&);
 cudaError_t dia_const_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, LaunchPlan*);
+// y = alpha*A*x + beta*y AND part[b] = block b's share of sum_i x_i*y_i (square matrix); *n_part = blocks
+cudaError_t dia_const_dot_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, double* part,
+                               int* n_part, LaunchPlan*);
 bool dia_win_supported(const Variant&);
 bool dia_win_fits(const Variant&, const DiaFormat&);
 cudaError_t dia_win_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, int sm_count, LaunchPlan*);

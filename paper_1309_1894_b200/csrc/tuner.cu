@@ -361,6 +361,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
       if (variant_from_string(it->second.variant.c_str(), &v) && variant_eligible(h, v, &why) &&
           adopt_variant(h, v, T.s) == SPMV_OK) {
         h->tuned = true;
+        h->leaders.assign(1, it->second.variant);
         handle_refresh_info(h);
         if (report) {
           strncpy(report->winner, it->second.variant.c_str(), sizeof(report->winner) - 1);
@@ -518,6 +519,17 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     return SPMV_ERR_VERIFY_FAILED;
   }
   const Scored win = ok[0];
+  h->leaders.clear();
+  for (size_t i = 0; i < ok.size() && h->leaders.size() < 3; ++i) {
+    // distinct kernels: a grid / carve-out sibling of a leader is not another leader
+    Variant base = ok[i].v; base.grid = 0; base.carve = -1;
+    bool dup = false;
+    for (const std::string& d : h->leaders) {
+      Variant q; variant_from_string(d.c_str(), &q); q.grid = 0; q.carve = -1;
+      dup |= variant_to_string(q) == variant_to_string(base);
+    }
+    if (!dup) h->leaders.push_back(variant_to_string(ok[i].v));
+  }
   st = adopt_variant(h, win.v, T.s);
   if (st != SPMV_OK) return fail(st);
   h->tuned = true;

@@ -349,7 +349,10 @@ cudaError_t allow_smem(const void* fn, size_t smem) {
   return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
 
-static inline cudaError_t run_call(const KernelCall& c, const ApplyArgs& a) {
+cudaError_t run_call(const KernelCall& c, const ApplyArgs& a0) {
+  ApplyArgs a = a0;
+  a.x = a0.x ? a0.x + c.x_off : a0.x;
+  a.y = a0.y ? a0.y + c.y_off : a0.y;
   // private copy of the argument block: concurrent applies of one handle never share mutable state
   alignas(16) unsigned char buf[sizeof(c.store)];
   memcpy(buf, c.store, (size_t)c.used);
@@ -378,6 +381,85 @@ cudaError_t run_plan(const LaunchPlan& p, const ApplyArgs& a) {
   cudaError_t e = run_call(aligned ? p.k[0] : p.alt, a);
   if (e == cudaSuccess && p.n > 1) e = run_call(p.k[1], a);
   return e;
+}
+
+// The plan's kernel re-aimed at rows [a, b): counts shrink, the format pointers move to the first row (slice,
+// block row) of the range, x / y get element offsets, the grid covers the range.  Argument positions are those
+// the families' *_plan functions build (kernels_*.cu).
+bool plan_for_rows(const LaunchPlan& p, int64_t rows, int64_t cols, int64_t a, int64_t b, bool aligned, KernelCall* out) {
+  if (p.n != 1 || p.range_kind == RANGE_NONE || a < 0 || b > rows || a >= b || a % p.range_align) return false;
+  if (b != rows && b % p.range_align) return false;
+  KernelCall c = (p.has_alt && !aligned) ? p.alt : p.k[0];
+  int64_t units = b - a;
+  auto shift = [&](int i, int64_t bytes) {
+    const char* ptr = c.get<const char*>(i);
+    if (ptr) c.set(i, ptr + bytes);
+  };
+  switch (p.range_kind) {
+    case RANGE_CSR:                      // rows, row_ptr (absolute positions: col_idx / val stay)
+      c.set(0, (int)(b - a));
+      shift(1, 4 * a);
+      c.y_off = a;
+      break;
+    case RANGE_BCSR:                     // block rows, brow_ptr
+      c.set(0, (int)((b - a) / 3));
+      shift(1, 4 * (a / 3));
+      c.y_off = a;
+      units = (b - a) / 3;
+      break;
+    case RANGE_SELL:
+    case RANGE_SELL_TMA: {               // slices [s0, s1)
+      const int C = p.range_elem;
+      const int64_t s0 = a / C, s1 = (b + C - 1) / C;
+      const bool tma = p.range_kind == RANGE_SELL_TMA;
+      const int i_sp = tma ? 3 : 4, i_sbase = tma ? 6 : 7, i_perm = tma ? 7 : 8;
+      const bool perm = c.get<const int*>(i_perm) != nullptr;
+      c.set(0, (int64_t)(b - a));                                    // rows of the range (no permutation: row < rows)
+      c.set(1, tma ? (int64_t)(s1 - s0) : (int64_t)(s1 - s0) * C);   // slices | padded rows
+      shift(i_sp, 8 * s0);
+      shift(i_sbase, 4 * s0);
+      shift(i_perm, 4 * s0 * C);
+      c.y_off = perm ? 0 : a;                                        // perm holds absolute rows
+      units = tma ? (s1 - s0) : (s1 - s0) * C;
+      break;
+    }
+    case RANGE_DIA: {                    // rows, ld, dval, mask
+      const int C = p.range_align, nd = p.range_elem;
+      const int64_t ld = (b - a + C - 1) / C * C;
+      c.set(0, (int64_t)(b - a));
+      c.set(1, ld);
+      shift(6, 8 * (a / C) * nd * C);
+      shift(7, 4 * a);
+      c.x_off = a; c.y_off = a;
+      units = ld;
+      break;
+    }
+    case RANGE_DIA_TMA: {                // rows, xlo, xhi, nslices, dval, mask
+      const int C = p.range_align, nd = p.range_elem;
+      const int64_t ns = (b - a + C - 1) / C;
+      c.set(0, (int64_t)(b - a));
+      c.set(1, (int64_t)-a);
+      c.set(2, (int64_t)(cols - 1 - a));
+      c.set(3, ns);
+      shift(7, 8 * (a / C) * nd * C);
+      shift(8, 4 * a);
+      c.x_off = a; c.y_off = a;
+      units = ns * C;
+      break;
+    }
+    case RANGE_DIA_CONST:                // rows, xlo, xhi, mask (range_elem bytes per word)
+      c.set(0, (int)(b - a));
+      c.set(1, (int)-a);
+      c.set(2, (int)(cols - 1 - a));
+      shift(6, (int64_t)p.range_elem * a);
+      c.x_off = a; c.y_off = a;
+      break;
+    default: return false;
+  }
+  const int64_t g = (units + c.per_block - 1) / std::max<int64_t>(c.per_block, 1);
+  c.grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(g, c.grid));
+  *out = c;
+  return true;
 }
 
 // Resolves everything a launch of `v` on this handle needs (the format must exist).  The carve-out
@@ -439,6 +521,16 @@ spmv_status_t build_plan(spmv_handle_s* h, const Variant& v, LaunchPlan* out) {
     set_last_error("cannot prepare the launch of %s: %s", variant_to_string(v).c_str(), cudaGetErrorString(e));
     return SPMV_ERR_CUDA;
   }
+  return SPMV_OK;
+}
+
+spmv_status_t build_dot_plan(spmv_handle_s* h, double* part, int* n_part, LaunchPlan* out) {
+  const Variant& v = h->sel;
+  if (v.fam != FAM_DIA_CONST || v.X != 0) return SPMV_ERR_UNSUPPORTED;
+  auto it = h->dias.find(v.C);
+  if (it == h->dias.end()) return SPMV_ERR_UNSUPPORTED;
+  cudaError_t e = dia_const_dot_plan(v, h->A.rows, h->A.cols, it->second, part, n_part, out);
+  if (e != cudaSuccess) { cudaGetLastError(); return SPMV_ERR_UNSUPPORTED; }
   return SPMV_OK;
 }
 

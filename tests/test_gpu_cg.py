@@ -40,6 +40,9 @@ def test_cg_solves_the_laplacian_like_the_oracle(cuda, desc):
         stream.synchronize()
         x = dx.cpu().numpy()
         assert res["converged"] == 1 and res["breakdown"] == 0 and res["graph_replays"] >= 1 and res["fused"] == 0
+        # p.q comes out of the SpMV epilogue for dia_const (no second pass over p and q), from a dot kernel otherwise
+        assert res["fused_dot"] == (1 if desc.startswith("dia_const") else 0)
+        assert res["kernels_per_iteration"] == (5 if desc.startswith("merge") else 4)
         assert abs(res["iters"] - k_ref) <= 3, (res, k_ref)
         assert res["rel_residual"] <= tol
         assert _true_rel_res(A, x, b) <= 2 * tol              # recurrence residual ~ true residual
@@ -140,3 +143,46 @@ def test_cg_fused_single_kernel_for_small_systems(cuda):
         assert res3["fused"] == 0 and abs(res3["iters"] - res["iters"]) <= 5
         assert np.abs(dx3.cpu().numpy() - x).max() <= 2 * tol * cond * np.abs(x).max()
         S.close()
+
+
+def test_cg_fused_dot_equals_separate_dot_and_loop_tuning(cuda):
+    """(i) the dot product fused into the dia_const kernel gives a valid CG run next to the
+    separate dot kernel (another summation shape: compared through the solution, not bitwise); (ii) tune_loop
+    times the leaders of spmv_tune inside the iteration and adopts one of them; the solve is still right."""
+    import torch
+    A = W.laplace3d_7pt(72)                                   # 373 248 rows: above the single-kernel limit
+    xt = W.uniform(131, A.rows)
+    b, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, xt, 0.0)
+    tol = 1e-9
+    S = binding.SpMV.from_csr(A)
+    rep = S.tune(alpha=1.0, beta=0.0, use_cache=2, reps=2, min_batch_ms=0.1, search=1)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        db = H.to_dev(b)
+        S.select("dia_const:b256:r1:x0")
+        out = {}
+        for key, kw in (("fused", {}), ("separate", {"no_fused_dot": True})):
+            dx = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
+            res = S.cg(db, dx, tol=tol, max_iters=2000, **kw)
+            torch.cuda.current_stream().synchronize()
+            out[key] = (res, dx.cpu().numpy())
+            assert res["converged"] == 1 and res["fused"] == 0
+            assert _true_rel_res(A, out[key][1], b) <= 2 * tol
+        assert out["fused"][0]["fused_dot"] == 1 and out["fused"][0]["kernels_per_iteration"] == 4
+        assert out["separate"][0]["fused_dot"] == 0 and out["separate"][0]["kernels_per_iteration"] == 4
+        assert abs(out["fused"][0]["iters"] - out["separate"][0]["iters"]) <= 3
+        assert np.abs(out["fused"][1] - out["separate"][1]).max() <= 2 * tol * 2200 * np.abs(xt).max()
+        # repeat of the fused form: bit-identical (fixed reduction shape, last-block sums in index order)
+        dx2 = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
+        res2 = S.cg(db, dx2, tol=tol, max_iters=2000)
+        torch.cuda.current_stream().synchronize()
+        assert np.array_equal(dx2.cpu().numpy(), out["fused"][1]) and res2["iters"] == out["fused"][0]["iters"]
+    # tune for the loop: needs the leaders of a tune in this process
+    T = binding.SpMV.from_csr(A)
+    rep = T.tune(alpha=1.0, beta=0.0, use_cache=2, reps=2, min_batch_ms=0.1, search=1)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        dx = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
+        res = T.cg(H.to_dev(b), dx, tol=tol, max_iters=2000, tune_loop=True)
+        torch.cuda.current_stream().synchronize()
+        assert res["converged"] == 1 and res["loop_variant"] == T.variant and len(res["loop_variant"]) > 0
+        assert _true_rel_res(A, dx.cpu().numpy(), b) <= 2 * tol
+    S.close(); T.close()

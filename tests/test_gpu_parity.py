@@ -142,6 +142,49 @@ def test_apply_host_matches_device_apply(cuda):
     S.close()
 
 
+@pytest.mark.parametrize("which", ["stencil7", "fem", "banded"])
+def test_apply_host_pipeline_is_bit_identical_to_device_apply(cuda, which):
+    """spmv_apply_host pipelines chunks of rows (upload | kernel on a row range | download) where the variant
+    has a range form.  Large enough for several chunks (~2 MB of y each) with a ragged last one; every family's
+    range launch must reproduce the one-launch result bit for bit, for beta == 0 and beta != 0, and match the
+    oracle."""
+    import torch
+    if which == "stencil7":
+        A = W.laplace3d_7pt(93)                                # 804 357 rows: odd, not a multiple of any slice height
+        descs = ["default", "csr_vector:b256:w8:u2:x0", "sell:b256:c128:s1:r2:u4:x0", "sell:b256:c128:s1024:r1:u2:x0",
+                 "sell_tma:b288:c256:s1:r1:u8:i3:x0", "sell_tma:b160:c128:s512:r1:u4:i4:x0", "sell16:b256:c128:s1:r2:u4:x0",
+                 "sell16_tma:b288:c256:s1:r1:u8:i3:x0", "dia:b256:c128:r2:u4:x0", "dia_tma:b288:c256:r1:u7:i3:x0",
+                 "dia_const:b256:r1:x0", "dia_const:b128:r2:x0", "dia_const:b256:r4:x0",
+                 "merge:b256:i7:x0", "ell:b256:r1:u2:x0"]       # the last two have no range form: one launch
+    elif which == "fem":
+        A = W.fem_block27(56)                                  # 526 848 rows, dense 3x3 blocks
+        descs = ["bcsr3:b256:w8:u2:x0", "bcsr3:b512:w16:u2:x0:g1", "csr_vector:b256:w32:u2:x0"]
+    else:
+        A = W.banded_random(700001, 9, 1500, stream=83)
+        descs = ["sell16:b256:c512:s1:r4:u2:x0", "sell16_tma:b544:c512:s1:r1:u4:i4:x0", "sell:b128:c128:s8192:r1:u2:x0", "csr_scalar:b256:r2:u2:x0:g2"]
+    x, y0 = W.uniform(84, A.cols), W.uniform(85, A.rows)
+    S = binding.SpMV.from_csr(A)
+    xh = torch.from_numpy(x).pin_memory()
+    ref = {}
+    for beta in (0.0, -0.75):
+        ref[beta] = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.25, x, beta, None if beta == 0.0 else y0, parallel=True)
+    for desc in descs:
+        S.select(desc)
+        for beta in (0.0, -0.75):
+            y_dev = H.gpu_apply(S, 1.25, x, beta, None if beta == 0.0 else y0)
+            yh = torch.from_numpy(np.full(A.rows, np.nan) if beta == 0.0 else y0.copy()).pin_memory()
+            S.apply_host(1.25, xh, beta, yh)
+            assert np.array_equal(yh.numpy(), y_dev), (desc, beta)
+            assert oracle.accept(yh.numpy(), ref[beta][0], ref[beta][1], H.TOL)[0], (desc, beta)
+    # pageable (unpinned) host memory and an unaligned host pointer work too
+    S.select(descs[0])
+    xu = np.empty(A.cols + 1); xu[1:] = x
+    yu = np.empty(A.rows + 1); yu[1:] = y0
+    S.apply_host(1.25, xu[1:], -0.75, yu[1:])
+    assert oracle.accept(yu[1:], ref[-0.75][0], ref[-0.75][1], H.TOL)[0]
+    S.close()
+
+
 @pytest.mark.slow
 def test_tma_pipeline_race_regression_full_size(cuda):
     """Regression: on full-size cfg5 with sorted slices the TMA refill (async proxy) used to land

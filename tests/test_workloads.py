@@ -98,3 +98,18 @@ def test_byte_model_matches_survey_table():
     g = json.load(open(GOLDEN))
     assert W.algorithmic_bytes(4096, 4096, 20224, 0.0) == g["cfg1"]["bytes"] == 324612
     assert W.algorithmic_bytes(2097152, 2097152, 14581760, 0.5) == g["cfg2"]["bytes"]
+
+
+def test_banded_random_structure():
+    """banded_random: fixed row length, distinct sorted columns inside the clipped band, reproducible."""
+    A = W.banded_random(3000, 12, 400, stream=7)
+    lens = A.row_lengths()
+    assert (lens == 12).all() and A.nnz == 36000
+    rid = np.repeat(np.arange(A.rows), lens)
+    d = A.col_idx.astype(np.int64) - rid
+    assert d.min() >= -400 and d.max() <= 400 and A.col_idx.min() >= 0 and A.col_idx.max() < A.cols
+    key = (rid.astype(np.int64) << 32) | A.col_idx
+    assert (np.diff(key) > 0).all()                       # sorted, no duplicates within a row
+    assert np.unique(d).size > 32                         # far more diagonals than DIA admits
+    B = W.banded_random(3000, 12, 400, stream=7)
+    assert np.array_equal(A.col_idx, B.col_idx) and np.array_equal(A.val, B.val)
