@@ -525,6 +525,63 @@ def bench_banded(args, torch, binding, W, device):
     return out
 
 
+def bench_sharded(args, torch, binding, W, dist_max, device, world, rank):
+    """--sharded: ONE matrix row-sharded over the N GPUs (strong scaling), instead of the default
+    N independent replicas.  Every rank builds the same seeded matrix and keeps its nnz-balanced row block; a step
+    is one sharded apply: halo exchange (torch.distributed point-to-point over NCCL) overlapped with the interior
+    rows, then the boundary rows.  Time: CUDA events on the launching stream, barrier on both sides, max over ranks."""
+    from paper_1309_1894_b200 import sharded
+    cfg = int(args.configs.split(",")[0])
+    prob = W.config(cfg)
+    A = prob.A
+    transport = sharded.TorchDistTransport() if world > 1 else sharded.LoopbackTransport(1).view(0)
+    align = 768 if cfg == 4 else 512
+    sh = sharded.ShardedSpMV(A, transport, device=device, align=align)
+    sh.finish_setup()
+    l2 = torch.cuda.get_device_properties(device).L2_cache_size
+    rep = sh.tune(alpha=prob.alpha, beta=prob.beta, use_cache=2, seed=cfg,
+                  flush_l2=(12 * sh.nnz_local + 24 * sh.rows_local < 4 * l2))
+    sh.x_owned.copy_(torch.from_numpy(prob.x[sh.lo:sh.hi]))
+    y0 = prob.y0 if prob.y0 is not None else np.zeros(A.rows)
+    y = torch.from_numpy(y0[sh.lo:sh.hi].copy()).to(device)
+    for _ in range(args.warmup):
+        sh.apply(prob.alpha, prob.beta, y)
+    torch.cuda.synchronize()
+    dist_max(0.0)
+    ts = []
+    while sum(ts) * args.steps * 1e3 < args.min_ms and len(ts) < 400 or not ts:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            sh.apply(prob.alpha, prob.beta, y)
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(dist_max(a.elapsed_time(b) * 1e-3 / args.steps))
+    t = float(np.median(ts))
+    # parity of this rank's block against the oracle on sampled rows (one apply from y0)
+    y.copy_(torch.from_numpy(y0[sh.lo:sh.hi]))
+    sh.apply(prob.alpha, prob.beta, y)
+    torch.cuda.synchronize()
+    sub = W.CSR(sh.rows_local, A.cols, (A.row_ptr[sh.lo:sh.hi + 1].astype(np.int64) - int(A.row_ptr[sh.lo])).astype(np.int32),
+                A.col_idx[int(A.row_ptr[sh.lo]):int(A.row_ptr[sh.hi])], A.val[int(A.row_ptr[sh.lo]):int(A.row_ptr[sh.hi])])
+    chk = oracle_check(W.Problem(prob.name, sub, prob.x, None if prob.y0 is None else y0[sh.lo:sh.hi], prob.alpha, prob.beta),
+                       y.cpu().numpy())
+    if not chk["ok"]:
+        raise SystemExit(f"bench --sharded: rank {rank} FAILED the oracle check: {chk}")
+    nbytes = W.algorithmic_bytes(A.rows, A.cols, A.nnz, prob.beta)
+    line = {"metric": METRIC, "value": nbytes / t / 1e9, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": headline_config(W, cfg, A.rows, A.nnz),
+            "selection": {"variant_rank0": rep["winner"], "parallelism": f"rows sharded over {world} GPUs, halo exchange + interior overlap",
+                          "rows_rank0": sh.rows_local, "halo_bytes_rank0": sh.halo.bytes_received(),
+                          "interior_split_rank0": sh.split},
+            "gpu_launches": args.steps * len(ts) * (1 if sh.split is None else 3), "parity": chk,
+            "timed_batches": len(ts), "gflops": 2.0 * A.nnz / t / 1e9}
+    if rank == 0:
+        print(json.dumps(line))
+    sh.close()
+
+
 def config_roofline(r, peak, ceil):
     """What bounds this config's winner and the fraction of that bound."""
     if r["cfg"] == 1:       # 0.1 MB per apply: launch-latency-bound (SURVEY sec. 8(d))
@@ -586,6 +643,8 @@ def main():
     ap.add_argument("--min-ms", type=float, default=50.0, help="batches of --steps repeat until the timed region lasts this long")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-oracle-check", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: row-shard ONE matrix (the first of --configs) over the GPUs instead of N replicas")
     ap.add_argument("--no-extras", action="store_true", help="skip the banded-matrix line (16-bit vs 32-bit column indices)")
     ap.add_argument("--variant-filter", default=None,
                     help="comma list of descriptor prefixes the tuner may use (spmv_tune variant_filter), e.g. "
@@ -623,6 +682,12 @@ def main():
     from paper_1309_1894_b200.dist import make_dist_max
     dist_max = make_dist_max(torch, world, device)
 
+    if args.sharded:
+        bench_sharded(args, torch, binding, W, dist_max, device, world, rank)
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
     cfgs = [int(c) for c in args.configs.split(",")]
     results = []
     for cfg in cfgs:

@@ -190,6 +190,31 @@ SPMV_API spmv_status_t spmv_graph_create(spmv_handle_t h, double alpha, const do
 SPMV_API spmv_status_t spmv_graph_launch(spmv_graph_t g, void* stream);
 SPMV_API spmv_status_t spmv_graph_destroy(spmv_graph_t g);
 
+/* ---- Row-sharded apply: rows are independent, so A and y split into
+ * nnz-balanced contiguous row blocks, one per GPU; before an apply each GPU needs the x entries its columns
+ * reference and does not own.  The library provides the compute-side pieces; the transport between processes
+ * is torch.distributed (NCCL over NVLink) in paper_1309_1894_b200/sharded.py.
+ *
+ * spmv_partition_rows: bounds[0..nparts] with bounds[0] = 0, bounds[nparts] = rows, interior bounds multiples
+ *   of `align`, chosen so that part g holds about nnz/nparts stored entries (h_row_ptr is a HOST array).
+ * spmv_external_columns: the sorted distinct columns referenced by the handle's matrix outside [own_lo, own_hi)
+ *   -- the halo this shard must receive.  *count receives their number; at most cap are written to h_cols (HOST).
+ *   Also reports, per row, whether it references an external column: [*int_lo, *int_hi) is the longest run of
+ *   rows that do not (the interior, computable before the halo arrives).  Synchronises `stream`.
+ * spmv_gather / spmv_scatter: dst[i] = src[idx[i]] / dst[idx[i]] = src[i] for i < n (device arrays, idx int32):
+ *   packing the entries a peer needs, unpacking what arrived.  Asynchronous on `stream`.
+ * spmv_apply_rows: spmv_apply restricted to rows [row_begin, row_end) (d_x, d_y: the whole vectors).  row_begin
+ *   must be a multiple of *align_out = the selected variant's range alignment (query with row_begin = row_end);
+ *   UNSUPPORTED when the variant has no row-range form (merge-path, row-split SELL, ELL, dia_win). */
+SPMV_API spmv_status_t spmv_partition_rows(int64_t rows, const int32_t* h_row_ptr, int32_t nparts, int64_t align,
+                                  int64_t* h_bounds);
+SPMV_API spmv_status_t spmv_external_columns(spmv_handle_t h, int64_t own_lo, int64_t own_hi, int32_t* h_cols,
+                                    int64_t cap, int64_t* count, int64_t* int_lo, int64_t* int_hi, void* stream);
+SPMV_API spmv_status_t spmv_gather(int64_t n, const int32_t* d_idx, const double* d_src, double* d_dst, void* stream);
+SPMV_API spmv_status_t spmv_scatter(int64_t n, const int32_t* d_idx, const double* d_src, double* d_dst, void* stream);
+SPMV_API spmv_status_t spmv_apply_rows(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y,
+                              int64_t row_begin, int64_t row_end, int64_t* align_out, void* stream);
+
 /* n independent applies, handle i on streams[i % nstreams] ("number of
  * asynchronous streams").  No synchronisation. */
 SPMV_API spmv_status_t spmv_apply_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,

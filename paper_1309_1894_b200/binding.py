@@ -22,7 +22,8 @@ EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_ap
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
            "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache", "spmv_graph_create", "spmv_graph_launch",
-           "spmv_graph_destroy"]
+           "spmv_graph_destroy", "spmv_partition_rows", "spmv_external_columns", "spmv_gather", "spmv_scatter",
+           "spmv_apply_rows"]
 
 
 class SpmvError(RuntimeError):
@@ -113,10 +114,16 @@ def lib():
     L.spmv_graph_create.argtypes = [vp, dbl, vp, dbl, vp, i32, C.POINTER(vp)]
     L.spmv_graph_launch.argtypes = [vp, vp]
     L.spmv_graph_destroy.argtypes = [vp]
+    L.spmv_partition_rows.argtypes = [i64, vp, i32, i64, vp]
+    L.spmv_external_columns.argtypes = [vp, i64, i64, vp, i64, C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]
+    L.spmv_gather.argtypes = [i64, vp, vp, vp, vp]
+    L.spmv_scatter.argtypes = [i64, vp, vp, vp, vp]
+    L.spmv_apply_rows.argtypes = [vp, dbl, vp, dbl, vp, i64, i64, C.POINTER(i64), vp]
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
               "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg",
-              "spmv_graph_create", "spmv_graph_launch", "spmv_graph_destroy"):
+              "spmv_graph_create", "spmv_graph_launch", "spmv_graph_destroy", "spmv_partition_rows",
+              "spmv_external_columns", "spmv_gather", "spmv_scatter", "spmv_apply_rows"):
         getattr(L, n).restype = C.c_int
     L.spmv_status_string.argtypes = [C.c_int]
     L.spmv_status_string.restype = C.c_char_p
@@ -262,6 +269,30 @@ class SpMV:
         out["loop_variant"] = out["loop_variant"].decode()
         return out
 
+    def apply_rows(self, alpha, x, beta, y, row_begin: int, row_end: int, stream=None):
+        """spmv_apply restricted to rows [row_begin, row_end); x, y are the whole vectors."""
+        al = C.c_int64(0)
+        _check(lib().spmv_apply_rows(self.h, float(alpha), _dptr(x), float(beta), _dptr(y), int(row_begin), int(row_end),
+                                     C.byref(al), _stream_ptr(stream)), "spmv_apply_rows")
+        return y
+
+    def range_align(self) -> int:
+        """Row alignment of the selected variant's row-range form (0: it has none)."""
+        al = C.c_int64(0)
+        _check(lib().spmv_apply_rows(self.h, 1.0, None, 0.0, None, 0, 0, C.byref(al), None), "spmv_apply_rows")
+        return int(al.value)
+
+    def external_columns(self, own_lo: int, own_hi: int):
+        """(sorted int32 array of the columns referenced outside [own_lo, own_hi), (interior_lo, interior_hi))."""
+        n, a, b = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        _check(lib().spmv_external_columns(self.h, int(own_lo), int(own_hi), None, 0, C.byref(n), C.byref(a), C.byref(b),
+                                           _stream_ptr()), "spmv_external_columns")
+        out = np.empty(n.value, dtype=np.int32)
+        if n.value:
+            _check(lib().spmv_external_columns(self.h, int(own_lo), int(own_hi), C.c_void_p(out.ctypes.data), n.value,
+                                               C.byref(n), C.byref(a), C.byref(b), _stream_ptr()), "spmv_external_columns")
+        return out, (int(a.value), int(b.value))
+
     def graph(self, alpha, x, beta, y, k: int) -> "Graph":
         """k back-to-back applies captured into one CUDA graph (spmv_graph_create); x, y are baked in."""
         assert x.is_cuda and y.is_cuda and x.numel() == self.cols and y.numel() == self.rows
@@ -381,6 +412,27 @@ def tune_batch(handles, alphas, xs, betas, ys, streams):
         c *= 2
         i += 1
     return best.value, counts
+
+
+def partition_rows(row_ptr: np.ndarray, nparts: int, align: int = 1) -> np.ndarray:
+    """spmv_partition_rows: nnz-balanced contiguous row blocks; returns int64 bounds [nparts + 1]."""
+    rp = np.ascontiguousarray(row_ptr, dtype=np.int32)
+    out = np.zeros(nparts + 1, dtype=np.int64)
+    _check(lib().spmv_partition_rows(rp.size - 1, C.c_void_p(rp.ctypes.data), int(nparts), int(align),
+                                     C.c_void_p(out.ctypes.data)), "spmv_partition_rows")
+    return out
+
+
+def gather(idx, src, dst, stream=None):
+    """dst[i] = src[idx[i]] (CUDA tensors; idx int32): the library's pack kernel."""
+    assert idx.is_cuda and src.is_cuda and dst.is_cuda and dst.numel() >= idx.numel()
+    _check(lib().spmv_gather(idx.numel(), _dptr(idx), _dptr(src), _dptr(dst), _stream_ptr(stream)), "spmv_gather")
+
+
+def scatter(idx, src, dst, stream=None):
+    """dst[idx[i]] = src[i] (CUDA tensors; idx int32): the library's unpack kernel."""
+    assert idx.is_cuda and src.is_cuda and dst.is_cuda and src.numel() >= idx.numel()
+    _check(lib().spmv_scatter(idx.numel(), _dptr(idx), _dptr(src), _dptr(dst), _stream_ptr(stream)), "spmv_scatter")
 
 
 def measure_ceiling(kind: int, nbytes: int = 1 << 30, reps: int = 10) -> float:
