@@ -149,7 +149,9 @@ typedef struct {
   char runner_up[128];
   double runner_up_us;
   /* optional per-candidate log: "descriptor status time_us max_err_over_scale\n"; status in
-   * {timed, timed1 (one batch only: > 25 % behind the leader), pruned_slow, pruned_format, rejected} */
+   * {timed, timed1 (one batch only: > 25 % behind the leader), retimed (tie-break: within 2 % of the best, timed
+   * again with 3x the batches; a tie within 0.5 % goes to the lexicographically smallest descriptor),
+   * pruned_slow, pruned_format, rejected} */
   char* log_buf;
   size_t log_cap;
   size_t log_len;

@@ -45,6 +45,64 @@ __global__ void scan_inclusive_kernel(T* __restrict__ a, int64_t n) {
   }
 }
 
+// ---- multi-block form: tiles of 1024 entries scanned in place, the tile totals scanned by the single-block
+// kernel above, then added back.  In place over a[1..n]; a[0] must already hold 0.
+template <typename T>
+__global__ void __launch_bounds__(1024) scan_tiles_kernel(T* __restrict__ a, int64_t n, T* __restrict__ totals) {
+  __shared__ T s_w[32];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int64_t i = 1 + (int64_t)blockIdx.x * 1024 + tid;
+  T v = i <= n ? a[i] : 0;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    T u = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += u;
+  }
+  if (lane == 31) s_w[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    T x = s_w[lane];
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      T u = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += u;
+    }
+    s_w[lane] = x;
+  }
+  __syncthreads();
+  v += w > 0 ? s_w[w - 1] : 0;
+  if (i <= n) a[i] = v;
+  if (tid == 1023) totals[blockIdx.x + 1] = v;      // totals[0] = 0 is set by the caller's memset
+}
+template <typename T>
+__global__ void scan_add_kernel(T* __restrict__ a, int64_t n, const T* __restrict__ totals) {
+  const int64_t i = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= n) a[i] += totals[(i - 1) >> 10];       // inclusive totals of the tiles before this one
+}
+template <typename T>
+static spmv_status_t scan_inclusive(T* a, int64_t n, Allocator& al, cudaStream_t s) {
+  if (n <= 0) return SPMV_OK;
+  const int64_t ntiles = (n + 1023) / 1024;
+  if (ntiles <= 4) {
+    scan_inclusive_kernel<T><<<1, 1024, 0, s>>>(a, n);
+    SPMV_CUDA_TRY(cudaGetLastError());
+    return SPMV_OK;
+  }
+  T* totals = (T*)al.alloc(sizeof(T) * (ntiles + 1), s);
+  if (!totals) return SPMV_ERR_ALLOC;
+  cudaError_t e = cudaMemsetAsync(totals, 0, sizeof(T), s);
+  if (e == cudaSuccess) {
+    scan_tiles_kernel<T><<<(unsigned)ntiles, 1024, 0, s>>>(a, n, totals);
+    scan_inclusive_kernel<T><<<1, 1024, 0, s>>>(totals, ntiles);
+    scan_add_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(a, n, totals);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);      // totals is freed below
+  al.free(totals, sizeof(T) * (ntiles + 1));
+  if (e != cudaSuccess) { set_last_error("scan: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+  return SPMV_OK;
+}
+
 // ------------------------------------------------------------------ SELL-C-sigma
 // perm[p] = original row stored at SELL position p (or -1).  Within each window of sigma
 // positions, rows are ordered by descending length, ties by ascending row (stable).
@@ -260,6 +318,8 @@ void free_sell(SellFormat& f, Allocator& al) {
 spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int split, Allocator& al, cudaStream_t s,
                          SellFormat* out) {
   SellFormat f;
+  // every error return below frees what was built so far (the converters are all-or-nothing)
+  struct Guard { SellFormat& f; Allocator& al; bool keep; ~Guard() { if (!keep) free_sell(f, al); } } guard{f, al, false};
   f.is_ell = ell;
   CsrView A = A0;
   f.vrows = A0.rows;
@@ -286,10 +346,10 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
     const unsigned g = (unsigned)((rows0 + 255) / 256);
     split_count_kernel<<<g, 256, 0, s>>>(rows0, split, A0.row_ptr, vstart, pstart, sidx);
     SPMV_CUDA_TRY(cudaGetLastError());
-    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(vstart, rows0);
-    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(pstart, rows0);
-    scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(sidx, rows0);
-    SPMV_CUDA_TRY(cudaGetLastError());
+    for (int* arr : {vstart, pstart, sidx}) {
+      spmv_status_t sst = scan_inclusive<int>(arr, rows0, al, s);
+      if (sst != SPMV_OK) return sst;
+    }
     int tot[3] = {0, 0, 0};
     SPMV_CUDA_TRY(cudaMemcpyAsync(&tot[0], vstart + rows0, sizeof(int), cudaMemcpyDeviceToHost, s));
     SPMV_CUDA_TRY(cudaMemcpyAsync(&tot[1], pstart + rows0, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -304,7 +364,7 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
     f.part = (double*)al.alloc(sizeof(double) * std::max<int64_t>(f.nparts, 1), s);
     f.srow = (int32_t*)al.alloc(sizeof(int32_t) * std::max<int64_t>(f.nsplit, 1), s);
     f.sptr = (int32_t*)al.alloc(sizeof(int32_t) * (f.nsplit + 1), s);
-    if (!vrp || !vtarget || !f.part || !f.srow || !f.sptr) { free_sell(f, al); return SPMV_ERR_ALLOC; }
+    if (!vrp || !vtarget || !f.part || !f.srow || !f.sptr) return SPMV_ERR_ALLOC;
     split_fill_kernel<<<g, 256, 0, s>>>(rows0, f.vrows, (int)A0.nnz, split, A0.row_ptr, vstart, pstart, sidx, vrp,
                                         vtarget, f.srow, f.sptr);
     SPMV_CUDA_TRY(cudaGetLastError());
@@ -332,7 +392,7 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
   if (!f.slice_ptr) return SPMV_ERR_ALLOC;
   if (f.sigma > 1) {
     f.perm = (int32_t*)al.alloc(sizeof(int32_t) * rows_padded, s);
-    if (!f.perm) { free_sell(f, al); return SPMV_ERR_ALLOC; }
+    if (!f.perm) return SPMV_ERR_ALLOC;
     const int64_t nwin = (rows_padded + f.sigma - 1) / f.sigma;
     const size_t smem = sizeof(unsigned long long) * f.sigma;
     if (smem > 48 * 1024)
@@ -344,8 +404,10 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
   sell_width_kernel<<<(unsigned)((f.nslices * 32 + 255) / 256), 256, 0, s>>>(A.rows, f.nslices, f.C, A.row_ptr, f.perm,
                                                                          f.slice_ptr);
   SPMV_CUDA_TRY(cudaGetLastError());
-  scan_inclusive_kernel<int64_t><<<1, 1024, 0, s>>>(f.slice_ptr, f.nslices);
-  SPMV_CUDA_TRY(cudaGetLastError());
+  {
+    spmv_status_t sst = scan_inclusive<int64_t>(f.slice_ptr, f.nslices, al, s);
+    if (sst != SPMV_OK) return sst;
+  }
   int64_t total = 0;
   SPMV_CUDA_TRY(cudaMemcpyAsync(&total, f.slice_ptr + f.nslices, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
@@ -353,8 +415,8 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
   const int64_t n_alloc = total > 0 ? total : 2;
   f.val = (double*)al.alloc(sizeof(double) * n_alloc, s);
   f.col = (int32_t*)al.alloc(sizeof(int32_t) * n_alloc, s);
-  if (!f.val || !f.col) { f.padded = n_alloc; free_sell(f, al); return SPMV_ERR_ALLOC; }
   f.padded = n_alloc;
+  if (!f.val || !f.col) return SPMV_ERR_ALLOC;
   if (total > 0) {
     sell_fill_kernel<<<(unsigned)((rows_padded + 127) / 128), 128, 0, s>>>(A.rows, rows_padded, f.C, f.logC, A.row_ptr,
                                                                         A.col_idx, A.val, f.perm, f.slice_ptr, f.val,
@@ -366,6 +428,7 @@ spmv_status_t build_sell(const CsrView& A0, int C, int sigma, bool ell, int spli
     SPMV_CUDA_TRY(cudaGetLastError());
   }
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  guard.keep = true;
   *out = f;
   return SPMV_OK;
 }
@@ -417,14 +480,17 @@ void free_bcsr3(BcsrFormat& f, Allocator& al) {
 spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out) {
   if (A.rows % 3 || A.cols % 3 || A.rows == 0) return SPMV_ERR_UNSUPPORTED;
   BcsrFormat f;
+  struct Guard { BcsrFormat& f; Allocator& al; bool keep; ~Guard() { if (!keep) free_bcsr3(f, al); } } guard{f, al, false};
   f.brows = A.rows / 3;
   f.brow_ptr = (int32_t*)al.alloc(sizeof(int32_t) * (f.brows + 1), s);
   if (!f.brow_ptr) return SPMV_ERR_ALLOC;
   const unsigned grid = (unsigned)((f.brows + 127) / 128);
   bcsr3_merge_kernel<false><<<grid, 128, 0, s>>>(f.brows, A.row_ptr, A.col_idx, A.val, f.brow_ptr, nullptr, nullptr);
   SPMV_CUDA_TRY(cudaGetLastError());
-  scan_inclusive_kernel<int><<<1, 1024, 0, s>>>(f.brow_ptr, f.brows);
-  SPMV_CUDA_TRY(cudaGetLastError());
+  {
+    spmv_status_t sst = scan_inclusive<int>(f.brow_ptr, f.brows, al, s);
+    if (sst != SPMV_OK) return sst;
+  }
   int total = 0;
   SPMV_CUDA_TRY(cudaMemcpyAsync(&total, f.brow_ptr + f.brows, sizeof(int), cudaMemcpyDeviceToHost, s));
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
@@ -432,12 +498,13 @@ spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrF
   const int64_t n_alloc = std::max<int64_t>(f.nblocks, 1);
   f.bcol = (int32_t*)al.alloc(sizeof(int32_t) * n_alloc, s);
   f.bval = (double*)al.alloc(sizeof(double) * 9 * n_alloc, s);
-  if (!f.bcol || !f.bval) { free_bcsr3(f, al); return SPMV_ERR_ALLOC; }
+  if (!f.bcol || !f.bval) return SPMV_ERR_ALLOC;
   SPMV_CUDA_TRY(cudaMemsetAsync(f.bval, 0, sizeof(double) * 9 * n_alloc, s));
   bcsr3_merge_kernel<true><<<grid, 128, 0, s>>>(f.brows, A.row_ptr, A.col_idx, A.val, f.brow_ptr, f.bcol, f.bval);
   SPMV_CUDA_TRY(cudaGetLastError());
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
   f.fill = f.nblocks ? (double)A.nnz / (9.0 * (double)f.nblocks) : 1.0;
+  guard.keep = true;
   *out = f;
   return SPMV_OK;
 }

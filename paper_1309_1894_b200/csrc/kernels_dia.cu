@@ -18,6 +18,7 @@
 #include "cg_reduce.cuh"
 #include "device_utils.cuh"
 #include "spmv_internal.h"
+#include "tma_utils.cuh"
 
 namespace spmv {
 
@@ -430,34 +431,6 @@ cudaError_t dia_const_plan(const Variant& v, int64_t rows, int64_t cols, const D
 // Same producer/consumer ring as kernels_sell_tma.cu: the values of J diagonals of one slice are ONE
 // contiguous run (slice-major layout), so a stage is a single cp.async.bulk.  The x addresses do not
 // depend on loaded data (row + offset), so the consumers issue their x loads BEFORE waiting for the stage.
-__device__ __forceinline__ uint32_t dsmem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void dbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(dsmem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void dbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(dsmem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void dbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(dsmem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void dbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "DWAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DWAIT_DONE;\n"
-      "bra DWAIT_LOOP;\n"
-      "DWAIT_DONE:\n"
-      "}\n" ::"r"(dsmem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void dbulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   dsmem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(dsmem_u32(bar))
-               : "memory");
-}
-
 // blockDim.x = C/R consumer threads + 32 (the last warp is the producer warp).
 // With the first stage of a slice the producer also brings the slice's mask words and (beta != 0, Y_BULK)
 // its old y values, so a consumer never waits on a dependent global load: the x loads are issued
@@ -479,10 +452,10 @@ dia_tma_kernel(int64_t rows, int64_t xlo, int64_t xhi, int64_t nslices, int C, i
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) {
-      dbar_init(&full[s], 1);
-      dbar_init(&empty[s], nconsumers / 32);
+      tma::bar_init(&full[s], 1);
+      tma::bar_init(&empty[s], nconsumers / 32);
     }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    tma::bar_init_fence();
   }
   __syncthreads();
   const bool want_y = beta != 0.0 && y_bulk;
@@ -495,16 +468,16 @@ dia_tma_kernel(int64_t rows, int64_t xlo, int64_t xhi, int64_t nslices, int C, i
         const bool ybulk = want_y && (s + 1) * C <= rows;
         for (int d0 = 0; d0 < nd; d0 += J) {
           const int nj = min(J, nd - d0);
-          dbar_wait(&empty[stage], phase ^ 1);
+          tma::bar_wait(&empty[stage], phase ^ 1);
           // generic-proxy reads of the previous occupant are ordered before this async-proxy refill
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          tma::fence_proxy_async();
           const uint32_t vb = (uint32_t)nj * C * sizeof(double);
           const uint32_t mb = d0 == 0 ? (uint32_t)C * sizeof(unsigned) : 0u;
           const uint32_t yb = (d0 == 0 && ybulk) ? (uint32_t)C * sizeof(double) : 0u;
-          dbar_expect_tx(&full[stage], vb + mb + yb);
-          dbulk_g2s(s_val + (size_t)stage * J * C, src + (int64_t)d0 * C, vb, &full[stage]);
-          if (mb) dbulk_g2s(s_mask + (size_t)stage * C, mask + s * C, mb, &full[stage]);
-          if (yb) dbulk_g2s(s_y + (size_t)stage * C, y + s * C, yb, &full[stage]);
+          tma::bar_expect_tx(&full[stage], vb + mb + yb);
+          tma::bulk_g2s(s_val + (size_t)stage * J * C, src + (int64_t)d0 * C, vb, &full[stage]);
+          if (mb) tma::bulk_g2s(s_mask + (size_t)stage * C, mask + s * C, mb, &full[stage]);
+          if (yb) tma::bulk_g2s(s_y + (size_t)stage * C, y + s * C, yb, &full[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -534,7 +507,7 @@ dia_tma_kernel(int64_t rows, int64_t xlo, int64_t xhi, int64_t nslices, int C, i
 #pragma unroll
         for (int r = 0; r < R; ++r) xv[j][r] = ldx<X>(x, min(max((int)(r0 + r) + o, xmin), xmax));
       }
-      dbar_wait(&full[stage], phase);
+      tma::bar_wait(&full[stage], phase);
       if (d0 == 0) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -556,7 +529,7 @@ dia_tma_kernel(int64_t rows, int64_t xlo, int64_t xhi, int64_t nslices, int C, i
       // the stage is in registers: hand it back before the FMAs
       asm volatile("fence.acq_rel.cta;" ::: "memory");
       __syncwarp();
-      if (lane == 0) dbar_arrive(&empty[stage]);
+      if (lane == 0) tma::bar_arrive(&empty[stage]);
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         const int d = d0 + j;
@@ -740,9 +713,10 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
   f.logC = C == 128 ? 7 : C == 256 ? 8 : 9;
   f.ld = ((A.rows + C - 1) / C) * C;
   dia_compute_windows(f);
+  struct Guard { DiaFormat& f; Allocator& al; bool keep; ~Guard() { if (!keep) free_dia(f, al); } } guard{f, al, false};
   f.val = (double*)al.alloc(sizeof(double) * nd * f.ld, s);
   f.mask = (unsigned*)al.alloc(sizeof(unsigned) * f.ld, s);
-  if (!f.val || !f.mask) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+  if (!f.val || !f.mask) return SPMV_ERR_ALLOC;
   SPMV_CUDA_TRY(cudaMemsetAsync(f.val, 0, sizeof(double) * nd * f.ld, s));
   DiaOffsets o;
   for (int i = 0; i < 32; ++i) o.off[i] = f.off[i];
@@ -753,7 +727,7 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
   {
     const size_t wbytes = sizeof(unsigned long long) * 64 + sizeof(unsigned) * 40;
     unsigned long long* d_ref = (unsigned long long*)al.alloc(wbytes, s);
-    if (!d_ref) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+    if (!d_ref) return SPMV_ERR_ALLOC;
     unsigned* d_seen = (unsigned*)(d_ref + 64);
     unsigned* d_mis = d_seen + 32;
     cudaError_t e2 = cudaMemsetAsync(d_ref, 0, wbytes, s);
@@ -769,7 +743,7 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
     if (e2 == cudaSuccess) e2 = cudaMemcpyAsync(&h_mis, d_mis, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
     if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(s);
     al.free(d_ref, wbytes);
-    if (e2 != cudaSuccess) { free_dia(f, al); set_last_error("build_dia: %s", cudaGetErrorString(e2)); return SPMV_ERR_CUDA; }
+    if (e2 != cudaSuccess) { set_last_error("build_dia: %s", cudaGetErrorString(e2)); return SPMV_ERR_CUDA; }
     f.is_const = h_mis == 0;
     for (int d = 0; d < 32; ++d) {
       const unsigned long long bits = h_ref[32 + std::min(d, nd - 1)];
@@ -778,15 +752,16 @@ spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, 
     if (f.is_const && nd <= 16) {
       f.mask_elem = nd <= 8 ? 1 : 2;
       f.mask_small = al.alloc((size_t)f.mask_elem * f.ld, s);
-      if (!f.mask_small) { free_dia(f, al); return SPMV_ERR_ALLOC; }
+      if (!f.mask_small) return SPMV_ERR_ALLOC;
       const unsigned gm = (unsigned)((f.ld + 255) / 256);
       if (f.mask_elem == 1) dia_mask_narrow_kernel<unsigned char><<<gm, 256, 0, s>>>(f.ld, f.mask, (unsigned char*)f.mask_small);
       else dia_mask_narrow_kernel<unsigned short><<<gm, 256, 0, s>>>(f.ld, f.mask, (unsigned short*)f.mask_small);
       cudaError_t e3 = cudaGetLastError();
-      if (e3 != cudaSuccess) { free_dia(f, al); set_last_error("build_dia: %s", cudaGetErrorString(e3)); return SPMV_ERR_CUDA; }
+      if (e3 != cudaSuccess) { set_last_error("build_dia: %s", cudaGetErrorString(e3)); return SPMV_ERR_CUDA; }
     }
   }
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  guard.keep = true;
   *out = f;
   return SPMV_OK;
 }

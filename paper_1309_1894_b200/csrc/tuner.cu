@@ -501,6 +501,53 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
   }
   std::sort(ok.begin(), ok.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; });
 
+  // ---- phase 3, tie-break: with a runner-up within a per cent or two the winner used to change from run to run
+  // (SURVEY sec. 7 hard part 11).  Every candidate within 2 % of the best is timed again with three times the
+  // batches; what is then within 0.5 % of the fastest counts as a tie, and a tie goes to the lexicographically
+  // smallest descriptor, so the same matrix selects the same variant in every process.
+  if (ok.size() > 1 && budget_left()) {
+    std::vector<Scored> close;
+    for (const Scored& c : ok)
+      if (c.us <= 1.02 * ok[0].us && close.size() < 6) close.push_back(c);
+    if (close.size() > 1) {
+      const int reps0 = T.reps;
+      T.reps = 3 * reps0;
+      for (Scored& c : close) {
+        release_formats_except(h, c.v);
+        if (ensure_format(h, c.v, T.s) != SPMV_OK) { c.us = 1e300; continue; }
+        LaunchPlan plan;
+        bool quick = false;
+        double us = 0;
+        if (build_plan(h, c.v, &plan) != SPMV_OK || T.time(plan, c.us, 1e300, &us, &quick) != SPMV_OK) { c.us = 1e300; continue; }
+        c.us = us;
+        T.log(variant_to_string(c.v), "retimed", us, 0);
+      }
+      T.reps = reps0;
+      double fastest = 1e300;
+      for (const Scored& c : close) fastest = std::min(fastest, c.us);
+      const Scored* pick = nullptr;
+      for (const Scored& c : close)
+        if (c.us <= 1.005 * fastest && (!pick || variant_to_string(c.v) < variant_to_string(pick->v))) pick = &c;
+      if (pick && fastest < 1e300) {
+        // the re-timed figures replace the first ones; the pick moves to the front
+        std::vector<Scored> rest;
+        const std::string pd = variant_to_string(pick->v);
+        const Scored chosen = *pick;
+        for (const Scored& c : ok) {
+          const std::string d = variant_to_string(c.v);
+          if (d == pd) continue;
+          Scored q = c;
+          for (const Scored& r : close) if (variant_to_string(r.v) == d) q.us = r.us;
+          rest.push_back(q);
+        }
+        std::sort(rest.begin(), rest.end(), [](const Scored& a, const Scored& b) { return a.us < b.us; });
+        ok.clear();
+        ok.push_back(chosen);
+        ok.insert(ok.end(), rest.begin(), rest.end());
+      }
+    }
+  }
+
   if (report) {
     report->n_enumerated = n_enum + 1;
     report->n_pruned_structural = n_pruned;
