@@ -92,6 +92,10 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
             const IT* __restrict__ scol, const int* __restrict__ sbase, const int* __restrict__ perm,
             double* __restrict__ part, double alpha, const double* __restrict__ x, double beta,
             double* __restrict__ y) {
+  // Programmatic dependent launch: the next kernel of the stream may start now; this one reads the format
+  // (immutable, owned by the handle) at once and waits for the previous kernel only before it touches x or y.
+  pdl_launch_dependents();
+  bool waited = false;
   const int64_t G = (int64_t)gridDim.x * blockDim.x;
   for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g * R < rows_padded; g += G) {
     const int64_t r0 = g * R;
@@ -115,6 +119,7 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
       if (PERM) orow[r] = __ldg(perm + row);
       else orow[r] = row < rows ? row : -1;
     }
+    if (!waited) { pdl_wait(); waited = true; }
 #pragma unroll
     for (int r = 0; r < R; ++r) yold[r] = (beta != 0.0 && orow[r] >= 0) ? y[orow[r]] : 0.0;
     // U steps per trip, every load of the trip issued before the first use; steps beyond
@@ -155,28 +160,36 @@ sell_kernel(int64_t rows, int64_t rows_padded, int C, int logC,
       else if (PERM && orow[r] < -1) part[-(orow[r] + 2)] = acc[r];   // segment of a split row
     }
   }
+  if (!waited) pdl_wait();
 }
 
-// One warp per split row: lane-strided sums over its segments, then the fixed butterfly -- the
-// order depends only on the format, so results are bit-identical across runs (reading A20).
+// W lanes per split row: lane-strided sums over its segments, then the fixed butterfly over the W lanes -- the
+// order depends only on the format, so results are bit-identical across runs (reading A20).  W = 8: a split
+// row has ceil(len / l) segments, a handful on the power-law matrix (a full warp per row left 3/4 of the lanes
+// idle and took 23 us for 105 K rows; profiles/r02_cfg3_sell_split_ncu_full.md).
+constexpr int kFixW = 8;
 __global__ void sell_split_fixup_kernel(int64_t nsplit, const int* __restrict__ srow, const int* __restrict__ sptr,
                                         const double* __restrict__ part, double alpha, double beta,
                                         double* __restrict__ y) {
-  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (w >= nsplit) return;
-  const int a = __ldg(sptr + w), b = __ldg(sptr + w + 1);
+  pdl_launch_dependents();
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kFixW;
+  const int lane = threadIdx.x & (kFixW - 1);
+  const bool live = w < nsplit;                      // every lane stays for the shuffles
+  const int a = live ? __ldg(sptr + w) : 0, b = live ? __ldg(sptr + w + 1) : 0;
+  const int row = live ? __ldg(srow + w) : 0;
+  pdl_wait();                                       // part[] is the previous kernel's output
   double s = 0.0;
-  for (int k = a + lane; k < b; k += 32) s += part[k];
-  s = butterfly_sum<32>(s);
-  if (lane == 0) store_y(y, __ldg(srow + w), alpha, s, beta);
+  for (int k = a + lane; k < b; k += kFixW) s += part[k];
+  s = butterfly_sum<kFixW>(s);
+  if (live && lane == 0) store_y(y, row, alpha, s, beta);
 }
 
 void sell_split_fixup_call(const SellFormat& f, KernelCall* c) {
   *c = KernelCall();
   c->fn = (const void*)sell_split_fixup_kernel;
-  c->grid = (unsigned)((f.nsplit * 32 + 255) / 256);
+  c->grid = (unsigned)((f.nsplit * kFixW + 255) / 256);
   c->block = 256;
+  c->pdl = true;
   c->add((int64_t)f.nsplit); c->add((const int*)f.srow); c->add((const int*)f.sptr); c->add((const double*)f.part);
   c->add_alpha(); c->add_beta(); c->add_y();
 }
@@ -217,6 +230,7 @@ cudaError_t sell_plan(const Variant& v, int64_t rows, const SellFormat& f, int s
   KernelCall& c = out->k[0];
   c.fn = k;
   c.block = v.block;
+  c.pdl = true;
   const int64_t rows_padded = f.nslices * (int64_t)f.C;
   const int64_t threads = (rows_padded + v.R - 1) / v.R;
   const int64_t exact = (threads + v.block - 1) / v.block;
