@@ -142,6 +142,40 @@ def test_apply_host_matches_device_apply(cuda):
     S.close()
 
 
+def test_graph_replay_equals_plain_applies(cuda):
+    """spmv_graph_create: k back-to-back applies captured into one CUDA graph give, bit for bit, what k plain
+    applies give (beta != 0, so every apply depends on the one before), for one- and two-kernel variants; the
+    graph can be replayed, and refuses bad arguments."""
+    import torch
+    prob = W.config(2, 0.3)
+    A = prob.A
+    S = binding.SpMV.from_csr(A)
+    dx = H.to_dev(prob.x)
+    for desc in ("dia_const:b256:r1:x0", "sell_tma:b288:c256:s1:r1:u8:i3:x0", "merge:b256:i7:x0", "default"):
+        S.select(desc)
+        y_plain = H.to_dev(prob.y0).clone()
+        for _ in range(7):
+            S.apply(0.75, dx, 0.5, y_plain)
+        y_graph = H.to_dev(prob.y0).clone()
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            g = S.graph(0.75, dx, 0.5, y_graph, 7)
+            g.launch()
+            st.synchronize()
+            assert torch.equal(y_graph, y_plain), desc
+            g.launch()                                           # a second replay continues from the current y
+            st.synchronize()
+        for _ in range(7):
+            S.apply(0.75, dx, 0.5, y_plain)
+        torch.cuda.synchronize()
+        assert torch.equal(y_graph, y_plain), desc
+        g.close()
+    with pytest.raises(binding.SpmvError) as e:
+        S.graph(1.0, dx, 0.0, y_plain, 0)
+    assert e.value.status == 1
+    S.close()
+
+
 @pytest.mark.parametrize("which", ["stencil7", "fem", "banded"])
 def test_apply_host_pipeline_is_bit_identical_to_device_apply(cuda, which):
     """spmv_apply_host pipelines chunks of rows (upload | kernel on a row range | download) where the variant
