@@ -17,6 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libspmv_b200.so")
+FAST_SRC = os.path.join(CSRC, "pyfast.c")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "-Xcompiler", "-fPIC,-fvisibility=hidden", "--expt-relaxed-constexpr"]
@@ -55,7 +56,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
         if verbose:
             print("linked", LIB)
+    _build_fast(force)
     return LIB
+
+
+def _build_fast(force: bool) -> None:
+    """_spmvfast: the CPython fast-call entry for spmv_apply (marshalling only), linked against libspmv_b200.so."""
+    import sysconfig
+    out = os.path.join(HERE, "_spmvfast" + sysconfig.get_config_var("EXT_SUFFIX"))
+    if not force and os.path.exists(out) and os.path.getmtime(out) >= max(os.path.getmtime(FAST_SRC), os.path.getmtime(LIB)):
+        return
+    cmd = ["gcc", "-O2", "-shared", "-fPIC", "-I" + sysconfig.get_paths()["include"], FAST_SRC, "-o", out,
+           "-L" + HERE, "-l:libspmv_b200.so", "-Wl,-rpath,$ORIGIN"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError(f"gcc failed for {FAST_SRC}:\n{r.stdout}\n{r.stderr}")
 
 
 if __name__ == "__main__":
