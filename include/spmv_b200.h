@@ -176,8 +176,12 @@ SPMV_API spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts, 
 SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta,
                          double* d_y, void* stream);
 
-/* Same operation with HOST vectors: copies x (and y when beta != 0) to the device,
- * applies, copies y back; synchronises `stream` before returning. */
+/* Same operation with HOST vectors (pinned memory overlaps; pageable memory works): copies x (and y when beta != 0) to
+ * the device, applies, copies y back; synchronises `stream` before returning.  Where the selected variant has a
+ * row-range form (see spmv_apply_rows) the call is a pipeline over chunks of rows on three internal streams --
+ * upload of x as far as the chunk's rows reach (its rows + the matrix bandwidth) and of the chunk of y | kernel on the
+ * chunk | download of the chunk of y -- bit-identical to the one-launch form.  Chunks hold ~3 MB of y (environment
+ * variable SPMV_HOST_CHUNK_MB overrides, for experiments). */
 SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
                               double* h_y, void* stream);
 

@@ -90,4 +90,20 @@ def test_apply_rows_refuses_what_has_no_range_form(cuda):
     got = y.cpu().numpy()
     assert oracle.accept(got[512:1024], y_ref[512:1024], scale[512:1024], H.TOL)[0]
     assert (got[:512] == 0).all() and (got[1024:] == 0).all()              # nothing outside the range is written
+    # dia_const: the pair-load instantiation (r2) falls back to one row per thread on unaligned vectors, range form too
+    L = W.laplace3d_7pt(24)
+    T = binding.SpMV.from_csr(L)
+    T.select("dia_const:b256:r2:x0")
+    xs = W.uniform(91, L.cols)
+    buf_x = torch.zeros(L.cols + 1, dtype=torch.float64, device="cuda"); buf_x[1:] = H.to_dev(xs)
+    buf_y = torch.zeros(L.rows + 1, dtype=torch.float64, device="cuda")
+    al = T.range_align()
+    a, b = 3 * al, 9 * al
+    T.apply_rows(2.0, buf_x[1:], 0.0, buf_y[1:], a, b)          # 8-byte aligned only
+    torch.cuda.synchronize()
+    y_ref, scale = oracle.spmv(L.row_ptr, L.col_idx, L.val, 2.0, xs, 0.0)
+    got = buf_y[1:].cpu().numpy()
+    assert oracle.accept(got[a:b], y_ref[a:b], scale[a:b], H.TOL)[0]
+    assert (got[:a] == 0).all() and (got[b:] == 0).all()
+    T.close()
     S.close()
