@@ -56,12 +56,29 @@ def test_null_and_bad_arguments_return_codes(L):
     assert L.spmv_select(None, b"default", None) == 1
     assert L.spmv_get_info(None, None) == 1
     L.spmv_clear_cache()
+    # round-2 entry points: graphs, row ranges, sharding helpers
+    g = ctypes.c_void_p(0)
+    assert L.spmv_graph_create(None, 1.0, None, 0.0, None, 4, ctypes.byref(g)) == 1 and not g.value
+    assert L.spmv_graph_launch(None, None) == 1 and L.spmv_graph_destroy(None) == 1
+    assert L.spmv_apply_rows(None, 1.0, None, 0.0, None, 0, 0, None, None) == 1
+    assert L.spmv_apply_host(None, 1.0, None, 0.0, None, None) == 1
+    assert L.spmv_gather(-1, None, None, None, None) == 1 and L.spmv_gather(0, None, None, None, None) == 0
+    assert L.spmv_scatter(3, None, None, None, None) == 1
+    assert L.spmv_external_columns(None, 0, 0, None, 0, None, None, None, None) == 1
+    assert L.spmv_partition_rows(4, None, 2, 1, None) == 1
+    assert L.spmv_cg(None, None, None, None, None, None) == 1
 
 
 def test_struct_sizes_match_header():
     # guards the ctypes mirrors against drift from include/spmv_b200.h (x86-64 layout)
     assert ctypes.sizeof(binding.Info) == 3 * 8 + 2 * 4 + 2 * 8 + 32 * 8 + 8 + 2 * 4 + 8 + 2 * 8 + 2 * 4 + 3 * 8 + 128 + 64
     assert ctypes.sizeof(binding.Allocator) == 24
+    # spmv_cg_opts_t: double + 6 int32; spmv_cg_result_t: 8 int32 + char[128] + 3 doubles
+    assert ctypes.sizeof(binding.CgOpts) == 8 + 6 * 4
+    assert ctypes.sizeof(binding.CgResult) == 8 * 4 + 128 + 3 * 8
+    assert binding.CgResult.rel_residual.offset == 160 and binding.CgResult.loop_variant.offset == 32
+    # spmv_tune_report_t: the log buffer triple closes the struct
+    assert binding.TuneReport.log_len.offset + 8 == ctypes.sizeof(binding.TuneReport)
 
 
 def test_sizes_over_the_int32_limits_are_unsupported(L):

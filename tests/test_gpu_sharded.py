@@ -107,3 +107,31 @@ def test_apply_rows_refuses_what_has_no_range_form(cuda):
     assert (got[:a] == 0).all() and (got[b:] == 0).all()
     T.close()
     S.close()
+
+
+def test_torch_distributed_transport_world1_nccl(cuda):
+    """The production transport (torch.distributed over NCCL) with the one rank this box has: process-group set-up,
+    the setup-time list exchange, an apply without peers.  (More ranks need more GPUs; the exchange itself is
+    covered by the gloo world-2 test on the CPU and by the loopback shards above.)"""
+    import os
+    import socket
+    import torch
+    import torch.distributed as dist
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda:0"))
+    try:
+        A = W.laplace3d_7pt(30)
+        sh = sharded.ShardedSpMV(A, sharded.TorchDistTransport(), device="cuda:0")
+        assert sh.plan is not None and sh.plan.halo_entries() == 0 and sh.split is None
+        assert list(sh.bounds) == [0, A.rows]
+        x, y0 = W.uniform(92, A.cols), W.uniform(93, A.rows)
+        sh.x_owned.copy_(H.to_dev(x))
+        y = H.to_dev(y0).clone()
+        sh.apply(1.5, -0.5, y)
+        torch.cuda.synchronize()
+        y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.5, x, -0.5, y0)
+        assert oracle.accept(y.cpu().numpy(), y_ref, scale, H.TOL)[0]
+        sh.close()
+    finally:
+        dist.destroy_process_group()
