@@ -77,6 +77,73 @@ def test_full_size_cfg5_batch_over_streams(cuda):
         h.close()
 
 
+def test_full_size_banded_matrix_16bit_indices(cuda):
+    """The bench's banded matrix (2^21 rows, 24 per row within +-2000 of the diagonal): the tuner's winner and the
+    best 16-bit-index variant both match the oracle on every row; the 16-bit format streams 10 B per entry."""
+    import torch
+    A = W.banded_random(1 << 21, 24, 2000)
+    x = W.uniform(90, A.cols)
+    prob = W.Problem("banded", A, x, None, 1.0, 0.0)
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x, 0.0, parallel=True)
+    S = binding.SpMV.from_csr(A)
+    dx = H.to_dev(x)
+    with pytest.raises(binding.SpmvError):                      # thousands of diagonals: not a DIA matrix
+        S.select("dia_tma:b288:c256:r1:u8:i3:x0")
+    for flt in (None, "sell16"):
+        rep = S.tune(alpha=1.0, beta=0.0, use_cache=2, variant_filter=flt, seed=7)
+        assert rep["n_rejected"] == 0
+        ok, mr, ff, nf = oracle.accept(_run(S, prob, dx, None).cpu().numpy(), y_ref, scale, H.TOL)
+        assert ok, (S.variant, nf, ff, mr)
+        print(f"banded: {flt or 'all'} -> {S.variant} {rep['winner_us']:.1f} us, format {S.info().format_bytes / 1e6:.0f} MB")
+    assert S.variant.startswith("sell16") and S.info().format_bytes < 10.1 * A.nnz + 16 * A.rows
+    S.close()
+
+
+@pytest.mark.parametrize("cfg,world", [(4, 2), (3, 3), (5, 2)])
+def test_full_size_host_pipeline_and_row_shards(cuda, cfg, world):
+    """At BASELINE.json sizes: (i) spmv_apply_host's chunk pipeline equals the device apply bit for bit with the
+    tuned variant; (ii) the matrix split into `world` nnz-balanced row shards (loopback transport, one GPU) gives
+    the oracle's result on every row, with the halo exchanged through the library's pack / unpack kernels."""
+    import torch
+    from paper_1309_1894_b200 import sharded
+    prob = W.config(cfg)
+    A = prob.A
+    y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, prob.alpha, prob.x, prob.beta, prob.y0, parallel=True)
+    S = binding.SpMV.from_csr(A)
+    S.tune(alpha=prob.alpha, beta=prob.beta, use_cache=0, seed=cfg)
+    dx = H.to_dev(prob.x)
+    dy0 = H.to_dev(prob.y0) if prob.y0 is not None else None
+    y_dev = _run(S, prob, dx, dy0).cpu().numpy()
+    xh = torch.from_numpy(prob.x).pin_memory()
+    yh = torch.from_numpy((prob.y0 if prob.y0 is not None else np.full(A.rows, np.nan)).copy()).pin_memory()
+    S.apply_host(prob.alpha, xh, prob.beta, yh)
+    assert np.array_equal(yh.numpy(), y_dev), S.variant
+    assert oracle.accept(y_dev, y_ref, scale, H.TOL)[0]
+    variant = S.variant
+    S.close()
+    del dx, dy0
+    torch.cuda.empty_cache()
+    hub = sharded.LoopbackTransport(world)
+    shards = [sharded.ShardedSpMV(A, hub.view(r), align=768) for r in range(world)]
+    for sh in shards:
+        sh.finish_setup()
+        sh.tune(alpha=prob.alpha, beta=prob.beta, use_cache=2, search=1, seed=cfg)
+        sh.x_owned.copy_(torch.from_numpy(prob.x[sh.lo:sh.hi]))
+    nnz = [sh.nnz_local for sh in shards]
+    assert max(nnz) <= 1.05 * A.nnz / world + 20000 * 768       # nnz-balanced up to the alignment
+    ys = [(H.to_dev(prob.y0[sh.lo:sh.hi]).clone() if prob.y0 is not None else
+           torch.full((sh.rows_local,), float("nan"), dtype=torch.float64, device="cuda")) for sh in shards]
+    sharded.run_lockstep(shards, prob.alpha, prob.beta, ys)
+    torch.cuda.synchronize()
+    y = np.concatenate([t.cpu().numpy() for t in ys])
+    ok, mr, ff, nf = oracle.accept(y, y_ref, scale, H.TOL)
+    assert ok, (cfg, world, [sh.S.variant for sh in shards], nf, ff, mr)
+    print(f"cfg{cfg}: whole {variant}; {world} shards {[sh.S.variant for sh in shards]}, halo {[sh.halo.bytes_received() for sh in shards]} B, "
+          f"split {[sh.split for sh in shards]}")
+    for sh in shards:
+        sh.close()
+
+
 def test_nnz_near_the_int32_limit(cuda):
     """Maximum sizes: 16 777 216 rows x 127 entries = 2 130 706 432 non-zeros (99.2 % of 2^31-1), built on
     the device from a closed-form pattern.  Values and x are small integers, so every variant must agree
