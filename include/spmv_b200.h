@@ -43,7 +43,8 @@
  *   keys      b threads per block | g grid: 0/absent exact cover, k = k waves of resident blocks |
  *             co shared-memory carve-out percent | u unroll (sell_tma/dia_tma: steps per stage) |
  *             r rows per thread | w lanes per (block) row | x x path: 0 ld.global.nc, 1 ld.global,
- *             2 window staged in shared memory (+ h = window half-width) | c slice height |
+ *             2 window staged in shared memory (+ h = window half-width), 3 (bcsr3) the 3-vector of a block as an
+ *             aligned 16-byte pair + one 8-byte load | c slice height |
  *             s sorting window sigma | l row-split length (rows longer than l become segments) |
  *             i merge items per thread (sell_tma/dia_tma: pipeline stages)
  *   "default" = csr_scalar:b256:r1:u1:x0, the fixed default variant.

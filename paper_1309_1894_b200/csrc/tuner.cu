@@ -94,8 +94,8 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     for (int I : {5, 7, 11}) {
       Variant v; v.fam = FAM_MERGE; v.block = b; v.I = I; all.push_back(v);
     }
-    for (int W : {4, 8, 16, 32}) for (int U : {1, 2}) {
-      Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; all.push_back(v);
+    for (int W : {4, 8, 16, 32}) for (int U : {1, 2}) for (int X : {0, 3}) {
+      Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; v.X = X; all.push_back(v);
     }
   }
   for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
