@@ -258,18 +258,16 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
         if constexpr (R == 1) {
           xv[u][0] = ldx<X>(x, min(max(r0 + o, xlo), xhi));
         } else {
-          // branch-free for either parity of the offset (p is warp-uniform: r0 is even): the run starts at
-          // the even index b = r0 + o - p; for p = 1 it is shifted left by one element and the right
-          // neighbour x[b + R] comes from the next lane's first element (lane 31 loads it)
-          const int p = o & 1;
-          const int b = r0 + o - p;
-          double e[R];
-          dia_load_pairs<R, X>(x, b, xlo, xhi, e);
-          double nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
-          if (p && (threadIdx.x & 31) == 31) nxt = ldx<X>(x, min(max(b + R, xlo), xhi));
+          // warp-uniform on the offset's parity (r0 is even): an even offset is R/2 aligned 16-byte pairs; an odd
+          // one is R 8-byte loads.  (Taking the odd run from the pair one element to the left plus a shuffle
+          // from the next lane puts a dependent exchange between the loads of consecutive diagonals and a
+          // second round trip for lane 31: measured 15.6 us against 11.4 us for one row per thread.)
+          if ((o & 1) == 0) {
+            dia_load_pairs<R, X>(x, r0 + o, xlo, xhi, xv[u]);
+          } else {
 #pragma unroll
-          for (int r = 0; r + 1 < R; ++r) xv[u][r] = p ? e[r + 1] : e[r];
-          xv[u][R - 1] = p ? nxt : e[R - 1];
+            for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max(r0 + o + r, xlo), xhi));
+          }
         }
       }
     }
@@ -313,9 +311,9 @@ dia_const_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ 
                  const double* __restrict__ x, double beta, double* __restrict__ y) {
   dia_const_body<R, ND, X, MT>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y);
 }
-// two rows per thread on a small stencil: 48 registers keep 1280 threads per SM resident without spilling
+// two rows per thread on a small stencil, blocks of at most 256 threads: 40 registers, 1536 threads per SM
 template <int ND, int X, typename MT>
-__global__ void __maxnreg__(48)
+__global__ void __launch_bounds__(256, 6)
 dia_const_kernel_r2(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                     const double* __restrict__ x, double beta, double* __restrict__ y) {
@@ -341,9 +339,9 @@ static const void* dia_const_dot_pick_nd(int nd) {
 }
 
 template <int R, int X, typename MT>
-static const void* dia_const_pick_nd(int nd) {
+static const void* dia_const_pick_nd(int nd, int block) {
   if constexpr (R == 2) {
-    switch (nd) {
+    if (block <= 256) switch (nd) {               // 40 registers under __launch_bounds__(256, 6)
       case 3: return (const void*)dia_const_kernel_r2<3, X, MT>;
       case 5: return (const void*)dia_const_kernel_r2<5, X, MT>;
       case 7: return (const void*)dia_const_kernel_r2<7, X, MT>;
@@ -361,12 +359,12 @@ static const void* dia_const_pick_nd(int nd) {
   }
 }
 template <int R, int X>
-static const void* dia_const_pick_mt(int mask_elem, int nd) {
-  return mask_elem == 1 ? dia_const_pick_nd<R, X, unsigned char>(nd)
-       : mask_elem == 2 ? dia_const_pick_nd<R, X, unsigned short>(nd) : dia_const_pick_nd<R, X, unsigned>(nd);
+static const void* dia_const_pick_mt(int mask_elem, int nd, int block) {
+  return mask_elem == 1 ? dia_const_pick_nd<R, X, unsigned char>(nd, block)
+       : mask_elem == 2 ? dia_const_pick_nd<R, X, unsigned short>(nd, block) : dia_const_pick_nd<R, X, unsigned>(nd, block);
 }
-static const void* dia_const_pick(int R, int X, int mask_elem, int nd) {
-#define P(r, xx) if (R == r && X == xx) return dia_const_pick_mt<r, xx>(mask_elem, nd);
+static const void* dia_const_pick(int R, int X, int mask_elem, int nd, int block = 512) {
+#define P(r, xx) if (R == r && X == xx) return dia_const_pick_mt<r, xx>(mask_elem, nd, block);
   P(1, 0) P(2, 0) P(4, 0) P(1, 1) P(2, 1) P(4, 1)
 #undef P
   return nullptr;
@@ -377,7 +375,7 @@ bool dia_const_supported(const Variant& v) {      // exact grid only (no g key):
 }
 static void dia_const_call(KernelCall& c, int R, const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f) {
   c = KernelCall();
-  c.fn = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd);
+  c.fn = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd, v.block);
   c.block = v.block;
   const int64_t threads = (rows + R - 1) / R;
   c.grid = (unsigned)((threads + v.block - 1) / v.block);
