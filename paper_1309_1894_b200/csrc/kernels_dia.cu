@@ -198,12 +198,21 @@ constexpr int dia_const_min_blocks(int R, int ND) { return (ND == 0 || ND > 9) ?
 // DOT (R == 1 only; the solver loop, solver.cu): the kernel also writes its block's share of sum_i x_i * y_i
 // (square matrix) to dot_part[blockIdx.x]; the caller adds the gridDim.x partials in index order.  No
 // arrival counter here: a fence + atomic at the tail of 8192 short blocks costs more than the dot pass saved.
-template <int R, int ND, int X, typename MT, bool DOT = false>
+// TRI (R == 2 only): the diagonals come in runs (o - 1, o, o + 1) with o even around every "base" offset -- the
+// natural ordering of a 5-, 7- or 27-point stencil on a grid of even extent: diagonal d with d % 3 == tri_phase is
+// the centre of a run, its left and right neighbours are NOT loaded: x[r0 + o - 1 .. ] and x[r0 + o + 1 .. ] are
+// assembled from the centre's aligned pair and one shuffle (the previous lane's second element, the next lane's
+// first); lanes 0 and 31 load their missing element in the load phase, so it stays one memory round trip.
+// Centres: every diagonal whose two neighbours in the list are at distance 1 (tri_mask, checked on the host).
+// BZ: beta == 0 (y is write-only).  Instruction count decides a kernel this short (ncu: 6.6 M warp instructions
+// took 15.5 us, 4.4 M took 11.9 us, same memory requests), so the two cases are separate instantiations chosen by
+// a uniform branch at kernel entry instead of predicated code, and the R > 1 forms require rows % R == 0 (the plan
+// falls back to R = 1 otherwise) so that a thread's rows are all live or all dead.
+template <int R, int ND, int X, typename MT, bool DOT, unsigned TRI, bool BZ>
 __device__ __forceinline__ void
 dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
                double alpha, const double* __restrict__ x, double beta, double* __restrict__ y,
                double* __restrict__ dot_part = nullptr) {
-  pdl_launch_dependents();
   constexpr int NDC = ND == 0 ? 8 : (ND % 9 == 0 ? 9 : (ND <= 8 ? ND : 8));     // diagonals per chunk
   constexpr int DMAX = ND == 0 ? 32 : ND;
   const int nd = ND == 0 ? nd_rt : ND;
@@ -212,6 +221,8 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
   // x indices are clamped, their mask words exist (the mask array is padded to a multiple of the slice
   // height >= 32*R), nothing is stored.
   const int r0 = (blockIdx.x * blockDim.x + threadIdx.x) * R;
+  const int lane = threadIdx.x & 31;
+  (void)lane;
   if (R == 1 && !DOT && r0 >= rows) return;
   unsigned m[R];
   if constexpr (R == 2) {
@@ -224,24 +235,21 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
     m[0] = mask[r0];
   }
   pdl_wait();                                                // x and y may be the previous kernel's output
-  const bool full = r0 + R <= rows;
+  const bool live = r0 < rows;                               // R > 1: rows % R == 0, so all R rows or none
   double yold[R], acc[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) { yold[r] = 0.0; acc[r] = 0.0; }
-  if (beta != 0.0) {
-    if constexpr (R > 1) {
-      if (full) {
+  if constexpr (!BZ) {
+    if (live) {
+      if constexpr (R > 1) {
 #pragma unroll
         for (int r = 0; r < R; r += 2) {
           const double2 p = *reinterpret_cast<const double2*>(y + r0 + r);
           yold[r] = p.x; yold[r + 1] = p.y;
         }
       } else {
-#pragma unroll
-        for (int r = 0; r < R; ++r) if (r0 + r < rows) yold[r] = y[r0 + r];
+        yold[0] = y[r0];
       }
-    } else {
-      if (!DOT || r0 < rows) yold[0] = y[r0];
     }
   }
   // statically unrolled over the chunks so that the by-value offset / coefficient parameters are never
@@ -257,6 +265,16 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
         const int o = offs.off[d < 32 ? d : 31];
         if constexpr (R == 1) {
           xv[u][0] = ldx<X>(x, min(max(r0 + o, xlo), xhi));
+        } else if constexpr (R == 2 && TRI != 0) {
+          if ((TRI >> (d & 31)) & 1u) {                        // centre of a run: its pair serves three diagonals
+            dia_load_pairs<R, X>(x, r0 + o, xlo, xhi, xv[u]);
+          } else if (d + 1 < DMAX && ((TRI >> ((d + 1) & 31)) & 1u)) {   // left neighbour: lane 0 loads x[r0 + o]
+            xv[u][0] = lane == 0 ? ldx<X>(x, min(max(r0 + o, xlo), xhi)) : 0.0;
+          } else if (d >= 1 && ((TRI >> ((d - 1) & 31)) & 1u)) {         // right neighbour: lane 31 loads x[r0 + o + 1]
+            xv[u][1] = lane == 31 ? ldx<X>(x, min(max(r0 + o + 1, xlo), xhi)) : 0.0;
+          } else {                                             // outside the runs every offset is even (host-checked):
+            dia_load_pairs<R, X>(x, r0 + o, xlo, xhi, xv[u]);  // a run-time parity test compiles to both paths, predicated
+          }
         } else {
           // warp-uniform on the offset's parity (r0 is even): an even offset is R/2 aligned 16-byte pairs; an odd
           // one is R 8-byte loads.  (Taking the odd run from the pair one element to the left plus a shuffle
@@ -268,6 +286,19 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
 #pragma unroll
             for (int r = 0; r < R; ++r) xv[u][r] = ldx<X>(x, min(max(r0 + o + r, xlo), xhi));
           }
+        }
+      }
+    }
+    if constexpr (R == 2 && TRI != 0) {
+      // second phase, after every load of the chunk has been issued: the neighbours of each centre
+#pragma unroll
+      for (int u = 0; u < NDC; ++u) {
+        const int d = d0 + u;
+        if (d < DMAX && ((TRI >> (d & 31)) & 1u)) {
+          const double up = __shfl_up_sync(0xffffffffu, xv[u][1], 1);       // previous lane's x[r0 - 1 + o]
+          const double dn = __shfl_down_sync(0xffffffffu, xv[u][0], 1);     // next lane's x[r0 + 2 + o]
+          if (u >= 1) { xv[u - 1][0] = lane == 0 ? xv[u - 1][0] : up; xv[u - 1][1] = xv[u][0]; }
+          if (u + 1 < NDC) { xv[u + 1][1] = lane == 31 ? xv[u + 1][1] : dn; xv[u + 1][0] = xv[u][1]; }
         }
       }
     }
@@ -283,41 +314,80 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
   }
   double out[R];
 #pragma unroll
-  for (int r = 0; r < R; ++r) out[r] = (beta == 0.0) ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
+  for (int r = 0; r < R; ++r) out[r] = BZ ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
   if constexpr (DOT) {
     __shared__ double s_warp[33];
-    const bool live = r0 < rows;
     if (live) y[r0] = out[0];
     const double mine = block_sum_fixed(live ? ldx<X>(x, r0) * out[0] : 0.0, s_warp);
     if (threadIdx.x == 0) dot_part[blockIdx.x] = mine;
     return;
   }
+  if (!live) return;
   if constexpr (R > 1) {
-    if (full) {
 #pragma unroll
-      for (int r = 0; r < R; r += 2) *reinterpret_cast<double2*>(y + r0 + r) = make_double2(out[r], out[r + 1]);
-      return;
-    }
+    for (int r = 0; r < R; r += 2) *reinterpret_cast<double2*>(y + r0 + r) = make_double2(out[r], out[r + 1]);
+  } else {
+    y[r0] = out[0];
   }
-#pragma unroll
-  for (int r = 0; r < R; ++r)
-    if (r0 + r < rows) y[r0 + r] = out[r];
 }
+
+// kernel entry: launch_dependents, then the beta == 0 / beta != 0 instantiation of the body
+#define DIA_CONST_ENTRY(R_, ND_, X_, MT_, DOT_, TRI_, ...)                                                         \
+  pdl_launch_dependents();                                                                                        \
+  if (beta == 0.0) dia_const_body<R_, ND_, X_, MT_, DOT_, TRI_, true>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y, ##__VA_ARGS__); \
+  else dia_const_body<R_, ND_, X_, MT_, DOT_, TRI_, false>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y, ##__VA_ARGS__)
 
 template <int R, int ND, int X, typename MT>
 __global__ void __launch_bounds__(512, dia_const_min_blocks(R, ND))
 dia_const_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                  const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                  const double* __restrict__ x, double beta, double* __restrict__ y) {
-  dia_const_body<R, ND, X, MT>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+  DIA_CONST_ENTRY(R, ND, X, MT, false, 0u);
 }
+
+// centres of the (o - 1, o, o + 1) runs of a 5-, 7- or 27-point stencil in natural ordering (0: no such form)
+constexpr unsigned dia_tri_mask(int ND) {
+  return ND == 5 ? 0x4u : ND == 7 ? 0x8u : ND == 27 ? 0x2492492u : 0u;     // d = 2 | d = 3 | d = 1, 4, ..., 25
+}
+// two rows per thread, the +-1 neighbours shuffled out of the centre pair (TRI): 5 loads instead of 7 on cfg2
+template <int ND, int X, typename MT>
+__global__ void __launch_bounds__(256, ND <= 9 ? 6 : 3)
+dia_const_kernel_r2t(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
+                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
+                     const double* __restrict__ x, double beta, double* __restrict__ y) {
+  DIA_CONST_ENTRY(2, ND, X, MT, false, dia_tri_mask(ND));
+}
+template <int X, typename MT>
+static const void* dia_const_pick_tri(int nd) {
+  switch (nd) {
+    case 5: return (const void*)dia_const_kernel_r2t<5, X, MT>;
+    case 7: return (const void*)dia_const_kernel_r2t<7, X, MT>;
+    case 27: return (const void*)dia_const_kernel_r2t<27, X, MT>;
+    default: return nullptr;
+  }
+}
+// host check of the run structure the TRI kernels assume
+static bool dia_tri_ok(const DiaFormat& f) {
+  const unsigned m = f.nd == 5 ? dia_tri_mask(5) : f.nd == 7 ? dia_tri_mask(7) : f.nd == 27 ? dia_tri_mask(27) : 0u;
+  if (!m) return false;
+  for (int c = 0; c < f.nd; ++c) {
+    if ((m >> c) & 1u) {
+      if (c < 1 || c + 1 >= f.nd || (f.off[c] & 1) || f.off[c - 1] != f.off[c] - 1 || f.off[c + 1] != f.off[c] + 1) return false;
+    } else {
+      const bool neighbour = (c + 1 < f.nd && ((m >> (c + 1)) & 1u)) || (c >= 1 && ((m >> (c - 1)) & 1u));
+      if (!neighbour && (f.off[c] & 1)) return false;        // every diagonal outside the runs is read as aligned pairs
+    }
+  }
+  return true;
+}
+
 // two rows per thread on a small stencil, blocks of at most 256 threads: 40 registers, 1536 threads per SM
 template <int ND, int X, typename MT>
 __global__ void __launch_bounds__(256, 6)
 dia_const_kernel_r2(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                     const double* __restrict__ x, double beta, double* __restrict__ y) {
-  dia_const_body<2, ND, X, MT>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y);
+  DIA_CONST_ENTRY(2, ND, X, MT, false, 0u);
 }
 
 // one row per thread with the fused dot product (the solver loop)
@@ -326,7 +396,7 @@ __global__ void __launch_bounds__(512, 2)
 dia_const_dot_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                      const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                      const double* __restrict__ x, double beta, double* __restrict__ y, double* __restrict__ dot_part) {
-  dia_const_body<1, ND, 0, MT, true>(rows, xlo, xhi, nd_rt, offs, coefs, mask, alpha, x, beta, y, dot_part);
+  DIA_CONST_ENTRY(1, ND, 0, MT, true, 0u, dot_part);
 }
 template <typename MT>
 static const void* dia_const_dot_pick_nd(int nd) {
@@ -376,6 +446,12 @@ bool dia_const_supported(const Variant& v) {      // exact grid only (no g key):
 static void dia_const_call(KernelCall& c, int R, const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f) {
   c = KernelCall();
   c.fn = dia_const_pick(R, v.X, f.mask_small ? f.mask_elem : 4, f.nd, v.block);
+  if (R == 2 && v.block <= 256 && dia_tri_ok(f)) {     // (o - 1, o, o + 1) runs: the neighbours come out of the centre pair
+    const int me = f.mask_small ? f.mask_elem : 4;
+    const void* t = v.X == 0 ? (me == 1 ? dia_const_pick_tri<0, unsigned char>(f.nd) : me == 2 ? dia_const_pick_tri<0, unsigned short>(f.nd) : dia_const_pick_tri<0, unsigned>(f.nd))
+                             : (me == 1 ? dia_const_pick_tri<1, unsigned char>(f.nd) : me == 2 ? dia_const_pick_tri<1, unsigned short>(f.nd) : dia_const_pick_tri<1, unsigned>(f.nd));
+    if (t) c.fn = t;
+  }
   c.block = v.block;
   const int64_t threads = (rows + R - 1) / R;
   c.grid = (unsigned)((threads + v.block - 1) / v.block);
@@ -415,7 +491,7 @@ cudaError_t dia_const_plan(const Variant& v, int64_t rows, int64_t cols, const D
   if (rows == 0) return cudaSuccess;
   // 16-byte pair accesses need an even column count (a pair is then never half inside [0, cols)) and aligned
   // vectors: the one-row-per-thread instantiation is the alternative taken per apply when x or y is not
-  const int R = cols % 2 == 0 ? v.R : 1;
+  const int R = (cols % 2 == 0 && rows % v.R == 0) ? v.R : 1;
   dia_const_call(out->k[0], R, v, rows, cols, f);
   if (R > 1) { dia_const_call(out->alt, 1, v, rows, cols, f); out->has_alt = true; }
   out->n = 1;
