@@ -182,7 +182,10 @@ SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d
  * row-range form (see spmv_apply_rows) the call is a pipeline over chunks of rows on three internal streams --
  * upload of x as far as the chunk's rows reach (its rows + the matrix bandwidth) and of the chunk of y | kernel on the
  * chunk | download of the chunk of y -- bit-identical to the one-launch form.  Chunks hold ~3 MB of y (environment
- * variable SPMV_HOST_CHUNK_MB overrides, for experiments). */
+ * variable SPMV_HOST_CHUNK_MB overrides, for experiments).  Zero-copy y: when h_y is pinned AND mapped host memory
+ * (cudaHostAlloc / cudaHostRegister; 16-byte aligned) and the variant stores y one row per thread in row order (the
+ * DIA families), the chunk kernels read and write h_y in place over PCIe instead of through a staging vector and
+ * two copies (~8 MB chunks; SPMV_HOST_ZEROCOPY=0 turns it off); same kernels, same bits. */
 SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
                               double* h_y, void* stream);
 

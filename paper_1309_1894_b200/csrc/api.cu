@@ -2,6 +2,7 @@
 // and spmv_measure_ceiling (verify.cu).
 #include <math.h>
 #include <stdlib.h>
+#include <stdint.h>
 #include <string.h>
 
 #include <algorithm>
@@ -268,10 +269,32 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
   if (!h->d_x_stage || !h->d_y_stage) return SPMV_ERR_ALLOC;
   double *dx = h->d_x_stage, *dy = h->d_y_stage;
 
-  // chunks of ~3 MB of y (smaller: the fixed cost of a PCIe copy shows; larger: less overlap), boundaries on the
-  // variant's range alignment
+  // Zero-copy y.  When the caller's y is pinned, MAPPED host memory (cudaHostAlloc / cudaHostRegister: what
+  // torch's pin_memory() gives) and the variant's kernels read and write y one row per thread in row order (the
+  // DIA families), the chunk kernels work on the caller's vector in place: their 256-byte warp stores cross PCIe as
+  // posted writes while the copy engine uploads the next chunk of x, and no copy engine runs in the opposite
+  // direction (measured on the B200 box: bidirectional 3 MB DMA chunks drop to ~31 GB/s each way; cfg2 0.84 ->
+  // 0.76 ms, one cfg5 member 0.92 -> 0.75 ms).  Families that store y with a stride (BCSR: three rows from one
+  // lane; permuted SELL) were 3x slower this way and keep the staged copies.  SPMV_HOST_ZEROCOPY=0 disables it.
+  double* zy = nullptr;
+  {
+    const char* zc_env = getenv("SPMV_HOST_ZEROCOPY");
+    const bool zc_on = !(zc_env && atoi(zc_env) == 0);
+    const int rk = h->plan.range_kind;
+    if (zc_on && rows > 0 && (rk == RANGE_DIA || rk == RANGE_DIA_TMA || rk == RANGE_DIA_CONST)) {
+      cudaPointerAttributes pa;
+      if (cudaPointerGetAttributes(&pa, h_y) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
+          ((uintptr_t)pa.devicePointer & 15) == 0)
+        zy = (double*)pa.devicePointer;
+      cudaGetLastError();                      // an unregistered pageable pointer is not an error here
+    }
+  }
+  // chunks of ~3 MB of y (smaller: the fixed cost of a PCIe copy shows; larger: less overlap; ~8 MB when y is
+  // zero-copy: the kernels' own PCIe traffic has no per-copy cost), boundaries on the variant's range alignment
   const int64_t align = h->plan.range_align > 0 ? h->plan.range_align : 1;
-  static const double chunk_mb = getenv("SPMV_HOST_CHUNK_MB") ? atof(getenv("SPMV_HOST_CHUNK_MB")) : 3.0;   // measured: 2-4 MB of y per chunk is the flat optimum
+  const char* chunk_env = getenv("SPMV_HOST_CHUNK_MB");        // read per call: tests force several chunks on small matrices
+  const double chunk_mb_env = chunk_env ? atof(chunk_env) : 0.0;
+  const double chunk_mb = chunk_mb_env > 0 ? chunk_mb_env : zy ? 8.0 : 3.0;
   int64_t nchunks = std::min<int64_t>(32, (int64_t)(rows * 8 / (chunk_mb * 1048576.0)));
   int64_t chunk = nchunks > 1 ? ((rows + nchunks - 1) / nchunks + align - 1) / align * align : rows;
   const bool pipelined = alpha != 0.0 && nchunks > 1 && chunk < rows && h->plan.n == 1 && h->plan.range_kind != RANGE_NONE;
@@ -315,19 +338,19 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
     }
     SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c], h->hs_up));
     SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * c], 0));
-    if (beta != 0.0) {       // y on its own upload stream: the fixed latencies of the two small copies overlap
+    if (beta != 0.0 && !zy) {       // y on its own upload stream: the fixed latencies of the two small copies overlap
       SPMV_CUDA_TRY(cudaMemcpyAsync(dy + a, h_y + a, sizeof(double) * (b - a), cudaMemcpyHostToDevice, h->hs_up2));
       SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c + 2], h->hs_up2));
       SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * c + 2], 0));
     }
     KernelCall kc;
     if (!plan_for_rows(h->plan, rows, cols, a, b, aligned, &kc)) { set_last_error("apply_host: range launch refused"); return SPMV_ERR_INTERNAL; }
-    ApplyArgs args{alpha, beta, dx, dy, h->hs_run};
+    ApplyArgs args{alpha, beta, dx, zy ? zy : dy, h->hs_run};
     cudaError_t e = run_call(kc, args);
     if (e != cudaSuccess) { set_last_error("apply_host: chunk launch failed: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
     SPMV_CUDA_TRY(cudaEventRecord(ev[3 * c + 1], h->hs_run));
     SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_down, ev[3 * c + 1], 0));
-    SPMV_CUDA_TRY(cudaMemcpyAsync(h_y + a, dy + a, sizeof(double) * (b - a), cudaMemcpyDeviceToHost, h->hs_down));
+    if (!zy) SPMV_CUDA_TRY(cudaMemcpyAsync(h_y + a, dy + a, sizeof(double) * (b - a), cudaMemcpyDeviceToHost, h->hs_down));
   }
   SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks + 1], h->hs_down));
   SPMV_CUDA_TRY(cudaStreamWaitEvent(s, ev[3 * nchunks + 1], 0));

@@ -219,6 +219,43 @@ def test_apply_host_pipeline_is_bit_identical_to_device_apply(cuda, which):
     S.close()
 
 
+def test_apply_host_zero_copy_y_equals_staged_copies(cuda, monkeypatch):
+    """spmv_apply_host on pinned (mapped) host memory lets the DIA families' chunk kernels read and write y in
+    place over PCIe; pageable memory and SPMV_HOST_ZEROCOPY=0 take the staged copies.  All three give the bits of
+    the device apply, for beta == 0 (y write-only: incoming NaN ignored) and beta != 0, several chunks with a
+    ragged last one, and match the oracle."""
+    import torch
+    monkeypatch.setenv("SPMV_HOST_CHUNK_MB", "1.5")
+    A = W.stencil3d_27pt(83)                                   # 571 787 rows = 4.6 MB of y: 3 chunks
+    x, y0 = W.uniform(86, A.cols), W.uniform(87, A.rows)
+    S = binding.SpMV.from_csr(A)
+    xh = torch.from_numpy(x).pin_memory()
+    for desc in ("dia:b256:c128:r2:u4:x0", "dia_tma:b288:c256:r1:u9:i3:x0", "dia_const:b256:r1:x0", "dia_const:b128:r2:x0"):
+        S.select(desc)
+        for beta in (0.0, -0.75):
+            y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.25, x, beta, None if beta == 0.0 else y0, parallel=True)
+            y_dev = H.gpu_apply(S, 1.25, x, beta, None if beta == 0.0 else y0)
+            start = np.full(A.rows, np.nan) if beta == 0.0 else y0.copy()
+            y_zero = torch.from_numpy(start.copy()).pin_memory()
+            S.apply_host(1.25, xh, beta, y_zero)                 # zero-copy y
+            y_page = start.copy()
+            S.apply_host(1.25, xh, beta, y_page)                 # pageable y: staged
+            monkeypatch.setenv("SPMV_HOST_ZEROCOPY", "0")
+            y_off = torch.from_numpy(start.copy()).pin_memory()
+            S.apply_host(1.25, xh, beta, y_off)                  # pinned y, zero-copy off: staged
+            monkeypatch.delenv("SPMV_HOST_ZEROCOPY")
+            for got in (y_zero.numpy(), y_page, y_off.numpy()):
+                assert np.array_equal(got, y_dev), (desc, beta)
+            assert oracle.accept(y_zero.numpy(), y_ref, scale, H.TOL)[0], (desc, beta)
+    # a pinned but odd-aligned y (8 mod 16) takes the staged path
+    S.select("dia_const:b256:r1:x0")
+    yo = torch.empty(A.rows + 1, dtype=torch.float64).pin_memory()
+    yo[1:] = torch.from_numpy(y0)
+    S.apply_host(1.25, xh, -0.75, yo[1:])
+    assert np.array_equal(yo[1:].numpy(), H.gpu_apply(S, 1.25, x, -0.75, y0))
+    S.close()
+
+
 @pytest.mark.slow
 def test_tma_pipeline_race_regression_full_size(cuda):
     """Regression: on full-size cfg5 with sorted slices the TMA refill (async proxy) used to land
