@@ -185,7 +185,9 @@ SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d
  * variable SPMV_HOST_CHUNK_MB overrides, for experiments).  Zero-copy y: when h_y is pinned AND mapped host memory
  * (cudaHostAlloc / cudaHostRegister; 16-byte aligned) and the variant stores y one row per thread in row order (the
  * DIA families), the chunk kernels read and write h_y in place over PCIe instead of through a staging vector and
- * two copies (~8 MB chunks; SPMV_HOST_ZEROCOPY=0 turns it off); same kernels, same bits. */
+ * two copies (~8 MB chunks; SPMV_HOST_ZEROCOPY=0 turns it off); same kernels, same bits.  For a DIA-family variant
+ * on a small system (x and y together <= 1 MB) with x mapped as well, the one kernel reads x and updates y in place:
+ * one launch + one synchronise instead of three copies. */
 SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
                               double* h_y, void* stream);
 

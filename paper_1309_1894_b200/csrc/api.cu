@@ -275,7 +275,8 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
   // posted writes while the copy engine uploads the next chunk of x, and no copy engine runs in the opposite
   // direction (measured on the B200 box: bidirectional 3 MB DMA chunks drop to ~31 GB/s each way; cfg2 0.84 ->
   // 0.76 ms, one cfg5 member 0.92 -> 0.75 ms).  Families that store y with a stride (BCSR: three rows from one
-  // lane; permuted SELL) were 3x slower this way and keep the staged copies.  SPMV_HOST_ZEROCOPY=0 disables it.
+  // lane; permuted SELL) were slower this way (BCSR with its y stores packed to 24 B per block row: 0.97 vs 0.68 ms)
+  // and keep the staged copies.  SPMV_HOST_ZEROCOPY=0 disables it.
   double* zy = nullptr;
   {
     const char* zc_env = getenv("SPMV_HOST_ZEROCOPY");
@@ -299,6 +300,22 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
   int64_t chunk = nchunks > 1 ? ((rows + nchunks - 1) / nchunks + align - 1) / align * align : rows;
   const bool pipelined = alpha != 0.0 && nchunks > 1 && chunk < rows && h->plan.n == 1 && h->plan.range_kind != RANGE_NONE;
   if (!pipelined) {
+    // small stencil systems: three DMA operations cost more than the data (cfg1: 32 KB each way).  When both
+    // vectors are mapped host memory and the variant reads x as coalesced shifted streams (the DIA families:
+    // zy != nullptr) the kernel works on the caller's x and y in place -- one launch and one synchronise.
+    // Measured: 5-point stencils 29.7 -> 20.8 us (32 KB vectors), 68.9 -> 49.6 us (512 KB); slower from 2 MB per
+    // vector on, and 4-13x slower for gathered x (small power-law matrices), hence the family and size limits.
+    if (zy && alpha != 0.0 && (rows + cols) * 8 <= (1 << 20) && cols > 0) {
+      cudaPointerAttributes px;
+      const bool okx = cudaPointerGetAttributes(&px, h_x) == cudaSuccess && px.type == cudaMemoryTypeHost && px.devicePointer;
+      cudaGetLastError();
+      if (okx) {
+        spmv_status_t st = spmv_apply(h, alpha, (const double*)px.devicePointer, beta, zy, stream);
+        if (st != SPMV_OK) return st;
+        SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+        return SPMV_OK;
+      }
+    }
     if (cols) SPMV_CUDA_TRY(cudaMemcpyAsync(dx, h_x, sizeof(double) * cols, cudaMemcpyHostToDevice, s));
     if (beta != 0.0 && rows) SPMV_CUDA_TRY(cudaMemcpyAsync(dy, h_y, sizeof(double) * rows, cudaMemcpyHostToDevice, s));
     spmv_status_t st = spmv_apply(h, alpha, dx, beta, dy, stream);

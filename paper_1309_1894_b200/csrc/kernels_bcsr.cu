@@ -64,11 +64,9 @@ bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol
     s0 = butterfly_sum<T>(s0);
     s1 = butterfly_sum<T>(s1);
     s2 = butterfly_sum<T>(s2);
-    if (ok && lane == 0) {
-      store_y(y, 3 * br + 0, alpha, s0, beta);
-      store_y(y, 3 * br + 1, alpha, s1, beta);
-      store_y(y, 3 * br + 2, alpha, s2, beta);
-    }
+    // after the butterfly every lane holds the three sums: lanes 0..2 store one row each (one store instruction,
+    // 24 contiguous bytes per block row)
+    if (ok && lane < 3) store_y(y, 3 * br + lane, alpha, lane == 0 ? s0 : lane == 1 ? s1 : s2, beta);
   }
 }
 

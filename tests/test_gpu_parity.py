@@ -247,6 +247,22 @@ def test_apply_host_zero_copy_y_equals_staged_copies(cuda, monkeypatch):
             for got in (y_zero.numpy(), y_page, y_off.numpy()):
                 assert np.array_equal(got, y_dev), (desc, beta)
             assert oracle.accept(y_zero.numpy(), y_ref, scale, H.TOL)[0], (desc, beta)
+    # small system, x and y both mapped: the kernel works on the host vectors in place (no copies at all)
+    A1 = W.laplace2d_5pt(64)
+    x1, y1 = W.uniform(88, A1.cols), W.uniform(89, A1.rows)
+    S1 = binding.SpMV.from_csr(A1)
+    x1h = torch.from_numpy(x1).pin_memory()
+    for desc in ("dia_const:b256:r1:x0", "dia_const:b128:r2:x0", "dia:b256:c128:r1:u4:x0", "default"):
+        S1.select(desc)
+        for beta in (0.0, 0.5):
+            y_dev = H.gpu_apply(S1, -1.5, x1, beta, None if beta == 0.0 else y1)
+            yh1 = torch.from_numpy(np.full(A1.rows, np.nan) if beta == 0.0 else y1.copy()).pin_memory()
+            S1.apply_host(-1.5, x1h, beta, yh1)
+            assert np.array_equal(yh1.numpy(), y_dev), (desc, beta)
+            yp1 = np.full(A1.rows, np.nan) if beta == 0.0 else y1.copy()
+            S1.apply_host(-1.5, x1, beta, yp1)                   # pageable: staged
+            assert np.array_equal(yp1, y_dev), (desc, beta)
+    S1.close()
     # a pinned but odd-aligned y (8 mod 16) takes the staged path
     S.select("dia_const:b256:r1:x0")
     yo = torch.empty(A.rows + 1, dtype=torch.float64).pin_memory()
