@@ -606,7 +606,11 @@ def config_roofline(r, peak, ceil):
 def profile_one(args, torch, binding, W):
     """A few applies of one variant on one config: the command the ncu captures under profiles/ run."""
     cfg = args.profile_one
-    prob = W.config(cfg)
+    if cfg == 6:        # the banded extra workload of bench_banded
+        A6 = W.banded_random(1 << 21, 24, 2000)
+        prob = W.Problem("banded-random 2^21 rows, 24/row within +-2000", A6, W.uniform(90, A6.cols), None, 1.0, 0.0)
+    else:
+        prob = W.config(cfg)
     A = prob.A
     S = binding.SpMV.from_csr(A)
     x = torch.from_numpy(prob.x).cuda()
@@ -652,7 +656,7 @@ def main():
                          "reads the matrix values (no constant-coefficient elision)")
     ap.add_argument("--tune-cache", default=None,
                     help="file persisting tuning winners (spmv_tune cache_path); a second run then skips the search")
-    ap.add_argument("--profile-one", type=int, default=0, metavar="CFG", help="ncu / sanitizer driver: a few cold applies of one variant")
+    ap.add_argument("--profile-one", type=int, default=0, metavar="CFG", help="ncu / sanitizer driver: a few cold applies of one variant (6 = the banded extra workload)")
     ap.add_argument("--variant", default=None, help="--profile-one: descriptor to force ('tuned' or absent: tune)")
     ap.add_argument("--iters", type=int, default=5)
     args = ap.parse_args()

@@ -112,12 +112,19 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     // x window staged in shared memory (a10 ii): only meaningful when the rows of a slice are contiguous
     if (S == 1 && (J == 4 || J == 8) && ST <= 3)
       for (int H : {72, 136}) { Variant w = v; w.X = 2; w.H = H; all.push_back(w); }
+    // banded matrix: a window as wide as the band takes EVERY gather of a slice out of shared memory
+    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth > 136 && in.bandwidth <= 4096) {
+      Variant w = v; w.X = 3; w.H = (int)((in.bandwidth + 7) / 8 * 8); all.push_back(w);
+    }
   }
   for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
     Variant v; v.fam = FAM_SELL16_TMA; v.C = C; v.S = S; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;
     if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
     if (S == 1 && skewed) { ++*n_pruned; continue; }
     all.push_back(v);
+    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth > 136 && in.bandwidth <= 4096) {
+      Variant w = v; w.X = 3; w.H = (int)((in.bandwidth + 7) / 8 * 8); all.push_back(w);
+    }
   }
   for (int C : {128, 256, 512}) for (int R : {1, 2}) for (int J : {4, 7, 8, 9, 14}) for (int ST : {2, 3, 4}) {
     Variant v; v.fam = FAM_DIA_TMA; v.C = C; v.R = R; v.U = J; v.I = ST; v.block = C / R + 32;

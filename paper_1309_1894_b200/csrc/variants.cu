@@ -68,7 +68,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_SELL_TMA: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); add("i", v.I); break;
   }
   add("x", v.X);
-  if (v.X == 2) add("h", v.H);
+  if (v.X == 2 || (v.X == 3 && (v.fam == FAM_SELL_TMA || v.fam == FAM_SELL16_TMA))) add("h", v.H);
   if (v.grid > 0) add("g", v.grid);
   if (v.carve >= 0) add("co", v.carve);
   return std::string(buf);
@@ -169,6 +169,12 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (v.L != 0) return no("sell16 has no row splitting");
     if (2 * in.bandwidth + std::max(v.C, v.S) >= 0xFFFF && in.rows > 0)
       return no("column span of a slice can reach 65535: 16-bit deltas do not fit");
+  }
+  if ((v.fam == FAM_SELL_TMA || v.fam == FAM_SELL16_TMA) && v.X == 3) {
+    // x3: every gather of a slice comes out of the shared-memory window, with no fallback path in the kernel
+    if (v.S != 1 || v.L != 0) return no("x3 needs the rows of a slice in natural order (s1, no splitting)");
+    if (v.H < in.bandwidth) return no("x3 needs a window half-width h >= the matrix bandwidth");
+    if ((in.cols & 1) || (v.H & 1) || (v.C & 1)) return no("x3 needs an even column count, h and c (16-byte aligned windows)");
   }
   if (v.L != 0) {
     if (v.fam != FAM_SELL && v.fam != FAM_SELL_TMA) return no("row splitting is a SELL option");

@@ -49,6 +49,9 @@ REPRESENTATIVE_VARIANTS = [
     # x window staged in shared memory (a10 ii)
     "sell_tma:b288:c256:s1:r1:u8:i3:x2:h136", "sell_tma:b160:c256:s1:r2:u4:i3:x2:h72", "sell_tma:b160:c128:s1:r1:u16:i2:x2:h8",
     "sell_tma:b288:c512:s1024:r2:u8:i2:x2:h136", "sell_tma:b160:c128:s8192:l32:r1:u4:i3:x2:h72",
+    # x3: the window covers the whole band -- every gather is a shared-memory read (eligible when h >= bandwidth)
+    "sell_tma:b288:c256:s1:r1:u8:i3:x3:h904", "sell_tma:b160:c128:s1:r1:u4:i6:x3:h4096",
+    "sell16_tma:b160:c128:s1:r1:u8:i4:x3:h1000", "sell16_tma:b288:c512:s1:r2:u4:i4:x3:h904",
     # long rows cut into segments of l entries (virtual rows) + ordered fix-up
     "sell:b256:c128:s8192:l16:r2:u2:x0", "sell:b128:c512:s1024:l64:r1:u4:x0", "sell:b256:c128:s256:l4:r1:u2:x1",
     "sell_tma:b160:c128:s8192:l32:r1:u4:i3:x0", "sell_tma:b160:c256:s2048:l128:r2:u8:i2:x0",

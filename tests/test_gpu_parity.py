@@ -324,6 +324,54 @@ def test_update_values_keeps_the_variant_and_matches_oracle(cuda):
     S.close()
 
 
+def test_full_band_window_x3(cuda):
+    """sell_tma / sell16_tma with x3: the shared-memory x window spans the matrix bandwidth, the kernel has no
+    L1 gather path at all.  Several slices with a ragged last one, windows clipped at both ends of x, beta == 0
+    and != 0, against the oracle; bit-identical to the x0 form of the same shape (same per-row order); an
+    8-byte-aligned x takes the x0 kernel (alt plan); the variant is refused when the window cannot cover the
+    band, when rows are sorted, and for an odd column count."""
+    import torch
+    A = W.banded_random(70001 * 2, 11, 1300, stream=91)        # 140 002 rows: 273.4 slices of 512
+    x, y0 = W.uniform(92, A.cols), W.uniform(93, A.rows)
+    S = binding.SpMV.from_csr(A)
+    bw = int(S.info().bandwidth)
+    assert 0 < bw <= 1300
+    for desc in ("sell_tma:b544:c512:s1:r1:u4:i4", "sell16_tma:b544:c512:s1:r1:u8:i3", "sell16_tma:b288:c512:s1:r2:u8:i3",
+                 "sell16_tma:b160:c128:s1:r1:u4:i6", "sell_tma:b288:c256:s1:r1:u16:i2"):
+        for beta in (0.0, -0.5):
+            S.select(desc + ":x0")
+            y_x0 = H.gpu_apply(S, 1.5, x, beta, None if beta == 0.0 else y0)
+            S.select(desc + ":x3:h1304")
+            y_x3, _, _ = H.check_against_oracle(S, A, 1.5, x, beta, None if beta == 0.0 else y0, what="x3")
+            assert np.array_equal(y_x3, y_x0), (desc, beta)
+            assert np.array_equal(H.gpu_apply(S, 1.5, x, beta, None if beta == 0.0 else y0), y_x3)      # repeatable
+    # 8-byte aligned x: no bulk copy possible, the plan's alternative (x0) kernel runs
+    S.select("sell16_tma:b544:c512:s1:r1:u8:i3:x3:h1304")
+    bx = torch.zeros(A.cols + 2, dtype=torch.float64, device="cuda")
+    dx = bx[1:1 + A.cols]
+    dx.copy_(torch.from_numpy(x))
+    dy = torch.from_numpy(y0).cuda()
+    assert dx.data_ptr() % 16 == 8
+    S.apply(1.5, dx, -0.5, dy)
+    torch.cuda.synchronize()
+    assert np.array_equal(dy.cpu().numpy(), y_x3)
+    for bad in ("sell16_tma:b544:c512:s1:r1:u8:i3:x3:h1000",      # window narrower than the band
+                "sell16_tma:b544:c512:s1024:r1:u8:i3:x3:h1304",   # sorted rows: a slice's rows are not contiguous
+                "sell_tma:b544:c512:s1:r1:u8:i3:x3:h4104"):       # h out of range
+        with pytest.raises(binding.SpmvError) as e:
+            S.select(bad)
+        assert e.value.status == 3, bad
+    S.close()
+    Aodd = W.banded_random(5001, 7, 300, stream=94)            # odd column count: the last column cannot be staged
+    So = binding.SpMV.from_csr(Aodd)
+    with pytest.raises(binding.SpmvError) as e:
+        So.select("sell_tma:b160:c128:s1:r1:u4:i6:x3:h304")
+    assert e.value.status == 3
+    So.select("sell_tma:b160:c128:s1:r1:u4:i3:x2:h304")        # x2 keeps its L1 path for what the window misses
+    H.check_against_oracle(So, Aodd, 1.0, W.uniform(95, Aodd.cols), 0.0, None, what="x2 odd")
+    So.close()
+
+
 def test_unaligned_vectors_take_the_fallback_paths(cuda):
     """x / y that are only 8-byte aligned: the bulk-copy (TMA) paths that need 16-byte aligned global
     addresses (dia_tma old-y stage, sell_tma x2 window) must fall back to plain loads, not fault."""
