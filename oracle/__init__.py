@@ -15,6 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle_spmv.c")
 _SRC_CG = os.path.join(_HERE, "oracle_cg.c")
+_SRC_JAC = os.path.join(_HERE, "oracle_jacobi.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
@@ -22,10 +23,10 @@ _lib = None
 def build(force: bool = False) -> str:
     """Compile oracle_spmv.c -> liboracle.so (-O2, no FMA contraction, OpenMP)."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_CG))):
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_CG), os.path.getmtime(_SRC_JAC))):
         return _LIB
     cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-           "-std=c11", "-Wall", "-o", _LIB, _SRC, _SRC_CG, "-lm"]
+           "-std=c11", "-Wall", "-o", _LIB, _SRC, _SRC_CG, _SRC_JAC, "-lm"]
     subprocess.run(cmd, check=True)
     return _LIB
 
@@ -49,6 +50,8 @@ def _load():
     lib.oracle_accept.restype = None
     lib.oracle_cg.argtypes = [i64, vp, vp, vp, vp, vp, dbl, i64, vp, vp]
     lib.oracle_cg.restype = i64
+    lib.oracle_jacobi.argtypes = [i64, vp, vp, vp, vp, vp, dbl, dbl, i64, vp, vp]
+    lib.oracle_jacobi.restype = i64
     _lib = lib
     return lib
 
@@ -139,3 +142,17 @@ def cg(row_ptr, col_idx, val, b, x0=None, tol=1e-10, max_iters=1000):
     k = lib.oracle_cg(rows, _p(rp), _p(ci), _p(va), _p(b), _p(x), float(tol), int(max_iters),
                       ctypes.byref(rel), _p(hist))
     return x, int(k), rel.value, hist[:int(k) + 1]
+
+
+def jacobi(row_ptr, col_idx, val, b, x0=None, omega=1.0, tol=1e-10, max_iters=1000):
+    """Weighted Jacobi (oracle_jacobi.c).  Returns (x, iters, rel_res, res_hist); iters == -1: zero diagonal."""
+    lib = _load()
+    rp, ci, va = _csr(row_ptr, col_idx, val)
+    rows = rp.size - 1
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    x = np.zeros(rows) if x0 is None else np.array(x0, dtype=np.float64, copy=True)
+    hist = np.full(int(max_iters) + 1, np.nan)
+    rel = ctypes.c_double(0.0)
+    k = lib.oracle_jacobi(rows, _p(rp), _p(ci), _p(va), _p(b), _p(x), float(omega), float(tol), int(max_iters),
+                          ctypes.byref(rel), _p(hist))
+    return x, int(k), rel.value, hist[:max(int(k), 0) + 1]

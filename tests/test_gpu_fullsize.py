@@ -96,6 +96,14 @@ def test_full_size_banded_matrix_16bit_indices(cuda):
         assert ok, (S.variant, nf, ff, mr)
         print(f"banded: {flt or 'all'} -> {S.variant} {rep['winner_us']:.1f} us, format {S.info().format_bytes / 1e6:.0f} MB")
     assert S.variant.startswith("sell16") and S.info().format_bytes < 10.1 * A.nnz + 16 * A.rows
+    # the shared-memory x window (x3: window = the band, double-buffered per slice, no L1 path): every row against
+    # the oracle and 25 back-to-back repeats bit for bit (a refill landing under a reader would show up here)
+    S.select("sell16_tma:b544:c512:s1:r1:u8:i3:x3:h2000")
+    first = _run(S, prob, dx, None).clone()
+    ok, mr, ff, nf = oracle.accept(first.cpu().numpy(), y_ref, scale, H.TOL)
+    assert ok, (S.variant, nf, ff, mr)
+    for _ in range(25):
+        assert torch.equal(_run(S, prob, dx, None), first)
     S.close()
 
 

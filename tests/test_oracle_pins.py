@@ -339,3 +339,101 @@ def test_c5_zero_iterations_and_initial_guess():
     xs = np.linalg.solve(_dense(A), b)
     _, k2, rel2, _ = oracle.cg(A.row_ptr, A.col_idx, A.val, b, x0=xs, tol=1e-10, max_iters=100)
     assert k2 == 0 and rel2 <= 1e-10
+
+
+# ------------------------------------------------------------------ J1-J5: the weighted-Jacobi oracle (oracle_jacobi.c)
+def _sine_mode(n, dim, m):
+    """Eigenvector / eigenvalue of the Dirichlet Laplacian (diag 2*dim, off -1) on an n^dim grid: product of sines."""
+    i = np.arange(1, n + 1)
+    lam = 0.0
+    v = np.ones(1)
+    for mm in m[:dim]:
+        v = np.kron(np.sin(mm * np.pi * i / (n + 1)), v)       # first index fastest: row = i + n*j
+        lam += 2.0 - 2.0 * np.cos(mm * np.pi / (n + 1))
+    return v, lam
+
+
+@pytest.mark.parametrize("dim,n,m,omega", [(2, 12, (1, 1), 1.0), (2, 12, (3, 7), 0.8), (2, 9, (9, 9), 2.0 / 3.0), (3, 6, (2, 5, 1), 0.9)])
+def test_j1_jacobi_closed_form_on_laplacian_eigenvectors(dim, n, m, omega):
+    """b = lambda v (v a sine eigenvector), x0 = 0: x_k = (1 - rho^k) v and ||r_k|| = |rho|^k ||b|| with
+    rho = 1 - omega lambda / d (textbook: the Jacobi iteration matrix I - omega D^-1 A shares A's eigenvectors
+    when the diagonal is constant)."""
+    A = W.laplace2d_5pt(n) if dim == 2 else W.laplace3d_7pt(n)
+    v, lam = _sine_mode(n, dim, m)
+    d = 2.0 * dim
+    rho = 1.0 - omega * lam / d
+    b = lam * v
+    for k in (1, 2, 7, 20):
+        x, it, rel, hist = oracle.jacobi(A.row_ptr, A.col_idx, A.val, b, omega=omega, tol=0.0, max_iters=k)
+        assert it == k and hist.size == k + 1
+        assert np.abs(x - (1.0 - rho ** k) * v).max() <= 1e-13
+        want = np.abs(rho) ** np.arange(k + 1) * np.linalg.norm(b)
+        assert np.abs(hist - want).max() <= 1e-12 * np.linalg.norm(b)
+        assert rel == pytest.approx(abs(rho) ** k, abs=1e-13)
+
+
+def test_j2_diagonal_matrix_is_solved_by_the_first_update_exactly():
+    n = 40
+    d = 0.5 + np.arange(n) % 7
+    Dg = W.CSR(n, n, np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32), d)
+    b = W.uniform(96, n)
+    x, k, rel, hist = oracle.jacobi(Dg.row_ptr, Dg.col_idx, Dg.val, b, omega=1.0, tol=1e-15, max_iters=10)
+    assert k == 1 and np.array_equal(x, b / d) and rel <= 1e-15
+    assert hist[0] == pytest.approx(np.linalg.norm(b), rel=1e-15)
+
+
+@pytest.mark.parametrize("seed,omega", [(0, 1.0), (1, 0.7), (2, 1.0)])
+def test_j3_jacobi_limit_is_the_dense_solution_nonsymmetric(seed, omega):
+    """Strictly row-diagonally-dominant, NON-symmetric, varying diagonal of both signs: Jacobi converges, and to
+    numpy.linalg.solve's answer.  A^T instead of A, d_j instead of d_i, or a sign slip cannot pass."""
+    rng = np.random.default_rng(seed)
+    n = 60
+    lens = rng.integers(2, 9, n)
+    A = W.csr_from_lengths(lens, n, 97 + seed)
+    D = _dense(A)
+    np.fill_diagonal(D, 0.0)
+    diag = (np.abs(D).sum(axis=1) * 1.5 + 1.0) * np.where(np.arange(n) % 3 == 0, -1.0, 1.0)
+    D[np.arange(n), np.arange(n)] = diag
+    rp = [0]; ci = []; va = []
+    for i in range(n):
+        nz = np.nonzero(D[i])[0]
+        ci += nz.tolist(); va += D[i, nz].tolist(); rp.append(len(ci))
+    rp, ci, va = np.array(rp, np.int32), np.array(ci, np.int32), np.array(va)
+    assert not np.allclose(D, D.T)
+    b = W.uniform(99 + seed, n)
+    x, k, rel, hist = oracle.jacobi(rp, ci, va, b, omega=omega, tol=1e-14, max_iters=2000)
+    xs = np.linalg.solve(D, b)
+    assert 0 < k < 2000 and rel <= 1e-14
+    assert np.abs(x - xs).max() <= 1e-12 * np.abs(xs).max()
+    assert np.all(np.diff(hist) < 0)                               # monotone in this (dominant) case
+
+
+def test_j4_zero_iterations_initial_guess_and_zero_rhs():
+    A = W.laplace2d_5pt(6)
+    b = W.uniform(94, A.rows)
+    x0 = W.uniform(95, A.rows)
+    x, k, rel, hist = oracle.jacobi(A.row_ptr, A.col_idx, A.val, b, x0=x0, tol=1e-12, max_iters=0)
+    Ax0, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, x0, 0.0)
+    assert k == 0 and np.array_equal(x, x0)
+    assert rel == pytest.approx(np.linalg.norm(b - Ax0) / np.linalg.norm(b), rel=1e-13)
+    xs = np.linalg.solve(_dense(A), b)                                  # starting at the solution: no update
+    x2, k2, rel2, _ = oracle.jacobi(A.row_ptr, A.col_idx, A.val, b, x0=xs, tol=1e-10, max_iters=100)
+    assert k2 == 0 and np.array_equal(x2, xs)
+    x3, k3, rel3, _ = oracle.jacobi(A.row_ptr, A.col_idx, A.val, np.zeros(A.rows), tol=1e-10, max_iters=100)
+    assert k3 == 0 and rel3 == 0.0 and not x3.any()
+
+
+def test_j5_duplicate_diagonal_entries_sum_and_zero_diagonal_is_refused():
+    # row 0: (0,0)=1.5 and (0,0)=2.5 -> d_0 = 4; row 1: d_1 = 2; off-diagonals small
+    rp = np.array([0, 3, 5], dtype=np.int32)
+    ci = np.array([0, 1, 0, 0, 1], dtype=np.int32)
+    va = np.array([1.5, 0.5, 2.5, -0.25, 2.0])
+    b = np.array([1.0, -2.0])
+    x, k, rel, _ = oracle.jacobi(rp, ci, va, b, omega=1.0, tol=0.0, max_iters=1)
+    assert k == 1 and np.array_equal(x, np.array([1.0 / 4.0, -2.0 / 2.0]))       # x0 = 0: x1 = b / d
+    xs = np.linalg.solve(np.array([[4.0, 0.5], [-0.25, 2.0]]), b)
+    x, k, rel, _ = oracle.jacobi(rp, ci, va, b, tol=1e-15, max_iters=200)
+    assert np.abs(x - xs).max() <= 1e-14
+    x0 = np.array([3.0, 4.0])
+    xz, kz, _, _ = oracle.jacobi(np.array([0, 1, 2], np.int32), np.array([1, 1], np.int32), np.array([1.0, 1.0]), b, x0=x0)
+    assert kz == -1 and np.array_equal(xz, x0)                           # row 0 has no diagonal entry
