@@ -291,6 +291,35 @@ typedef struct {
 SPMV_API spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x, const spmv_cg_opts_t* opts,
                       spmv_cg_result_t* result, void* stream);
 
+/* Second solver loop (SURVEY.md sec. 8(f) rank 3 names "CG / Jacobi using spmv_apply"): the weighted Jacobi
+ * iteration  x_{k+1} = x_k + omega * D^-1 (b - A x_k)  for a square A with a non-zero diagonal (d_i = the sum of
+ * the stored entries (i, i)), the selected SpMV variant as the product.  Per iteration: t = A x_k, then one fused
+ * pass (residual, its norm, next iterate).  The stop test precedes the update: the call stops first when
+ * ||b - A x_k|| <= tol * ||b||, or when k == max_iters; d_x then holds x_k and rel_residual ITS residual.
+ *   d_b [rows] right-hand side (device, read only); d_x [rows] initial guess in, iterate out (device).
+ * Scalars stay on the device; `check_every` (rounded up to even) iterations are replayed as one CUDA graph
+ * between host polls.  A zero diagonal entry: result->zero_diagonal = 1, d_x untouched, SPMV_OK.
+ * Workspace (3 vectors) comes from the handle's allocator for the duration of the call.  Synchronises `stream`.
+ * Errors: INVALID_ARG (rows != cols, NULL), ALLOC, CUDA. */
+typedef struct {
+  double omega;          /* 0 -> 1.0 */
+  double tol;            /* 0 -> 1e-10 */
+  int32_t max_iters;     /* 0 -> 1000; negative -> 0 iterations (residual of the initial guess only) */
+  int32_t check_every;   /* 0 -> 8 */
+  int32_t no_graph;      /* 1: never use a CUDA graph */
+} spmv_jacobi_opts_t;
+typedef struct {
+  int32_t iters, converged, zero_diagonal;
+  int32_t iterations_launched;   /* > iters: the pass that meets the stop rule, and passes issued after it, update nothing */
+  int32_t graph_replays;
+  int32_t kernels_per_iteration;
+  double rel_residual;           /* ||b - A x|| / ||b|| of the returned x  (the norm itself when b == 0) */
+  double device_seconds;         /* CUDA events around the whole call */
+  double wall_seconds;
+} spmv_jacobi_result_t;
+SPMV_API spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double* d_x, const spmv_jacobi_opts_t* opts,
+                          spmv_jacobi_result_t* result, void* stream);
+
 /* Writes the newline-separated descriptors of every candidate the tuner would
  * enumerate for this matrix (after structural pruning) into buf; *len = bytes needed. */
 SPMV_API spmv_status_t spmv_list_variants(spmv_handle_t h, char* buf, size_t cap, size_t* len);

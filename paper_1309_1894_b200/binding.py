@@ -20,7 +20,7 @@ STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "S
 
 EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_status_string",
+           "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache", "spmv_graph_create", "spmv_graph_launch",
            "spmv_graph_destroy", "spmv_partition_rows", "spmv_external_columns", "spmv_gather", "spmv_scatter",
            "spmv_apply_rows"]
@@ -76,6 +76,17 @@ class CgResult(C.Structure):
                 ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
 
 
+class JacobiOpts(C.Structure):
+    _fields_ = [("omega", C.c_double), ("tol", C.c_double), ("max_iters", C.c_int32), ("check_every", C.c_int32),
+                ("no_graph", C.c_int32)]
+
+
+class JacobiResult(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("zero_diagonal", C.c_int32),
+                ("iterations_launched", C.c_int32), ("graph_replays", C.c_int32), ("kernels_per_iteration", C.c_int32),
+                ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
+
+
 class TuneReport(C.Structure):
     _fields_ = [("winner", C.c_char * 128), ("winner_us", C.c_double), ("default_us", C.c_double),
                 ("n_enumerated", C.c_int32), ("n_pruned_structural", C.c_int32),
@@ -111,6 +122,7 @@ def lib():
     L.spmv_measure_ceiling.argtypes = [i32, C.c_size_t, i32, vp, C.POINTER(dbl)]
     L.spmv_update_values.argtypes = [vp, vp, C.POINTER(i32), vp]
     L.spmv_cg.argtypes = [vp, vp, vp, C.POINTER(CgOpts), C.POINTER(CgResult), vp]
+    L.spmv_jacobi.argtypes = [vp, vp, vp, C.POINTER(JacobiOpts), C.POINTER(JacobiResult), vp]
     L.spmv_graph_create.argtypes = [vp, dbl, vp, dbl, vp, i32, C.POINTER(vp)]
     L.spmv_graph_launch.argtypes = [vp, vp]
     L.spmv_graph_destroy.argtypes = [vp]
@@ -121,7 +133,7 @@ def lib():
     L.spmv_apply_rows.argtypes = [vp, dbl, vp, dbl, vp, i64, i64, C.POINTER(i64), vp]
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
-              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg",
+              "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi",
               "spmv_graph_create", "spmv_graph_launch", "spmv_graph_destroy", "spmv_partition_rows",
               "spmv_external_columns", "spmv_gather", "spmv_scatter", "spmv_apply_rows"):
         getattr(L, n).restype = C.c_int
@@ -290,6 +302,15 @@ class SpMV:
         out = {k: getattr(r, k) for k, _ in CgResult._fields_}
         out["loop_variant"] = out["loop_variant"].decode()
         return out
+
+    def jacobi(self, b, x, *, omega=1.0, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, stream=None) -> dict:
+        """Weighted Jacobi with the selected variant (spmv_jacobi).  x: initial guess in, iterate out."""
+        assert b.is_cuda and x.is_cuda and b.numel() == self.rows and x.numel() == self.rows
+        o = JacobiOpts(float(omega), float(tol), int(max_iters) if max_iters > 0 else -1, int(check_every),
+                       int(bool(no_graph)))
+        r = JacobiResult()
+        _check(lib().spmv_jacobi(self.h, _dptr(b), _dptr(x), C.byref(o), C.byref(r), _stream_ptr(stream)), "spmv_jacobi")
+        return {k: getattr(r, k) for k, _ in JacobiResult._fields_}
 
     def apply_rows(self, alpha, x, beta, y, row_begin: int, row_end: int, stream=None):
         """spmv_apply restricted to rows [row_begin, row_end); x, y are the whole vectors."""

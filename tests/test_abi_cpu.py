@@ -67,6 +67,7 @@ def test_null_and_bad_arguments_return_codes(L):
     assert L.spmv_external_columns(None, 0, 0, None, 0, None, None, None, None) == 1
     assert L.spmv_partition_rows(4, None, 2, 1, None) == 1
     assert L.spmv_cg(None, None, None, None, None, None) == 1
+    assert L.spmv_jacobi(None, None, None, None, None, None) == 1
 
 
 def test_struct_sizes_match_header():
@@ -77,6 +78,9 @@ def test_struct_sizes_match_header():
     assert ctypes.sizeof(binding.CgOpts) == 8 + 6 * 4
     assert ctypes.sizeof(binding.CgResult) == 8 * 4 + 128 + 3 * 8
     assert binding.CgResult.rel_residual.offset == 160 and binding.CgResult.loop_variant.offset == 32
+    # spmv_jacobi_opts_t: 2 doubles + 3 int32 (+ 4 padding); spmv_jacobi_result_t: 6 int32 + 3 doubles
+    assert ctypes.sizeof(binding.JacobiOpts) == 2 * 8 + 3 * 4 + 4
+    assert ctypes.sizeof(binding.JacobiResult) == 6 * 4 + 3 * 8 and binding.JacobiResult.rel_residual.offset == 24
     # spmv_tune_report_t: the log buffer triple closes the struct
     assert binding.TuneReport.log_len.offset + 8 == ctypes.sizeof(binding.TuneReport)
 
