@@ -425,7 +425,8 @@ spmv_status_t spmv_format_download(spmv_handle_t h, const char* name, void* h_bu
     else if (!strcmp(name, "perm") && sf->perm) { src = sf->perm; n = sizeof(int32_t) * sf->nslices * sf->C; }
   } else if (v.fam == FAM_BCSR3 && h->has_bcsr) {
     if (!strcmp(name, "brow_ptr")) { src = h->bcsr.brow_ptr; n = sizeof(int32_t) * (h->bcsr.brows + 1); }
-    else if (!strcmp(name, "bcol")) { src = h->bcsr.bcol; n = sizeof(int32_t) * h->bcsr.nblocks; }
+    else if (!strcmp(name, "bcol") && h->bcsr.bcol) { src = h->bcsr.bcol; n = sizeof(int32_t) * h->bcsr.nblocks; }
+    else if (!strcmp(name, "bcol16") && h->bcsr.bcol16) { src = h->bcsr.bcol16; n = sizeof(uint16_t) * h->bcsr.nblocks; }
     else if (!strcmp(name, "bval")) { src = h->bcsr.bval; n = sizeof(double) * 9 * h->bcsr.nblocks; }
   } else if ((v.fam == FAM_DIA || v.fam == FAM_DIA_TMA || v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_WIN || v.fam == FAM_DIA_CWIN) && h->dias.count(v.C)) {
     const DiaFormat& df = h->dias[v.C];

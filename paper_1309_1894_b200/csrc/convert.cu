@@ -470,8 +470,50 @@ __global__ void bcsr3_merge_kernel(int64_t brows, const int* __restrict__ rp, co
   }
 }
 
+// 16-bit block columns (the BCSR counterpart of sell16): a block row of a banded matrix
+// references block columns near its own index, so bcol - block row + 32768 fits 16 bits: 74 B per block, not 76
+__global__ void bcsr3_narrow_kernel(int64_t brows, const int* __restrict__ bp, const int* __restrict__ bcol,
+                                    unsigned short* __restrict__ bcol16, int* __restrict__ bad) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= brows) return;
+  for (int k = bp[b]; k < bp[b + 1]; ++k) {
+    const int64_t d = (int64_t)bcol[k] - b + 32768;
+    if (d < 0 || d > 65535) { *bad = 1; bcol16[k] = 0; }
+    else bcol16[k] = (unsigned short)d;
+  }
+}
+
+// bytes of the bcol16 allocation: the indices, padded to 4 bytes, then the converter's flag word
+static size_t bcol16_bytes(int64_t nblocks) { return (((size_t)std::max<int64_t>(nblocks, 1) * 2 + 3) & ~(size_t)3) + sizeof(int); }
+
+spmv_status_t bcsr3_narrow_indices(BcsrFormat& f, Allocator& al, cudaStream_t s) {
+  if (f.bcol16) return SPMV_OK;
+  if (!f.bcol) return SPMV_ERR_INTERNAL;
+  const size_t bytes = bcol16_bytes(f.nblocks);
+  uint16_t* c16 = (uint16_t*)al.alloc(bytes, s);
+  if (!c16) return SPMV_ERR_ALLOC;
+  struct Guard { uint16_t* p; size_t n; Allocator& al; bool keep; ~Guard() { if (!keep) al.free(p, n); } } guard{c16, bytes, al, false};
+  int* d_bad = (int*)((char*)c16 + bytes - sizeof(int));
+  SPMV_CUDA_TRY(cudaMemsetAsync(d_bad, 0, sizeof(int), s));
+  bcsr3_narrow_kernel<<<(unsigned)((f.brows + 127) / 128), 128, 0, s>>>(f.brows, f.brow_ptr, f.bcol, c16, d_bad);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  int bad = 0;
+  SPMV_CUDA_TRY(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
+  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+  if (bad) { set_last_error("bcsr3 i16: a block column is 32768 or more block rows away from its block row"); return SPMV_ERR_UNSUPPORTED; }
+  guard.keep = true;
+  f.bcol16 = c16;
+  return SPMV_OK;
+}
+
+void bcsr3_drop_indices(BcsrFormat& f, Allocator& al, bool drop16) {
+  if (drop16 && f.bcol16) { al.free(f.bcol16, bcol16_bytes(f.nblocks)); f.bcol16 = nullptr; }
+  if (!drop16 && f.bcol && f.bcol16) { al.free(f.bcol, sizeof(int32_t) * std::max<int64_t>(f.nblocks, 1)); f.bcol = nullptr; }
+}
+
 void free_bcsr3(BcsrFormat& f, Allocator& al) {
   if (f.brow_ptr) al.free(f.brow_ptr, sizeof(int32_t) * (f.brows + 1));
+  if (f.bcol16) al.free(f.bcol16, bcol16_bytes(f.nblocks));
   if (f.bcol) al.free(f.bcol, sizeof(int32_t) * std::max<int64_t>(f.nblocks, 1));
   if (f.bval) al.free(f.bval, sizeof(double) * 9 * std::max<int64_t>(f.nblocks, 1));
   f = BcsrFormat();

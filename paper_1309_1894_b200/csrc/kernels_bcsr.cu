@@ -4,7 +4,7 @@
 // are stored TRANSPOSED inside the block row (element k of block j at 9*start + k*nb + j),
 // a library-owned layout, so that each of the 9 value loads is contiguous across lanes
 // instead of striding by 72 bytes.  One int32 block column per 9 values: 8.44 B/nnz
-// instead of CSR's 12.  x is read as the 3-vector x[3*bc .. 3*bc+2]: three 8-byte loads (X = 0, 1), or -- X = 3 --
+// instead of CSR's 12 (8.22 B/nnz with the 16-bit block columns of variant key i16).  x is read as the 3-vector x[3*bc .. 3*bc+2]: three 8-byte loads (X = 0, 1), or -- X = 3 --
 // one aligned 16-byte pair plus one 8-byte load (the pair starts at 3*bc for an even block column, at 3*bc + 1
 // for an odd one): a third fewer L1 requests on the x path, which is where this kernel's L1TEX time goes
 // (each lane of a warp touches another line of x).  X = 3 needs a 16-byte aligned x; otherwise it runs as X = 0.
@@ -13,11 +13,23 @@
 
 namespace spmv {
 
-template <int T, int U, int X>
+__device__ __forceinline__ int ld_bcol(const int* p, int) { return ld_stream(p); }
+// 16-bit form (variant key i16): block column = stored delta - 32768 + the block row's index in the whole matrix.
+// Measured on cfg4 (74 instead of 76 B per block): wins with three 8-byte x loads (x0: 296.6 vs 306.0 us) but loses
+// with the pair loads of x3 (312 vs 286 us; loading the index as its aligned 32-bit word: 320 us), so the tuner
+// keeps the 32-bit x3 form there -- the variant stays enumerated, the measurement decides per matrix.
+__device__ __forceinline__ int ld_bcol(const unsigned short* p, int br_global) {
+  unsigned short v;
+  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(v) : "l"(p));
+  return (int)v - 32768 + br_global;
+}
+
+// br0: index of the range's first block row in the whole matrix (row-range launches; 0 otherwise)
+template <int T, int U, int X, typename IT>
 __global__ void __launch_bounds__(1024)
-bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol,
+bcsr3_kernel(int brows, const int* __restrict__ bp, const IT* __restrict__ bcol,
              const double* __restrict__ bval, double alpha, const double* __restrict__ x,
-             double beta, double* __restrict__ y) {
+             double beta, double* __restrict__ y, int br0) {
   const int lane = threadIdx.x & (T - 1);
   const bool xpair = (reinterpret_cast<uintptr_t>(x) & 15) == 0;
   const int sub_in_warp = (threadIdx.x & 31) / T;
@@ -29,7 +41,7 @@ bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol
     const int start = ok ? __ldg(bp + br) : 0;
     const int nb = ok ? __ldg(bp + br + 1) - start : 0;
     const double* pv = bval + 9 * (int64_t)start;
-    const int* pc = bcol + start;
+    const IT* pc = bcol + start;
     double s0 = 0.0, s1 = 0.0, s2 = 0.0;
     for (int j = lane; j < nb; j += T * U) {
       double v[U][9];
@@ -38,7 +50,7 @@ bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol
       for (int u = 0; u < U; ++u) {
         const int jj = j + u * T;
         const bool in = jj < nb;
-        c[u] = in ? ld_stream(pc + jj) : -1;
+        c[u] = in ? ld_bcol(pc + jj, (int)br + br0) : -1;
 #pragma unroll
         for (int k = 0; k < 9; ++k) v[u][k] = in ? ld_stream(pv + (int64_t)k * nb + jj) : 0.0;
       }
@@ -70,37 +82,40 @@ bcsr3_kernel(int brows, const int* __restrict__ bp, const int* __restrict__ bcol
   }
 }
 
-typedef void (*bcsr_kernel_t)(int, const int*, const int*, const double*, double, const double*, double,
-                              double*);
-
-template <int X>
-static bcsr_kernel_t pick_tu(int T, int U) {
-#define P(t, u) if (T == t && U == u) return bcsr3_kernel<t, u, X>;
+template <int X, typename IT>
+static const void* pick_tu(int T, int U) {
+#define P(t, u) if (T == t && U == u) return (const void*)bcsr3_kernel<t, u, X, IT>;
   P(4, 1) P(4, 2) P(8, 1) P(8, 2) P(16, 1) P(16, 2) P(32, 1) P(32, 2)
 #undef P
   return nullptr;
 }
-static bcsr_kernel_t pick(const Variant& v) {
-  return v.X == 0 ? pick_tu<0>(v.W, v.U) : v.X == 1 ? pick_tu<1>(v.W, v.U) : v.X == 3 ? pick_tu<3>(v.W, v.U) : nullptr;
+template <typename IT>
+static const void* pick_x(const Variant& v) {
+  return v.X == 0 ? pick_tu<0, IT>(v.W, v.U) : v.X == 1 ? pick_tu<1, IT>(v.W, v.U) : v.X == 3 ? pick_tu<3, IT>(v.W, v.U) : nullptr;
+}
+static const void* pick(const Variant& v) {
+  return v.I == 16 ? pick_x<unsigned short>(v) : v.I == 0 ? pick_x<int>(v) : nullptr;
 }
 
 bool bcsr_supported(const Variant& v) {
   return v.block >= 32 && v.block <= 1024 && v.block % 32 == 0 && pick(v) != nullptr;
 }
 cudaError_t bcsr_plan(const Variant& v, const BcsrFormat& f, int sm_count, LaunchPlan* out) {
-  bcsr_kernel_t k = pick(v);
-  if (!k) return cudaErrorInvalidValue;
+  const void* k = pick(v);
+  if (!k || (v.I == 16 ? !f.bcol16 : !f.bcol)) return cudaErrorInvalidValue;
   *out = LaunchPlan();
   if (f.brows == 0) return cudaSuccess;
   KernelCall& c = out->k[0];
-  c.fn = (const void*)k;
+  c.fn = k;
   c.block = v.block;
   const int64_t per_block = v.block / v.W;
   const int64_t exact = (f.brows + per_block - 1) / per_block;
   cudaError_t e = resolve_grid(v.grid, c.fn, v.block, 0, sm_count, exact, &c.grid);
   if (e != cudaSuccess) return e;
-  c.add((int)f.brows); c.add((const int*)f.brow_ptr); c.add((const int*)f.bcol); c.add((const double*)f.bval);
+  c.add((int)f.brows); c.add((const int*)f.brow_ptr);
+  c.add(v.I == 16 ? (const void*)f.bcol16 : (const void*)f.bcol); c.add((const double*)f.bval);
   c.add_alpha(); c.add_x(); c.add_beta(); c.add_y();
+  c.add((int)0);                 // argument 8: br0, set by plan_for_rows
   c.per_block = per_block;       // block rows
   out->n = 1;
   out->range_kind = RANGE_BCSR;

@@ -58,6 +58,7 @@ struct BcsrFormat {
   int64_t brows = 0, nblocks = 0;
   int32_t* brow_ptr = nullptr;   // [brows+1]
   int32_t* bcol = nullptr;       // [nblocks] block column
+  uint16_t* bcol16 = nullptr;    // [nblocks] 16-bit form (variant key i16): bcol - block row + 32768; built on demand
   double* bval = nullptr;        // [9*nblocks]
   double fill = 0.0;             // nnz / (9*nblocks)
 };
@@ -279,6 +280,9 @@ spmv_status_t sell_narrow_indices(SellFormat& f, Allocator& al, cudaStream_t s);
 void free_sell(SellFormat& f, Allocator& al);
 spmv_status_t build_bcsr3(const CsrView& A, Allocator& al, cudaStream_t s, BcsrFormat* out);
 void free_bcsr3(BcsrFormat& f, Allocator& al);
+// bcol16 from bcol (UNSUPPORTED when some |bcol - block row| >= 32768); drop one of the two index arrays
+spmv_status_t bcsr3_narrow_indices(BcsrFormat& f, Allocator& al, cudaStream_t s);
+void bcsr3_drop_indices(BcsrFormat& f, Allocator& al, bool drop16);
 spmv_status_t build_dia(const CsrView& A, int C, Allocator& al, cudaStream_t s, DiaFormat* out);
 void free_dia(DiaFormat& f, Allocator& al);
 spmv_status_t build_merge_plan(const CsrView& A, int tile_items, Allocator& al, cudaStream_t s,

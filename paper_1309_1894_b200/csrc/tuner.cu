@@ -94,8 +94,8 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     for (int I : {5, 7, 11}) {
       Variant v; v.fam = FAM_MERGE; v.block = b; v.I = I; all.push_back(v);
     }
-    for (int W : {4, 8, 16, 32}) for (int U : {1, 2}) for (int X : {0, 3}) {
-      Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; v.X = X; all.push_back(v);
+    for (int W : {4, 8, 16, 32}) for (int U : {1, 2}) for (int X : {0, 3}) for (int I : {0, 16}) {
+      Variant v; v.fam = FAM_BCSR3; v.block = b; v.W = W; v.U = U; v.X = X; v.I = I; all.push_back(v);
     }
   }
   for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
@@ -113,8 +113,8 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     if (S == 1 && (J == 4 || J == 8) && ST <= 3)
       for (int H : {72, 136}) { Variant w = v; w.X = 2; w.H = H; all.push_back(w); }
     // banded matrix: a window as wide as the band takes EVERY gather of a slice out of shared memory
-    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth > 136 && in.bandwidth <= 4096) {
-      Variant w = v; w.X = 3; w.H = (int)((in.bandwidth + 7) / 8 * 8); all.push_back(w);
+    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth <= 4096 && in.rows > 0) {
+      Variant w = v; w.X = 3; w.H = (int)std::max<int64_t>(8, (in.bandwidth + 7) / 8 * 8); all.push_back(w);
     }
   }
   for (int C : {128, 256, 512}) for (int S : {1, 8192}) for (int R : {1, 2}) for (int J : {4, 8, 16}) for (int ST : {2, 3, 4, 6}) {
@@ -122,8 +122,8 @@ std::vector<Variant> enumerate_candidates(const spmv_handle_s* h, const char* fi
     if (S > 1 && in.var_row_len == 0.0) { ++*n_pruned; continue; }
     if (S == 1 && skewed) { ++*n_pruned; continue; }
     all.push_back(v);
-    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth > 136 && in.bandwidth <= 4096) {
-      Variant w = v; w.X = 3; w.H = (int)((in.bandwidth + 7) / 8 * 8); all.push_back(w);
+    if (S == 1 && (J == 4 || J == 8) && ST >= 3 && in.bandwidth <= 4096 && in.rows > 0) {
+      Variant w = v; w.X = 3; w.H = (int)std::max<int64_t>(8, (in.bandwidth + 7) / 8 * 8); all.push_back(w);
     }
   }
   for (int C : {128, 256, 512}) for (int R : {1, 2}) for (int J : {4, 7, 8, 9, 14}) for (int ST : {2, 3, 4}) {

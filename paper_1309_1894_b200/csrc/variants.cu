@@ -58,7 +58,7 @@ std::string variant_to_string(const Variant& v) {
     case FAM_SELL: add("c", v.C); add("s", v.S); if (v.L > 0) add("l", v.L); add("r", v.R); add("u", v.U); break;
     case FAM_ELL: add("r", v.R); add("u", v.U); break;
     case FAM_MERGE: add("i", v.I); break;
-    case FAM_BCSR3: add("w", v.W); add("u", v.U); break;
+    case FAM_BCSR3: add("w", v.W); add("u", v.U); if (v.I == 16) add("i", 16); break;
     case FAM_DIA: add("c", v.C); add("r", v.R); add("u", v.U); break;
     case FAM_DIA_TMA: add("c", v.C); add("r", v.R); add("u", v.U); add("i", v.I); break;
     case FAM_DIA_CONST: add("r", v.R); break;
@@ -156,6 +156,8 @@ bool variant_eligible(const spmv_handle_s* h, const Variant& v, std::string* why
     if (in.rows % 3 || in.cols % 3 || in.rows == 0) return no("rows/cols not multiples of 3");
     if (!in.cols_sorted) return no("BCSR needs sorted unique columns");
     if (!in.block3_full) return no("3x3 block fill < 1.0 (zero fill would multiply x; reading A7)");
+    // i16: |block column - block row| <= (|col - row| + 2) / 3 must stay below 32768
+    if (v.I == 16 && (in.bandwidth + 2) / 3 >= 32768) return no("bcsr3 i16: block columns up to 32768 block rows away: 16-bit deltas do not fit");
   }
   if ((v.fam == FAM_DIA_CONST || v.fam == FAM_DIA_CWIN) && h->dia_state == 2)
     return no("coefficients are not constant along the diagonals");
@@ -218,10 +220,17 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
       return st;
     }
     case FAM_BCSR3: {
-      if (h->has_bcsr) return SPMV_OK;
-      spmv_status_t st = build_bcsr3(h->A, h->al, s, &h->bcsr);
-      if (st == SPMV_OK) h->has_bcsr = true;
-      return st;
+      if (h->has_bcsr && !h->bcsr.bcol) {          // only the 16-bit indices were kept: rebuild for either form
+        cudaDeviceSynchronize();
+        free_bcsr3(h->bcsr, h->al);
+        h->has_bcsr = false;
+      }
+      if (!h->has_bcsr) {
+        spmv_status_t st = build_bcsr3(h->A, h->al, s, &h->bcsr);
+        if (st != SPMV_OK) return st;
+        h->has_bcsr = true;
+      }
+      return v.I == 16 ? bcsr3_narrow_indices(h->bcsr, h->al, s) : SPMV_OK;
     }
     case FAM_DIA_WIN:
     case FAM_DIA_CWIN:
@@ -268,7 +277,7 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   const bool keeps_sell = is_sell_family(keep);
   const bool keeps_dia = keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST ||
                          keep.fam == FAM_DIA_WIN || keep.fam == FAM_DIA_CWIN;
-  size_t n_free = (h->has_ell && keep.fam != FAM_ELL) + (h->has_bcsr && keep.fam != FAM_BCSR3);
+  size_t n_free = (h->has_ell && keep.fam != FAM_ELL) + (h->has_bcsr && (keep.fam != FAM_BCSR3 || h->bcsr.bcol16));
   for (const auto& kv : h->sells) n_free += !(keeps_sell && kv.first == sell_key(keep));
   for (const auto& kv : h->dias) n_free += !(keeps_dia && kv.first == keep.C);
   for (const auto& kv : h->plans) n_free += !(keep.fam == FAM_MERGE && kv.first == keep.block * keep.I);
@@ -280,6 +289,7 @@ void release_formats_except(spmv_handle_s* h, const Variant& keep) {
   }
   if (h->has_ell && keep.fam != FAM_ELL) { free_sell(h->ell, h->al); h->has_ell = false; }
   if (h->has_bcsr && keep.fam != FAM_BCSR3) { free_bcsr3(h->bcsr, h->al); h->has_bcsr = false; }
+  else if (h->has_bcsr) bcsr3_drop_indices(h->bcsr, h->al, keep.I != 16);        // the index array the kept variant does not read
   for (auto it = h->dias.begin(); it != h->dias.end();) {
     if ((keep.fam == FAM_DIA || keep.fam == FAM_DIA_TMA || keep.fam == FAM_DIA_CONST || keep.fam == FAM_DIA_WIN ||
          keep.fam == FAM_DIA_CWIN) && it->first == keep.C) { ++it; continue; }
@@ -313,7 +323,7 @@ int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v) {
              (f.perm ? f.nslices * (int64_t)f.C * 4 : 0) + f.nparts * 16 + f.nsplit * 8;
     }
     case FAM_ELL: return h->has_ell ? h->ell.padded * 12 + 16 : 0;
-    case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * 76 + (h->bcsr.brows + 1) * 4 : 0;
+    case FAM_BCSR3: return h->has_bcsr ? h->bcsr.nblocks * (v.I == 16 ? 74 : 76) + (h->bcsr.brows + 1) * 4 : 0;
     case FAM_DIA_CWIN:
     case FAM_DIA_CONST: {
       auto it = h->dias.find(v.C);
@@ -410,6 +420,7 @@ bool plan_for_rows(const LaunchPlan& p, int64_t rows, int64_t cols, int64_t a, i
     case RANGE_BCSR:                     // block rows, brow_ptr
       c.set(0, (int)((b - a) / 3));
       shift(1, 4 * (a / 3));
+      c.set(8, (int)(a / 3));            // br0: the 16-bit block columns are relative to the block row's own index
       c.y_off = a;
       units = (b - a) / 3;
       break;

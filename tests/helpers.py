@@ -65,6 +65,8 @@ REPRESENTATIVE_VARIANTS = [
     "dia_tma:b288:c256:r1:u8:i3:x0", "dia_tma:b96:c128:r2:u4:i2:x0", "dia_tma:b544:c512:r1:u7:i4:x0", "dia_tma:b160:c256:r2:u9:i2:x0:g2",
     "merge:b128:i5:x0", "merge:b256:i7:x0", "merge:b256:i11:x1", "merge:b512:i7:x0", "merge:b128:i11:x0",
     "bcsr3:b256:w4:u1:x0", "bcsr3:b128:w8:u2:x0", "bcsr3:b256:w16:u1:x1", "bcsr3:b256:w32:u2:x0:g1", "bcsr3:b512:w16:u2:x3:g1", "bcsr3:b128:w8:u1:x3",
+    # 16-bit block columns
+    "bcsr3:b128:w8:u2:i16:x0", "bcsr3:b256:w16:u1:i16:x3:g1", "bcsr3:b256:w4:u2:i16:x1",
 ]
 
 

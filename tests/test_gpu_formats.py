@@ -279,6 +279,38 @@ def test_bcsr3_layout_matches_numpy(cuda):
             ra, re = A.row_ptr[3 * b + r], A.row_ptr[3 * b + r + 1]
             assert np.array_equal(blk[3 * r:3 * r + 3, :].T.reshape(-1), A.val[ra:re])
     assert S.info().format_bytes == int(bp[-1]) * 76 + (brows + 1) * 4
+    # 16-bit block columns (variant key i16): bcol - block row + 32768; selecting it drops the 32-bit array
+    S.select("bcsr3:b256:w8:u1:i16:x0")
+    assert S.variant == "bcsr3:b256:w8:u1:i16:x0"
+    bc16 = S.download("bcol16", np.uint16)
+    brow_of = np.repeat(np.arange(brows), np.diff(bp))
+    assert np.array_equal(bc16.astype(np.int64), bc.astype(np.int64) - brow_of + 32768)
+    assert S.info().format_bytes == int(bp[-1]) * 74 + (brows + 1) * 4
+    with pytest.raises(binding.SpmvError):
+        S.download("bcol", np.int32)
+    S.select("bcsr3:b256:w8:u1:x0")                                    # and back: the 32-bit form is rebuilt
+    assert np.array_equal(S.download("bcol", np.int32), bc)
+    S.close()
+
+
+def test_bcsr3_i16_refused_when_block_columns_are_far(cuda):
+    """bcsr3 i16 stores bcol - block row + 32768 in 16 bits: a matrix with a block 35 000 block rows away from the
+    diagonal is refused for i16 (structurally, from the bandwidth statistic) and runs with 32-bit block columns."""
+    brows = 40000
+    far = (np.arange(brows) + 35000) % brows
+    bcols = np.sort(np.stack([np.arange(brows), far], axis=1), axis=1)            # two dense 3x3 blocks per block row
+    cols = (3 * bcols[:, None, :, None] + np.arange(3)[None, None, None, :]).repeat(3, axis=1).reshape(3 * brows, 6)
+    rp = (6 * np.arange(3 * brows + 1)).astype(np.int32)
+    A = W.CSR(3 * brows, 3 * brows, rp, cols.reshape(-1).astype(np.int32), W.normal(27, 18 * brows))
+    x = W.uniform(28, A.cols)
+    S = binding.SpMV.from_csr(A)
+    assert S.info().block3_full == 1
+    with pytest.raises(binding.SpmvError) as e:
+        S.select("bcsr3:b256:w8:u1:i16:x0")
+    assert e.value.status == 3
+    assert not any(":i16" in d for d in S.variants() if d.startswith("bcsr3"))
+    S.select("bcsr3:b256:w4:u1:x0")
+    H.check_against_oracle(S, A, 1.0, x, 0.0, None, what="bcsr3 far blocks")
     S.close()
 
 

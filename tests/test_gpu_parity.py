@@ -192,7 +192,7 @@ def test_apply_host_pipeline_is_bit_identical_to_device_apply(cuda, which):
                  "merge:b256:i7:x0", "ell:b256:r1:u2:x0"]       # the last two have no range form: one launch
     elif which == "fem":
         A = W.fem_block27(56)                                  # 526 848 rows, dense 3x3 blocks
-        descs = ["bcsr3:b256:w8:u2:x0", "bcsr3:b512:w16:u2:x0:g1", "csr_vector:b256:w32:u2:x0"]
+        descs = ["bcsr3:b256:w8:u2:x0", "bcsr3:b512:w16:u2:x0:g1", "bcsr3:b128:w16:u2:i16:x3:g8", "csr_vector:b256:w32:u2:x0"]
     else:
         A = W.banded_random(700001, 9, 1500, stream=83)
         descs = ["sell16:b256:c512:s1:r4:u2:x0", "sell16_tma:b544:c512:s1:r1:u4:i4:x0", "sell:b128:c128:s8192:r1:u2:x0", "csr_scalar:b256:r2:u2:x0:g2"]
