@@ -15,9 +15,9 @@ namespace spmv {
 
 __device__ __forceinline__ int ld_bcol(const int* p, int) { return ld_stream(p); }
 // 16-bit form (variant key i16): block column = stored delta - 32768 + the block row's index in the whole matrix.
-// Measured on cfg4 (74 instead of 76 B per block): wins with three 8-byte x loads (x0: 296.6 vs 306.0 us) but loses
-// with the pair loads of x3 (312 vs 286 us; loading the index as its aligned 32-bit word: 320 us), so the tuner
-// keeps the 32-bit x3 form there -- the variant stays enumerated, the measurement decides per matrix.
+// Measured on cfg4 (74 instead of 76 B per block): with three 8-byte x loads (x0) 281.5 us against 288.7 us for 32-bit
+// block columns and 286 us for the 32-bit x3 form (the round-2 winner until then); with the pair loads of x3 it loses
+// (312 vs 286 us; loading the index as its aligned 32-bit word: 320 us).  The tuner's measurement decides per matrix.
 __device__ __forceinline__ int ld_bcol(const unsigned short* p, int br_global) {
   unsigned short v;
   asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(v) : "l"(p));
@@ -26,7 +26,7 @@ __device__ __forceinline__ int ld_bcol(const unsigned short* p, int br_global) {
 
 // br0: index of the range's first block row in the whole matrix (row-range launches; 0 otherwise)
 template <int T, int U, int X, typename IT>
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(X == 3 ? 1024 : 512)
 bcsr3_kernel(int brows, const int* __restrict__ bp, const IT* __restrict__ bcol,
              const double* __restrict__ bval, double alpha, const double* __restrict__ x,
              double beta, double* __restrict__ y, int br0) {
@@ -54,22 +54,44 @@ bcsr3_kernel(int brows, const int* __restrict__ bp, const IT* __restrict__ bcol,
 #pragma unroll
         for (int k = 0; k < 9; ++k) v[u][k] = in ? ld_stream(pv + (int64_t)k * nb + jj) : 0.0;
       }
+      if constexpr (X == 3) {
+        // pair loads: per-block branches (measured on cfg4: 286 us; with the loads of both blocks hoisted above the
+        // FMAs as in the other branch the kernel needs 70 registers and takes 310 us, 297 us when held to 64)
 #pragma unroll
-      for (int u = 0; u < U; ++u) {
-        if (c[u] >= 0) {
-          const double* px = x + 3 * (int64_t)c[u];
-          double x0, x1, x2;
-          if (X == 3 && xpair) {
-            const int p = c[u] & 1;
-            const double2 a = __ldg(reinterpret_cast<const double2*>(px + p));
-            const double b = __ldg(px + (p ? 0 : 2));
-            x0 = p ? b : a.x; x1 = p ? a.x : a.y; x2 = p ? a.y : b;
-          } else {
-            x0 = ldx<(X == 3 ? 0 : X)>(px, 0); x1 = ldx<(X == 3 ? 0 : X)>(px, 1); x2 = ldx<(X == 3 ? 0 : X)>(px, 2);
+        for (int u = 0; u < U; ++u) {
+          if (c[u] >= 0) {
+            const double* px = x + 3 * (int64_t)c[u];
+            double x0, x1, x2;
+            if (xpair) {
+              const int p = c[u] & 1;
+              const double2 a = __ldg(reinterpret_cast<const double2*>(px + p));
+              const double b = __ldg(px + (p ? 0 : 2));
+              x0 = p ? b : a.x; x1 = p ? a.x : a.y; x2 = p ? a.y : b;
+            } else {
+              x0 = ldx<0>(px, 0); x1 = ldx<0>(px, 1); x2 = ldx<0>(px, 2);
+            }
+            s0 = fma(v[u][0], x0, fma(v[u][1], x1, fma(v[u][2], x2, s0)));
+            s1 = fma(v[u][3], x0, fma(v[u][4], x1, fma(v[u][5], x2, s1)));
+            s2 = fma(v[u][6], x0, fma(v[u][7], x1, fma(v[u][8], x2, s2)));
           }
-          s0 = fma(v[u][0], x0, fma(v[u][1], x1, fma(v[u][2], x2, s0)));
-          s1 = fma(v[u][3], x0, fma(v[u][4], x1, fma(v[u][5], x2, s1)));
-          s2 = fma(v[u][6], x0, fma(v[u][7], x1, fma(v[u][8], x2, s2)));
+        }
+      } else {
+        // every x load of the trip is issued before the first FMA (measured on cfg4, x0: 306.0 -> 288.7 us; with 16-bit
+        // block columns 296.6 -> 281.5 us).  A lane past the end of the block row reads block column 0 and is never
+        // multiplied: its sums are selected, not its products zeroed, so a non-finite x[0..2] cannot leak into the row.
+        double xx[U][3];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const double* px = x + 3 * (int64_t)max(c[u], 0);
+          xx[u][0] = ldx<X>(px, 0); xx[u][1] = ldx<X>(px, 1); xx[u][2] = ldx<X>(px, 2);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const double t0 = fma(v[u][0], xx[u][0], fma(v[u][1], xx[u][1], fma(v[u][2], xx[u][2], s0)));
+          const double t1 = fma(v[u][3], xx[u][0], fma(v[u][4], xx[u][1], fma(v[u][5], xx[u][2], s1)));
+          const double t2 = fma(v[u][6], xx[u][0], fma(v[u][7], xx[u][1], fma(v[u][8], xx[u][2], s2)));
+          const bool on = c[u] >= 0;
+          s0 = on ? t0 : s0; s1 = on ? t1 : s1; s2 = on ? t2 : s2;
         }
       }
     }
@@ -98,7 +120,7 @@ static const void* pick(const Variant& v) {
 }
 
 bool bcsr_supported(const Variant& v) {
-  return v.block >= 32 && v.block <= 1024 && v.block % 32 == 0 && pick(v) != nullptr;
+  return v.block >= 32 && v.block <= (v.X == 3 ? 1024 : 512) && v.block % 32 == 0 && pick(v) != nullptr;
 }
 cudaError_t bcsr_plan(const Variant& v, const BcsrFormat& f, int sm_count, LaunchPlan* out) {
   const void* k = pick(v);
