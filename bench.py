@@ -62,7 +62,9 @@ def ncu_traffic(variant: str, cfg: int):
         t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
         e = t.get(f"cfg{cfg}", {})
         # the capture is of one instantiation of the family; DRAM traffic is a property of the format
-        return e.get("dram_bytes_per_launch") if e.get("variant", "").split(":")[0] == variant.split(":")[0] else None
+        # (the index width is part of the format: bcsr3 with and without i16 stream different bytes)
+        key = lambda v: (v.split(":")[0], ":i16" in v)
+        return e.get("dram_bytes_per_launch") if key(e.get("variant", "")) == key(variant) else None
     except Exception:
         return None
 
