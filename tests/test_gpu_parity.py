@@ -435,3 +435,42 @@ def test_fuzz_random_matrices_random_variants(cuda):
             n_checked += 1
         S.close()
     assert n_checked > 200
+
+
+def test_fuzz_banded_and_block_matrices(cuda):
+    """Seeded fuzz over the structured classes: banded matrices with random width (the tuner then enumerates the
+    16-bit index formats and the full-band x window, x3) and 3x3-block FEM matrices (bcsr3 with 32- and 16-bit
+    block columns): random candidates of the tuner's own enumeration, preferring those new forms, random scalars,
+    non-finite x entries in every other trial, each against the oracle."""
+    rng = np.random.default_rng(4242)
+    n_checked, n_new = 0, 0
+    for trial in range(14):
+        if trial % 7 == 6:
+            A = W.fem_block27(int(rng.integers(3, 8)), val_stream=500 + trial)
+        else:
+            rows = int(rng.integers(300, 9000))
+            per_row = int(rng.integers(1, 14))
+            half = int(rng.integers(per_row + 1, 3000))
+            A = W.banded_random(rows, per_row, half, stream=500 + trial)
+        x = W.uniform(600 + trial, A.cols)
+        if trial % 2:
+            x[int(rng.integers(0, A.cols))] = np.nan
+            x[int(rng.integers(0, A.cols))] = -np.inf
+        y0 = W.uniform(700 + trial, A.rows)
+        alpha, beta = float(rng.normal()), float(rng.choice([0.0, 1.0, -0.75]))
+        y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, alpha, x, beta, y0 if beta != 0.0 else None)
+        S = binding.SpMV.from_csr(A)
+        cands = S.variants()
+        new = [c for c in cands if ":x3:h" in c or ":i16" in c or c.startswith("sell16")]
+        pick = list(rng.choice(new, size=min(12, len(new)), replace=False)) if new else []
+        pick += list(rng.choice(cands, size=min(6, len(cands)), replace=False))
+        for desc in pick:
+            if not _select_or_skip(S, str(desc)):
+                continue
+            y = H.gpu_apply(S, alpha, x, beta, y0 if beta != 0.0 else None)
+            ok, mr, ff, nf = oracle.accept(y, y_ref, scale, H.TOL)
+            assert ok, (trial, A.rows, str(desc), nf, ff, mr)
+            n_checked += 1
+            n_new += str(desc) in new
+        S.close()
+    assert n_checked > 150 and n_new > 80
