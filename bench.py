@@ -403,13 +403,15 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
         if not parity["ok"]:
             raise SystemExit(f"bench: cfg{cfg} {variant} FAILED the oracle check: {checks}")
 
-    # ---- e2e through spmv_apply_host with pinned host vectors (every member, one after the other)
+    # ---- e2e through spmv_apply_host (cfg5: spmv_apply_host_batch over the four members) with pinned host vectors
     xh = [torch.from_numpy(p.x).pin_memory() for p in probs]
     yh = [torch.from_numpy((p.y0 if p.y0 is not None else np.zeros(p.A.rows)).copy()).pin_memory() for p in probs]
 
     def e2e_step():
-        for m in range(members):
-            handles[m].apply_host(alpha, xh[m], beta, yh[m])     # synchronises the stream itself
+        if members == 1:
+            handles[0].apply_host(alpha, xh[0], beta, yh[0])     # synchronises the stream itself
+        else:                                                    # cfg5: the members' pipelines enqueued together, one synchronise
+            binding.apply_host_batch(handles[:members], [alpha] * members, xh[:members], [beta] * members, yh[:members])
     for _ in range(3):
         e2e_step()
     n_e2e = max(5, min(args.steps, 50))

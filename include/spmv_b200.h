@@ -191,6 +191,15 @@ SPMV_API spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d
 SPMV_API spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta,
                               double* h_y, void* stream);
 
+/* n host-vector applies (n DIFFERENT handles; BASELINE.json configs[4]: "four independent ... matrices ... applied
+ * concurrently") as one call: every member's pipeline is enqueued first -- each runs on its handle's own internal
+ * streams behind the work queued on `stream` when the call began, so the members' copies and kernels interleave --
+ * then `stream` is synchronised once.  Results equal n spmv_apply_host calls bit for bit.
+ * Errors: INVALID_ARG (NULL, a handle twice), ALLOC, CUDA. */
+SPMV_API spmv_status_t spmv_apply_host_batch(int32_t n, const spmv_handle_t* hs, const double* alphas,
+                                    const double* const* h_xs, const double* betas, double* const* h_ys,
+                                    void* stream);
+
 /* k back-to-back applies y <- alpha*A*x + beta*y of the selected variant captured into ONE CUDA graph (SURVEY.md
  * sec. 8(d): "a CUDA-graph replay of K applies may be reported as an additional, clearly labelled line"
  * lists the launch configuration among the tuned parameters -- for a launch-bound matrix the launch itself is the

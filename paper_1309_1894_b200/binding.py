@@ -18,7 +18,7 @@ SPMV_OK = 0
 STATUS_NAMES = ["SPMV_OK", "SPMV_ERR_INVALID_ARG", "SPMV_ERR_INVALID_MATRIX", "SPMV_ERR_UNSUPPORTED",
                 "SPMV_ERR_ALLOC", "SPMV_ERR_CUDA", "SPMV_ERR_VERIFY_FAILED", "SPMV_ERR_INTERNAL"]
 
-EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
+EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_host_batch", "spmv_apply_batch",
            "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
            "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache", "spmv_graph_create", "spmv_graph_launch",
@@ -110,6 +110,7 @@ def lib():
     L.spmv_tune.argtypes = [vp, C.POINTER(TuneOpts), C.POINTER(TuneReport)]
     L.spmv_apply.argtypes = [vp, dbl, vp, dbl, vp, vp]
     L.spmv_apply_host.argtypes = [vp, dbl, vp, dbl, vp, vp]
+    L.spmv_apply_host_batch.argtypes = [i32, C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), vp]
     L.spmv_apply_batch.argtypes = [i32, C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), C.POINTER(dbl),
                                    C.POINTER(vp), C.POINTER(vp), i32]
     L.spmv_tune_batch.argtypes = [i32, C.POINTER(vp), C.POINTER(dbl), C.POINTER(vp), C.POINTER(dbl),
@@ -131,7 +132,7 @@ def lib():
     L.spmv_gather.argtypes = [i64, vp, vp, vp, vp]
     L.spmv_scatter.argtypes = [i64, vp, vp, vp, vp]
     L.spmv_apply_rows.argtypes = [vp, dbl, vp, dbl, vp, i64, i64, C.POINTER(i64), vp]
-    for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_batch",
+    for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_host_batch", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
               "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi",
               "spmv_graph_create", "spmv_graph_launch", "spmv_graph_destroy", "spmv_partition_rows",
@@ -434,6 +435,18 @@ def apply_batch(handles, alphas, xs, betas, ys, streams):
     dy = (vp * n)(*[y.data_ptr() for y in ys])
     ss = (vp * len(streams))(*[s.cuda_stream for s in streams])
     _check(lib().spmv_apply_batch(n, hs, al, dx, be, dy, ss, len(streams)), "spmv_apply_batch")
+
+
+def apply_host_batch(handles, alphas, xs_host, betas, ys_host, stream=None):
+    """spmv_apply_host_batch: host-vector applies of n different handles, enqueued together, one synchronise."""
+    n = len(handles)
+    ptr = lambda a: a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+    hs = (C.c_void_p * n)(*[h.h for h in handles])
+    al = (C.c_double * n)(*[float(a) for a in alphas])
+    be = (C.c_double * n)(*[float(b) for b in betas])
+    xp = (C.c_void_p * n)(*[ptr(x) for x in xs_host])
+    yp = (C.c_void_p * n)(*[ptr(y) for y in ys_host])
+    _check(lib().spmv_apply_host_batch(n, hs, al, xp, be, yp, _stream_ptr(stream)), "spmv_apply_host_batch")
 
 
 def tune_batch(handles, alphas, xs, betas, ys, streams):

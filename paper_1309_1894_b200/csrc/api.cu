@@ -258,8 +258,10 @@ spmv_status_t spmv_graph_destroy(spmv_graph_t g) {
 // PCIe is full duplex, so the download of chunk k-1 overlaps the upload of chunk k+1 and the kernel of chunk k;
 // for a banded matrix the first kernel starts long before x is complete.  Results are bit-identical to the
 // one-launch form: a row is summed by the same kernel code in the same order.
-spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
-                              void* stream) {
+// entry: event the pipeline's internal streams wait on (nullptr: the current tail of `stream`); wait: synchronise
+// `stream` before returning (spmv_apply_host_batch enqueues every member first and synchronises once)
+static spmv_status_t apply_host_impl(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
+                                     void* stream, cudaEvent_t entry, bool wait) {
   if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
   if ((h->A.rows > 0 && !h_y) || (h->A.cols > 0 && !h_x)) return SPMV_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
@@ -312,7 +314,7 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
       if (okx) {
         spmv_status_t st = spmv_apply(h, alpha, (const double*)px.devicePointer, beta, zy, stream);
         if (st != SPMV_OK) return st;
-        SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+        if (wait) SPMV_CUDA_TRY(cudaStreamSynchronize(s));
         return SPMV_OK;
       }
     }
@@ -321,7 +323,7 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
     spmv_status_t st = spmv_apply(h, alpha, dx, beta, dy, stream);
     if (st != SPMV_OK) return st;
     if (rows) SPMV_CUDA_TRY(cudaMemcpyAsync(h_y, dy, sizeof(double) * rows, cudaMemcpyDeviceToHost, s));
-    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+    if (wait) SPMV_CUDA_TRY(cudaStreamSynchronize(s));
     return SPMV_OK;
   }
   nchunks = (rows + chunk - 1) / chunk;
@@ -337,12 +339,16 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
     h->hs_events.push_back(e);
   }
   cudaEvent_t* ev = h->hs_events.data();
-  // work already queued on the caller's stream comes first
-  SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks], s));
-  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up, ev[3 * nchunks], 0));
-  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up2, ev[3 * nchunks], 0));
-  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev[3 * nchunks], 0));
-  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_down, ev[3 * nchunks], 0));
+  // work already queued on the caller's stream comes first (a batch: what was queued when the batch began)
+  cudaEvent_t ev_in = entry;
+  if (!ev_in) {
+    SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks], s));
+    ev_in = ev[3 * nchunks];
+  }
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up, ev_in, 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_up2, ev_in, 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_run, ev_in, 0));
+  SPMV_CUDA_TRY(cudaStreamWaitEvent(h->hs_down, ev_in, 0));
   const bool aligned = true;                 // the staging vectors come from the allocator: 16-byte aligned
   const int64_t bw = h->info.bandwidth;
   int64_t x_up = 0;                          // x[0, x_up) is queued for upload
@@ -371,10 +377,41 @@ spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, 
   }
   SPMV_CUDA_TRY(cudaEventRecord(ev[3 * nchunks + 1], h->hs_down));
   SPMV_CUDA_TRY(cudaStreamWaitEvent(s, ev[3 * nchunks + 1], 0));
-  SPMV_CUDA_TRY(cudaStreamSynchronize(s));
-  SPMV_CUDA_TRY(cudaStreamSynchronize(h->hs_up));       // (nothing pending: every upload precedes a kernel that has finished)
+  if (wait) {
+    SPMV_CUDA_TRY(cudaStreamSynchronize(s));
+    SPMV_CUDA_TRY(cudaStreamSynchronize(h->hs_up));     // (nothing pending: every upload precedes a kernel that has finished)
+  }
   return SPMV_OK;
 }
+
+spmv_status_t spmv_apply_host(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
+                              void* stream) {
+  return apply_host_impl(h, alpha, h_x, beta, h_y, stream, nullptr, true);
+}
+
+// n host-vector applies as ONE call: every member's chunk pipeline is enqueued behind the same entry event (its
+// own internal streams: the members' copies and kernels interleave, PCIe never idles between members), then
+// `stream` is synchronised once.
+spmv_status_t spmv_apply_host_batch(int32_t n, const spmv_handle_t* hs, const double* alphas, const double* const* h_xs,
+                                    const double* betas, double* const* h_ys, void* stream) {
+  if (n < 0 || (n > 0 && (!hs || !alphas || !h_xs || !betas || !h_ys))) return SPMV_ERR_INVALID_ARG;
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < i; ++j)
+      if (hs[i] == hs[j]) { set_last_error("spmv_apply_host_batch: a handle appears twice (its staging vectors would be shared)"); return SPMV_ERR_INVALID_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaEvent_t entry = nullptr;
+  SPMV_CUDA_TRY(cudaEventCreateWithFlags(&entry, cudaEventDisableTiming));
+  cudaError_t e = cudaEventRecord(entry, s);
+  spmv_status_t st = e == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
+  for (int i = 0; i < n && st == SPMV_OK; ++i) st = apply_host_impl(hs[i], alphas[i], h_xs[i], betas[i], h_ys[i], stream, entry, false);
+  e = cudaStreamSynchronize(s);                    // also after a failure: nothing of this call may stay in flight
+  for (int i = 0; i < n; ++i)
+    if (handle_alive(hs[i]) && hs[i]->hs_up) cudaStreamSynchronize(hs[i]->hs_up);
+  cudaEventDestroy(entry);
+  if (st == SPMV_OK && e != cudaSuccess) { set_last_error("spmv_apply_host_batch: %s", cudaGetErrorString(e)); st = SPMV_ERR_CUDA; }
+  return st;
+}
+
 
 spmv_status_t spmv_apply_batch(int32_t n, const spmv_handle_t* hs, const double* alphas, const double* const* d_xs,
                                const double* betas, double* const* d_ys, void* const* streams, int32_t nstreams) {

@@ -62,6 +62,7 @@ def test_null_and_bad_arguments_return_codes(L):
     assert L.spmv_graph_launch(None, None) == 1 and L.spmv_graph_destroy(None) == 1
     assert L.spmv_apply_rows(None, 1.0, None, 0.0, None, 0, 0, None, None) == 1
     assert L.spmv_apply_host(None, 1.0, None, 0.0, None, None) == 1
+    assert L.spmv_apply_host_batch(2, None, None, None, None, None, None) == 1 and L.spmv_apply_host_batch(-1, None, None, None, None, None, None) == 1
     assert L.spmv_gather(-1, None, None, None, None) == 1 and L.spmv_gather(0, None, None, None, None) == 0
     assert L.spmv_scatter(3, None, None, None, None) == 1
     assert L.spmv_external_columns(None, 0, 0, None, 0, None, None, None, None) == 1

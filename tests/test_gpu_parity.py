@@ -272,6 +272,42 @@ def test_apply_host_zero_copy_y_equals_staged_copies(cuda, monkeypatch):
     S.close()
 
 
+def test_apply_host_batch_equals_member_calls(cuda, monkeypatch):
+    """spmv_apply_host_batch: the members' pipelines are enqueued together and synchronised once; results equal
+    one spmv_apply_host call per member bit for bit -- pipelined members (several chunks, staged and zero-copy
+    y), a member without a range form (one launch) and a small one; a handle passed twice is refused."""
+    import torch
+    monkeypatch.setenv("SPMV_HOST_CHUNK_MB", "1.0")
+    mats = [W.stencil3d_27pt(70, perturb_stream=61), W.laplace3d_7pt(75), W.fem_block27(40), W.powerlaw(20000), W.laplace2d_5pt(20)]
+    descs = ["dia_tma:b288:c256:r1:u9:i3:x0", "dia_const:b256:r1:x0", "bcsr3:b128:w16:u2:i16:x0:g8", "merge:b256:i7:x0", "dia_const:b256:r1:x0"]
+    hs = [binding.SpMV.from_csr(A) for A in mats]
+    for S, d in zip(hs, descs):
+        S.select(d)
+    alphas = [1.0, -0.5, 2.0, 1.25, 1.0]
+    betas = [1.0, 0.5, 0.0, -0.75, 0.0]
+    xs = [W.uniform(130 + i, A.cols) for i, A in enumerate(mats)]
+    y0 = [W.uniform(140 + i, A.rows) for i, A in enumerate(mats)]
+    xh = [torch.from_numpy(x).pin_memory() for x in xs]
+    want = []
+    for S, a, b, x, y in zip(hs, alphas, betas, xh, y0):
+        yy = torch.from_numpy(y.copy()).pin_memory()
+        S.apply_host(a, x, b, yy)
+        want.append(yy.numpy().copy())
+    for rep in range(3):
+        yh = [torch.from_numpy(y.copy()).pin_memory() for y in y0]
+        binding.apply_host_batch(hs, alphas, xh, betas, yh)
+        for i in range(len(hs)):
+            assert np.array_equal(yh[i].numpy(), want[i]), (rep, i, descs[i])
+    for i, A in enumerate(mats):                       # and the oracle
+        y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, alphas[i], xs[i], betas[i], y0[i] if betas[i] != 0.0 else None, parallel=True)
+        assert oracle.accept(want[i], y_ref, scale, H.TOL)[0], descs[i]
+    with pytest.raises(binding.SpmvError) as e:
+        binding.apply_host_batch([hs[0], hs[0]], [1.0, 1.0], [xh[0], xh[0]], [0.0, 0.0], [torch.zeros(mats[0].rows, dtype=torch.float64)] * 2)
+    assert e.value.status == 1
+    for S in hs:
+        S.close()
+
+
 @pytest.mark.slow
 def test_tma_pipeline_race_regression_full_size(cuda):
     """Regression: on full-size cfg5 with sorted slices the TMA refill (async proxy) used to land
