@@ -99,10 +99,11 @@ extern "C" spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double*
   if (n == 0) { result->converged = 1; return SPMV_OK; }
 
   const int nb = (int)std::min<int64_t>((n + kJacBlock - 1) / kJacBlock, (int64_t)h->dev.sm_count * 8);
-  const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + (size_t)nb) + sizeof(JacobiState);
+  const size_t ns = ((size_t)n + 15) & ~(size_t)15;          // 128-byte stride: every vector 16-byte aligned (pair loads)
+  const size_t ws_bytes = sizeof(double) * (3 * ns + (size_t)nb) + sizeof(JacobiState);
   double* ws = (double*)h->al.alloc(ws_bytes, s);
   if (!ws) return SPMV_ERR_ALLOC;
-  double *d = ws, *t = d + n, *x1 = t + n, *part = x1 + n;
+  double *d = ws, *t = d + ns, *x1 = t + ns, *part = x1 + ns;
   JacobiState* st = (JacobiState*)(part + nb);
   double* buf[2] = {d_x, x1};
   cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -297,10 +297,11 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
   // partial arrays: one slot per block of whichever kernel writes them (the SpMV kernel with the fused dot
   // runs an exact grid of >= 32 rows per block)
   const size_t npart = std::max<size_t>((size_t)nb, (size_t)((n + 31) / 32));    // (fused: nb is the cooperative grid)
-  const size_t ws_bytes = sizeof(double) * (3 * (size_t)n + 3 * npart) + sizeof(CgState);
+  const size_t ns = ((size_t)n + 15) & ~(size_t)15;          // 128-byte stride: every vector 16-byte aligned (pair loads)
+  const size_t ws_bytes = sizeof(double) * (3 * ns + 3 * npart) + sizeof(CgState);
   double* ws = (double*)h->al.alloc(ws_bytes, s);
   if (!ws) return SPMV_ERR_ALLOC;
-  double *r = ws, *p = r + n, *q = p + n, *part_rr = q + n, *part_bb = part_rr + npart, *part_pq = part_bb + npart;
+  double *r = ws, *p = r + ns, *q = p + ns, *part_rr = q + ns, *part_bb = part_rr + npart, *part_pq = part_bb + npart;
   CgState* st = (CgState*)(part_pq + npart);
   if (cudaMemsetAsync(st, 0, sizeof(CgState), s) != cudaSuccess) { h->al.free(ws, ws_bytes); return SPMV_ERR_CUDA; }
   // q = A p with p.q fused into the SpMV kernel's epilogue where the selected family has that form
