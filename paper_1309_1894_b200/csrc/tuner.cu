@@ -425,6 +425,7 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
       if (in.block3_full) return v.fam == FAM_BCSR3;
       if (skew) return v.fam == FAM_MERGE || ((v.fam == FAM_SELL || v.fam == FAM_SELL_TMA) && v.L > 0);
       if (is_sell16(v)) return true;                                                       // banded, not diagonal: 10 B per entry
+      if (v.fam == FAM_SELL_TMA && v.X == 3) return true;                                  // band fits a shared-memory x window
       return v.fam == FAM_SELL && v.S == 1;
     };
     std::vector<Variant> cut;
