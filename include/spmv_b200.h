@@ -43,10 +43,13 @@
  *   keys      b threads per block | g grid: 0/absent exact cover, k = k waves of resident blocks |
  *             co shared-memory carve-out percent | u unroll (sell_tma/dia_tma: steps per stage) |
  *             r rows per thread | w lanes per (block) row | x x path: 0 ld.global.nc, 1 ld.global,
- *             2 window staged in shared memory (+ h = window half-width), 3 (bcsr3) the 3-vector of a block as an
- *             aligned 16-byte pair + one 8-byte load | c slice height |
+ *             2 (sell_tma, sell16_tma) the x window of a slice staged in shared memory (+ h = window half-width;
+ *             gathers outside it go through L1), 3 (sell_tma, sell16_tma) the same with h >= the matrix bandwidth:
+ *             every gather is a shared-memory read (sigma 1, even column count); 3 (bcsr3) the 3-vector of a
+ *             block as an aligned 16-byte pair + one 8-byte load | c slice height |
  *             s sorting window sigma | l row-split length (rows longer than l become segments) |
- *             i merge items per thread (sell_tma/dia_tma: pipeline stages)
+ *             i merge items per thread (sell_tma/dia_tma: pipeline stages; bcsr3: i16 = 16-bit block columns
+ *             relative to the block row, 74 instead of 76 bytes per block)
  *   "default" = csr_scalar:b256:r1:u1:x0, the fixed default variant.
  */
 #ifndef SPMV_B200_H
