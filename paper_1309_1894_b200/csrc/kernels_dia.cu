@@ -151,7 +151,7 @@ cudaError_t dia_plan(const Variant& v, int64_t rows, const DiaFormat& f, int sm_
 // (which entries exist near the boundary), x and y only.  Same summation order as dia_kernel, and the
 // coefficients are the stored bit patterns, so the result equals dia_kernel's bit for bit.
 //
-// Shape (round 2; measured on cfg2 with _work/stencil_probe.cu): one trip per thread over an EXACT grid
+// Shape (round 2; measured on cfg2 with a stand-alone probe of the same stencil, not kept): one trip per thread over an EXACT grid
 // -- the hardware block scheduler keeps every SM's load queue full, a persistent grid-stride loop with
 // software pipelining (round 1: 124 registers, 21 us) does not -- a thread owns R adjacent rows and reads
 // x[r0 + off .. r0 + off + R) as aligned 16-byte pairs; for an odd offset the pair is taken one element
