@@ -358,6 +358,17 @@ def test_update_values_keeps_the_variant_and_matches_oracle(cuda):
     assert S.update_values(torch.from_numpy(v4).cuda()) is True and S.variant.startswith("dia_tma")
     H.check_against_oracle(S, W.CSR(L.rows, L.cols, L.row_ptr, L.col_idx, v4), 1.0, xl, 0.0, None, what="fallback")
     S.close()
+    # formats with a derived index array (16-bit block columns, 16-bit slice deltas, the x3 window) are rebuilt whole
+    F = W.fem_block27(6)
+    Bm = W.banded_random(5000, 8, 600, stream=88)
+    for M, desc in ((F, "bcsr3:b128:w16:u2:i16:x0:g8"), (Bm, "sell16_tma:b288:c256:s1:r1:u8:i3:x3:h600"), (Bm, "sell16:b256:c128:s1:r2:u4:x0")):
+        S = binding.SpMV.from_csr(M)
+        S.select(desc)
+        xm, ym = W.uniform(86, M.cols), W.uniform(87, M.rows)
+        v5 = W.normal(89, M.nnz)
+        assert S.update_values(torch.from_numpy(v5).cuda()) is False and S.variant == desc
+        H.check_against_oracle(S, W.CSR(M.rows, M.cols, M.row_ptr, M.col_idx, v5), -1.5, xm, 0.5, ym, what="update_values " + desc)
+        S.close()
 
 
 def test_full_band_window_x3(cuda):
