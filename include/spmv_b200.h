@@ -319,12 +319,15 @@ typedef struct {
   int32_t max_iters;     /* 0 -> 1000; negative -> 0 iterations (residual of the initial guess only) */
   int32_t check_every;   /* 0 -> 8 */
   int32_t no_graph;      /* 1: never use a CUDA graph */
+  int32_t no_fused;      /* 1: never fuse the step into the product kernel (available for the dia_const family: product,
+                            residual, update and norm partials in one pass; the iterates are bit-identical either way) */
 } spmv_jacobi_opts_t;
 typedef struct {
   int32_t iters, converged, zero_diagonal;
   int32_t iterations_launched;   /* > iters: the pass that meets the stop rule, and passes issued after it, update nothing */
   int32_t graph_replays;
   int32_t kernels_per_iteration;
+  int32_t fused_step;            /* 1: the step ran inside the product kernel */
   double rel_residual;           /* ||b - A x|| / ||b|| of the returned x  (the norm itself when b == 0) */
   double device_seconds;         /* CUDA events around the whole call */
   double wall_seconds;

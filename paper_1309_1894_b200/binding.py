@@ -78,13 +78,13 @@ class CgResult(C.Structure):
 
 class JacobiOpts(C.Structure):
     _fields_ = [("omega", C.c_double), ("tol", C.c_double), ("max_iters", C.c_int32), ("check_every", C.c_int32),
-                ("no_graph", C.c_int32)]
+                ("no_graph", C.c_int32), ("no_fused", C.c_int32)]
 
 
 class JacobiResult(C.Structure):
     _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("zero_diagonal", C.c_int32),
                 ("iterations_launched", C.c_int32), ("graph_replays", C.c_int32), ("kernels_per_iteration", C.c_int32),
-                ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
+                ("fused_step", C.c_int32), ("rel_residual", C.c_double), ("device_seconds", C.c_double), ("wall_seconds", C.c_double)]
 
 
 class TuneReport(C.Structure):
@@ -304,11 +304,12 @@ class SpMV:
         out["loop_variant"] = out["loop_variant"].decode()
         return out
 
-    def jacobi(self, b, x, *, omega=1.0, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, stream=None) -> dict:
+    def jacobi(self, b, x, *, omega=1.0, tol=1e-10, max_iters=1000, check_every=8, no_graph=False, no_fused=False,
+               stream=None) -> dict:
         """Weighted Jacobi with the selected variant (spmv_jacobi).  x: initial guess in, iterate out."""
         assert b.is_cuda and x.is_cuda and b.numel() == self.rows and x.numel() == self.rows
         o = JacobiOpts(float(omega), float(tol), int(max_iters) if max_iters > 0 else -1, int(check_every),
-                       int(bool(no_graph)))
+                       int(bool(no_graph)), int(bool(no_fused)))
         r = JacobiResult()
         _check(lib().spmv_jacobi(self.h, _dptr(b), _dptr(x), C.byref(o), C.byref(r), _stream_ptr(stream)), "spmv_jacobi")
         return {k: getattr(r, k) for k, _ in JacobiResult._fields_}

@@ -2,7 +2,9 @@
 // weighted Jacobi iteration  x_{k+1} = x_k + omega * D^-1 (b - A x_k)  with the selected SpMV variant as the
 // matrix product.  Two kernels per iteration: t = A x_k (the variant's own launch plan), then ONE fused pass that
 // forms r_k = b - t, its squared norm (block partials, finished by the last block to arrive: cg_reduce.cuh) and the
-// next iterate.  The stop test belongs BEFORE the update (textbook order, and the oracle's): the pass therefore
+// next iterate (for a constant-coefficient stencil variant the product joins that pass: dia_const_jacobi_kernel reads
+// mask, x, b, d and writes the next iterate -- ONE pass over the vectors per iteration, plus a one-block finishing
+// kernel).  The stop test belongs BEFORE the update (textbook order, and the oracle's): the pass therefore
 // writes x_{k+1} into the OTHER of two buffers, and the block that finishes the norm decides whether the step
 // counts -- when it does not, the result simply stays in the buffer the step read.  Iteration j reads buffer j & 1,
 // so a CUDA graph of an even number of iterations can be replayed; scalars live on the device, kernels are no-ops
@@ -77,6 +79,24 @@ jacobi_step_kernel(int64_t n, const double* __restrict__ b, const double* __rest
   }
 }
 
+// Finishing kernel of the FUSED step (constant-coefficient stencils: the product, the residual, the update and the
+// block partials of ||r||^2 all come out of dia_const_jacobi_kernel): one block adds the partials in index order and
+// applies the stop rule -- the same rule as jacobi_step_kernel's last block.
+__global__ void __launch_bounds__(1024)
+jacobi_finish_kernel(int n_part, const double* __restrict__ part, JacobiState* __restrict__ st, double tol, int max_iters) {
+  __shared__ double s_warp[33];
+  if (st->done) return;
+  double v = 0.0;
+  for (int i = threadIdx.x; i < n_part; i += blockDim.x) v += part[i];
+  v = block_sum_fixed(v, s_warp);
+  if (threadIdx.x == 0) {
+    st->rr = v;
+    const int conv = sqrt(v) <= tol * sqrt(st->bb);
+    if (conv || st->iters >= max_iters) { st->converged = conv; st->done = 1; }
+    else st->iters += 1;
+  }
+}
+
 }  // namespace spmv
 
 using namespace spmv;
@@ -99,12 +119,20 @@ extern "C" spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double*
   if (n == 0) { result->converged = 1; return SPMV_OK; }
 
   const int nb = (int)std::min<int64_t>((n + kJacBlock - 1) / kJacBlock, (int64_t)h->dev.sm_count * 8);
+  // constant-coefficient stencil selected: the whole step is ONE pass (product, residual, update, norm partials)
+  const DiaFormat* fused_f = nullptr;
+  if (o.no_fused == 0 && h->sel.fam == FAM_DIA_CONST && h->sel.X == 0) {
+    auto it = h->dias.find(h->sel.C);
+    if (it != h->dias.end() && it->second.is_const) fused_f = &it->second;
+  }
+  const int n_fpart = fused_f ? dia_const_jacobi_blocks(h->sel, n) : 0;
+  const size_t npart = (size_t)std::max(nb, n_fpart);
   const size_t ns = ((size_t)n + 15) & ~(size_t)15;          // 128-byte stride: every vector 16-byte aligned (pair loads)
-  const size_t ws_bytes = sizeof(double) * (3 * ns + (size_t)nb) + sizeof(JacobiState);
+  const size_t ws_bytes = sizeof(double) * (3 * ns + npart) + sizeof(JacobiState);
   double* ws = (double*)h->al.alloc(ws_bytes, s);
   if (!ws) return SPMV_ERR_ALLOC;
   double *d = ws, *t = d + ns, *x1 = t + ns, *part = x1 + ns;
-  JacobiState* st = (JacobiState*)(part + nb);
+  JacobiState* st = (JacobiState*)(part + npart);
   double* buf[2] = {d_x, x1};
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   cudaGraph_t graph = nullptr;
@@ -129,6 +157,12 @@ extern "C" spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double*
   auto iteration = [&]() -> spmv_status_t {                 // iteration j reads buffer j & 1
     const double* xc = buf[launched & 1];
     double* xn = buf[(launched + 1) & 1];
+    if (fused_f) {
+      if (dia_const_jacobi_launch(h->sel, n, n, *fused_f, omega, xc, xn, d_b, part, &st->done, s) != cudaSuccess) return SPMV_ERR_CUDA;
+      jacobi_finish_kernel<<<1, 1024, 0, s>>>(n_fpart, part, st, tol, max_iters);
+      ++launched;
+      return cudaGetLastError() == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
+    }
     ApplyArgs a{1.0, 0.0, xc, t, s};
     spmv_status_t st1 = launch_plan(h->plan, a);            // t = A x_k
     if (st1 != SPMV_OK) return st1;
@@ -182,7 +216,8 @@ extern "C" spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double*
   result->wall_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
   result->iterations_launched = launched;
   result->graph_replays = graph_replays;
-  result->kernels_per_iteration = 1 + h->plan.n;
+  result->kernels_per_iteration = fused_f ? 2 : 1 + h->plan.n;
+  result->fused_step = fused_f ? 1 : 0;
   cleanup();
   return SPMV_OK;
 }

@@ -208,11 +208,16 @@ constexpr int dia_const_min_blocks(int R, int ND) { return (ND == 0 || ND > 9) ?
 // took 15.5 us, 4.4 M took 11.9 us, same memory requests), so the two cases are separate instantiations chosen by
 // a uniform branch at kernel entry instead of predicated code, and the R > 1 forms require rows % R == 0 (the plan
 // falls back to R = 1 otherwise) so that a thread's rows are all live or all dead.
-template <int R, int ND, int X, typename MT, bool DOT, unsigned TRI, bool BZ>
+// DOT == 2 (R == 1, BZ, square matrix; the Jacobi loop, jacobi.cu): the whole weighted-Jacobi step in this kernel.
+// alpha carries omega, y is the NEXT iterate: r_i = jb[i] - (A x)_i, y[i] = x[i] + omega * r_i / jd, and the block's
+// share of sum_i r_i^2 goes to dot_part[blockIdx.x] (added in index order by the caller's finishing kernel).  jd is
+// the coefficient of the offset-0 diagonal: with constant coefficients every row that stores its diagonal entry has
+// that value, and the caller has established on the device that every row does (else it never lets this kernel run).
+template <int R, int ND, int X, typename MT, int DOT, unsigned TRI, bool BZ>
 __device__ __forceinline__ void
 dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
                double alpha, const double* __restrict__ x, double beta, double* __restrict__ y,
-               double* __restrict__ dot_part = nullptr) {
+               double* __restrict__ dot_part = nullptr, const double* __restrict__ jb = nullptr, double jd = 1.0) {
   constexpr int NDC = ND == 0 ? 8 : (ND % 9 == 0 ? 9 : (ND <= 8 ? ND : 8));     // diagonals per chunk
   constexpr int DMAX = ND == 0 ? 32 : ND;
   const int nd = ND == 0 ? nd_rt : ND;
@@ -223,7 +228,7 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
   const int r0 = (blockIdx.x * blockDim.x + threadIdx.x) * R;
   const int lane = threadIdx.x & 31;
   (void)lane;
-  if (R == 1 && !DOT && r0 >= rows) return;
+  if (R == 1 && DOT == 0 && r0 >= rows) return;
   unsigned m[R];
   if constexpr (R == 2) {
     const typename DiaMaskVec<MT>::V2 mm = *reinterpret_cast<const typename DiaMaskVec<MT>::V2*>(mask + r0);
@@ -239,6 +244,10 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
   double yold[R], acc[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) { yold[r] = 0.0; acc[r] = 0.0; }
+  double jbi = 0.0;                                          // Jacobi step: right-hand side of this row,
+  if constexpr (DOT == 2) {                                  // loaded in the same round trip as x
+    if (live) jbi = jb[r0];
+  }
   if constexpr (!BZ) {
     if (live) {
       if constexpr (R > 1) {
@@ -315,7 +324,19 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
   double out[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) out[r] = BZ ? alpha * acc[r] : fma(alpha, acc[r], beta * yold[r]);
-  if constexpr (DOT) {
+  if constexpr (DOT == 2) {
+    __shared__ double s_warp[33];
+    double rr = 0.0;
+    if (live) {
+      const double ri = jbi - acc[0];
+      y[r0] = fma(alpha, ri / jd, ldx<X>(x, r0));
+      rr = ri * ri;
+    }
+    const double mine = block_sum_fixed(rr, s_warp);
+    if (threadIdx.x == 0) dot_part[blockIdx.x] = mine;
+    return;
+  }
+  if constexpr (DOT == 1) {
     __shared__ double s_warp[33];
     if (live) y[r0] = out[0];
     const double mine = block_sum_fixed(live ? ldx<X>(x, r0) * out[0] : 0.0, s_warp);
@@ -342,7 +363,7 @@ __global__ void __launch_bounds__(512, dia_const_min_blocks(R, ND))
 dia_const_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                  const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                  const double* __restrict__ x, double beta, double* __restrict__ y) {
-  DIA_CONST_ENTRY(R, ND, X, MT, false, 0u);
+  DIA_CONST_ENTRY(R, ND, X, MT, 0, 0u);
 }
 
 // centres of the (o - 1, o, o + 1) runs of a 5-, 7- or 27-point stencil in natural ordering (0: no such form)
@@ -355,7 +376,7 @@ __global__ void __launch_bounds__(256, ND <= 9 ? 6 : 3)
 dia_const_kernel_r2t(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                      const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                      const double* __restrict__ x, double beta, double* __restrict__ y) {
-  DIA_CONST_ENTRY(2, ND, X, MT, false, dia_tri_mask(ND));
+  DIA_CONST_ENTRY(2, ND, X, MT, 0, dia_tri_mask(ND));
 }
 template <int X, typename MT>
 static const void* dia_const_pick_tri(int nd) {
@@ -387,7 +408,7 @@ __global__ void __launch_bounds__(256, 6)
 dia_const_kernel_r2(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                     const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                     const double* __restrict__ x, double beta, double* __restrict__ y) {
-  DIA_CONST_ENTRY(2, ND, X, MT, false, 0u);
+  DIA_CONST_ENTRY(2, ND, X, MT, 0, 0u);
 }
 
 // one row per thread with the fused dot product (the solver loop)
@@ -396,8 +417,52 @@ __global__ void __launch_bounds__(512, 2)
 dia_const_dot_kernel(int rows, int xlo, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
                      const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double alpha,
                      const double* __restrict__ x, double beta, double* __restrict__ y, double* __restrict__ dot_part) {
-  DIA_CONST_ENTRY(1, ND, 0, MT, true, 0u, dot_part);
+  DIA_CONST_ENTRY(1, ND, 0, MT, 1, 0u, dot_part);
 }
+// the weighted-Jacobi step fused into the stencil product (jacobi.cu); a no-op once *done is set
+template <int ND, typename MT>
+__global__ void __launch_bounds__(512, 2)
+dia_const_jacobi_kernel(int rows, int xhi, int nd_rt, const __grid_constant__ DiaOffsets offs,
+                        const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double omega,
+                        const double* __restrict__ x, double* __restrict__ x_next, const double* __restrict__ b,
+                        double d, double* __restrict__ part, const int* __restrict__ done) {
+  if (*done) return;
+  dia_const_body<1, ND, 0, MT, 2, 0u, true>(rows, 0, xhi, nd_rt, offs, coefs, mask, omega, x, 0.0, x_next, part, b, d);
+}
+template <typename MT>
+static cudaError_t dia_const_jacobi_launch_mt(const DiaFormat& f, int block, int rows, int cols, const MT* mask, double omega,
+                                              const double* x, double* x_next, const double* b, double d,
+                                              double* part, const int* done, cudaStream_t s) {
+  DiaCoefs co;
+  for (int i = 0; i < 32; ++i) co.c[i] = f.coef[i];
+  const DiaOffsets of = dia_offsets(f);
+  const unsigned grid = (unsigned)((rows + block - 1) / block);
+  switch (f.nd) {
+    case 5: dia_const_jacobi_kernel<5, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
+    case 7: dia_const_jacobi_kernel<7, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
+    case 27: dia_const_jacobi_kernel<27, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
+    default: dia_const_jacobi_kernel<0, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
+  }
+  return cudaGetLastError();
+}
+int dia_const_jacobi_blocks(const Variant& v, int64_t rows) {
+  const int block = std::min(std::max(v.block, 32), 512);
+  return (int)((rows + block - 1) / block);
+}
+cudaError_t dia_const_jacobi_launch(const Variant& v, int64_t rows, int64_t cols, const DiaFormat& f, double omega,
+                                    const double* x, double* x_next, const double* b, double* part,
+                                    const int* done, cudaStream_t s) {
+  if (!f.is_const || rows != cols || rows == 0) return cudaErrorInvalidValue;
+  double d = 1.0;                                  // (no offset-0 diagonal: every row lacks it, the caller's `done` is set)
+  for (int i = 0; i < f.nd; ++i)
+    if (f.off[i] == 0) d = f.coef[i];
+  const int block = std::min(std::max(v.block, 32), 512);
+  const int me = f.mask_small ? f.mask_elem : 4;
+  if (me == 1) return dia_const_jacobi_launch_mt<unsigned char>(f, block, (int)rows, (int)cols, (const unsigned char*)f.mask_small, omega, x, x_next, b, d, part, done, s);
+  if (me == 2) return dia_const_jacobi_launch_mt<unsigned short>(f, block, (int)rows, (int)cols, (const unsigned short*)f.mask_small, omega, x, x_next, b, d, part, done, s);
+  return dia_const_jacobi_launch_mt<unsigned>(f, block, (int)rows, (int)cols, (const unsigned*)f.mask, omega, x, x_next, b, d, part, done, s);
+}
+
 template <typename MT>
 static const void* dia_const_dot_pick_nd(int nd) {
   switch (nd) {

@@ -221,6 +221,13 @@ cudaError_t dia_const_plan(const Variant&, int64_t rows, int64_t cols, const Dia
 // y = alpha*A*x + beta*y AND part[b] = block b's share of sum_i x_i*y_i (square matrix); *n_part = blocks
 cudaError_t dia_const_dot_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, double* part,
                                int* n_part, LaunchPlan*);
+// one weighted-Jacobi step fused into the constant-coefficient stencil product: x_next = x + omega * (b - A x) / d (d =
+// the coefficient of the offset-0 diagonal; the caller guarantees every row stores it, else *done is set) and
+// part[block] = the block's share of ||b - A x||^2; a no-op once *done != 0.  blocks: how many partials it writes
+int dia_const_jacobi_blocks(const Variant&, int64_t rows);
+cudaError_t dia_const_jacobi_launch(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, double omega,
+                                    const double* x, double* x_next, const double* b, double* part,
+                                    const int* done, cudaStream_t s);
 bool dia_win_supported(const Variant&);
 bool dia_win_fits(const Variant&, const DiaFormat&);
 cudaError_t dia_win_plan(const Variant&, int64_t rows, int64_t cols, const DiaFormat&, int sm_count, LaunchPlan*);

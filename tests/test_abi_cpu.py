@@ -79,9 +79,9 @@ def test_struct_sizes_match_header():
     assert ctypes.sizeof(binding.CgOpts) == 8 + 6 * 4
     assert ctypes.sizeof(binding.CgResult) == 8 * 4 + 128 + 3 * 8
     assert binding.CgResult.rel_residual.offset == 160 and binding.CgResult.loop_variant.offset == 32
-    # spmv_jacobi_opts_t: 2 doubles + 3 int32 (+ 4 padding); spmv_jacobi_result_t: 6 int32 + 3 doubles
-    assert ctypes.sizeof(binding.JacobiOpts) == 2 * 8 + 3 * 4 + 4
-    assert ctypes.sizeof(binding.JacobiResult) == 6 * 4 + 3 * 8 and binding.JacobiResult.rel_residual.offset == 24
+    # spmv_jacobi_opts_t: 2 doubles + 4 int32; spmv_jacobi_result_t: 7 int32 (+ 4 padding) + 3 doubles
+    assert ctypes.sizeof(binding.JacobiOpts) == 2 * 8 + 4 * 4
+    assert ctypes.sizeof(binding.JacobiResult) == 7 * 4 + 4 + 3 * 8 and binding.JacobiResult.rel_residual.offset == 32
     # spmv_tune_report_t: the log buffer triple closes the struct
     assert binding.TuneReport.log_len.offset + 8 == ctypes.sizeof(binding.TuneReport)
 

@@ -53,6 +53,15 @@ def test_jacobi_fixed_step_count_matches_the_oracle(cuda, desc):
             stream.synchronize()
             assert torch.equal(dx, dx2) and torch.equal(dx, dx3)
             assert res3["graph_replays"] == 0 and (k <= 2 or res2["graph_replays"] >= 1)
+            # constant-coefficient stencil: the step runs inside the product kernel; the iterates are the same bits
+            # as with the separate pass (the update is element-wise; only the shape of the norm's sum differs)
+            assert res["fused_step"] == (1 if desc.startswith("dia_const") else 0)
+            if desc.startswith("dia_const"):
+                dx4 = H.to_dev(x0).clone()
+                res4 = S.jacobi(db, dx4, omega=omega, tol=1e-300, max_iters=k, check_every=6, no_fused=True)
+                stream.synchronize()
+                assert res4["fused_step"] == 0 and res4["iters"] == k and torch.equal(dx, dx4)
+                assert res4["rel_residual"] == pytest.approx(res["rel_residual"], rel=1e-12)
     S.close()
 
 
@@ -78,6 +87,36 @@ def test_jacobi_closed_form_on_a_laplacian_eigenvector(cuda):
             assert np.abs(dx.cpu().numpy() - (1.0 - rho ** k) * v).max() <= 1e-13
             assert res["rel_residual"] == pytest.approx(abs(rho) ** k, rel=1e-11)
     S.close()
+
+
+def test_jacobi_fused_step_on_the_27_point_stencil_and_a_2d_grid(cuda):
+    """The fused step for other diagonal counts (27-point: the generic-count instantiation of the mask type; 5-point:
+    exact-ND), ragged sizes, stop rule included: against the oracle and bit-identical to the unfused path."""
+    import torch
+    stream = torch.cuda.Stream()
+    for A, desc in ((W.stencil3d_27pt(13), "dia_const:b128:r1:x0"), (W.laplace2d_5pt(77), "dia_const:b512:r2:x0"),
+                    (W.laplace3d_7pt(30), "dia_const:b256:r4:x0")):
+        xt = W.uniform(128, A.rows)
+        b, _ = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.0, xt, 0.0)
+        S = binding.SpMV.from_csr(A)
+        S.select(desc)
+        with torch.cuda.stream(stream):
+            db = H.to_dev(b)
+            for tol, max_iters in ((1e-300, 37), (1e-3, 5000)):
+                x_ref, k_ref, rel_ref, _ = oracle.jacobi(A.row_ptr, A.col_idx, A.val, b, omega=0.9, tol=tol, max_iters=max_iters)
+                dx = torch.zeros(A.rows, dtype=torch.float64, device="cuda")
+                res = S.jacobi(db, dx, omega=0.9, tol=tol, max_iters=max_iters)
+                dx2 = torch.zeros_like(dx)
+                res2 = S.jacobi(db, dx2, omega=0.9, tol=tol, max_iters=max_iters, no_fused=True)
+                stream.synchronize()
+                assert res["fused_step"] == 1 and res2["fused_step"] == 0 and res["kernels_per_iteration"] == 2
+                assert abs(res["iters"] - k_ref) <= 1 and res["iters"] == res2["iters"], (desc, res, k_ref)
+                assert torch.equal(dx, dx2)
+                if res["iters"] == k_ref:
+                    assert np.abs(dx.cpu().numpy() - x_ref).max() <= 1e-12 * np.abs(x_ref).max()
+                    assert res["rel_residual"] == pytest.approx(rel_ref, rel=1e-10)
+                assert res["converged"] == (1 if tol > 1e-100 else 0)
+        S.close()
 
 
 def test_jacobi_converges_like_the_oracle_on_a_dominant_nonsymmetric_matrix(cuda):
