@@ -17,6 +17,7 @@
 #include <chrono>
 
 #include "cg_reduce.cuh"
+#include "device_utils.cuh"
 #include "handle.h"
 
 namespace spmv {
@@ -85,6 +86,8 @@ jacobi_step_kernel(int64_t n, const double* __restrict__ b, const double* __rest
 __global__ void __launch_bounds__(1024)
 jacobi_finish_kernel(int n_part, const double* __restrict__ part, JacobiState* __restrict__ st, double tol, int max_iters) {
   __shared__ double s_warp[33];
+  pdl_launch_dependents();                         // the next step's kernel may load its mask words meanwhile
+  pdl_wait();                                      // the partials are the previous kernel's output
   if (st->done) return;
   double v = 0.0;
   for (int i = threadIdx.x; i < n_part; i += blockDim.x) v += part[i];
@@ -159,9 +162,13 @@ extern "C" spmv_status_t spmv_jacobi(spmv_handle_t h, const double* d_b, double*
     double* xn = buf[(launched + 1) & 1];
     if (fused_f) {
       if (dia_const_jacobi_launch(h->sel, n, n, *fused_f, omega, xc, xn, d_b, part, &st->done, s) != cudaSuccess) return SPMV_ERR_CUDA;
-      jacobi_finish_kernel<<<1, 1024, 0, s>>>(n_fpart, part, st, tol, max_iters);
+      int np_arg = n_fpart, mi = max_iters;
+      const double* part_c = part;
+      double tol_arg = tol;
+      JacobiState* st_arg = st;
+      void* fargs[] = {&np_arg, &part_c, &st_arg, &tol_arg, &mi};
       ++launched;
-      return cudaGetLastError() == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
+      return launch_kernel_pdl((const void*)jacobi_finish_kernel, 1, 1024, 0, s, fargs, true) == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
     }
     ApplyArgs a{1.0, 0.0, xc, t, s};
     spmv_status_t st1 = launch_plan(h->plan, a);            // t = A x_k

@@ -217,7 +217,8 @@ template <int R, int ND, int X, typename MT, int DOT, unsigned TRI, bool BZ>
 __device__ __forceinline__ void
 dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, const DiaCoefs& coefs, const MT* __restrict__ mask,
                double alpha, const double* __restrict__ x, double beta, double* __restrict__ y,
-               double* __restrict__ dot_part = nullptr, const double* __restrict__ jb = nullptr, double jd = 1.0) {
+               double* __restrict__ dot_part = nullptr, const double* __restrict__ jb = nullptr, double jd = 1.0,
+               const int* __restrict__ jdone = nullptr) {
   constexpr int NDC = ND == 0 ? 8 : (ND % 9 == 0 ? 9 : (ND <= 8 ? ND : 8));     // diagonals per chunk
   constexpr int DMAX = ND == 0 ? 32 : ND;
   const int nd = ND == 0 ? nd_rt : ND;
@@ -240,6 +241,9 @@ dia_const_body(int rows, int xlo, int xhi, int nd_rt, const DiaOffsets& offs, co
     m[0] = mask[r0];
   }
   pdl_wait();                                                // x and y may be the previous kernel's output
+  if constexpr (DOT == 2) {
+    if (*jdone) return;                                      // the loop has stopped (uniform; written by the finishing kernel)
+  }
   const bool live = r0 < rows;                               // R > 1: rows % R == 0, so all R rows or none
   double yold[R], acc[R];
 #pragma unroll
@@ -426,8 +430,8 @@ dia_const_jacobi_kernel(int rows, int xhi, int nd_rt, const __grid_constant__ Di
                         const __grid_constant__ DiaCoefs coefs, const MT* __restrict__ mask, double omega,
                         const double* __restrict__ x, double* __restrict__ x_next, const double* __restrict__ b,
                         double d, double* __restrict__ part, const int* __restrict__ done) {
-  if (*done) return;
-  dia_const_body<1, ND, 0, MT, 2, 0u, true>(rows, 0, xhi, nd_rt, offs, coefs, mask, omega, x, 0.0, x_next, part, b, d);
+  pdl_launch_dependents();
+  dia_const_body<1, ND, 0, MT, 2, 0u, true>(rows, 0, xhi, nd_rt, offs, coefs, mask, omega, x, 0.0, x_next, part, b, d, done);
 }
 template <typename MT>
 static cudaError_t dia_const_jacobi_launch_mt(const DiaFormat& f, int block, int rows, int cols, const MT* mask, double omega,
@@ -437,13 +441,11 @@ static cudaError_t dia_const_jacobi_launch_mt(const DiaFormat& f, int block, int
   for (int i = 0; i < 32; ++i) co.c[i] = f.coef[i];
   const DiaOffsets of = dia_offsets(f);
   const unsigned grid = (unsigned)((rows + block - 1) / block);
-  switch (f.nd) {
-    case 5: dia_const_jacobi_kernel<5, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
-    case 7: dia_const_jacobi_kernel<7, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
-    case 27: dia_const_jacobi_kernel<27, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
-    default: dia_const_jacobi_kernel<0, MT><<<grid, block, 0, s>>>(rows, cols - 1, f.nd, of, co, mask, omega, x, x_next, b, d, part, done); break;
-  }
-  return cudaGetLastError();
+  const void* fn = f.nd == 5 ? (const void*)dia_const_jacobi_kernel<5, MT> : f.nd == 7 ? (const void*)dia_const_jacobi_kernel<7, MT>
+                 : f.nd == 27 ? (const void*)dia_const_jacobi_kernel<27, MT> : (const void*)dia_const_jacobi_kernel<0, MT>;
+  int xhi = cols - 1, nd = f.nd;
+  void* args[] = {&rows, &xhi, &nd, (void*)&of, (void*)&co, &mask, &omega, &x, &x_next, &b, &d, &part, &done};
+  return launch_kernel_pdl(fn, grid, (unsigned)block, 0, s, args, true);      // programmatic dependent launch
 }
 int dia_const_jacobi_blocks(const Variant& v, int64_t rows) {
   const int block = std::min(std::max(v.block, 32), 512);
