@@ -212,3 +212,34 @@ def test_feature_guided_search_finds_the_same_class_of_winner(cuda, cfg, scale):
     assert quick["winner_us"] <= 1.15 * full["winner_us"], (quick["winner"], full["winner"])
     H.check_against_oracle(S2, A, prob.alpha, prob.x, prob.beta, prob.y0, what=f"cfg{cfg} guided winner")
     S.close(); S2.close()
+
+
+def test_full_tune_on_unusual_large_matrices(cuda):
+    """The exhaustive tuner on shapes the five configs do not cover (rectangular banded, tall, wide, mostly empty
+    rows, odd column count, a 2D grid with a wide band): every enumerated candidate must agree with the ORACLE's
+    reference (passed in as d_y_ref: no candidate may be rejected), and the winner matches the oracle."""
+    import torch
+    rng = np.random.default_rng(11)
+    band = W.banded_random(120000, 9, 900, stream=12)
+    mats = [
+        ("lap2d_400", W.laplace2d_5pt(400)),
+        ("rect_banded_wide", W.CSR(band.rows, band.cols + 1000, band.row_ptr, band.col_idx, band.val)),
+        ("tall_random", W.csr_from_lengths(rng.integers(0, 12, 200000), 40000, 13)),
+        ("wide_random", W.csr_from_lengths(rng.integers(1, 40, 20000), 800000, 14)),
+        ("banded_odd_cols", W.banded_random(80001, 7, 3000, stream=15)),
+        ("fem_20", W.fem_block27(20)),
+        ("empty_heavy", W.csr_from_lengths(np.where(rng.random(150000) < 0.9, 0, rng.integers(1, 300, 150000)), 150000, 16)),
+    ]
+    for name, A in mats:
+        x, y0 = W.uniform(20, A.cols), W.uniform(21, A.rows)
+        y_ref, scale = oracle.spmv(A.row_ptr, A.col_idx, A.val, 1.25, x, -0.5, y0, parallel=True)
+        S = binding.SpMV.from_csr(A)
+        dx, dy0 = H.to_dev(x), H.to_dev(y0)
+        rep = S.tune(alpha=1.25, beta=-0.5, x=dx, y0=dy0, y_ref=H.to_dev(y_ref), scale=H.to_dev(scale), use_cache=2)
+        assert rep["n_rejected"] == 0 and rep["n_timed"] > 100, (name, rep["n_rejected"], rep["n_timed"])
+        dy = dy0.clone()
+        S.apply(1.25, dx, -0.5, dy)
+        torch.cuda.synchronize()
+        ok, mr, ff, nf = oracle.accept(dy.cpu().numpy(), y_ref, scale, H.TOL)
+        assert ok, (name, S.variant, nf, ff, mr)
+        S.close()
