@@ -253,6 +253,45 @@ SPMV_API spmv_status_t spmv_tune_batch(int32_t n, const spmv_handle_t* hs, const
                               double* const* d_ys, void* const* streams, int32_t max_streams,
                               int32_t* best_nstreams, double* us_per_count);
 
+/* ---- The product for callers that may not allocate device memory.
+ *
+ * Every other compute entry point obtains device memory at some stage: spmv_create / spmv_select / spmv_tune build
+ * converted formats and workspaces through cudaMalloc (or the allocator callbacks), spmv_cg and spmv_jacobi take
+ * three vectors per call.  Some users of the library cannot afford that at the place where they need y = alpha*A*x +
+ * beta*y: a component living inside an application that has already handed all of the GPU's memory to its own pool
+ * (cudaMalloc then fails, and the pool is not the library's to draw from); or a step of a latency-bound loop,
+ * where cudaMalloc / cudaFree are unwelcome because they serialise against all work running on the device.
+ *
+ * spmv_merge_apply_noalloc is for them.  It runs the merge-path CSR kernels (north_star (c) "merge-path CSR for
+ * skewed row lengths"; descriptor merge:b256:i7:x0) straight from the caller's CSR arrays: no handle, no conversion,
+ * no cudaMalloc / cudaFree, no allocating library routine, on any call.  The scratch memory these kernels need (a
+ * table of tile starts and one carry per tile, 16 bytes per tile of 1792 merge-path items) is a fixed 1 MiB + 256 B
+ * array compiled into the library; each GPU that loads the library carries it until the process exits, whether or
+ * not this entry point is ever called.
+ *   Limit: rows + nnz <= spmv_merge_noalloc_max_path() = 117 440 512 (65 536 tiles).  Above it the call returns
+ *     SPMV_ERR_UNSUPPORTED, spmv_last_error() says by how much, and nothing is launched.
+ *   Arguments: device pointers; the CSR arrays, x (cols entries) and y (rows entries) are the caller's, as for
+ *     spmv_create / spmv_apply, and must not alias.  The matrix is NOT validated (that would need a read-back): pass
+ *     arrays that satisfy spmv_create's rules (monotone row_ptr with row_ptr[0] = 0 and row_ptr[rows] = nnz, columns
+ *     in [0, cols)).  beta == 0: y is write-only.  alpha == 0: y = beta*y, the matrix and x are not referenced.
+ *   Result: bit-identical to spmv_select(h, "merge:b256:i7:x0") + spmv_apply on the same arrays, and to itself on
+ *     every repeat (no floating-point atomics).
+ *   First call on a device: looks up the array's address on the CURRENT device (cudaGetSymbolAddress, once per
+ *     device, remembered per device ordinal; ordinals 0..63).  That makes the driver load the library's device code
+ *     if it has not yet, so make the first call on each device during set-up, before any stream capture begins
+ *     and outside the part of the program that must not stall.  Later calls are three kernel launches on `stream`.
+ *   Sharing: there is ONE array per GPU, used by every call on that GPU from any thread, and it keeps what the last
+ *     call wrote.  A call never relies on those contents (each call first rewrites every word it later reads), so
+ *     back-to-back calls on one stream need nothing in between.  Two calls whose kernels can overlap on the GPU --
+ *     different streams without an event between them, or two host threads -- race on the array and produce
+ *     garbage: order them.
+ *   Asynchronous on `stream`; never synchronises.  Errors: INVALID_ARG (negative size, NULL array that is needed,
+ *     d_x == d_y), UNSUPPORTED (over the limit above or over int32 sizes), CUDA. */
+SPMV_API spmv_status_t spmv_merge_apply_noalloc(int64_t rows, int64_t cols, int64_t nnz, const int32_t* d_row_ptr,
+                                       const int32_t* d_col_idx, const double* d_val, double alpha,
+                                       const double* d_x, double beta, double* d_y, void* stream);
+SPMV_API int64_t spmv_merge_noalloc_max_path(void);
+
 /* Force a variant by descriptor ("default" = the fixed default).  Builds the format it
  * needs.  Errors: INVALID_ARG (unparsable), UNSUPPORTED (not eligible for this matrix). */
 SPMV_API spmv_status_t spmv_select(spmv_handle_t h, const char* variant_descriptor, void* stream);

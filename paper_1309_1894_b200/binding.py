@@ -23,7 +23,7 @@ EXPORTS = ["spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_ap
            "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi", "spmv_status_string",
            "spmv_last_error", "spmv_version", "spmv_clear_cache", "spmv_graph_create", "spmv_graph_launch",
            "spmv_graph_destroy", "spmv_partition_rows", "spmv_external_columns", "spmv_gather", "spmv_scatter",
-           "spmv_apply_rows"]
+           "spmv_apply_rows", "spmv_merge_apply_noalloc", "spmv_merge_noalloc_max_path"]
 
 
 class SpmvError(RuntimeError):
@@ -132,6 +132,10 @@ def lib():
     L.spmv_gather.argtypes = [i64, vp, vp, vp, vp]
     L.spmv_scatter.argtypes = [i64, vp, vp, vp, vp]
     L.spmv_apply_rows.argtypes = [vp, dbl, vp, dbl, vp, i64, i64, C.POINTER(i64), vp]
+    L.spmv_merge_apply_noalloc.argtypes = [i64, i64, i64, vp, vp, vp, dbl, vp, dbl, vp, vp]
+    L.spmv_merge_apply_noalloc.restype = C.c_int
+    L.spmv_merge_noalloc_max_path.argtypes = []
+    L.spmv_merge_noalloc_max_path.restype = i64
     for n in ("spmv_create", "spmv_tune", "spmv_apply", "spmv_apply_host", "spmv_apply_host_batch", "spmv_apply_batch",
               "spmv_tune_batch", "spmv_select", "spmv_list_variants", "spmv_get_info",
               "spmv_format_download", "spmv_destroy", "spmv_measure_ceiling", "spmv_update_values", "spmv_cg", "spmv_jacobi",
@@ -490,6 +494,28 @@ def scatter(idx, src, dst, stream=None):
     """dst[idx[i]] = src[i] (CUDA tensors; idx int32): the library's unpack kernel."""
     assert idx.is_cuda and src.is_cuda and dst.is_cuda and src.numel() >= idx.numel()
     _check(lib().spmv_scatter(idx.numel(), _dptr(idx), _dptr(src), _dptr(dst), _stream_ptr(stream)), "spmv_scatter")
+
+
+def merge_apply_noalloc(rows, cols, row_ptr, col_idx, val, alpha, x, beta, y, stream=None):
+    """spmv_merge_apply_noalloc: y = alpha*A*x + beta*y by the merge-path kernels, straight from CSR arrays that are
+    already CUDA tensors (row_ptr / col_idx int32, val / x / y float64), for callers that must not allocate device
+    memory where they need the product -- their memory pool owns the whole GPU, or they sit in a loop that cannot
+    take the device-wide stall of cudaMalloc / cudaFree.  This wrapper allocates nothing either: it passes pointers.
+    The kernels' scratch is a fixed array inside the library, shared by every call on the GPU: calls that may
+    overlap (two streams, two threads) must be ordered by the caller.  rows + nnz <= merge_noalloc_max_path().
+    Make the first call on each device during set-up (it resolves the array's device address)."""
+    nnz = int(val.numel())
+    for t in (row_ptr, col_idx, val, x, y):
+        assert t.is_cuda and t.is_contiguous()
+    assert row_ptr.numel() == rows + 1 and col_idx.numel() == nnz and x.numel() >= cols and y.numel() >= rows
+    _check(lib().spmv_merge_apply_noalloc(int(rows), int(cols), nnz, _dptr(row_ptr), _dptr(col_idx), _dptr(val),
+                                          float(alpha), _dptr(x), float(beta), _dptr(y), _stream_ptr(stream)),
+           "spmv_merge_apply_noalloc")
+
+
+def merge_noalloc_max_path() -> int:
+    """Largest rows + nnz spmv_merge_apply_noalloc accepts (what its built-in scratch array can serve)."""
+    return int(lib().spmv_merge_noalloc_max_path())
 
 
 def measure_ceiling(kind: int, nbytes: int = 1 << 30, reps: int = 10) -> float:

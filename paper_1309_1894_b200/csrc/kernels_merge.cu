@@ -9,6 +9,8 @@
 // boundaries go to (carry_row, carry_val) and are added in tile order by merge_fixup_kernel.
 #include <limits.h>
 
+#include <mutex>
+
 #include "device_utils.cuh"
 #include "spmv_internal.h"
 
@@ -240,3 +242,115 @@ void free_merge_plan(MergePlan& p, Allocator& al) {
 }
 
 }  // namespace spmv
+
+// ---------------------------------------------------------------------------------------------------------
+// spmv_merge_apply_noalloc (include/spmv_b200.h): the merge-path product above for callers that cannot
+// allocate device memory.  Same three kernels as the handle path (merge_partition_kernel, merge_kernel<256,7,0>,
+// merge_fixup_kernel), same tile size, hence the same bits as spmv_select("merge:b256:i7:x0") + spmv_apply; the
+// only difference is where the tile table and the tile carries live: not in buffers a handle obtained from
+// cudaMalloc (build_merge_plan), but in the file-scope array below, which is part of the library image and is
+// placed on every GPU that loads the library, for as long as the process runs.
+//
+// Layout of the array for kNoAllocMaxTiles tiles T:   [0, 8T) carry_val (double) | [8T, 12T) carry_row (int) |
+// [12T, 16T + 4) tile_row (int, T + 1 entries).  1 MiB + 256 B in all.
+//
+// Nothing in it has to start at zero: a call reads only words the same call wrote earlier on the same stream
+// (the partition kernel writes tile_row[0..ntiles], every tile of merge_kernel writes its own carry_row /
+// carry_val, and the fix-up reads those ntiles entries only), so what an earlier call -- possibly with more
+// tiles -- left behind is never looked at.
+namespace spmv {
+
+constexpr int kNoAllocBlock = 256, kNoAllocItems = 7;
+constexpr int kNoAllocTileItems = kNoAllocBlock * kNoAllocItems;        // 1792 merge-path items per tile
+constexpr int64_t kNoAllocMaxTiles = 65536;
+constexpr int64_t kNoAllocMaxPath = kNoAllocMaxTiles * kNoAllocTileItems;  // rows + nnz <= 117 440 512
+constexpr size_t kNoAllocBytes = (size_t)((16 * kNoAllocMaxTiles + 4 + 255) / 256 * 256);
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// In host code `g_noalloc_scratch` is only a stand-in the runtime uses to look the array up: its value is not a
+// device address and must never reach a kernel.  The address on a given GPU comes from cudaGetSymbolAddress,
+// asked once per device with that device current, and is kept here.
+constexpr int kNoAllocMaxDevices = 64;
+static std::mutex g_noalloc_mu;
+static unsigned char* g_noalloc_addr[kNoAllocMaxDevices] = {nullptr};
+
+static spmv_status_t noalloc_scratch_for_current_device(unsigned char** out) {
+  int dev = -1;
+  SPMV_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) {
+    set_last_error("spmv_merge_apply_noalloc: device ordinal %d is outside the %d this entry point keeps track of",
+                   dev, kNoAllocMaxDevices);
+    return SPMV_ERR_UNSUPPORTED;
+  }
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  if (!g_noalloc_addr[dev]) {
+    unsigned char* p = nullptr;
+    SPMV_CUDA_TRY(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+    if (!p) {
+      set_last_error("spmv_merge_apply_noalloc: cudaGetSymbolAddress returned a null address on device %d", dev);
+      return SPMV_ERR_CUDA;
+    }
+    g_noalloc_addr[dev] = p;
+  }
+  *out = g_noalloc_addr[dev];
+  return SPMV_OK;
+}
+
+}  // namespace spmv
+
+extern "C" {
+
+int64_t spmv_merge_noalloc_max_path(void) { return spmv::kNoAllocMaxPath; }
+
+spmv_status_t spmv_merge_apply_noalloc(int64_t rows, int64_t cols, int64_t nnz, const int32_t* d_row_ptr,
+                                       const int32_t* d_col_idx, const double* d_val, double alpha,
+                                       const double* d_x, double beta, double* d_y, void* stream) {
+  using namespace spmv;
+  if (rows < 0 || cols < 0 || nnz < 0) return SPMV_ERR_INVALID_ARG;
+  if (rows > 0 && (!d_row_ptr || !d_y)) return SPMV_ERR_INVALID_ARG;
+  if (nnz > 0 && (!d_col_idx || !d_val)) return SPMV_ERR_INVALID_ARG;
+  if (rows > 0x7fffffffll || cols > 0x7fffffffll || nnz > 0x7fffffffll) {
+    set_last_error("spmv_merge_apply_noalloc: sizes over the int32 index range");
+    return SPMV_ERR_UNSUPPORTED;
+  }
+  const int64_t path = rows + nnz;
+  if (path > kNoAllocMaxPath) {
+    set_last_error("spmv_merge_apply_noalloc: rows + nnz = %lld is over the limit of %lld that the built-in "
+                   "scratch array (%zu bytes) can serve; use spmv_create / spmv_select / spmv_apply instead",
+                   (long long)path, (long long)kNoAllocMaxPath, kNoAllocBytes);
+    return SPMV_ERR_UNSUPPORTED;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  if (rows == 0) return SPMV_OK;
+  if (alpha == 0.0) {                                // y = beta*y: A, x and the scratch are not touched
+    cudaError_t e = scale_y_launch(rows, beta, d_y, s);
+    if (e != cudaSuccess) { set_last_error("scale kernel: %s", cudaGetErrorString(e)); return SPMV_ERR_CUDA; }
+    return SPMV_OK;
+  }
+  if (cols > 0 && nnz > 0 && !d_x) return SPMV_ERR_INVALID_ARG;
+  if (d_x == d_y) return SPMV_ERR_INVALID_ARG;       // x and y must not alias
+
+  unsigned char* base = nullptr;
+  spmv_status_t st = noalloc_scratch_for_current_device(&base);
+  if (st != SPMV_OK) return st;
+  int64_t ntiles = (path + kNoAllocTileItems - 1) / kNoAllocTileItems;
+  if (ntiles == 0) ntiles = 1;
+  double* carry_val = reinterpret_cast<double*>(base);
+  int32_t* carry_row = reinterpret_cast<int32_t*>(base + 8 * kNoAllocMaxTiles);
+  int32_t* tile_row = reinterpret_cast<int32_t*>(base + 12 * kNoAllocMaxTiles);
+
+  merge_partition_kernel<<<(unsigned)((ntiles + 1 + 255) / 256), 256, 0, s>>>((int)rows, (int)nnz, d_row_ptr,
+                                                                          kNoAllocTileItems, ntiles, tile_row);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  constexpr size_t smem = MergeSmem<kNoAllocBlock, kNoAllocItems>::bytes;
+  static_assert(smem <= 48 * 1024, "needs no opt-in shared memory attribute");
+  merge_kernel<kNoAllocBlock, kNoAllocItems, 0><<<(unsigned)ntiles, kNoAllocBlock, smem, s>>>(
+      (int)rows, (int)nnz, d_row_ptr, d_col_idx, d_val, tile_row, carry_row, carry_val, alpha, d_x, beta, d_y);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  merge_fixup_kernel<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(ntiles, carry_row, carry_val, alpha, d_y);
+  SPMV_CUDA_TRY(cudaGetLastError());
+  return SPMV_OK;
+}
+
+}  // extern "C"
