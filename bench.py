@@ -6,8 +6,10 @@
 
 One "step" is one pass of the hot path, y = alpha*A*x + beta*y through spmv_apply with the autotuned
 variant (cfg5: the batch of four applies through spmv_apply_batch), inputs resident in HBM.  Every
-config of --configs is tuned, checked against the oracle and timed; the FIRST one is the headline of
-the JSON line (default cfg4, the largest single matrix: 2.58 GB as CSR), the rest sit in `per_config`.
+config of --configs is tuned (every candidate verified against oracle/'s result for the config's inputs),
+checked against the oracle on every row and timed; the FIRST one is the headline (default cfg4, the largest
+single matrix: 2.58 GB as CSR).  stdout carries ONE compact JSON line (< 2 KB: contract fields, roofline,
+cpu_baseline, e2e, clocks, one summary entry per config); the full record goes to gpurun_out/bench_detail.json.
 
 Three numbers per config, never conflated:
   eff_gbs       algorithmic bytes of the CSR byte model (nnz*12 + (rows+1)*4 + 8*cols + 8*rows
@@ -45,7 +47,7 @@ METRIC = "fp64 SpMV effective GB/s & fraction of B200 HBM peak (autotuned vs def
 NOMINAL_HBM_GBS = 8000.0      # BASELINE.json:north_star "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 DEFAULT_CONFIGS = "4,1,2,3,5"
-ORACLE_SAMPLE_ROWS = 16384
+VALUE_STREAMING_FILTER = "csr_scalar,csr_vector,sell:,sell_tma,sell16,ell,merge,bcsr3,dia:,dia_tma,dia_win"
 
 
 def measured_peak():
@@ -154,26 +156,22 @@ def cpu_baseline(prob, W, steps_parallel=5, steps_serial=2):
             "gflops": 2.0 * prob.A.nnz / tp / 1e9}
 
 
-def oracle_check(prob, y_gpu: np.ndarray, n_sample: int = ORACLE_SAMPLE_ROWS, tol: float = 1e-12):
-    """Sampled-row parity of what was timed: the oracle (oracle/, plain CPU row loop) recomputes
-    `n_sample` seeded rows (+ the first and last 64) from the same inputs; acceptance rule and
-    tolerance are north_star's (1e-12 relative to scale_i).  Returns a small report dict."""
+def oracle_reference(prob):
+    """(y_ref, scale) of the whole config from oracle/ (its row-parallel form, bit-identical to the serial loop)."""
     import oracle
     A = prob.A
-    rows = A.rows
-    rng = np.random.default_rng(12345)
-    pick = np.unique(np.concatenate([rng.integers(0, rows, size=min(n_sample, rows)),
-                                     np.arange(min(64, rows)), np.arange(max(rows - 64, 0), rows)]))
-    rp = A.row_ptr.astype(np.int64)
-    lens = (rp[pick + 1] - rp[pick])
-    sub_rp = np.zeros(pick.size + 1, dtype=np.int64)
-    np.cumsum(lens, out=sub_rp[1:])
-    idx = np.repeat(rp[pick] - sub_rp[:-1], lens) + np.arange(int(sub_rp[-1]), dtype=np.int64)
-    y0 = prob.y0[pick] if prob.y0 is not None else None
-    y_ref, scale = oracle.spmv(sub_rp.astype(np.int32), A.col_idx[idx], A.val[idx], prob.alpha, prob.x, prob.beta, y0)
-    ok, mr, ff, nf = oracle.accept(y_gpu[pick], y_ref, scale, tol)
-    return {"rows_checked": int(pick.size), "ok": bool(ok), "max_err_over_scale": float(mr), "n_fail": int(nf),
-            "first_fail_row": int(pick[ff]) if nf else -1, "tolerance": tol}
+    return oracle.spmv(A.row_ptr, A.col_idx, A.val, prob.alpha, prob.x, prob.beta, prob.y0, parallel=True)
+
+
+def oracle_check(prob, y_gpu: np.ndarray, ref=None, tol: float = 1e-12):
+    """Parity of what was timed, on EVERY row: the oracle (oracle/, plain CPU row loop) recomputes the whole
+    product from the same inputs (`ref`: its (y_ref, scale) when already computed for the tuner); acceptance rule
+    and tolerance are north_star's (1e-12 relative to scale_i).  Returns a small report dict."""
+    import oracle
+    y_ref, scale = ref if ref is not None else oracle_reference(prob)
+    ok, mr, ff, nf = oracle.accept(y_gpu, y_ref, scale, tol)
+    return {"rows_checked": int(prob.A.rows), "ok": bool(ok), "max_err_over_scale": float(mr), "n_fail": int(nf),
+            "first_fail_row": int(ff) if nf else -1, "tolerance": tol}
 
 
 def run_reference(args, W):
@@ -206,7 +204,9 @@ def run_reference(args, W):
 
 def headline_config(W, cfg, rows, nnz):
     """The `config` object: identical in both arms (workload only; what was selected is `selection`)."""
-    return {"workload": W.CONFIG_NAMES[cfg], "rows": int(rows), "nnz": int(nnz)}
+    big = 12 * int(nnz) + 20 * int(rows) >= 4 * 126 * (1 << 20)
+    return {"workload": W.CONFIG_NAMES[cfg], "rows": int(rows), "nnz": int(nnz),
+            "l2": "inputs >= 4x L2: no flush" if big else "cold: rotated copies > 3x L2, or 2x L2 flush per step"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -233,6 +233,12 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
             ys.append(y0s[-1].clone())
 
     add_copy()
+    # the oracle's result for the config's own inputs: the reference EVERY tuner candidate is verified against
+    # (north_star (d)) and, after the timed region, the every-row parity check of the timed variant
+    refs, drefs = [], []
+    if not args.no_oracle_check:
+        refs = [oracle_reference(p) for p in probs]
+        drefs = [(torch.from_numpy(yr).to(device), torch.from_numpy(sc).to(device)) for yr, sc in refs]
     state = {"copies": 1, "mode": "warm", "step": 0, "nstreams": 1}
     streams = [torch.cuda.current_stream()]
     flush = None
@@ -289,19 +295,30 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
 
     # ---- tune first (setup, outside the timed region); the two fixed baselines are timed below under the
     # same cache protocol as the winner
-    def tune(h, first):
+    def tune(i, first, **kw):
         # the cold protocol applies when the CSR-model footprint is below 4x L2 (decided before the winner is known)
-        return h.tune(alpha=alpha, beta=beta, use_cache=(0 if (not first or args.tune_cache) else 2),
-                      cache_path=args.tune_cache, flush_l2=(nbytes < 4 * l2), seed=cfg,
-                      variant_filter=args.variant_filter)
+        m = i % members
+        ref = dict(x=xs[i], y0=y0s[i], y_ref=drefs[m][0], scale=drefs[m][1]) if drefs else {}
+        opts = dict(alpha=alpha, beta=beta, use_cache=(0 if (not first or args.tune_cache) else 2),
+                    cache_path=args.tune_cache, flush_l2=(nbytes < 4 * l2), seed=cfg,
+                    variant_filter=args.variant_filter)
+        opts.update(ref)
+        opts.update(kw)
+        return handles[i].tune(**opts)
     t0 = time.perf_counter()
-    reports = [tune(h, i == 0) for i, h in enumerate(handles)]
+    reports = [tune(i, i == 0) for i in range(len(handles))]
     stream_times = {}
     if members > 1:
         streams = [torch.cuda.current_stream()] + [torch.cuda.Stream(device=device) for _ in range(3)]
         state["nstreams"], stream_times = binding.tune_batch(handles, [alpha] * members, xs, [beta] * members, ys, streams)
     tune_s = time.perf_counter() - t0
     variant = handles[0].variant
+    # the feature-guided search on the same matrix and reference: its cost and its winner
+    rg = tune(0, True, use_cache=2, cache_path=None, search=1)
+    guided = {"tune_seconds": rg["tune_seconds"], "winner": rg["winner"], "winner_us": rg["winner_us"],
+              "n_timed": rg["n_timed"], "exhaustive_tune_seconds": reports[0]["tune_seconds"],
+              "exhaustive_winner_us": reports[0]["winner_us"], "exhaustive_n_timed": reports[0]["n_timed"]}
+    handles[0].select(variant)
     fmt_bytes = int(sum(h.info().format_bytes for h in handles[:members]))
     bytes_actual = fmt_bytes + vec_bytes
     # merge-path and row-split SELL add one small ordered fix-up kernel per apply
@@ -316,7 +333,7 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
             state["mode"] = "rotate"
             for _ in range(copies - 1):
                 add_copy()
-                tune(handles[-1], False)          # in-process cache hit: same variant
+                tune(len(handles) - 1, False)     # in-process cache hit: same variant
             state["copies"] = copies
         else:
             state["mode"] = "flush"
@@ -362,6 +379,21 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
             torch.cuda.synchronize()
     clocks = sampler.stop() if sampler is not None else None
 
+    # ---- where the winner reads no matrix values (constant-coefficient stencil): the best variant that DOES stream
+    # them, same cache protocol -- what the stencil kernels do on a variable-coefficient matrix of this shape
+    with_values = None
+    if members == 1 and variant.split(":")[0] in ("dia_const", "dia_cwin"):
+        rv = tune(0, True, use_cache=2, cache_path=None, variant_filter=VALUE_STREAMING_FILTER)
+        for h in handles:
+            h.select(rv["winner"])
+        tv = float(np.median(timed(k_base, 3, 5.0, max_batches=20)))
+        fbv = int(handles[0].info().format_bytes) + vec_bytes
+        with_values = {"variant": rv["winner"], "t_us": tv * 1e6, "eff_gbs": nbytes / tv / 1e9,
+                       "bytes_actual": fbv, "actual_gbs": fbv / tv / 1e9, "frac_actual_of_measured": fbv / tv / 1e9 / measured_peak()[0],
+                       "filter": VALUE_STREAMING_FILTER}
+        for h in handles:
+            h.select(variant)
+
     # ---- the other cache state: warm (same buffers back to back) where the headline is cold
     t_warm = t_step
     if state["mode"] != "warm" and members == 1:
@@ -395,11 +427,12 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     deterministic = all(torch.equal(a, b) for a, b in zip(first, first_members()))
     parity = None
     if primary and not args.no_oracle_check:
-        checks = [oracle_check(p, y.cpu().numpy()) for p, y in zip(probs, first)]
+        checks = [oracle_check(p, y.cpu().numpy(), ref=r) for p, y, r in zip(probs, first, refs)]
         parity = {"ok": all(c["ok"] for c in checks), "rows_checked": sum(c["rows_checked"] for c in checks),
                   "max_err_over_scale": max(c["max_err_over_scale"] for c in checks),
                   "n_fail": sum(c["n_fail"] for c in checks), "tolerance": 1e-12,
-                  "what": "one apply of the timed variant from y0 vs oracle/ on seeded sample rows"}
+                  "rows": int(sum(p.A.rows for p in probs)),
+                  "what": "one apply of the timed variant from y0 vs oracle/ on every row"}
         if not parity["ok"]:
             raise SystemExit(f"bench: cfg{cfg} {variant} FAILED the oracle check: {checks}")
 
@@ -507,7 +540,8 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
            "tune_seconds": tune_s, "tune_reports": [{k: v for k, v in r.items() if k != "log"} for r in reports[:members]],
            "launches_per_step": launches_per_step, "timing": timing_note, "cache_mode": state["mode"],
            "deterministic": deterministic, "parity": parity, "e2e": e2e, "clocks": clocks, "cg": cg,
-           "graph_replay": graph, "sm_count": info.sm_count, "l2_bytes": info.l2_bytes,
+           "graph_replay": graph, "guided_search": guided, "with_values": with_values,
+           "tune_reference": "oracle" if drefs else "library reference kernel", "sm_count": info.sm_count, "l2_bytes": info.l2_bytes,
            "device": info.device_name.decode()}
     for h in handles:
         h.close()
@@ -621,6 +655,110 @@ def config_roofline(r, peak, ceil):
                     "CSR byte model of the metric and exceeds 1 when the format streams fewer bytes than CSR"}
 
 
+COMPACT_LIMIT = 2048      # bytes: the LAST stdout line must stay a short, driver-parseable JSON object
+
+
+def _r(v, nd=4):
+    """Round floats for the compact line (significant digits, not decimals)."""
+    if isinstance(v, float):
+        return float(f"{v:.{nd + 2}g}")
+    return v
+
+
+def compact_line(full: dict, detail_path: str | None) -> dict:
+    """The one JSON line of the contract: headline fields of the first config, the roofline / cpu_baseline / e2e
+    objects, and a one-entry-per-config summary.  Everything else (tune reports, ceilings, solver loops, the banded
+    extra) goes to the detail file.  Kept under COMPACT_LIMIT bytes (tests/test_bench_line_cpu.py)."""
+    out = {k: _r(full.get(k)) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                                        "higher_is_better", "scaling", "vs_baseline", "dtype", "data")}
+    out["config"] = dict(full["config"])
+    rf = full.get("roofline") or {}
+    out["roofline"] = {k: _r(rf.get(k)) for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
+                                                  "bytes_per_launch", "effective_gbs", "kernel") if k in rf}
+    cb = full.get("cpu_baseline")
+    if cb:
+        out["cpu_baseline"] = {"value": _r(cb["value"]), "unit": cb["unit"], "cores": cb["cores"], "kind": cb["kind"],
+                               "sample": str(cb.get("sample", ""))[:64]}
+    e = full["e2e"]
+    out["e2e"] = {k: _r(e[k]) for k in ("value", "unit", "ms_per_step", "h2d_bytes_per_step", "d2h_bytes_per_step")}
+    out["gpu_launches"] = full["gpu_launches"]
+    ck = full.get("clocks") or {}
+    out["clocks"] = {"sm_mhz": ck.get("sm_mhz"), "sm_max_mhz": ck.get("sm_max_mhz"), "reasons": ck.get("reasons", [])}
+    par = full.get("parity") or {}
+    out["parity"] = {k: _r(par.get(k)) for k in ("ok", "rows_checked", "rows", "max_err_over_scale", "tolerance")}
+    out["deterministic"] = full.get("deterministic")
+    out["speedup_vs_default"] = _r(full.get("speedup_vs_default"))
+    g = full.get("guided_search") or {}
+    out["tune"] = {"reference": full.get("tune_reference"), "exhaustive_s": _r(g.get("exhaustive_tune_seconds"), 2),
+                   "guided_s": _r(g.get("tune_seconds"), 2), "exhaustive_us": _r(g.get("exhaustive_winner_us")),
+                   "guided_us": _r(g.get("winner_us"))}
+    rows = []
+    for r in full.get("per_config", []):
+        rr = r.get("roofline") or {}
+        row = {"cfg": r["cfg"], "variant": r["variant"], "us": _r(r["t_step_us"], 2), "frac": _r(rr.get("frac"), 1)}
+        wv = r.get("with_values")
+        if wv and wv["frac_actual_of_measured"] > 0.05:    # (not for launch-bound sizes)
+                  # the best variant that still streams the matrix values: [descriptor, us, fraction of the HBM peak]
+            row["with_values"] = [wv["variant"], _r(wv["t_us"], 2), _r(wv["frac_actual_of_measured"], 1)]
+        rows.append(row)
+    out["detail"] = detail_path
+    # never let the summary break the contract line: drop its optional parts until it fits
+    for drop in ((), ("with_values",), ("with_values", "variant")):
+        out["per_config"] = [{k: v for k, v in row.items() if k not in drop} for row in rows]
+        if len(json.dumps(out, separators=(",", ":"))) < COMPACT_LIMIT - 100:
+            break
+    return out
+
+
+def write_detail(full: dict) -> str | None:
+    """The full record (per-config tune reports, ceilings, solver loops, banded extra) as a side file."""
+    for d in (os.path.join(ROOT, "gpurun_out"), tempfile.gettempdir()):
+        try:
+            os.makedirs(d, exist_ok=True)
+            path = os.path.join(d, "bench_detail.json")
+            with open(path, "w") as f:
+                json.dump(full, f, indent=1)
+            return os.path.relpath(path, ROOT) if path.startswith(ROOT) else path
+        except OSError:
+            continue
+    return None
+
+
+def relaunch_under_torchrun(args) -> None:
+    """`python bench.py --gpus N` with N > 1 and no launcher around it: start N ranks ourselves (one process per GPU,
+    torch.distributed.run on 127.0.0.1) -- the same launch the driver uses -- and become that launcher."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    sys.stdout.flush()
+    os.execv(sys.executable, cmd)
+
+
+def rendezvous_only(args) -> None:
+    """--rendezvous-only: every rank joins the process group (nccl with a GPU per rank, else gloo), one all-reduce
+    counts them, rank 0 prints {"ranks_joined": N}.  The launch-readiness check of `--gpus N` (no SpMV work)."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    n = 1
+    if world > 1:
+        use_nccl = torch.cuda.is_available() and torch.cuda.device_count() >= world
+        if use_nccl:
+            torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        dist.init_process_group("nccl" if use_nccl else "gloo")
+        t = torch.ones(1, device="cuda" if use_nccl else "cpu")
+        dist.all_reduce(t)
+        n = int(t.item())
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"ranks_joined": n, "n_gpus": args.gpus, "world_size": world}))
+
+
 def profile_one(args, torch, binding, W):
     """A few applies of one variant on one config: the command the ncu captures under profiles/ run."""
     cfg = args.profile_one
@@ -677,8 +815,14 @@ def main():
     ap.add_argument("--profile-one", type=int, default=0, metavar="CFG", help="ncu / sanitizer driver: a few cold applies of one variant (6 = the banded extra workload)")
     ap.add_argument("--variant", default=None, help="--profile-one: descriptor to force ('tuned' or absent: tune)")
     ap.add_argument("--iters", type=int, default=5)
+    ap.add_argument("--rendezvous-only", action="store_true", help="join the N ranks, count them, print, exit (launch check)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.profile_one:
+        relaunch_under_torchrun(args)           # does not return
+    if args.rendezvous_only:
+        rendezvous_only(args)
+        return
 
     from paper_1309_1894_b200 import workloads as W
     if args.impl == "reference":
@@ -696,6 +840,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and rank == 0:
+        print(f"bench: --gpus {args.gpus} but the launcher started {world} rank(s); n_gpus = {world}", file=sys.stderr)
     torch.cuda.set_device(local)
     device = f"cuda:{local}"
     if world > 1:
@@ -727,6 +873,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": head["t_step_us"] * 1e-3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": headline_config(W, head["cfg"], head["rows"], head["nnz"]),
+        "guided_search": head["guided_search"], "tune_reference": head["tune_reference"],
         "selection": {"variant": head["variant"], "nstreams": head["nstreams"], "variant_filter": args.variant_filter,
                       "l2": head["timing"],
                       "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
@@ -764,7 +911,9 @@ def main():
         line["cg"] = next((r["cg"] for r in results if r["cg"]), None)
         if not args.no_extras:
             line["banded"] = bench_banded(args, torch, binding, W, device)
-        print(json.dumps(line))
+        detail = write_detail(line)
+        sys.stdout.flush()
+        print(json.dumps(compact_line(line, detail), separators=(",", ":")), flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
