@@ -212,13 +212,14 @@ class SpMV:
     """Handle wrapper.  row_ptr/col_idx (int32) and val (float64) are CUDA torch tensors that
     this object keeps alive (the C handle borrows them)."""
 
-    def __init__(self, rows, cols, row_ptr, col_idx, val, *, use_torch_allocator=True, stream=None):
+    def __init__(self, rows, cols, row_ptr, col_idx, val, *, use_torch_allocator=True, stream=None, allocator=None):
         import torch
         assert row_ptr.is_cuda and row_ptr.dtype == torch.int32 and row_ptr.is_contiguous()
         assert col_idx.dtype == torch.int32 and val.dtype == torch.float64
         assert col_idx.is_contiguous() and val.is_contiguous()
         self._keep = (row_ptr, col_idx, val)
-        self._alloc = _torch_allocator() if use_torch_allocator else None
+        # allocator: a ready-made Allocator struct (spmv_allocator_t callbacks; the tests pass a failing one)
+        self._alloc = allocator if allocator is not None else (_torch_allocator() if use_torch_allocator else None)
         self.rows, self.cols, self.nnz = int(rows), int(cols), int(val.numel())
         h = C.c_void_p(0)
         st = lib().spmv_create(C.byref(h), self.rows, self.cols, self.nnz, _dptr(row_ptr),

@@ -32,12 +32,43 @@ static void refresh_info(spmv_handle_s* h) {
 }
 void handle_refresh_info(spmv_handle_s* h) { refresh_info(h); }
 
+// Does the format the SELECTED variant's launch plan points into still exist?  (The plan holds raw device
+// pointers into it; error paths of select / tune / update_values may have released it.)
+bool selected_format_alive(const spmv_handle_s* h) {
+  const Variant& v = h->sel;
+  switch (v.fam) {
+    case FAM_CSR_SCALAR: case FAM_CSR_VECTOR: return true;          // caller-owned CSR arrays only
+    case FAM_SELL: case FAM_SELL_TMA: case FAM_SELL16: case FAM_SELL16_TMA: return h->sells.count(sell_key(v)) != 0;
+    case FAM_ELL: return h->has_ell;
+    case FAM_MERGE: return h->plans.count(v.block * v.I) != 0;
+    case FAM_BCSR3: return h->has_bcsr && (v.I == 16 ? h->bcsr.bcol16 != nullptr : h->bcsr.bcol != nullptr);
+    case FAM_DIA: case FAM_DIA_TMA: case FAM_DIA_CONST: case FAM_DIA_WIN: case FAM_DIA_CWIN: return h->dias.count(v.C) != 0;
+    default: return false;
+  }
+}
+
+// The fixed default variant reads the caller's CSR arrays only, so its plan needs no allocation and can never
+// point at freed memory: where a selection's format has been (or may have been) released, the handle goes here.
+void reset_to_default(spmv_handle_s* h) {
+  const Variant d = default_variant();
+  LaunchPlan p;
+  if (build_plan(h, d, &p) != SPMV_OK) p = LaunchPlan();
+  h->sel = d;
+  h->plan = p;
+  h->tuned = false;
+  h->leaders.clear();
+  refresh_info(h);
+}
+void repair_selection_after_failure(spmv_handle_s* h) {
+  if (!selected_format_alive(h)) reset_to_default(h);
+}
+
 spmv_status_t adopt_variant(spmv_handle_s* h, const Variant& v, cudaStream_t s) {
   spmv_status_t st = ensure_format(h, v, s);
-  if (st != SPMV_OK) return st;
+  if (st != SPMV_OK) { repair_selection_after_failure(h); return st; }
   LaunchPlan p;
   st = build_plan(h, v, &p);
-  if (st != SPMV_OK) return st;
+  if (st != SPMV_OK) { repair_selection_after_failure(h); return st; }
   h->sel = v;
   h->plan = p;
   release_formats_except(h, v);
@@ -171,19 +202,26 @@ spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* 
   cudaStream_t s = (cudaStream_t)stream;
   SPMV_CUDA_TRY(cudaDeviceSynchronize());           // no apply on any stream may still be reading the old formats
   h->A.val = d_val;
+  const Variant want = h->sel;
+  const bool was_tuned = h->tuned;
+  const std::vector<std::string> leaders = h->leaders;
   release_all_formats(h);
+  reset_to_default(h);                              // the old plan points into what was just freed: whatever fails
+                                                    // below, the handle stays usable (on the default variant)
   if (h->dia_state > 0) h->dia_state = 0;           // constness must be re-established on the new values
   if (fell_back) *fell_back = 0;
-  spmv_status_t st = adopt_variant(h, h->sel, s);
+  spmv_status_t st = adopt_variant(h, want, s);
+  if (st == SPMV_OK) { h->tuned = was_tuned; h->leaders = leaders; refresh_info(h); }
   if (st == SPMV_ERR_UNSUPPORTED) {
     if (fell_back) *fell_back = 1;
-    Variant alt = h->sel;
+    Variant alt = want;
     st = SPMV_ERR_UNSUPPORTED;
-    if ((h->sel.fam == FAM_DIA_CONST || h->sel.fam == FAM_DIA_CWIN) && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
+    if ((want.fam == FAM_DIA_CONST || want.fam == FAM_DIA_CWIN) && variant_from_string("dia_tma:b288:c256:r1:u8:i3:x0", &alt)) {
       std::string why;
       if (variant_eligible(h, alt, &why)) st = adopt_variant(h, alt, s);
+      if (st == SPMV_OK) { h->tuned = was_tuned; refresh_info(h); }
     }
-    if (st != SPMV_OK) { h->tuned = false; st = adopt_variant(h, default_variant(), s); }
+    if (st != SPMV_OK) st = adopt_variant(h, default_variant(), s);
   }
   if (st != SPMV_OK) return st;
   SPMV_CUDA_TRY(cudaStreamSynchronize(s));
@@ -202,6 +240,7 @@ spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, doubl
     return SPMV_OK;
   }
   if (h->A.cols > 0 && !d_x) return SPMV_ERR_INVALID_ARG;
+  if (d_x == d_y) { set_last_error("spmv_apply: x and y are the same vector (they must not alias)"); return SPMV_ERR_INVALID_ARG; }
   ApplyArgs a{alpha, beta, d_x, d_y, s};
   return launch_plan(h->plan, a);
 }

@@ -60,6 +60,11 @@ spmv_status_t build_dot_plan(spmv_handle_s* h, double* part, int* n_part, Launch
 spmv_status_t launch_plan(const LaunchPlan& p, const ApplyArgs& a);
 // Makes `v` the selected variant: format, plan, info.  Waits for the device first when formats are freed.
 spmv_status_t adopt_variant(spmv_handle_s* h, const Variant& v, cudaStream_t s);
+// Error paths that may have released the selected variant's format call this: if the format is gone, the handle
+// goes back to the fixed default variant (plan on the caller's CSR arrays), tuned = false.
+bool selected_format_alive(const spmv_handle_s* h);
+void repair_selection_after_failure(spmv_handle_s* h);
+void reset_to_default(spmv_handle_s* h);
 // Bytes of matrix data the variant streams per apply (format-actual, not algorithmic).
 int64_t variant_format_bytes(const spmv_handle_s* h, const Variant& v);
 // Frees every owned format the given variant does not need.

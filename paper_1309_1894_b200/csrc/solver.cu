@@ -260,6 +260,8 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
     std::string best;
     double best_s = 1e300;
     const std::vector<std::string> leaders = h->leaders;
+    const Variant incoming = h->sel;                         // what the caller had selected (the apply winner)
+    const bool incoming_tuned = h->tuned;
     for (const std::string& d : leaders) {
       Variant v;
       std::string why;
@@ -275,11 +277,15 @@ extern "C" spmv_status_t spmv_cg(spmv_handle_t h, const double* d_b, double* d_x
     }
     cudaStreamSynchronize(s);
     h->al.free(xs, sizeof(double) * (size_t)n);
-    Variant v;
-    if (!best.empty() && variant_from_string(best.c_str(), &v)) {
-      spmv_status_t st = adopt_variant(h, v, s);
-      if (st != SPMV_OK) return st;
-    }
+    // no probe produced a time (b == 0, breakdown, a failed probe): back to the caller's selection, not to
+    // whichever leader happened to be probed last
+    Variant v = incoming;
+    if (!best.empty() && !variant_from_string(best.c_str(), &v)) v = incoming;
+    spmv_status_t st = adopt_variant(h, v, s);
+    if (st != SPMV_OK && !best.empty()) st = adopt_variant(h, incoming, s);
+    if (st != SPMV_OK) return st;
+    h->tuned = incoming_tuned;
+    h->leaders = leaders;
   }
 
   // small systems: one cooperative kernel for the whole solve (see cg_fused_kernel)

@@ -358,33 +358,39 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
   const int64_t rows = h->A.rows, cols = h->A.cols;
 
   const std::string key = signature_key(h, T.beta != 0.0);
-  if (o.use_cache != 2 && !(o.fault_inject && *o.fault_inject)) {
+  // A cached winner is a CLAIM (the signature covers the structure, not the values; the file may be stale, edited
+  // or written by another build): it is looked up here and adopted further down only after one launch of it has
+  // passed the same verification every candidate passes.  A failed entry is dropped and the full search runs.
+  bool have_cached = false;
+  Variant cached_v;
+  CacheEntry cached_e;
+  if (o.use_cache != 2) {
     std::lock_guard<std::mutex> lk(g_cache_mu);
     if (o.cache_path && *o.cache_path) cache_file_load(o.cache_path);
     auto it = g_cache.find(key);
-    if (it != g_cache.end()) {
-      Variant v;
-      std::string why;
-      if (variant_from_string(it->second.variant.c_str(), &v) && variant_eligible(h, v, &why) &&
-          adopt_variant(h, v, T.s) == SPMV_OK) {
-        h->tuned = true;
-        h->leaders.assign(1, it->second.variant);
-        handle_refresh_info(h);
-        if (report) {
-          strncpy(report->winner, it->second.variant.c_str(), sizeof(report->winner) - 1);
-          report->winner_us = it->second.us;
-          report->cache_hit = 1;
-          report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
-        }
-        return SPMV_OK;
-      }
+    std::string why;
+    if (it != g_cache.end() && variant_from_string(it->second.variant.c_str(), &cached_v) && variant_eligible(h, cached_v, &why)) {
+      have_cached = true;
+      cached_e = it->second;
     }
   }
 
   // ---- probes, reference result, scratch
   Allocator& al = h->al;
   spmv_status_t st = SPMV_OK;
-  auto fail = [&](spmv_status_t code) { T.cleanup(); return code; };
+  // the candidate loop releases formats as it goes, possibly the one the pre-tune selection's plan points into
+  // and ensure_format may rebuild a format at another address: after a failure re-resolve the pre-tune selection
+  // (format found or rebuilt, plan rebuilt); if that fails too, the fixed default variant (no owned memory)
+  const Variant pre_sel = h->sel;
+  const bool pre_tuned = h->tuned;
+  auto fail = [&](spmv_status_t code) {
+    T.cleanup();
+    const std::string err = last_error_text();
+    if (adopt_variant(h, pre_sel, T.s) == SPMV_OK) { h->tuned = pre_tuned; handle_refresh_info(h); }
+    else reset_to_default(h);
+    set_last_error("%s", err.c_str());
+    return code;
+  };
   if (cudaEventCreate(&T.e0) != cudaSuccess || cudaEventCreate(&T.e1) != cudaSuccess) return fail(SPMV_ERR_CUDA);
   T.x = (double*)o.d_x_probe;
   if (!T.x) { T.x = (double*)al.alloc(sizeof(double) * cols, T.s); T.own_x = true; if (!T.x) return fail(SPMV_ERR_ALLOC);
@@ -408,6 +414,32 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
     T.flush_n = (int64_t)(2 * h->dev.l2_bytes / sizeof(double));
     T.flushbuf = (double*)al.alloc(sizeof(double) * T.flush_n, T.s);
     if (!T.flushbuf) return fail(SPMV_ERR_ALLOC);
+  }
+
+  // ---- cache hit: verify the cached winner once, then adopt it
+  if (have_cached) {
+    bool pass = false; double err = 0, vus = 0;
+    LaunchPlan plan;
+    spmv_status_t sc = ensure_format(h, cached_v, T.s);
+    if (sc == SPMV_OK) sc = build_plan(h, cached_v, &plan);
+    if (sc == SPMV_OK) sc = T.verify(cached_v, plan, &pass, &err, &vus);
+    if (sc == SPMV_OK && pass && adopt_variant(h, cached_v, T.s) == SPMV_OK) {
+      T.log(cached_e.variant, "cache_hit_verified", vus, err);
+      h->tuned = true;
+      h->leaders.assign(1, cached_e.variant);
+      T.cleanup();
+      handle_refresh_info(h);
+      if (report) {
+        strncpy(report->winner, cached_e.variant.c_str(), sizeof(report->winner) - 1);
+        report->winner_us = cached_e.us;
+        report->cache_hit = 1;
+        report->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+      }
+      return SPMV_OK;
+    }
+    T.log(cached_e.variant, "cache_entry_rejected", vus, err);
+    std::lock_guard<std::mutex> lk(g_cache_mu);
+    g_cache.erase(key);
   }
 
   // ---- phase 1: every candidate, verify then time

@@ -224,6 +224,7 @@ spmv_status_t ensure_format(spmv_handle_s* h, const Variant& v, cudaStream_t s) 
         cudaDeviceSynchronize();
         free_bcsr3(h->bcsr, h->al);
         h->has_bcsr = false;
+        if (h->sel.fam == FAM_BCSR3) reset_to_default(h);   // its plan pointed into the format just freed
       }
       if (!h->has_bcsr) {
         spmv_status_t st = build_bcsr3(h->A, h->al, s, &h->bcsr);

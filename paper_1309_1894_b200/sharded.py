@@ -114,15 +114,28 @@ class _LoopbackEnd:
         return [self.hub.lists[q][self.rank] for q in range(self.world)]
 
     def start(self, sends, recvs):
-        self.hub.posted[self.rank] = (sends, recvs)
+        # The sender packed its buffers on ITS current stream (a shard's comm stream); the receiver copies them on
+        # another stream that has no dependency on it.  An event recorded here, after the packing kernels, travels
+        # with the posted sends and the receiver waits on it before it reads (without it the copy could read the
+        # send buffer before the gather had written it).
+        ev = None
+        if any(t.is_cuda for _, t in sends):
+            import torch
+            ev = torch.cuda.Event()
+            ev.record(torch.cuda.current_stream())
+        self.hub.posted[self.rank] = (sends, recvs, ev)
         return self.rank
 
     def wait(self, _):
         # deliver everything addressed to me (every end has posted before anyone waits: lock-step driver)
-        _, my_recvs = self.hub.posted[self.rank]
+        _, my_recvs, _ = self.hub.posted[self.rank]
         for peer, dst in my_recvs:
-            src = [t for p, t in self.hub.posted[peer][0] if p == self.rank]
+            peer_sends, _, peer_ev = self.hub.posted[peer]
+            src = [t for p, t in peer_sends if p == self.rank]
             assert len(src) == 1 and src[0].numel() == dst.numel()
+            if peer_ev is not None and dst.is_cuda:
+                import torch
+                torch.cuda.current_stream().wait_event(peer_ev)
             dst.copy_(src[0])
 
 

@@ -52,6 +52,10 @@ def test_sharded_apply_matches_oracle(cuda, name, world, variant):
     if name in ("stencil7", "stencil27", "fem", "banded") and variant.split(":")[0] != "merge":
         assert n_split == world                                # banded: interior rows overlap the exchange
     for alpha, beta in ((1.0, 0.0), (-1.5, 0.5)):
+        if beta != 0.0:                                        # a NEW x for the second pass: halo buffers that still hold
+            x = W.uniform(91, A.cols)                          # the first pass's entries would now give a wrong result
+            for s in shards:
+                s.x_owned.copy_(torch.from_numpy(x[s.lo:s.hi]))
         ys = [H.to_dev(y0[s.lo:s.hi]).clone() if beta != 0.0 else
               torch.full((s.rows_local,), float("nan"), dtype=torch.float64, device="cuda") for s in shards]
         sharded.run_lockstep(shards, alpha, beta, ys)
