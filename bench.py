@@ -815,6 +815,7 @@ def main():
     ap.add_argument("--profile-one", type=int, default=0, metavar="CFG", help="ncu / sanitizer driver: a few cold applies of one variant (6 = the banded extra workload)")
     ap.add_argument("--variant", default=None, help="--profile-one: descriptor to force ('tuned' or absent: tune)")
     ap.add_argument("--iters", type=int, default=5)
+    ap.add_argument("--ceilings", action="store_true", help="run only the library's ceiling kernels (spmv_measure_ceiling) and print them")
     ap.add_argument("--rendezvous-only", action="store_true", help="join the N ranks, count them, print, exit (launch check)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
@@ -836,6 +837,15 @@ def main():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     if args.profile_one:
         profile_one(args, torch, binding, W)
+        return
+    if args.ceilings:          # the library's ceiling kernels alone (the command the ceiling captures in profiles/ run)
+        torch.cuda.set_device(0)
+        print(json.dumps({"copy_gbs_1GiB": binding.measure_ceiling(0, 1 << 30, 5),
+                          "read_gbs_1GiB": binding.measure_ceiling(1, 1 << 30, 5),
+                          "read_gbs_1777MB": binding.measure_ceiling(1, 1777136820, 5),
+                          "blockrow_read_gbs_1684MB": binding.measure_ceiling(4, 1684343232, 7),
+                          "empty_launch_us": binding.measure_ceiling(2, 0, 200),
+                          "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}))
         return
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -895,7 +905,8 @@ def main():
         ceil = {"copy_gbs_1GiB": binding.measure_ceiling(0, 1 << 30, 5),
                 "read_gbs_1GiB": binding.measure_ceiling(1, 1 << 30, 5),
                 "empty_launch_us": binding.measure_ceiling(2, 0, 200),
-                "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3)}
+                "random_gather_G_per_s_32MiB_table": binding.measure_ceiling(3, 1 << 25, 3),
+                "bcsr3_value_loads_only_gbs": binding.measure_ceiling(4, 1684343232, 5)}
         line["ceilings"] = ceil
         try:
             cpu_model = [l.split(":", 1)[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")][0]

@@ -29,9 +29,12 @@
  *   - There is no CPU fallback: without a CUDA device every compute entry point
  *     returns SPMV_ERR_CUDA.
  *   - Concurrency: distinct handles are independent.  One handle may have several applies in
- *     flight on different streams only if its selected variant has no workspace; merge-path
- *     (tile carries) and row-split SELL (segment sums) own one workspace per handle, so their
- *     applies must be ordered (same stream, or events).  spmv_cg allocates per call.
+ *     flight on different streams.  Variants that own a workspace -- merge-path (tile carries)
+ *     and row-split SELL (segment sums), one workspace per handle -- are ordered by the library:
+ *     an spmv_apply on another stream than the handle's previous apply first makes its stream wait
+ *     (on the device, through an event) for that apply.  Exceptions the caller orders: applies
+ *     enqueued inside a stream capture, and replays of an spmv_graph_t next to other applies of the
+ *     same handle.  spmv_apply itself may be called from several host threads.  spmv_cg allocates per call.
  *
  * Variant descriptors (spmv_select, tune reports, spmv_list_variants): "family:key<int>:..."
  *   families  csr_scalar (thread per row), csr_vector (w lanes per row), sell / sell_tma
@@ -395,7 +398,8 @@ SPMV_API spmv_status_t spmv_destroy(spmv_handle_t h);
  * launches back to back over rotating windows (cold);
  * 2: empty-kernel launch latency in microseconds, 3: random 8-byte gathers out of a vector of
  * `bytes` bytes, in giga-gathers per second (the ceiling of the x path when columns are
- * unstructured). */
+ * unstructured), 4: the value loads of the bcsr3 kernel alone (records of 27 3x3 blocks in the block-row layout,
+ * 16 lanes per record, no x / index / FMA; GB/s, median batch): what the layout's load pattern allows. */
 SPMV_API spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_t reps, void* stream,
                                    double* result);
 

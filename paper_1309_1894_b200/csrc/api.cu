@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <mutex>
 #include <set>
+#include <string>
 
 #include "handle.h"
 
@@ -172,6 +173,7 @@ spmv_status_t spmv_destroy(spmv_handle_t h) {
   if (h->d_x_stage) h->al.free(h->d_x_stage, sizeof(double) * h->A.cols);
   if (h->d_y_stage) h->al.free(h->d_y_stage, sizeof(double) * h->A.rows);
   for (cudaEvent_t e : h->hs_events) cudaEventDestroy(e);
+  if (h->ws_event) cudaEventDestroy(h->ws_event);
   if (h->hs_up) { cudaStreamDestroy(h->hs_up); cudaStreamDestroy(h->hs_up2); cudaStreamDestroy(h->hs_run); cudaStreamDestroy(h->hs_down); }
   h->magic = 0;
   delete h;
@@ -228,6 +230,27 @@ spmv_status_t spmv_update_values(spmv_handle_t h, const double* d_val, int32_t* 
   return SPMV_OK;
 }
 
+// Variants with a second, ordered fix-up kernel own one workspace per handle.  Two applies of such a variant on
+// DIFFERENT streams would overlap on the GPU and mix their carries, so the library orders them itself: every such
+// apply records an event, and an apply on another stream than the previous one first makes its stream wait for it
+// (no host synchronisation; same-stream applies pay one event record).  Inside a stream capture the graph's own
+// edges order the launches and no event is touched; replaying such a graph concurrently with other applies of the
+// same handle remains the caller's to order.
+static spmv_status_t apply_with_workspace(spmv_handle_s* h, const ApplyArgs& a) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(a.stream, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+  if (cap != cudaStreamCaptureStatusNone) return launch_plan(h->plan, a);
+  std::lock_guard<std::mutex> lk(h->ws_mu);
+  if (!h->ws_event) SPMV_CUDA_TRY(cudaEventCreateWithFlags(&h->ws_event, cudaEventDisableTiming));
+  if (h->ws_used && h->ws_stream != a.stream) SPMV_CUDA_TRY(cudaStreamWaitEvent(a.stream, h->ws_event, 0));
+  const spmv_status_t st = launch_plan(h->plan, a);
+  if (st != SPMV_OK) return st;
+  SPMV_CUDA_TRY(cudaEventRecord(h->ws_event, a.stream));
+  h->ws_stream = a.stream;
+  h->ws_used = true;
+  return SPMV_OK;
+}
+
 // The apply path: argument checks, then one (two for merge-path / row-split SELL) kernel launch from the
 // plan resolved at select / tune time.  No locks, no lookups, no CUDA attribute or occupancy calls.
 spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, double beta, double* d_y, void* stream) {
@@ -242,6 +265,7 @@ spmv_status_t spmv_apply(spmv_handle_t h, double alpha, const double* d_x, doubl
   if (h->A.cols > 0 && !d_x) return SPMV_ERR_INVALID_ARG;
   if (d_x == d_y) { set_last_error("spmv_apply: x and y are the same vector (they must not alias)"); return SPMV_ERR_INVALID_ARG; }
   ApplyArgs a{alpha, beta, d_x, d_y, s};
+  if (h->plan.n == 2) return apply_with_workspace(h, a);     // merge-path / row-split SELL
   return launch_plan(h->plan, a);
 }
 
@@ -299,7 +323,28 @@ spmv_status_t spmv_graph_destroy(spmv_graph_t g) {
 // one-launch form: a row is summed by the same kernel code in the same order.
 // entry: event the pipeline's internal streams wait on (nullptr: the current tail of `stream`); wait: synchronise
 // `stream` before returning (spmv_apply_host_batch enqueues every member first and synchronises once)
+static spmv_status_t apply_host_body(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
+                                     void* stream, cudaEvent_t entry, bool wait);
+
+// Nothing of a host-vector apply may outlive the call that failed: copies and kernels already queued on the
+// pipeline's internal streams still read h_x and write h_y, which the caller is free to release after an error.
+static void drain_host_streams(spmv_handle_s* h, cudaStream_t s) {
+  const std::string err = last_error_text();
+  for (cudaStream_t q : {h->hs_up, h->hs_up2, h->hs_run, h->hs_down})
+    if (q) cudaStreamSynchronize(q);
+  cudaStreamSynchronize(s);
+  cudaGetLastError();
+  set_last_error("%s", err.c_str());
+}
+
 static spmv_status_t apply_host_impl(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
+                                     void* stream, cudaEvent_t entry, bool wait) {
+  const spmv_status_t st = apply_host_body(h, alpha, h_x, beta, h_y, stream, entry, wait);
+  if (st != SPMV_OK && st != SPMV_ERR_INVALID_ARG && handle_alive(h)) drain_host_streams(h, (cudaStream_t)stream);
+  return st;
+}
+
+static spmv_status_t apply_host_body(spmv_handle_t h, double alpha, const double* h_x, double beta, double* h_y,
                                      void* stream, cudaEvent_t entry, bool wait) {
   if (!handle_alive(h)) return SPMV_ERR_INVALID_ARG;
   if ((h->A.rows > 0 && !h_y) || (h->A.cols > 0 && !h_x)) return SPMV_ERR_INVALID_ARG;
@@ -444,8 +489,11 @@ spmv_status_t spmv_apply_host_batch(int32_t n, const spmv_handle_t* hs, const do
   spmv_status_t st = e == cudaSuccess ? SPMV_OK : SPMV_ERR_CUDA;
   for (int i = 0; i < n && st == SPMV_OK; ++i) st = apply_host_impl(hs[i], alphas[i], h_xs[i], betas[i], h_ys[i], stream, entry, false);
   e = cudaStreamSynchronize(s);                    // also after a failure: nothing of this call may stay in flight
-  for (int i = 0; i < n; ++i)
-    if (handle_alive(hs[i]) && hs[i]->hs_up) cudaStreamSynchronize(hs[i]->hs_up);
+  for (int i = 0; i < n; ++i) {
+    if (!handle_alive(hs[i])) continue;
+    if (st != SPMV_OK) drain_host_streams(hs[i], s);       // a member failed: every member's pipeline is drained
+    else if (hs[i]->hs_up) cudaStreamSynchronize(hs[i]->hs_up);
+  }
   cudaEventDestroy(entry);
   if (st == SPMV_OK && e != cudaSuccess) { set_last_error("spmv_apply_host_batch: %s", cudaGetErrorString(e)); st = SPMV_ERR_CUDA; }
   return st;

@@ -1,6 +1,7 @@
 // The handle behind spmv_handle_t and the helpers api.cu / tuner.cu share.
 #pragma once
 #include <map>
+#include <mutex>
 #include <string>
 #include <tuple>
 #include <utility>
@@ -28,6 +29,13 @@ struct spmv_handle_s {
   std::map<int, spmv::MergePlan> plans;                    // key tile_items
   std::map<int, spmv::DiaFormat> dias;                     // key C
   int dia_state = 0;                                       // 0 not tried, 1 built once, -1 pattern is not diagonal
+
+  // merge-path and row-split SELL keep ONE workspace per handle (tile carries / segment sums): applies of such a
+  // variant are chained through this event, so that an apply enqueued on another stream starts after the previous one
+  std::mutex ws_mu;
+  cudaEvent_t ws_event = nullptr;
+  cudaStream_t ws_stream = nullptr;
+  bool ws_used = false;
 
   // staging for spmv_apply_host, and the three internal streams + events of its chunk pipeline
   double* d_x_stage = nullptr;

@@ -576,6 +576,12 @@ extern "C" spmv_status_t spmv_tune(spmv_handle_t h, const spmv_tune_opts_t* opts
           for (size_t i = 0; i < close.size() && ready; ++i) {
             bool quick = false;
             double us = 0;
+            // the carve-out is a per-FUNCTION attribute: siblings that share a kernel and differ in `co` would all
+            // run with whichever value was set last, so it is set again before each sibling's batch
+            if (plans[i].n > 0) {
+              cudaFuncSetAttribute(plans[i].k[0].fn, cudaFuncAttributePreferredSharedMemoryCarveout, close[i].v.carve);
+              if (plans[i].has_alt) cudaFuncSetAttribute(plans[i].alt.fn, cudaFuncAttributePreferredSharedMemoryCarveout, close[i].v.carve);
+            }
             ready = T.time(plans[i], close[i].us, 1e300, &us, &quick) == SPMV_OK;
             ts[i].push_back(us);
           }

@@ -9,6 +9,7 @@
 
 #include <algorithm>
 
+#include "device_utils.cuh"
 #include "spmv_internal.h"
 
 namespace spmv {
@@ -168,6 +169,36 @@ __global__ void ceiling_gather_kernel(const double* __restrict__ x, const int* _
   if (s == 1.2345e300) out[0] = s;
 }
 
+// The VALUE loads of bcsr3_kernel<16, 2, ...> and nothing else (no block columns, no x, no FMA chain, no y): `nrec`
+// records of 9 * nb doubles, element k of block j of record r at r * 9 * nb + k * nb + j; 16 lanes per record, lane l
+// reads blocks l and l + 16 of each of the nine element streams -- runs of nb doubles that start at any 8-byte
+// boundary.  Answers: is the block-row layout's load pattern (many short unaligned runs through LSU) what keeps the
+// bcsr3 winner below the one-stream read ceiling, or is it the rest of the kernel?
+__global__ void __launch_bounds__(512)
+ceiling_blockrow_kernel(const double* __restrict__ src, int64_t nrec, int nb, double* __restrict__ out) {
+  constexpr int T = 16, U = 2;
+  const int lane = threadIdx.x & (T - 1);
+  const int64_t nsub = ((int64_t)gridDim.x * blockDim.x) / T;
+  double s = 0.0;
+  for (int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / T; r < nrec; r += nsub) {
+    const double* pv = src + r * 9 * (int64_t)nb;
+    for (int j = lane; j < nb; j += T * U) {
+      double v[U][9];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int jj = j + u * T;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) v[u][k] = jj < nb ? ld_stream(pv + (int64_t)k * nb + jj) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int k = 0; k < 9; ++k) s += v[u][k];
+    }
+  }
+  if (s == 1.2345e300) out[0] = s;
+}
+
 }  // namespace spmv
 
 extern "C" spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_t reps, void* stream, double* result) {
@@ -243,6 +274,33 @@ extern "C" spmv_status_t spmv_measure_ceiling(int32_t kind, size_t bytes, int32_
     *result = best;
     cudaFree(xv);
     cudaFree(idx);
+    cudaFree(o);
+  } else if (kind == 4) {
+    // `bytes` per launch as records of 27 blocks (cfg4's interior block rows: 1944 B each), launches back to back
+    // over rotating windows of a >= 768 MB buffer like kinds 0 / 1; MEDIAN batch (the protocol of the applies)
+    const int nb = 27;
+    const int64_t nrec = (int64_t)(bytes / (72 * nb)), n = nrec * 9 * nb;
+    if (nrec <= 0) return SPMV_ERR_INVALID_ARG;
+    const int64_t nwin = std::max<int64_t>(1, ((int64_t)768 << 20) / (n * 8) + 1);
+    double *a = nullptr, *o = nullptr;
+    SPMV_CUDA_TRY(cudaMalloc(&a, nwin * n * 8));
+    SPMV_CUDA_TRY(cudaMalloc(&o, 8));
+    SPMV_CUDA_TRY(cudaMemsetAsync(a, 0, nwin * n * 8, s));
+    const int K = (int)std::max<int64_t>(4, std::min<int64_t>(64, ((int64_t)2 << 30) / (n * 8)));
+    std::vector<double> all;
+    int64_t w = 0;
+    for (int i = 0; i < reps + 2; ++i) {
+      SPMV_CUDA_TRY(cudaEventRecord(e0, s));
+      for (int k = 0; k < K; ++k, w = (w + 1) % nwin)
+        ceiling_blockrow_kernel<<<148 * 8 * 8, 128, 0, s>>>(a + w * n, nrec, nb, o);
+      SPMV_CUDA_TRY(cudaEventRecord(e1, s));
+      SPMV_CUDA_TRY(cudaEventSynchronize(e1));
+      SPMV_CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+      if (i >= 2) all.push_back((double)K * (double)n * 8.0 / ((double)ms * 1e6));
+    }
+    std::sort(all.begin(), all.end());
+    *result = all[all.size() / 2];
+    cudaFree(a);
     cudaFree(o);
   } else {
     return SPMV_ERR_INVALID_ARG;
