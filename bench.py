@@ -314,11 +314,13 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     tune_s = time.perf_counter() - t0
     variant = handles[0].variant
     # the feature-guided search on the same matrix and reference: its cost and its winner
-    rg = tune(0, True, use_cache=2, cache_path=None, search=1)
-    guided = {"tune_seconds": rg["tune_seconds"], "winner": rg["winner"], "winner_us": rg["winner_us"],
-              "n_timed": rg["n_timed"], "exhaustive_tune_seconds": reports[0]["tune_seconds"],
-              "exhaustive_winner_us": reports[0]["winner_us"], "exhaustive_n_timed": reports[0]["n_timed"]}
-    handles[0].select(variant)
+    guided = None
+    if not args.no_extras:
+        rg = tune(0, True, use_cache=2, cache_path=None, search=1)
+        guided = {"tune_seconds": rg["tune_seconds"], "winner": rg["winner"], "winner_us": rg["winner_us"],
+                  "n_timed": rg["n_timed"], "exhaustive_tune_seconds": reports[0]["tune_seconds"],
+                  "exhaustive_winner_us": reports[0]["winner_us"], "exhaustive_n_timed": reports[0]["n_timed"]}
+        handles[0].select(variant)
     fmt_bytes = int(sum(h.info().format_bytes for h in handles[:members]))
     bytes_actual = fmt_bytes + vec_bytes
     # merge-path and row-split SELL add one small ordered fix-up kernel per apply
@@ -382,7 +384,7 @@ def bench_config(cfg, args, torch, binding, W, dist_max, device, primary):
     # ---- where the winner reads no matrix values (constant-coefficient stencil): the best variant that DOES stream
     # them, same cache protocol -- what the stencil kernels do on a variable-coefficient matrix of this shape
     with_values = None
-    if members == 1 and variant.split(":")[0] in ("dia_const", "dia_cwin"):
+    if members == 1 and variant.split(":")[0] in ("dia_const", "dia_cwin") and not args.no_extras:
         rv = tune(0, True, use_cache=2, cache_path=None, variant_filter=VALUE_STREAMING_FILTER)
         for h in handles:
             h.select(rv["winner"])
@@ -805,7 +807,8 @@ def main():
     ap.add_argument("--no-oracle-check", action="store_true")
     ap.add_argument("--sharded", action="store_true",
                     help="N > 1: row-shard ONE matrix (the first of --configs) over the GPUs instead of N replicas")
-    ap.add_argument("--no-extras", action="store_true", help="skip the banded-matrix line (16-bit vs 32-bit column indices)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extras: the banded-matrix line, the guided-search comparison, the value-streaming "
+                                                              "runner-up (profiling runs: only the tuned variant's launches)")
     ap.add_argument("--variant-filter", default=None,
                     help="comma list of descriptor prefixes the tuner may use (spmv_tune variant_filter), e.g. "
                          "'csr_scalar,csr_vector,sell:,sell_tma,ell,merge,bcsr3,dia:,dia_tma' = everything that still "
