@@ -83,3 +83,19 @@ def test_gpus_n_without_a_launcher_starts_n_ranks():
     last = [l for l in r.stdout.splitlines() if l.startswith("{")][-1]
     rec = json.loads(last)
     assert rec == {"ranks_joined": 2, "n_gpus": 2, "world_size": 2}
+
+
+def test_reference_arm_under_n_ranks_prints_one_line_with_n_gpus():
+    """`bench.py --impl reference --gpus 2` (no launcher): two ranks are started, rank 0 alone runs the oracle and prints
+    ONE line whose n_gpus and config agree with what the product arm would print for the same workload."""
+    from paper_1309_1894_b200 import workloads as W
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "2",
+                        "--warmup", "3", "--configs", "1"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, lines
+    rec = json.loads(lines[0])
+    assert rec["impl"] == "reference" and rec["n_gpus"] == 2 and rec["value"] > 0
+    assert rec["config"] == bench.headline_config(W, 1, 4096, 20224)
+    assert rec["cpu_baseline"]["kind"] == "oracle" and rec["e2e"]["h2d_bytes_per_step"] == 0
