@@ -132,7 +132,9 @@ typedef struct {
   int32_t n_carveouts;        /* 0 -> {-1 (driver default)}                             */
   int32_t carveouts[8];       /* shared-memory carve-out percentages, -1 = default      */
   int32_t use_cache;          /* 0 -> use the in-process cache; 2 -> bypass it           */
-  const char* cache_path;     /* optional file persisted across processes               */
+  const char* cache_path;     /* optional file persisted across processes.  A cached winner (in process or from
+                                 this file) is a claim: it is adopted only after one launch of it has passed the same
+                                 verification as every candidate; an entry that fails is dropped and the search runs */
   const char* fault_inject;   /* TEST ONLY: descriptor prefix of candidates whose output
                                  is perturbed before verification                       */
   uint64_t seed;
